@@ -1,0 +1,291 @@
+"""Pins P7-P14 of SURVEY.md 8(c): noise, CG, loops, derivative loops and the TSM
+combination of the oracle, against known answers, dense brute force, closed forms and
+the statistical laws of Eq. 2.1-2.4."""
+import itertools
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1211_0126_b200 import workloads as W
+from dense_helpers import coords, dense_from_apply, parity, timeslice_projector_trace, volume
+
+G5 = np.diag([1.0, 1.0, -1.0, -1.0]).astype(np.complex128)
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# ---------------------------------------------------------------- P12 noise
+def test_p12_philox_known_answers():
+    n = 0
+    for line in open(os.path.join(GOLD, "philox4x32_10_kat.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        w = [int(t, 16) for t in line.split()]
+        assert oracle.philox4x32_10(w[0:4], w[4:6]).tolist() == w[6:10]
+        n += 1
+    assert n == 3
+
+
+def test_p12_noise_encoding_and_statistics():
+    dims = (8, 8, 8, 8)
+    seed = 0x1211012600000001
+    eta = oracle.noise(dims, seed, 5, 0)
+    # encoding O3, checked site by site against the raw generator on a few sites
+    for lex in (0, 1, 777, 4095):
+        w0 = int(oracle.philox4x32_10([lex, 0, 5, 0x5A340000], [seed & 0xFFFFFFFF, seed >> 32])[0])
+        for q in range(12):
+            k = (w0 >> (2 * q)) & 3
+            assert eta[lex].reshape(-1)[q] == [1, 1j, -1, -1j][k]
+    vals = eta.reshape(-1)
+    assert np.array_equal(np.abs(vals), np.ones_like(vals.real))
+    n = vals.size
+    counts = np.array([(vals == v).sum() for v in (1, 1j, -1, -1j)])
+    assert counts.sum() == n
+    chi2 = ((counts - n / 4) ** 2 / (n / 4)).sum()
+    assert chi2 < 25.0                                   # 3 dof; P(chi2 > 25) ~ 1.5e-5
+    assert abs(vals.mean()) < 5 / np.sqrt(n)             # Eq. 2.1, first property
+    # Eq. 2.1 second property on a few components: (1/N) sum_j eta_j eta_j^dag = 1 + O(1/sqrt N)
+    N = 400
+    sub = np.stack([oracle.noise((2, 2, 2, 2), seed, j, 0).reshape(-1)[:24] for j in range(N)])
+    cov = sub.T @ sub.conj() / N
+    assert np.allclose(np.diag(cov), 1.0, atol=1e-14)
+    off = cov - np.eye(24)
+    assert np.abs(off).max() < 5 / np.sqrt(N)
+    # different sources / seeds / kinds are different streams
+    assert (oracle.noise(dims, seed, 6, 0) != eta).mean() > 0.7
+    assert (oracle.noise(dims, seed + 1, 5, 0) != eta).mean() > 0.7
+    z2 = oracle.noise(dims, seed, 5, 1).reshape(-1)
+    assert set(np.unique(z2).tolist()) == {-1, 1}
+    assert abs(z2.real.mean()) < 5 / np.sqrt(n)
+
+
+# ---------------------------------------------------------------- P7 / P10 dense brute force
+@pytest.fixture(scope="module")
+def tiny():
+    dims = (2, 2, 2, 4)
+    kappa, mu, theta = 0.16, 0.25, -1
+    U = W.random_su3_links(dims, 0.7, 51)
+    V = volume(dims)
+    M = dense_from_apply(lambda v: oracle.apply_M(dims, theta, kappa, mu, U, v), V)
+    Minv = np.linalg.inv(M)
+    return dict(dims=dims, kappa=kappa, mu=mu, theta=theta, U=U, M=M, Minv=Minv, V=V)
+
+
+def test_p7_hp_solve_and_loops_equal_dense(tiny):
+    d = tiny
+    eta = oracle.noise(d["dims"], 99, 0)
+    s, info = oracle.solve(d["dims"], d["theta"], d["kappa"], d["mu"], d["U"], eta, 1e-13, 500)
+    s_dense = (d["Minv"] @ eta.reshape(-1)).reshape(eta.shape)
+    assert np.allclose(s, s_dense, atol=1e-11)
+    L = oracle.loops(d["dims"], eta, s)
+    Lt, Vs = d["dims"][3], d["V"] // d["dims"][3]
+    for G in range(16):
+        Gam = oracle.gamma(G)
+        ref = np.einsum("txac,ab,txbc->t", eta.reshape(Lt, Vs, 4, 3).conj(), Gam, s_dense.reshape(Lt, Vs, 4, 3))
+        assert np.allclose(L[G], ref, atol=1e-10)
+
+
+def test_p7_brute_force_2x2x2x2():
+    """Extent 2: x+mu and x-mu are the same site and both hop terms contribute (8(b))."""
+    dims = (2, 2, 2, 2)
+    kappa, mu, theta = 0.15, 0.3, -1
+    U = W.random_su3_links(dims, 0.7, 52)
+    M = dense_from_apply(lambda v: oracle.apply_M(dims, theta, kappa, mu, U, v), 16)
+    eta = oracle.noise(dims, 5, 1)
+    s, info = oracle.solve(dims, theta, kappa, mu, U, eta, 1e-13, 500)
+    assert np.allclose(M @ s.reshape(-1), eta.reshape(-1), atol=1e-11)
+
+
+def test_p10_one_end_identity(tiny):
+    """Eq. 2.5 in dense form: Im Tr[g5 M^-1] = -a Tr[(M^dag M)^-1]."""
+    d = tiny
+    a = 2 * d["kappa"] * d["mu"]
+    tr5 = timeslice_projector_trace(d["dims"], oracle.gamma(1), d["Minv"]).sum()
+    rhs = -a * np.trace(np.linalg.inv(d["M"].conj().T @ d["M"])).real
+    assert np.isclose(tr5.imag, rhs, rtol=1e-11)
+    # and as the paper writes it: M_u^-1 - M_d^-1 = -2 i a M_d^-1 g5 M_u^-1
+    Md = dense_from_apply(lambda v: oracle.apply_M(d["dims"], d["theta"], d["kappa"], -d["mu"], d["U"], v), d["V"])
+    G5f = np.kron(np.eye(d["V"]), np.kron(G5, np.eye(3)))
+    assert np.allclose(d["Minv"] - np.linalg.inv(Md), -2j * a * np.linalg.inv(Md) @ G5f @ d["Minv"], atol=1e-11)
+
+
+# ---------------------------------------------------------------- P8 estimator statistics (Eq. 2.1-2.3)
+def test_p8_estimator_unbiased_with_predicted_variance(tiny):
+    d = tiny
+    dims, Lt = d["dims"], d["dims"][3]
+    Vs = d["V"] // Lt
+    N = 300
+    acc = np.zeros((16, Lt), dtype=np.complex128)
+    samples = np.zeros((N, 16, Lt), dtype=np.complex128)
+    for j in range(N):
+        eta = oracle.noise(dims, 1234, j)
+        s, _ = oracle.solve(dims, d["theta"], d["kappa"], d["mu"], d["U"], eta, 1e-12, 500)
+        samples[j] = oracle.loops(dims, eta, s)
+    mean = samples.mean(axis=0)
+    for G in (0, 1, 3, 7, 12):
+        Gam = oracle.gamma(G)
+        exact = timeslice_projector_trace(dims, Gam, d["Minv"])
+        A = np.kron(np.eye(d["V"]), np.kron(Gam, np.eye(3))) @ d["Minv"]     # eta^dag P_t A eta
+        for t in range(Lt):
+            rows = slice(12 * Vs * t, 12 * Vs * (t + 1))
+            blk = A[rows, :].copy()
+            blk[:, rows] -= np.diag(np.diag(A[rows, rows]))
+            var = (np.abs(blk) ** 2).sum()            # exact Z4 variance: sum_{a in t, b != a} |A_ab|^2
+            assert abs(mean[G, t] - exact[t]) < 4.5 * np.sqrt(var / N)
+            samp_var = (np.abs(samples[:, G, t] - exact[t]) ** 2).mean()
+            assert 0.7 * var < samp_var < 1.4 * var
+
+
+# ---------------------------------------------------------------- P9 free-field loops closed form
+def test_p9_free_field_loops_closed_form():
+    dims = (2, 2, 4, 4)
+    kappa, mu, theta = 0.11, 0.4, -1
+    a = 2 * kappa * mu
+    U = W.unit_links(dims)
+    V = volume(dims)
+    M = dense_from_apply(lambda v: oracle.apply_M(dims, theta, kappa, mu, U, v), V)
+    Minv = np.linalg.inv(M)
+    sA = sI = 0.0
+    for n in itertools.product(*[range(L) for L in dims]):
+        p = [2 * np.pi * n[i] / dims[i] for i in range(3)] + [(2 * n[3] + 1) * np.pi / dims[3]]
+        A = 1 - 2 * kappa * sum(np.cos(p))
+        den = A * A + sum((2 * kappa * np.sin(q)) ** 2 for q in p) + a * a
+        sA += A / den
+        sI += 1.0 / den
+    Vs = V // dims[3]
+    L1 = timeslice_projector_trace(dims, oracle.gamma(0), Minv)
+    L5 = timeslice_projector_trace(dims, oracle.gamma(1), Minv)
+    assert np.allclose(L1, 12 * Vs / V * sA, atol=1e-12)
+    assert np.allclose(L5, -1j * a * 12 * Vs / V * sI, atol=1e-12)
+    for m in range(4):
+        assert np.allclose(timeslice_projector_trace(dims, oracle.gamma(2 + m), Minv), 0, atol=1e-12)
+
+
+# ---------------------------------------------------------------- P13 CG
+def test_p13_truncated_cg_is_the_krylov_minimiser(tiny):
+    d = tiny
+    dims, theta, kappa, mu, U, V = d["dims"], d["theta"], d["kappa"], d["mu"], d["U"], d["V"]
+    a = 2 * kappa * mu
+    e = parity(dims) == 0
+    Mhat = dense_from_apply(lambda v: oracle.apply_Mhat(dims, theta, kappa, mu, U, v), V, site_mask=e)
+    eta = oracle.noise(dims, 4321, 0)
+    # bhat = eta_e + kappa D_eo R^-1 eta_o from the dense full matrix: bhat = eta_e - M_eo M_oo^-1 eta_o
+    idx = np.arange(12 * V).reshape(V, 12)
+    se, so = idx[e].reshape(-1), idx[~e].reshape(-1)
+    M = d["M"]
+    bhat = eta.reshape(-1)[se] - M[np.ix_(se, so)] @ np.linalg.solve(M[np.ix_(so, so)], eta.reshape(-1)[so])
+    A = Mhat.conj().T @ Mhat
+    bp = Mhat.conj().T @ bhat
+    prev = np.inf
+    for k in (1, 2, 3, 5, 8):
+        s, info = oracle.solve(dims, theta, kappa, mu, U, eta, 0.0, k)
+        assert info["iters"] == k and info["status"] == 0
+        xk = s.reshape(-1)[se]
+        K = [bp]
+        for _ in range(k - 1):
+            K.append(A @ K[-1])
+        Kq, _ = np.linalg.qr(np.stack(K, axis=1))
+        c, *_ = np.linalg.lstsq(Mhat @ Kq, bhat, rcond=None)
+        assert np.allclose(xk, Kq @ c, atol=1e-10 * np.linalg.norm(xk))
+        res = np.linalg.norm(bhat - Mhat @ xk)
+        assert res < prev                      # preconditioned true residual non-increasing
+        prev = res
+        # recursive residual reported by the oracle is that of the normal system
+        assert np.isclose(info["rel_resid_rec"], np.linalg.norm(bp - A @ xk) / np.linalg.norm(bp), rtol=1e-8)
+    # tolerance mode stops at the first k with |r_k|/|b'| <= tol
+    s, info = oracle.solve(dims, theta, kappa, mu, U, eta, 1e-3, 500)
+    k = info["iters"]
+    assert info["rel_resid_rec"] <= 1e-3
+    _, prev_info = oracle.solve(dims, theta, kappa, mu, U, eta, 0.0, k - 1)
+    assert prev_info["rel_resid_rec"] > 1e-3
+    s_fixed, _ = oracle.solve(dims, theta, kappa, mu, U, eta, 0.0, k)
+    assert np.array_equal(s, s_fixed)
+    # tolerance not reached within max_iter is flagged (8(b) TSM_ENOCONV) and keeps the iterate
+    s3, info3 = oracle.solve(dims, theta, kappa, mu, U, eta, 1e-12, 3)
+    assert info3["status"] == -6 and info3["iters"] == 3
+    assert np.array_equal(s3, oracle.solve(dims, theta, kappa, mu, U, eta, 0.0, 3)[0])
+
+
+# ---------------------------------------------------------------- P14 derivative
+def test_p14_covariant_difference():
+    dims = (4, 4, 6, 8)
+    xs = coords(dims)
+    U1 = W.unit_links(dims)
+    n = (1, 3, 2, 5)
+    p = np.array([2 * np.pi * n[i] / dims[i] for i in range(4)])
+    u = np.arange(12).reshape(4, 3) + 1j
+    psi = np.exp(1j * (xs @ p))[:, None, None] * u[None]
+    for m in range(4):   # U=1, periodic: D_mu e^{ipx} = i sin(p_mu) e^{ipx}
+        assert np.allclose(oracle.cov_diff(dims, +1, U1, m, psi), 1j * np.sin(p[m]) * psi, atol=1e-13)
+    # delta source: (D_mu delta_y)(y - mu) = U_mu(y-mu)/2, (D_mu delta_y)(y + mu) = -U_mu(y)^dag/2
+    U = W.random_su3_links(dims, 0.8, 61)
+    lex = lambda x: x[0] + dims[0] * (x[1] + dims[1] * (x[2] + dims[2] * x[3]))
+    for theta in (+1, -1):
+        for y in [(1, 2, 3, 0), (3, 3, 5, 7)]:
+            src = np.zeros((volume(dims), 4, 3), dtype=np.complex128)
+            src[lex(y), 2, 1] = 1.0
+            for m in range(4):
+                out = oracle.cov_diff(dims, theta, U, m, src)
+                xm = list(y); xm[m] = (y[m] - 1) % dims[m]
+                xp = list(y); xp[m] = (y[m] + 1) % dims[m]
+                php = theta if (m == 3 and xm[3] == dims[3] - 1) else 1
+                phm = theta if (m == 3 and xp[3] == 0) else 1
+                expect = np.zeros_like(out)
+                expect[lex(xm), 2] += 0.5 * php * U[m, lex(xm)][:, 1]
+                expect[lex(xp), 2] += -0.5 * phm * U[m, lex(y)].conj().T[:, 1]
+                assert np.allclose(out, expect, atol=1e-15)
+    # loops_deriv = loops(eta, D_mu s), ordering [mu][Gamma][t]
+    eta = oracle.noise(dims, 8, 0)
+    s = W.random_spinor(dims, 62)
+    Ld = oracle.loops_deriv(dims, -1, U, eta, s)
+    for m in range(4):
+        assert np.array_equal(Ld[m], oracle.loops(dims, eta, oracle.cov_diff(dims, -1, U, m, s)))
+    full = oracle.all_loops(dims, -1, U, eta, s, True)
+    assert full.shape == (80, dims[3]) and np.array_equal(full[16:].reshape(4, 16, -1), Ld)
+
+
+def test_loops_match_plain_einsum():
+    dims = (4, 2, 4, 6)
+    eta = oracle.noise(dims, 3, 2)
+    s = W.random_spinor(dims, 63)
+    Lt, Vs = dims[3], volume(dims) // dims[3]
+    L = oracle.loops(dims, eta, s)
+    for G in range(16):
+        ref = np.einsum("txac,ab,txbc->t", eta.reshape(Lt, Vs, 4, 3).conj(), oracle.gamma(G), s.reshape(Lt, Vs, 4, 3))
+        assert np.allclose(L[G], ref, atol=1e-11)
+
+
+# ---------------------------------------------------------------- P11 TSM algebra (Eq. 2.4)
+def test_p11_tsm_reduces_to_plain_estimator_when_lp_is_hp(tiny):
+    d = tiny
+    args = (d["dims"], d["theta"], d["kappa"], d["mu"], d["U"], 555)
+    n_hp, n_lp = 3, 5
+    per = {}
+    L = oracle.tsm_loops(*args, n_hp, n_lp, 1e-9, 500, 1e-9, 500, with_derivative=True, per_source=per)
+    plain = sum(per[j]["lp"] for j in range(n_hp, n_hp + n_lp)) / n_lp     # Eq. 2.2 over the LP set
+    assert np.array_equal(L, plain)
+    for j in range(n_hp):
+        assert np.array_equal(per[j]["hp"], per[j]["lp"])
+    assert set(per) == set(range(n_hp + n_lp))      # A10: exactly N_HP + N_LP sources, disjoint sets
+
+
+def test_p11_tsm_unbiased_with_crude_lp(tiny):
+    d = tiny
+    dims = d["dims"]
+    per = {}
+    n_hp, n_lp = 150, 300
+    L = oracle.tsm_loops(dims, d["theta"], d["kappa"], d["mu"], d["U"], 777, n_hp, n_lp,
+                         1e-12, 500, 0.0, 2, per_source=per)
+    corr = np.stack([per[j]["hp"] - per[j]["lp"] for j in range(n_hp)])
+    lps = np.stack([per[j]["lp"] for j in range(n_hp, n_hp + n_lp)])
+    assert np.allclose(L, corr.mean(axis=0) + lps.mean(axis=0), atol=1e-12)
+    err = np.sqrt(corr.var(axis=0).real / n_hp + lps.var(axis=0).real / n_lp)
+    biased = False
+    for G in (0, 1, 4, 9, 15):
+        exact = timeslice_projector_trace(dims, oracle.gamma(G), d["Minv"])
+        assert (np.abs(L[G] - exact) < 5 * err[G] + 1e-12).all()
+        lp_only = lps.mean(axis=0)[G]
+        lp_err = np.sqrt(lps.var(axis=0).real[G] / n_lp)
+        biased |= bool((np.abs(lp_only - exact) > 6 * lp_err).any())
+    assert biased, "a 2-iteration LP estimate should be visibly biased without the correction"
