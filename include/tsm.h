@@ -1,0 +1,157 @@
+/*
+ * tsm.h -- C ABI of the B200-native truncated-solver-method (TSM) loop library.
+ *
+ * The calls follow the paper's statement of the problem (arXiv:1211.0126; line numbers
+ * are /root/reference/PAPER.md, "Ax/Ox/Cx" are the readings listed in DESIGN.md):
+ *   - noise sources |eta_j> with Z2/Z4 components          (Eq. 2.1)
+ *   - solve M|s_j> = |eta_j>                               (Eq. 2.2)
+ *   - high precision, or truncated "at a large residual or equivalently a fixed
+ *     number of iterations"
+ *   - loops (1/N) sum <eta^dag X s> for all insertion times
+ *   - the TSM combination                                  (Eq. 2.4)
+ *
+ * Conventions
+ *   - Every call returns an int status: TSM_OK or a negative TSM_E* code.  Nothing throws
+ *     or aborts.  tsm_last_error() gives a human-readable message for the last failure.
+ *   - Pointers named host_* are HOST memory, dev_* are DEVICE memory on the context's GPU.
+ *     Host arrays are caller-owned fp64 in lexicographic layouts (C1, C2):
+ *       lex(x) = x0 + L0*(x1 + L1*(x2 + L2*x3)), x = (x,y,z,t);
+ *       spinor  [lex][alpha 0..3][colour 0..2][re,im];
+ *       links   [mu 0..3][lex][row c][col c'][re,im], (U psi)_c = sum_c' U_cc' psi_c';
+ *       loops   [op][t][re,im], op = 0..15 the 16 Gamma of C3 (1, g5, g_mu, g5 g_mu,
+ *               sigma_01,02,03,12,13,23), then 16 + 16*mu + Gamma for the derivative loops.
+ *   - The library allocates no large device memory.  All of it (link copies, solver
+ *     vectors, solution slots, reduction scratch) lives in ONE caller-provided workspace
+ *     (a torch tensor's data_ptr()), sized by tsm_workspace_bytes().  The context owns
+ *     only metadata, a few KB of pinned host memory and a few KB of device scalars.
+ *   - Work is enqueued on the stream given to tsm_set_stream() (default: the legacy
+ *     default stream).  Calls that return host scalars or arrays synchronise that stream
+ *     before returning; calls that only take dev_* pointers are asynchronous.
+ *   - "Native layout" of a single-parity spinor field with V_h = V/2 sites, nrhs sources:
+ *       [rhs][chunk][cb] of 16-byte vectors; fp64: 12 chunks of double2 (one complex each,
+ *       q = 3*alpha + c); fp32: 6 chunks of float4 (complex q = 2*chunk, 2*chunk+1);
+ *       bf16: 3 chunks of 8 x bf16 (complex q = 4*chunk .. 4*chunk+3);
+ *       cb = lex >> 1 is the checkerboard index, parity = (x+y+z+t) & 1 (H1).
+ *       A full-lattice field is [parity 0,1] of those.  tsm_field_bytes() gives sizes.
+ *   - Error behaviour: wrong-state calls (no workspace / gauge / params yet) -> TSM_ESTATE;
+ *     bad dims, enum, nrhs, slot or NULL pointer -> TSM_EINVAL; CUDA failure -> TSM_ECUDA.
+ */
+#ifndef TSM_H
+#define TSM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tsm_ctx tsm_ctx; /* opaque; owned by the library */
+
+enum { TSM_OK = 0, TSM_EINVAL = -1, TSM_ESTATE = -2, TSM_ECUDA = -3, TSM_ENOTUNITARY = -4,
+       TSM_EBREAKDOWN = -5, TSM_ENOCONV = -6 };
+enum { TSM_F64 = 0, TSM_F32 = 1, TSM_BF16 = 2 };          /* spinor storage precision */
+enum { TSM_Z4 = 0, TSM_Z2 = 1 };                           /* noise kind (A5)          */
+enum { TSM_OP_D_EO = 0,      /* out_e = D_eo in_o                         (H5)           */
+       TSM_OP_D_OE = 1,      /* out_o = D_oe in_e                                        */
+       TSM_OP_MHAT = 2,      /* out_e = (R - kappa^2 D_eo R^-1 D_oe) in_e (O4)           */
+       TSM_OP_MHAT_DAG = 3,  /* out_e = Mhat^dagger in_e                                 */
+       TSM_OP_M_FULL = 4 };  /* out = M in on the full lattice, [parity] fields (O2)     */
+#define TSM_MAX_NRHS 16
+#define TSM_N_LOCAL_OPS 16
+#define TSM_N_DERIV_OPS 64
+
+/* Geometry (H1).  dims = (Lx,Ly,Lz,Lt), every extent even and >= 4.  t_boundary = +1
+ * periodic or -1 antiperiodic in time (A3).  device = CUDA ordinal. */
+int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device);
+int tsm_destroy(tsm_ctx* ctx);
+const char* tsm_last_error(const tsm_ctx* ctx);
+
+/* Bytes of one single-parity native field of `nrhs` sources in precision `prec`. */
+size_t tsm_field_bytes(const tsm_ctx* ctx, int prec, int nrhs);
+
+/* Workspace: bytes needed for up to max_nrhs simultaneous sources (all precisions, both
+ * link copies, two solution slots, staging for host<->device conversion).  The pointer
+ * must be 256-byte aligned device memory that outlives every later call. */
+size_t tsm_workspace_bytes(const tsm_ctx* ctx, int max_nrhs);
+int tsm_set_workspace(tsm_ctx* ctx, void* dev_ptr, size_t bytes, int max_nrhs);
+int tsm_set_stream(tsm_ctx* ctx, void* cuda_stream);
+
+/* kappa, mu of the kappa-normalised twisted-mass operator of O2:
+ * M = 1 + 2 i kappa mu gamma5 - kappa D_hop  (= 2 kappa x the paper's M_u). */
+int tsm_set_params(tsm_ctx* ctx, double kappa, double mu);
+
+/* H2: upload one gauge configuration.  host_links is [4][V][3][3][2] fp64,
+ * copied (the caller keeps its array); it may be pinned or pageable.  The fp64 copy always
+ * keeps 18 reals; `reconstruct` (18 or 12) selects the storage of the fp32 copy used by the
+ * F32/BF16 paths (12: first two rows, third row rebuilt in-kernel, A22).  Links further than
+ * 1e-10 from SU(3) give TSM_ENOTUNITARY when reconstruct == 12.  max_unitarity_dev (may be
+ * NULL) receives max(|U^dag U - 1|_max, |det U - 1|). */
+int tsm_set_gauge(tsm_ctx* ctx, const double* host_links, int reconstruct, double* max_unitarity_dev);
+
+/* H3: generate noise source `source_id` of stream `seed` (O3: Philox4x32-10, counter
+ * (lex, source_id, kind)) on the device and copy it to host_out [V][4][3][2] in lex order
+ * (parity-test hook; the solver generates its sources itself). */
+int tsm_noise(tsm_ctx* ctx, uint64_t seed, uint32_t source_id, int kind, double* host_out);
+
+/* Host lex fp64 [nrhs][V][4][3][2]  <->  device native full-lattice field [parity][rhs][chunk][cb]. */
+int tsm_pack(tsm_ctx* ctx, int prec, int nrhs, const double* host_lex, void* dev_native);
+int tsm_unpack(tsm_ctx* ctx, int prec, int nrhs, const void* dev_native, double* host_lex);
+
+/* H5: one application of the stencil on caller buffers in native layout (asynchronous).
+ * D_EO/D_OE/MHAT/MHAT_DAG take and give single-parity fields; M_FULL full-lattice fields.
+ * dev_in and dev_out must not overlap. */
+int tsm_dslash(tsm_ctx* ctx, int op, int prec, int nrhs, const void* dev_in, void* dev_out);
+
+/* H3+H4+H6+H7: generate sources source_ids[0..nrhs) and solve M s = eta for all of them
+ * at once by even-odd preconditioned CG on Mhat^dag Mhat (O4, O5; batched, not block, CG:
+ * every source has its own alpha, beta, stopping iteration, A14).
+ *   tol > 0 : stop source j at the first iteration with |r_k|/|b'| <= tol (A8); a source
+ *             that has not got there after max_iter iterations reports TSM_ENOCONV.
+ *   tol == 0: exactly max_iter iterations, no residual test (A9).
+ * The full-lattice solutions stay in workspace slot `slot` (0 or 1), in precision `prec`
+ * (BF16 solves leave fp32 solutions).  info (may be NULL) is a host array [nrhs];
+ * rel_resid_true (the fp64 |eta - M s|/|eta| of the full system) is filled only when
+ * want_true_resid != 0.  Returns TSM_OK if every source ended TSM_OK, else the first
+ * non-OK per-source status (solutions are kept either way). */
+typedef struct {
+    int iters;              /* CG iterations done for this source              */
+    int status;             /* TSM_OK, TSM_EBREAKDOWN (A13) or TSM_ENOCONV     */
+    double rel_resid_rec;   /* sqrt(|r_k|^2/|b'|^2) of the CG recursion (A8)   */
+    double rel_resid_true;  /* fp64 true residual of the full system, or -1    */
+    double secs;            /* device time of the whole batch (same for all j) */
+} tsm_solve_info;
+int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs, int kind,
+              int prec, double tol, int max_iter, int slot, int want_true_resid,
+              tsm_solve_info* info);
+int tsm_get_solution(tsm_ctx* ctx, int slot, int rhs, double* host_out /* [V][4][3][2] */);
+/* Overwrite the solution held in a slot (contraction parity with the oracle's s, A16(i));
+ * the slot keeps the seed/source ids/kind/nrhs of the last tsm_solve into it. */
+int tsm_set_solution(tsm_ctx* ctx, int slot, int rhs, const double* host_in /* [V][4][3][2] */);
+
+/* H8-H10: per-timeslice loops and the TSM accumulators (Eq. 2.4, O6, O6b, O7). */
+int tsm_loops_reset(tsm_ctx* ctx, int with_derivative);            /* n_ops = 16 or 16+64     */
+int tsm_loops_add_correction(tsm_ctx* ctx, int slot_hp, int slot_lp); /* += L(HP)-L(LP); N_HP += nrhs */
+int tsm_loops_add_lp(tsm_ctx* ctx, int slot_lp);                   /* += L(LP); N_LP += nrhs  */
+int tsm_loops_source(tsm_ctx* ctx, int slot, int rhs, double* host_out /* [n_ops][Lt][2] */);
+int tsm_loops_finalize(tsm_ctx* ctx, double* host_out /* [n_ops][Lt][2] */);
+/* Accumulator access for checkpoint/resume (state = seed, next id, sums). */
+int tsm_loops_get_state(tsm_ctx* ctx, double* host_corr, double* host_lp, int* n_hp, int* n_lp);
+int tsm_loops_set_state(tsm_ctx* ctx, const double* host_corr, const double* host_lp, int n_hp, int n_lp);
+
+/* Convenience driver: the whole of Eq. 2.4 for one gauge configuration.  Sources
+ * 0..n_hp-1 get an HP (fp64, hp_tol) and an LP solve; sources n_hp..n_hp+n_lp-1 an LP solve
+ * (lp_prec; lp_tol > 0 or exactly lp_iters iterations); batches of nrhs sources.
+ * secs_out (may be NULL) receives the device time from the first noise kernel to the
+ * final loops (reading A23). */
+int tsm_run_loop_set(tsm_ctx* ctx, uint64_t seed, int kind, int n_hp, int n_lp, int lp_prec,
+                     double lp_tol, int lp_iters, double hp_tol, int hp_max_iter, int nrhs,
+                     int with_derivative, double* host_out, double* secs_out);
+
+/* Number of kernels this library has launched on the context since creation. */
+long long tsm_launch_count(const tsm_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TSM_H */

@@ -1,0 +1,336 @@
+// api_solve.cu -- C ABI (include/tsm.h): the solver driver (H3, H4, H6, H7), the loop
+// accumulators (H8-H10) and the whole-configuration TSM driver (Eq. 2.4).
+#include <cmath>
+#include <cstring>
+
+#include "tsm_internal.cuh"
+
+namespace {
+
+struct Twists {
+    TwistCoef zero, one, R, Rinv, Rb, Rbinv, mk2, k, kRinv;
+};
+
+Twists make_twists(const tsm_ctx* ctx)
+{
+    const double k = ctx->kappa, a = 2.0 * ctx->kappa * ctx->mu, n = 1.0 / (1.0 + a * a);
+    Twists t;
+    t.zero = {0, 0, 0, 0};
+    t.one = {1, 0, 1, 0};
+    t.R = {1, a, 1, -a};                 // 1 + i a gamma5
+    t.Rinv = {n, -a * n, n, a * n};      // (1 - i a gamma5)/(1 + a^2)
+    t.Rb = {1, -a, 1, a};                // R(-mu)
+    t.Rbinv = {n, a * n, n, -a * n};
+    t.mk2 = {-k * k, 0, -k * k, 0};
+    t.k = {k, 0, k, 0};
+    t.kRinv = {k * n, -k * a * n, k * n, k * a * n};
+    return t;
+}
+
+// One CG iteration on Mhat^dag Mhat (O5): four stencil launches and two fused BLAS launches.
+int cg_iteration(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, void* r, void* p, void* q, void* w, void* t, double tol)
+{
+    int rc;
+    if ((rc = launch_dslash(ctx, prec, 1, false, nrhs, p, nullptr, t, {tw.zero, tw.Rinv}, nullptr, 2))) return rc;   // t = R^-1 D_oe p
+    if ((rc = launch_dslash(ctx, prec, 0, false, nrhs, t, p, w, {tw.R, tw.mk2}, nullptr, 2))) return rc;             // w = Mhat p
+    if ((rc = launch_dslash(ctx, prec, 1, true, nrhs, w, nullptr, t, {tw.zero, tw.Rbinv}, nullptr, 2))) return rc;   // t = Rb^-1 D_oe^dag w
+    if ((rc = launch_dslash(ctx, prec, 0, true, nrhs, t, w, q, {tw.Rb, tw.mk2}, p, 3))) return rc;                   // q = Mhat^dag w; <p,q>
+    if ((rc = launch_cg_update_xr(ctx, prec, nrhs, x, p, r, q, tol))) return rc;
+    return launch_cg_update_p(ctx, prec, nrhs, p, r);
+}
+
+int fetch_scalars(tsm_ctx* ctx)
+{
+    TSM_CUDA(ctx, cudaMemcpyAsync(ctx->cg_host, ctx->cg, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx->stream));
+    TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return TSM_OK;
+}
+
+// fp64 |eta - M s| / |eta| of the full system for every source of a slot (reading A8/A17).
+int true_residuals(tsm_ctx* ctx, int slot, double* out)
+{
+    const int nrhs = ctx->slot_nrhs[slot], sp = ctx->slot_prec[slot];
+    const size_t fb = field_bytes(TSM_F64, ctx->g.Vh, nrhs);
+    // the six solver vectors are one contiguous region: three full-lattice fp64 fields
+    char* base = (char*)ctx->vec[0];
+    const size_t stride = 2 * ((char*)ctx->vec[1] - (char*)ctx->vec[0]);
+    char *s64 = base, *eta = base + stride, *ms = base + 2 * stride;
+    int rc;
+    // convert both parities; a full field [parity][rhs] is 2*nrhs single-source parity fields
+    if ((rc = launch_convert(ctx, sp, TSM_F64, 2 * nrhs, ctx->slot[slot], s64))) return rc;
+    if ((rc = launch_noise(ctx, TSM_F64, nrhs, ctx->slot_seed[slot], ctx->ids_dev + slot * TSM_MAX_NRHS, ctx->slot_kind[slot], eta))) return rc;
+    const Twists tw = make_twists(ctx);
+    const TwistCoef mk = {-ctx->kappa, 0, -ctx->kappa, 0};
+    if ((rc = launch_dslash(ctx, TSM_F64, 0, false, nrhs, s64 + fb, s64, ms, {tw.R, mk}, nullptr, 0))) return rc;
+    if ((rc = launch_dslash(ctx, TSM_F64, 1, false, nrhs, s64, s64 + fb, ms + fb, {tw.R, mk}, nullptr, 0))) return rc;
+    if ((rc = launch_diff_norm2(ctx, nrhs, eta, ms))) return rc;
+    if ((rc = fetch_scalars(ctx))) return rc;
+    const double eta2 = 12.0 * (double)ctx->g.V;   // |eta_{alpha c}(x)| = 1 for Z4 and Z2
+    for (int j = 0; j < nrhs; j++) out[j] = std::sqrt(ctx->cg_host->pq[j] / eta2);
+    return TSM_OK;
+}
+
+int check_slot(tsm_ctx* ctx, int slot, int rhs)
+{
+    if (slot < 0 || slot > 1) return tsm_fail(ctx, TSM_EINVAL, "slot must be 0 or 1");
+    if (ctx->slot_prec[slot] < 0) return tsm_fail(ctx, TSM_ESTATE, "slot holds no solution");
+    if (rhs < 0 || rhs >= ctx->slot_nrhs[slot]) return tsm_fail(ctx, TSM_EINVAL, "rhs out of range for this slot");
+    return TSM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs, int kind, int prec, double tol,
+              int max_iter, int slot, int want_true_resid, tsm_solve_info* info)
+{
+    int rc = ctx_enter(ctx, true, true, true);
+    if (rc) return rc;
+    if (!source_ids || nrhs < 1 || nrhs > ctx->max_nrhs || (kind != TSM_Z4 && kind != TSM_Z2) || prec < 0 || prec > 2 ||
+        !(tol >= 0) || max_iter < 0 || slot < 0 || slot > 1)
+        return tsm_fail(ctx, TSM_EINVAL, "bad solve arguments");
+    if (prec == TSM_BF16) return tsm_fail(ctx, TSM_EINVAL, "bf16 solves are not built yet");
+    const int sp = prec;   // precision of the stored solution
+    const int Vh = ctx->g.Vh;
+    const Twists tw = make_twists(ctx);
+    ctx->slot_prec[slot] = sp;
+    ctx->slot_nrhs[slot] = nrhs;
+    ctx->slot_kind[slot] = kind;
+    ctx->slot_seed[slot] = seed;
+    memcpy(ctx->slot_ids[slot], source_ids, nrhs * sizeof(uint32_t));
+    uint32_t* ids_dev = ctx->ids_dev + slot * TSM_MAX_NRHS;
+    TSM_CUDA(ctx, cudaMemcpyAsync(ids_dev, ctx->slot_ids[slot], nrhs * sizeof(uint32_t), cudaMemcpyHostToDevice, ctx->stream));
+    TSM_CUDA(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
+
+    char* s_e = (char*)ctx->slot[slot];
+    char* s_o = s_e + field_bytes(sp, Vh, nrhs);
+    void *r = ctx->vec[0], *p = ctx->vec[1], *q = ctx->vec[2], *w = ctx->vec[3], *t = ctx->vec[4], *aux = ctx->vec[5];
+    // H3: eta straight into the slot (eta_e where s_e will be, eta_o where s_o will be)
+    if ((rc = launch_noise(ctx, sp, nrhs, seed, ids_dev, kind, s_e))) return rc;
+    // H4: bhat = eta_e + kappa D_eo R^-1 eta_o (into w);  b' = Mhat^dag bhat (into r)
+    if ((rc = launch_twist(ctx, sp, nrhs, s_o, aux, tw.Rinv))) return rc;
+    if ((rc = launch_dslash(ctx, sp, 0, false, nrhs, aux, s_e, w, {tw.one, tw.k}, nullptr, 0))) return rc;
+    if ((rc = launch_dslash(ctx, sp, 1, true, nrhs, w, nullptr, t, {tw.zero, tw.Rbinv}, nullptr, 0))) return rc;
+    if ((rc = launch_dslash(ctx, sp, 0, true, nrhs, t, w, r, {tw.Rb, tw.mk2}, nullptr, 0))) return rc;
+    // O5: x0 = 0 (x lives in the slot's even half), r0 = p0 = b'
+    void* x = s_e;
+    if ((rc = launch_cg_init(ctx, prec, nrhs, r, p, x))) return rc;
+    const int poll = 4;
+    for (int k = 1; k <= max_iter; k++) {
+        if ((rc = cg_iteration(ctx, prec, nrhs, tw, x, r, p, q, w, t, tol))) return rc;
+        if (tol > 0 && (k % poll == 0) && k < max_iter) {
+            TSM_CUDA(ctx, cudaMemcpyAsync(&ctx->cg_host->all_done, &ctx->cg->all_done, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+            TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+            if (ctx->cg_host->all_done) break;
+        }
+    }
+    // H7: s_e = x, s_o = R^-1 (eta_o + kappa D_oe x)
+    if ((rc = launch_dslash(ctx, sp, 1, false, nrhs, x, s_o, aux, {tw.Rinv, tw.kRinv}, nullptr, 0))) return rc;
+    TSM_CUDA(ctx, cudaMemcpyAsync(s_o, aux, field_bytes(sp, Vh, nrhs), cudaMemcpyDeviceToDevice, ctx->stream));
+    TSM_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
+    if ((rc = fetch_scalars(ctx))) return rc;
+    float ms = 0;
+    TSM_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
+    const CgScalars sc = *ctx->cg_host;   // true_residuals() reuses the pinned copy
+    double tr[TSM_MAX_NRHS];
+    for (int j = 0; j < nrhs; j++) tr[j] = -1.0;
+    if (want_true_resid && (rc = true_residuals(ctx, slot, tr))) return rc;
+    int first = TSM_OK;
+    for (int j = 0; j < nrhs; j++) {
+        int st = sc.status[j];
+        if (st == TSM_OK && tol > 0 && !sc.done[j]) st = TSM_ENOCONV;
+        if (first == TSM_OK && st != TSM_OK) first = st;
+        if (info) {
+            info[j].iters = sc.iters[j];
+            info[j].status = st;
+            info[j].rel_resid_rec = sc.bb[j] > 0 ? std::sqrt(sc.rr[j] / sc.bb[j]) : 0.0;
+            info[j].rel_resid_true = tr[j];
+            info[j].secs = ms * 1e-3;
+        }
+    }
+    if (first != TSM_OK) ctx->err = first == TSM_ENOCONV ? "tolerance not reached in max_iter" : "CG breakdown";
+    return first;
+}
+
+int tsm_get_solution(tsm_ctx* ctx, int slot, int rhs, double* host_out)
+{
+    int rc = ctx_enter(ctx, true, false, false);
+    if (rc) return rc;
+    if ((rc = check_slot(ctx, slot, rhs))) return rc;
+    if (!host_out) return tsm_fail(ctx, TSM_EINVAL, "null output");
+    const int sp = ctx->slot_prec[slot], nrhs = ctx->slot_nrhs[slot], Vh = ctx->g.Vh;
+    // gather the two parities of source `rhs` into a one-source full-lattice field, then unpack
+    char* tmp = (char*)ctx->vec[5];
+    const size_t f1 = field_bytes(sp, Vh, 1);
+    for (int par = 0; par < 2; par++)
+        TSM_CUDA(ctx, cudaMemcpyAsync(tmp + par * f1, (char*)ctx->slot[slot] + field_bytes(sp, Vh, nrhs) * par + f1 * rhs, f1,
+                                      cudaMemcpyDeviceToDevice, ctx->stream));
+    return tsm_unpack(ctx, sp, 1, tmp, host_out);
+}
+
+int tsm_set_solution(tsm_ctx* ctx, int slot, int rhs, const double* host_in)
+{
+    int rc = ctx_enter(ctx, true, false, false);
+    if (rc) return rc;
+    if ((rc = check_slot(ctx, slot, rhs))) return rc;
+    if (!host_in) return tsm_fail(ctx, TSM_EINVAL, "null input");
+    const int sp = ctx->slot_prec[slot], nrhs = ctx->slot_nrhs[slot], Vh = ctx->g.Vh;
+    char* tmp = (char*)ctx->vec[5];
+    if ((rc = tsm_pack(ctx, sp, 1, host_in, tmp))) return rc;
+    const size_t f1 = field_bytes(sp, Vh, 1);
+    for (int par = 0; par < 2; par++)
+        TSM_CUDA(ctx, cudaMemcpyAsync((char*)ctx->slot[slot] + field_bytes(sp, Vh, nrhs) * par + f1 * rhs, tmp + par * f1, f1,
+                                      cudaMemcpyDeviceToDevice, ctx->stream));
+    TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return TSM_OK;
+}
+
+int tsm_loops_reset(tsm_ctx* ctx, int with_derivative)
+{
+    int rc = ctx_enter(ctx, true, false, false);
+    if (rc) return rc;
+    ctx->with_deriv = with_derivative ? 1 : 0;
+    ctx->n_ops = TSM_N_LOCAL_OPS + (with_derivative ? TSM_N_DERIV_OPS : 0);
+    ctx->n_hp = ctx->n_lp = 0;
+    const size_t lb = (size_t)ctx->n_ops * ctx->g.L[3] * 2 * sizeof(double);
+    TSM_CUDA(ctx, cudaMemsetAsync(ctx->acc_corr, 0, lb, ctx->stream));
+    TSM_CUDA(ctx, cudaMemsetAsync(ctx->acc_lp, 0, lb, ctx->stream));
+    return TSM_OK;
+}
+
+int tsm_loops_add_correction(tsm_ctx* ctx, int slot_hp, int slot_lp)
+{
+    int rc = ctx_enter(ctx, true, true, false);
+    if (rc) return rc;
+    if ((rc = check_slot(ctx, slot_hp, 0)) || (rc = check_slot(ctx, slot_lp, 0))) return rc;
+    if (slot_hp == slot_lp) return tsm_fail(ctx, TSM_EINVAL, "HP and LP slots must differ");
+    const int nrhs = ctx->slot_nrhs[slot_hp];
+    if (nrhs != ctx->slot_nrhs[slot_lp] || ctx->slot_seed[slot_hp] != ctx->slot_seed[slot_lp] ||
+        ctx->slot_kind[slot_hp] != ctx->slot_kind[slot_lp] ||
+        memcmp(ctx->slot_ids[slot_hp], ctx->slot_ids[slot_lp], nrhs * sizeof(uint32_t)) != 0)
+        return tsm_fail(ctx, TSM_ESTATE, "HP and LP slots hold different sources (Eq. 2.4 needs the same eta_j)");
+    if ((rc = launch_contract(ctx, slot_hp))) return rc;
+    if ((rc = launch_accumulate(ctx, ctx->acc_corr, ctx->loops_src[slot_hp], nrhs, +1.0))) return rc;
+    if ((rc = launch_contract(ctx, slot_lp))) return rc;
+    if ((rc = launch_accumulate(ctx, ctx->acc_corr, ctx->loops_src[slot_lp], nrhs, -1.0))) return rc;
+    ctx->n_hp += nrhs;
+    return TSM_OK;
+}
+
+int tsm_loops_add_lp(tsm_ctx* ctx, int slot_lp)
+{
+    int rc = ctx_enter(ctx, true, true, false);
+    if (rc) return rc;
+    if ((rc = check_slot(ctx, slot_lp, 0))) return rc;
+    const int nrhs = ctx->slot_nrhs[slot_lp];
+    if ((rc = launch_contract(ctx, slot_lp))) return rc;
+    if ((rc = launch_accumulate(ctx, ctx->acc_lp, ctx->loops_src[slot_lp], nrhs, +1.0))) return rc;
+    ctx->n_lp += nrhs;
+    return TSM_OK;
+}
+
+int tsm_loops_source(tsm_ctx* ctx, int slot, int rhs, double* host_out)
+{
+    int rc = ctx_enter(ctx, true, true, false);
+    if (rc) return rc;
+    if ((rc = check_slot(ctx, slot, rhs))) return rc;
+    if (!host_out) return tsm_fail(ctx, TSM_EINVAL, "null output");
+    if ((rc = launch_contract(ctx, slot))) return rc;
+    const size_t lb = (size_t)ctx->n_ops * ctx->g.L[3] * 2 * sizeof(double);
+    TSM_CUDA(ctx, cudaMemcpyAsync(ctx->host_small, (char*)ctx->loops_src[slot] + lb * rhs, lb, cudaMemcpyDeviceToHost, ctx->stream));
+    TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    memcpy(host_out, ctx->host_small, lb);
+    return TSM_OK;
+}
+
+int tsm_loops_finalize(tsm_ctx* ctx, double* host_out)
+{
+    int rc = ctx_enter(ctx, true, false, false);
+    if (rc) return rc;
+    if (!host_out) return tsm_fail(ctx, TSM_EINVAL, "null output");
+    if ((rc = launch_finalize(ctx))) return rc;
+    const size_t lb = (size_t)ctx->n_ops * ctx->g.L[3] * 2 * sizeof(double);
+    TSM_CUDA(ctx, cudaMemcpyAsync(ctx->host_small, ctx->loops_out, lb, cudaMemcpyDeviceToHost, ctx->stream));
+    TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    memcpy(host_out, ctx->host_small, lb);
+    return TSM_OK;
+}
+
+int tsm_loops_get_state(tsm_ctx* ctx, double* host_corr, double* host_lp, int* n_hp, int* n_lp)
+{
+    int rc = ctx_enter(ctx, true, false, false);
+    if (rc) return rc;
+    if (!host_corr || !host_lp || !n_hp || !n_lp) return tsm_fail(ctx, TSM_EINVAL, "null output");
+    const size_t lb = (size_t)ctx->n_ops * ctx->g.L[3] * 2 * sizeof(double);
+    TSM_CUDA(ctx, cudaMemcpyAsync(host_corr, ctx->acc_corr, lb, cudaMemcpyDeviceToHost, ctx->stream));
+    TSM_CUDA(ctx, cudaMemcpyAsync(host_lp, ctx->acc_lp, lb, cudaMemcpyDeviceToHost, ctx->stream));
+    TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    *n_hp = ctx->n_hp;
+    *n_lp = ctx->n_lp;
+    return TSM_OK;
+}
+
+int tsm_loops_set_state(tsm_ctx* ctx, const double* host_corr, const double* host_lp, int n_hp, int n_lp)
+{
+    int rc = ctx_enter(ctx, true, false, false);
+    if (rc) return rc;
+    if (!host_corr || !host_lp || n_hp < 0 || n_lp < 0) return tsm_fail(ctx, TSM_EINVAL, "bad state");
+    const size_t lb = (size_t)ctx->n_ops * ctx->g.L[3] * 2 * sizeof(double);
+    TSM_CUDA(ctx, cudaMemcpyAsync(ctx->acc_corr, host_corr, lb, cudaMemcpyHostToDevice, ctx->stream));
+    TSM_CUDA(ctx, cudaMemcpyAsync(ctx->acc_lp, host_lp, lb, cudaMemcpyHostToDevice, ctx->stream));
+    TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->n_hp = n_hp;
+    ctx->n_lp = n_lp;
+    return TSM_OK;
+}
+
+int tsm_run_loop_set(tsm_ctx* ctx, uint64_t seed, int kind, int n_hp, int n_lp, int lp_prec, double lp_tol, int lp_iters,
+                     double hp_tol, int hp_max_iter, int nrhs, int with_derivative, double* host_out, double* secs_out)
+{
+    int rc = ctx_enter(ctx, true, true, true);
+    if (rc) return rc;
+    if (n_hp < 0 || n_lp < 0 || nrhs < 1 || nrhs > ctx->max_nrhs || !host_out) return tsm_fail(ctx, TSM_EINVAL, "bad loop-set arguments");
+    cudaEvent_t e0, e1;
+    TSM_CUDA(ctx, cudaEventCreate(&e0));
+    TSM_CUDA(ctx, cudaEventCreate(&e1));
+    TSM_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
+    int worst = TSM_OK;
+    if ((rc = tsm_loops_reset(ctx, with_derivative))) goto fail;
+    for (int j0 = 0; j0 < n_hp + n_lp;) {
+        const bool hp = j0 < n_hp;
+        const int end = hp ? n_hp : n_hp + n_lp;
+        const int nb = (end - j0 < nrhs) ? end - j0 : nrhs;
+        uint32_t ids[TSM_MAX_NRHS];
+        for (int k = 0; k < nb; k++) ids[k] = (uint32_t)(j0 + k);
+        if (hp) {
+            rc = tsm_solve(ctx, seed, ids, nb, kind, TSM_F64, hp_tol, hp_max_iter, 0, 0, nullptr);
+            if (rc == TSM_ECUDA || rc == TSM_EINVAL || rc == TSM_ESTATE) goto fail;
+            if (rc && !worst) worst = rc;
+        }
+        rc = tsm_solve(ctx, seed, ids, nb, kind, lp_prec, lp_tol, lp_iters, 1, 0, nullptr);
+        // an LP solve that hits its iteration cap is still a valid truncated estimate
+        if (rc == TSM_ECUDA || rc == TSM_EINVAL || rc == TSM_ESTATE) goto fail;
+        if (rc == TSM_EBREAKDOWN && !worst) worst = rc;
+        rc = hp ? tsm_loops_add_correction(ctx, 0, 1) : tsm_loops_add_lp(ctx, 1);
+        if (rc) goto fail;
+        j0 += nb;
+    }
+    if ((rc = launch_finalize(ctx))) goto fail;
+    TSM_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
+    if ((rc = tsm_loops_finalize(ctx, host_out))) goto fail;
+    if (secs_out) {
+        float ms = 0;
+        TSM_CUDA(ctx, cudaEventElapsedTime(&ms, e0, e1));
+        *secs_out = ms * 1e-3;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return worst;
+fail:
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return rc;
+}
+
+}  // extern "C"

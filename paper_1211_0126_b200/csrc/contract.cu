@@ -1,0 +1,234 @@
+// contract.cu -- H8-H10: per-timeslice loop contractions and the TSM accumulators.
+//
+// H8  C_{ab}(t) = sum_{x in t, c} conj(eta_{ac}(x)) s_{bc}(x); L_Gamma(t) = sum_{ab} Gamma_{ab} C_{ab}(t)
+//     ("(1/N) sum <eta^dag X s>", "all possible insertion times"; O6).
+// H9  the same with s replaced by (D_mu s)(x) = 1/2 [phi+ U_mu(x) s(x+mu) - phi- U_mu(x-mu)^dag s(x-mu)]
+//     for mu = 0..3 (reading A18; O6b).
+// eta is never read from memory: it is regenerated from the Philox counter (PAPER.md:80,
+// "noise sources were generated on-the-fly").  Sums are fp64 with a fixed tree (A19).
+// H10 Eq. 2.4 accumulators (O7).
+#include "reduce.cuh"
+
+namespace {
+
+constexpr int CT_BS = 128;
+constexpr int CT_MAXBLK = 8;   // blocks per (timeslice, parity)
+
+// grid = (nblk * ngroup_in_launch, Lt, nrhs * 2); GROUP0 = 0: local; GROUP0 = 1: derivative, mu = blockIdx.x / nblk.
+// partials: [rhs][group 0..4][t][par][blk][32]
+template <int PREC, int RECON, bool DERIV>
+__global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs, const int nblk, const void* __restrict__ sol,
+                                                    const void* __restrict__ pack0, const void* __restrict__ pack1,
+                                                    const uint64_t seed, const uint32_t* __restrict__ ids, const int kind,
+                                                    double* __restrict__ partials)
+{
+    using T = typename PT<PREC>::real;
+    const int Vh = g.Vh;
+    const int blk = blockIdx.x % nblk, mu = blockIdx.x / nblk;
+    const int t = blockIdx.y;
+    const int rhs = blockIdx.z >> 1, par = blockIdx.z & 1;
+    const size_t fpar = field_bytes(PREC, Vh, nrhs), frhs = field_bytes(PREC, Vh, 1);
+    const char* s_same = (const char*)sol + fpar * par + frhs * rhs;
+    const char* s_other = (const char*)sol + fpar * (1 - par) + frhs * rhs;
+    const void* pack = par ? pack1 : pack0;
+    const uint32_t sid = ids[rhs];
+
+    double C[32];
+#pragma unroll
+    for (int k = 0; k < 32; k++) C[k] = 0;
+
+    for (int j = blk * CT_BS + threadIdx.x; j < g.Vsh; j += nblk * CT_BS) {
+        const int i = t * g.Vsh + j;
+        const SiteCoord sc = decode_site(g, i, par);
+        const uint32_t bits = noise_bits(lex_of_site(g, sc), seed, sid, kind);
+        T v[24];
+        if (!DERIV) {
+            load_spinor<PREC>(s_same, Vh, i, v);
+        } else {
+            int nb[8];
+            neighbours(g, i, sc, nb);
+            T uf[18], ub[18], sf[24], sb[24], a[6], b[6];
+            // runtime mu: the four directions are four block groups of the same launch
+            switch (mu) {
+                case 0: load_link_pair<PREC, RECON>(pack, Vh, i, 0, uf, ub); break;
+                case 1: load_link_pair<PREC, RECON>(pack, Vh, i, 1, uf, ub); break;
+                case 2: load_link_pair<PREC, RECON>(pack, Vh, i, 2, uf, ub); break;
+                default: load_link_pair<PREC, RECON>(pack, Vh, i, 3, uf, ub); break;
+            }
+            load_spinor<PREC>(s_other, Vh, nb[2 * mu], sf);
+            load_spinor<PREC>(s_other, Vh, nb[2 * mu + 1], sb);
+            const T ph_f = (mu == 3 && sc.t == g.L[3] - 1) ? (T)g.theta : (T)1;
+            const T ph_b = (mu == 3 && sc.t == 0) ? (T)g.theta : (T)1;
+#pragma unroll
+            for (int al = 0; al < 4; al++) {
+                su3_mul(uf, sf + 6 * al, a);
+                su3_mul(ub, sb + 6 * al, b);
+#pragma unroll
+                for (int k = 0; k < 6; k++) v[6 * al + k] = (T)0.5 * (ph_f * a[k] - ph_b * b[k]);
+            }
+        }
+#pragma unroll
+        for (int al = 0; al < 4; al++)
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+                float er, ei;
+                noise_value((bits >> (2 * (3 * al + c))) & 3, kind, er, ei);
+                const double cr = er, ci = -ei;   // conj(eta)
+#pragma unroll
+                for (int be = 0; be < 4; be++) {
+                    const double sr = (double)v[2 * (3 * be + c)], si = (double)v[2 * (3 * be + c) + 1];
+                    C[2 * (4 * al + be)] += cr * sr - ci * si;
+                    C[2 * (4 * al + be) + 1] += cr * si + ci * sr;
+                }
+            }
+    }
+    // block reduction of the 32 sums: shuffle tree per warp, fixed serial sum over warps
+    __shared__ double sm[CT_BS / 32][32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < 32; k++) {
+        const double r = warp_sum(C[k]);
+        if (lane == 0) sm[w][k] = r;
+    }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double tot = 0;
+        for (int ww = 0; ww < CT_BS / 32; ww++) tot += sm[ww][threadIdx.x];
+        const int group = DERIV ? 1 + mu : 0;
+        const size_t o = ((((size_t)rhs * 5 + group) * g.L[3] + t) * 2 + par) * nblk + blk;
+        partials[o * 32 + threadIdx.x] = tot;
+    }
+}
+
+// grid = (Lt, ngroups, nrhs), 32 threads: finish the sums and apply the 16 Gamma.
+__global__ void k_contract_finish(const int Lt, const int nblk, const int n_ops, const GammaTable gt,
+                                  const double* __restrict__ partials, double* __restrict__ loops)
+{
+    const int t = blockIdx.x, group = blockIdx.y, rhs = blockIdx.z, k = threadIdx.x;
+    __shared__ double C[32];
+    double tot = 0;
+    for (int pb = 0; pb < 2 * nblk; pb++) {
+        const size_t o = (((size_t)rhs * 5 + group) * Lt + t) * 2 * nblk + pb;
+        tot += partials[o * 32 + k];
+    }
+    C[k] = tot;
+    __syncthreads();
+    if (k < 16) {
+        double re = 0, im = 0;
+        for (int al = 0; al < 4; al++) {
+            const int be = gt.col[k][al], ph = gt.ph[k][al] & 3;
+            const double cr = C[2 * (4 * al + be)], ci = C[2 * (4 * al + be) + 1];
+            // multiply by i^ph
+            re += (ph == 0) ? cr : (ph == 1) ? -ci : (ph == 2) ? -cr : ci;
+            im += (ph == 0) ? ci : (ph == 1) ? cr : (ph == 2) ? -ci : -cr;
+        }
+        const int op = (group == 0) ? k : 16 + 16 * (group - 1) + k;
+        double* dst = loops + (((size_t)rhs * n_ops + op) * Lt + t) * 2;
+        dst[0] = re;
+        dst[1] = im;
+    }
+}
+
+__global__ void k_accumulate(const int n, const int nrhs, double* __restrict__ acc, const double* __restrict__ src, const double sign)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= n) return;
+    double s = 0;
+    for (int r = 0; r < nrhs; r++) s += src[(size_t)r * n + idx];
+    acc[idx] += sign * s;
+}
+
+__global__ void k_finalize(const int n, const double* __restrict__ corr, const double* __restrict__ lp, const double w_hp,
+                           const double w_lp, double* __restrict__ out)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx < n) out[idx] = w_hp * corr[idx] + w_lp * lp[idx];
+}
+
+}  // namespace
+
+// The CUDA path's own Gamma tables: each Gamma is a monomial matrix, Gamma_{a, col[a]} = i^ph[a].
+// gamma_mu are typed from C3 (gamma_k = [[0,-i sigma_k],[i sigma_k,0]], gamma_3 = [[0,1],[1,0]]);
+// gamma5 gamma_mu and sigma_{mu nu} = i gamma_mu gamma_nu (mu != nu) follow by monomial products.
+void build_gamma_table(GammaTable& t)
+{
+    struct Mono { int col[4]; int ph[4]; };
+    auto mul = [](const Mono& a, const Mono& b) {   // (AB)_{r, b.col[a.col[r]]} = a.ph[r] * b.ph[a.col[r]]
+        Mono o;
+        for (int r = 0; r < 4; r++) { o.col[r] = b.col[a.col[r]]; o.ph[r] = (a.ph[r] + b.ph[a.col[r]]) & 3; }
+        return o;
+    };
+    const Mono one = {{0, 1, 2, 3}, {0, 0, 0, 0}};
+    const Mono g5 = {{0, 1, 2, 3}, {0, 0, 2, 2}};
+    const Mono gm[4] = {
+        {{3, 2, 1, 0}, {3, 3, 1, 1}},   // gamma_0: rows (0:-i@3, 1:-i@2, 2:+i@1, 3:+i@0)
+        {{3, 2, 1, 0}, {2, 0, 0, 2}},   // gamma_1: (-1@3, +1@2, +1@1, -1@0)
+        {{2, 3, 0, 1}, {3, 1, 1, 3}},   // gamma_2: (-i@2, +i@3, +i@0, -i@1)
+        {{2, 3, 0, 1}, {0, 0, 0, 0}},   // gamma_3
+    };
+    const Mono eye_i = {{0, 1, 2, 3}, {1, 1, 1, 1}};   // i * 1
+    Mono all[16];
+    all[0] = one;
+    all[1] = g5;
+    for (int m = 0; m < 4; m++) { all[2 + m] = gm[m]; all[6 + m] = mul(g5, gm[m]); }
+    const int pr[6][2] = {{0, 1}, {0, 2}, {0, 3}, {1, 2}, {1, 3}, {2, 3}};
+    for (int k = 0; k < 6; k++) all[10 + k] = mul(eye_i, mul(gm[pr[k][0]], gm[pr[k][1]]));
+    for (int G = 0; G < 16; G++)
+        for (int r = 0; r < 4; r++) { t.col[G][r] = all[G].col[r]; t.ph[G][r] = all[G].ph[r]; }
+}
+
+int launch_contract(tsm_ctx* ctx, int slot)
+{
+    const Geom& g = ctx->g;
+    const int nrhs = ctx->slot_nrhs[slot], prec = ctx->slot_prec[slot];
+    int nblk = (g.Vsh + CT_BS - 1) / CT_BS;
+    if (nblk > CT_MAXBLK) nblk = CT_MAXBLK;
+    const size_t need = (size_t)nrhs * 5 * g.L[3] * 2 * nblk * 32;
+    if (need > ctx->partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
+    const uint32_t* ids = ctx->ids_dev + slot * TSM_MAX_NRHS;
+    const uint64_t seed = ctx->slot_seed[slot];
+    const int kind = ctx->slot_kind[slot];
+    const dim3 grid_l(nblk, g.L[3], nrhs * 2), grid_d(nblk * 4, g.L[3], nrhs * 2);
+    const void* sol = ctx->slot[slot];
+#define CT(P, R)                                                                                                             \
+    do {                                                                                                                     \
+        const void* p0 = (P == TSM_F64) ? ctx->gauge64[0] : ctx->gauge32[0];                                                 \
+        const void* p1 = (P == TSM_F64) ? ctx->gauge64[1] : ctx->gauge32[1];                                                 \
+        k_contract<P, R, false><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, p0, p1, seed, ids, kind, ctx->partials); \
+        ctx->launches++;                                                                                                     \
+        if (ctx->with_deriv) {                                                                                               \
+            k_contract<P, R, true><<<grid_d, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, p0, p1, seed, ids, kind, ctx->partials); \
+            ctx->launches++;                                                                                                 \
+        }                                                                                                                    \
+    } while (0)
+    if (prec == TSM_F64) CT(TSM_F64, 18);
+    else if (prec == TSM_F32 && ctx->recon == 18) CT(TSM_F32, 18);
+    else if (prec == TSM_F32) CT(TSM_F32, 12);
+    else return tsm_fail(ctx, TSM_ESTATE, "slot holds no fp64/fp32 solution");
+#undef CT
+    TSM_CUDA(ctx, cudaGetLastError());
+    const dim3 grid_f(g.L[3], ctx->with_deriv ? 5 : 1, nrhs);
+    k_contract_finish<<<grid_f, 32, 0, ctx->stream>>>(g.L[3], nblk, ctx->n_ops, ctx->gam, ctx->partials, ctx->loops_src[slot]);
+    ctx->launches++;
+    TSM_CUDA(ctx, cudaGetLastError());
+    return TSM_OK;
+}
+
+int launch_accumulate(tsm_ctx* ctx, double* acc, const double* src, int nrhs, double sign)
+{
+    const int n = ctx->n_ops * ctx->g.L[3] * 2;
+    k_accumulate<<<(n + 255) / 256, 256, 0, ctx->stream>>>(n, nrhs, acc, src, sign);
+    ctx->launches++;
+    TSM_CUDA(ctx, cudaGetLastError());
+    return TSM_OK;
+}
+
+int launch_finalize(tsm_ctx* ctx)
+{
+    const int n = ctx->n_ops * ctx->g.L[3] * 2;
+    const double w_hp = ctx->n_hp > 0 ? 1.0 / ctx->n_hp : 0.0, w_lp = ctx->n_lp > 0 ? 1.0 / ctx->n_lp : 0.0;
+    k_finalize<<<(n + 255) / 256, 256, 0, ctx->stream>>>(n, ctx->acc_corr, ctx->acc_lp, w_hp, w_lp, ctx->loops_out);
+    ctx->launches++;
+    TSM_CUDA(ctx, cudaGetLastError());
+    return TSM_OK;
+}

@@ -1,0 +1,369 @@
+// tsm_internal.cuh -- shared declarations of the CUDA path (sm_100a).
+// Layouts, precision traits, load/store helpers, block reductions, context struct.
+// Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <string>
+
+#include "../../include/tsm.h"
+
+// ------------------------------------------------------------------ geometry (H1)
+struct Geom {
+    int L[4];      // Lx, Ly, Lz, Lt (all even)
+    int Lxh;       // Lx / 2
+    int Vsh;       // Lx*Ly*Lz / 2: checkerboard sites per timeslice and parity
+    int Vh;        // V / 2
+    long long V;
+    int theta;     // time boundary phase, +1 or -1 (A3)
+};
+
+struct SiteCoord { int xh, y, z, t, rowpar; };
+
+// cb index of parity `par` -> coordinates; x = 2*xh + rowpar, rowpar = (y+z+t+par)&1.
+__device__ __forceinline__ SiteCoord decode_site(const Geom& g, int i, int par)
+{
+    SiteCoord s;
+    s.xh = i % g.Lxh;
+    int r = i / g.Lxh;
+    s.y = r % g.L[1];
+    r /= g.L[1];
+    s.z = r % g.L[2];
+    s.t = r / g.L[2];
+    s.rowpar = (s.y + s.z + s.t + par) & 1;
+    return s;
+}
+
+__device__ __forceinline__ long long lex_of_site(const Geom& g, const SiteCoord& s)
+{
+    const int x = 2 * s.xh + s.rowpar;
+    return x + (long long)g.L[0] * (s.y + (long long)g.L[1] * (s.z + (long long)g.L[2] * s.t));
+}
+
+// cb indices (in the other-parity field) of the 8 neighbours: nb[2*mu] = x+mu, nb[2*mu+1] = x-mu
+__device__ __forceinline__ void neighbours(const Geom& g, int i, const SiteCoord& s, int nb[8])
+{
+    const int Lxh = g.Lxh, sy = g.Lxh, sz = g.Lxh * g.L[1], st = g.Vsh;
+    nb[0] = s.rowpar ? (s.xh == Lxh - 1 ? i - (Lxh - 1) : i + 1) : i;
+    nb[1] = s.rowpar ? i : (s.xh == 0 ? i + (Lxh - 1) : i - 1);
+    nb[2] = (s.y == g.L[1] - 1) ? i - (g.L[1] - 1) * sy : i + sy;
+    nb[3] = (s.y == 0) ? i + (g.L[1] - 1) * sy : i - sy;
+    nb[4] = (s.z == g.L[2] - 1) ? i - (g.L[2] - 1) * sz : i + sz;
+    nb[5] = (s.z == 0) ? i + (g.L[2] - 1) * sz : i - sz;
+    nb[6] = (s.t == g.L[3] - 1) ? i - (g.L[3] - 1) * st : i + st;
+    nb[7] = (s.t == 0) ? i + (g.L[3] - 1) * st : i - st;
+}
+
+// ------------------------------------------------------------------ precision traits
+// A site's spinor is 24 reals r[2*q + ri], q = 3*alpha + c.  Storage: [chunk][cb] of 16-byte vectors.
+template <int PREC> struct PT;
+template <> struct PT<TSM_F64> {
+    using real = double;
+    static constexpr int NCHUNK = 12;   // double2 = one complex
+    static constexpr int GAUGE_F64 = 1;
+};
+template <> struct PT<TSM_F32> {
+    using real = float;
+    static constexpr int NCHUNK = 6;    // float4 = two complex
+    static constexpr int GAUGE_F64 = 0;
+};
+template <> struct PT<TSM_BF16> {
+    using real = float;                 // arithmetic type
+    static constexpr int NCHUNK = 3;    // 8 x bf16 = four complex
+    static constexpr int GAUGE_F64 = 0;
+};
+
+__host__ __device__ inline size_t field_bytes(int prec, long long Vh, int nrhs)
+{
+    const size_t per_site = prec == TSM_F64 ? 192 : (prec == TSM_F32 ? 96 : 48);
+    return per_site * (size_t)Vh * (size_t)nrhs;
+}
+__host__ __device__ inline int nchunk_of(int prec) { return prec == TSM_F64 ? 12 : (prec == TSM_F32 ? 6 : 3); }
+
+__device__ __forceinline__ void bf16x8_to_float(const uint4& v, float* o)
+{
+    const unsigned w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        o[2 * j] = __uint_as_float(w[j] << 16);
+        o[2 * j + 1] = __uint_as_float(w[j] & 0xffff0000u);
+    }
+}
+__device__ __forceinline__ uint4 float_to_bf16x8(const float* o)
+{
+    unsigned w[4];
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        __nv_bfloat162 b = __floats2bfloat162_rn(o[2 * j], o[2 * j + 1]);
+        w[j] = *reinterpret_cast<unsigned*>(&b);
+    }
+    return make_uint4(w[0], w[1], w[2], w[3]);
+}
+
+// Load / store 8 consecutive reals (reals 8*k8 .. 8*k8+7 of site i) of a field.
+template <int PREC> __device__ __forceinline__ void load8(const void* f, int Vh, int i, int k8, typename PT<PREC>::real* o)
+{
+    if constexpr (PREC == TSM_F64) {
+        const double2* p = reinterpret_cast<const double2*>(f) + (size_t)(4 * k8) * Vh + i;
+#pragma unroll
+        for (int j = 0; j < 4; j++) { const double2 v = __ldg(p + (size_t)j * Vh); o[2 * j] = v.x; o[2 * j + 1] = v.y; }
+    } else if constexpr (PREC == TSM_F32) {
+        const float4* p = reinterpret_cast<const float4*>(f) + (size_t)(2 * k8) * Vh + i;
+#pragma unroll
+        for (int j = 0; j < 2; j++) { const float4 v = __ldg(p + (size_t)j * Vh); o[4 * j] = v.x; o[4 * j + 1] = v.y; o[4 * j + 2] = v.z; o[4 * j + 3] = v.w; }
+    } else {
+        const uint4 v = __ldg(reinterpret_cast<const uint4*>(f) + (size_t)k8 * Vh + i);
+        bf16x8_to_float(v, o);
+    }
+}
+template <int PREC> __device__ __forceinline__ void store8(void* f, int Vh, int i, int k8, const typename PT<PREC>::real* o)
+{
+    if constexpr (PREC == TSM_F64) {
+        double2* p = reinterpret_cast<double2*>(f) + (size_t)(4 * k8) * Vh + i;
+#pragma unroll
+        for (int j = 0; j < 4; j++) p[(size_t)j * Vh] = make_double2(o[2 * j], o[2 * j + 1]);
+    } else if constexpr (PREC == TSM_F32) {
+        float4* p = reinterpret_cast<float4*>(f) + (size_t)(2 * k8) * Vh + i;
+#pragma unroll
+        for (int j = 0; j < 2; j++) p[(size_t)j * Vh] = make_float4(o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
+    } else {
+        reinterpret_cast<uint4*>(f)[(size_t)k8 * Vh + i] = float_to_bf16x8(o);
+    }
+}
+template <int PREC> __device__ __forceinline__ void load_spinor(const void* f, int Vh, int i, typename PT<PREC>::real* s)
+{
+#pragma unroll
+    for (int k = 0; k < 3; k++) load8<PREC>(f, Vh, i, k, s + 8 * k);
+}
+template <int PREC> __device__ __forceinline__ void store_spinor(void* f, int Vh, int i, const typename PT<PREC>::real* s)
+{
+#pragma unroll
+    for (int k = 0; k < 3; k++) store8<PREC>(f, Vh, i, k, s + 8 * k);
+}
+
+// ------------------------------------------------------------------ gauge packs (H2)
+// For output parity p and cb site i the pack holds 8 matrices, d = 2*mu + b:
+//   b = 0: U_mu(x)          (forward hop)      b = 1: U_mu(x - mu)^dagger (backward hop, stored daggered)
+// fp64: [72][Vh] double2, link d = chunks 9d .. 9d+8 (row-major complex entries).
+// fp32, 18 reals: [36][Vh] float4, direction mu = chunks 9mu .. 9mu+8 = 36 floats (fwd 18, bwd 18).
+// fp32, 12 reals: [24][Vh] float4, link d = chunks 3d .. 3d+2 (rows 0,1; row 2 = conj(row0 x row1)).
+__host__ __device__ inline size_t gauge_pack_bytes(int f64, int recon, long long Vh)
+{
+    return (size_t)Vh * 8 * (f64 ? 18 * 8 : recon * 4);
+}
+
+template <typename T> __device__ __forceinline__ void reconstruct_row2(T* u)
+{
+    // u[0..11] rows 0,1 as (re,im) pairs; row2 = conj(row0 x row1)
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const int a = (c + 1) % 3, b = (c + 2) % 3;
+        const T re = (u[2 * a] * u[6 + 2 * b] - u[2 * a + 1] * u[6 + 2 * b + 1]) - (u[2 * b] * u[6 + 2 * a] - u[2 * b + 1] * u[6 + 2 * a + 1]);
+        const T im = (u[2 * a] * u[6 + 2 * b + 1] + u[2 * a + 1] * u[6 + 2 * b]) - (u[2 * b] * u[6 + 2 * a + 1] + u[2 * b + 1] * u[6 + 2 * a]);
+        u[12 + 2 * c] = re;
+        u[12 + 2 * c + 1] = -im;
+    }
+}
+
+// Loads both links of direction mu for site i: uf = U_mu(x), ub = U_mu(x-mu)^dagger (18 reals each).
+template <int PREC, int RECON> __device__ __forceinline__ void load_link_pair(const void* pack, int Vh, int i, int mu,
+                                                                             typename PT<PREC>::real* uf, typename PT<PREC>::real* ub)
+{
+    if constexpr (PT<PREC>::GAUGE_F64) {
+        const double2* p = reinterpret_cast<const double2*>(pack) + (size_t)(18 * mu) * Vh + i;
+#pragma unroll
+        for (int j = 0; j < 9; j++) { const double2 v = __ldcs(p + (size_t)j * Vh); uf[2 * j] = v.x; uf[2 * j + 1] = v.y; }
+#pragma unroll
+        for (int j = 0; j < 9; j++) { const double2 v = __ldcs(p + (size_t)(9 + j) * Vh); ub[2 * j] = v.x; ub[2 * j + 1] = v.y; }
+    } else if constexpr (RECON == 18) {
+        const float4* p = reinterpret_cast<const float4*>(pack) + (size_t)(9 * mu) * Vh + i;
+        float l[36];
+#pragma unroll
+        for (int j = 0; j < 9; j++) { const float4 v = __ldcs(p + (size_t)j * Vh); l[4 * j] = v.x; l[4 * j + 1] = v.y; l[4 * j + 2] = v.z; l[4 * j + 3] = v.w; }
+#pragma unroll
+        for (int j = 0; j < 18; j++) { uf[j] = l[j]; ub[j] = l[18 + j]; }
+    } else {
+        const float4* p = reinterpret_cast<const float4*>(pack) + (size_t)(6 * mu) * Vh + i;
+#pragma unroll
+        for (int j = 0; j < 3; j++) { const float4 v = __ldcs(p + (size_t)j * Vh); uf[4 * j] = v.x; uf[4 * j + 1] = v.y; uf[4 * j + 2] = v.z; uf[4 * j + 3] = v.w; }
+#pragma unroll
+        for (int j = 0; j < 3; j++) { const float4 v = __ldcs(p + (size_t)(3 + j) * Vh); ub[4 * j] = v.x; ub[4 * j + 1] = v.y; ub[4 * j + 2] = v.z; ub[4 * j + 3] = v.w; }
+        reconstruct_row2(uf);
+        reconstruct_row2(ub);
+    }
+}
+
+// out[c] (+)= sum_c' U[c][c'] h[c'] for one spin row (3 complex), U 18 reals row-major.
+template <typename T> __device__ __forceinline__ void su3_mul(const T* u, const T* h, T* o)
+{
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        T re = u[6 * c] * h[0] - u[6 * c + 1] * h[1];
+        T im = u[6 * c] * h[1] + u[6 * c + 1] * h[0];
+        re += u[6 * c + 2] * h[2] - u[6 * c + 3] * h[3];
+        im += u[6 * c + 2] * h[3] + u[6 * c + 3] * h[2];
+        re += u[6 * c + 4] * h[4] - u[6 * c + 5] * h[5];
+        im += u[6 * c + 4] * h[5] + u[6 * c + 5] * h[4];
+        o[2 * c] = re;
+        o[2 * c + 1] = im;
+    }
+}
+
+// ------------------------------------------------------------------ Philox4x32-10 (H3, O3)
+__device__ __forceinline__ uint32_t philox_word0(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1)
+{
+#pragma unroll
+    for (int r = 0; r < 10; r++) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        c0 = hi1 ^ c1 ^ k0;
+        c1 = lo1;
+        c2 = hi0 ^ c3 ^ k1;
+        c3 = lo0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    return c0;
+}
+// 24 noise bits of site `lex` for source `sid`: component q uses bits 2q, 2q+1.
+__device__ __forceinline__ uint32_t noise_bits(long long lex, uint64_t seed, uint32_t sid, int kind)
+{
+    return philox_word0((uint32_t)((uint64_t)lex & 0xffffffffu), (uint32_t)((uint64_t)lex >> 32), sid,
+                        0x5A340000u | (uint32_t)kind, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32));
+}
+// eta component as (re, im) from its 2-bit code: Z4 -> i^k, Z2 -> 1 - 2(k&1).
+__device__ __forceinline__ void noise_value(int k, int kind, float& re, float& im)
+{
+    if (kind == TSM_Z4) {
+        re = (k == 0) ? 1.f : (k == 2 ? -1.f : 0.f);
+        im = (k == 1) ? 1.f : (k == 3 ? -1.f : 0.f);
+    } else {
+        re = (k & 1) ? -1.f : 1.f;
+        im = 0.f;
+    }
+}
+
+// ------------------------------------------------------------------ block reduction (A19)
+// Deterministic: fixed shuffle tree inside a warp, then a fixed serial sum over warps.
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+// Sum over the threads of one threadIdx.y row (blockDim.x a multiple of 32, <= 1024).
+// Result valid in threadIdx.x == 0.  smem: at least 32 * blockDim.y doubles.
+__device__ __forceinline__ double block_row_sum(double v, double* smem)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    v = warp_sum(v);
+    double* row = smem + 32 * threadIdx.y;
+    if (lane == 0) row[w] = v;
+    __syncthreads();
+    double t = 0;
+    if (threadIdx.x == 0)
+        for (int k = 0; k < nw; k++) t += row[k];
+    __syncthreads();
+    return t;
+}
+
+// Per-source CG scalars, device resident (A14: every source has its own).
+struct CgScalars {
+    double rr[TSM_MAX_NRHS];      // |r|^2 of the current residual
+    double bb[TSM_MAX_NRHS];      // |b'|^2
+    double pq[TSM_MAX_NRHS];      // Re <p, q>
+    double beta[TSM_MAX_NRHS];
+    int iters[TSM_MAX_NRHS];
+    int done[TSM_MAX_NRHS];       // frozen: converged, broken down, or zero source
+    int status[TSM_MAX_NRHS];
+    int all_done;
+    unsigned ticket;              // last-block counter, always left at 0
+};
+
+// ------------------------------------------------------------------ epilogue coefficients
+// out = Tx * x + Td * (D in), T = c_up on spins 0,1 and c_lo on spins 2,3 (complex), i.e.
+// T = alpha + i beta gamma5 with c_up = alpha + i beta, c_lo = alpha - i beta (C3: gamma5 diagonal).
+struct TwistCoef { double up_re, up_im, lo_re, lo_im; };
+struct DslashCoef { TwistCoef x, d; };
+
+// ------------------------------------------------------------------ context
+struct GammaTable {          // Gamma_{alpha, col[alpha]} = i^ph[alpha], all other entries 0
+    int col[16][4];
+    int ph[16][4];
+};
+
+struct tsm_ctx {
+    Geom g;
+    int device;
+    cudaStream_t stream;
+    double kappa, mu;
+    bool have_params, have_gauge, have_ws;
+    int recon;                       // storage of the fp32 link copy (18 / 12)
+    int max_nrhs;
+    int nsm;
+    // workspace carving (device pointers into the caller's buffer)
+    char* ws;
+    size_t ws_bytes;
+    void* gauge64[2];                // fp64 packs for output parity 0 / 1
+    void* gauge32[2];                // fp32 packs
+    void* staging;                   // raw host-layout staging (links or spinors), fp64
+    size_t staging_bytes;
+    void* vec[6];                    // CG vectors r, p, q, w, t, aux: single-parity, max_nrhs, fp64-sized
+    void* slot[2];                   // solutions: [parity][rhs][chunk][cb], fp64-sized
+    int slot_prec[2], slot_nrhs[2], slot_kind[2];
+    uint64_t slot_seed[2];
+    uint32_t slot_ids[2][TSM_MAX_NRHS];
+    double* partials;                // reduction scratch
+    size_t partials_count;
+    double* loops_src[2];            // per-source loops of a slot [rhs][n_ops][T][2]
+    double* acc_corr;                // [n_ops][T][2]
+    double* acc_lp;
+    double* loops_out;               // finalize output
+    // library-owned small allocations
+    CgScalars* cg;                   // device
+    CgScalars* cg_host;              // pinned
+    double* host_small;              // pinned scratch (loops, unitarity)
+    uint32_t* ids_dev;               // [2][TSM_MAX_NRHS]
+    GammaTable gam;
+    int n_ops, with_deriv, n_hp, n_lp;
+    long long launches;
+    cudaEvent_t ev0, ev1;
+    std::string err;
+};
+
+#define TSM_CUDA(ctx, expr)                                                                      \
+    do {                                                                                         \
+        cudaError_t e_ = (expr);                                                                 \
+        if (e_ != cudaSuccess) {                                                                 \
+            (ctx)->err = std::string(#expr) + ": " + cudaGetErrorString(e_);                     \
+            return TSM_ECUDA;                                                                    \
+        }                                                                                        \
+    } while (0)
+
+inline int tsm_fail(tsm_ctx* ctx, int code, const char* msg)
+{
+    if (ctx) ctx->err = msg;
+    return code;
+}
+
+// ------------------------------------------------------------------ launchers (defined in the .cu files)
+int launch_dslash(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs, const void* in, const void* x,
+                  void* out, const DslashCoef& c, const void* dot_y, int dot_mode);
+int launch_twist(tsm_ctx* ctx, int prec, int nrhs, const void* in, void* out, const TwistCoef& c);
+int launch_gauge_pack(tsm_ctx* ctx, double* max_dev_out);
+int launch_pack_spinor(tsm_ctx* ctx, int prec, int nrhs, const double* dev_lex, void* dev_native);
+int launch_unpack_spinor(tsm_ctx* ctx, int prec, int nrhs, const void* dev_native, double* dev_lex);
+int launch_noise(tsm_ctx* ctx, int prec, int nrhs, uint64_t seed, const uint32_t* dev_ids, int kind, void* dev_full);
+int launch_cg_init(tsm_ctx* ctx, int prec, int nrhs, const void* r, void* p, void* x);
+int launch_cg_update_xr(tsm_ctx* ctx, int prec, int nrhs, void* x, const void* p, void* r, const void* q, double tol);
+int launch_cg_update_p(tsm_ctx* ctx, int prec, int nrhs, void* p, const void* r);
+int launch_convert(tsm_ctx* ctx, int prec_in, int prec_out, int nrhs_fields, const void* in, void* out);
+int launch_contract(tsm_ctx* ctx, int slot);
+int launch_accumulate(tsm_ctx* ctx, double* acc, const double* src, int nrhs, double sign);
+int launch_finalize(tsm_ctx* ctx);
+void build_gamma_table(GammaTable& t);
+int ctx_enter(tsm_ctx* ctx, bool need_ws, bool need_gauge, bool need_params);
+// |a - b|^2 per source over full-lattice fp64 fields, left in cg->pq[rhs] (true-residual helper)
+int launch_diff_norm2(tsm_ctx* ctx, int nrhs, const void* a, const void* b);

@@ -1,0 +1,351 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element on
+the same seeded inputs.  Tolerances: bit-exact noise and
+indexing; 1e-12 relative for fp64 stencil and HP loops; 1e-5 for fp32 stencil; 1e-2 for
+bf16 storage (A20); LP solves by true residual (A17)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1211_0126_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+F64, F32, BF16 = 0, 1, 2
+
+
+def rel(a, b):
+    return np.abs(a - b).max() / np.abs(b).max()
+
+
+def rel_l2(a, b):
+    return np.linalg.norm((a - b).reshape(-1)) / np.linalg.norm(b.reshape(-1))
+
+
+@pytest.fixture(scope="module")
+def tsm_mod():
+    from paper_1211_0126_b200 import tsm
+    return tsm
+
+
+class Case:
+    def __init__(self, tsm_mod, dims, eps, seed, kappa, mu, theta, max_nrhs=4, recon=18):
+        self.dims, self.kappa, self.mu, self.theta = dims, kappa, mu, theta
+        self.U = W.random_su3_links(dims, eps, seed)
+        self.t = tsm_mod.Tsm(dims, t_boundary=theta, max_nrhs=max_nrhs)
+        self.t.set_params(kappa, mu)
+        self.dev = self.t.set_gauge(self.U, recon)
+        par = np.zeros(dims[::-1], dtype=np.int64)
+        for ax in range(4):
+            shape = [1, 1, 1, 1]
+            shape[ax] = dims[::-1][ax]
+            par = par + np.arange(dims[::-1][ax]).reshape(shape)
+        self.par = (par.reshape(-1) & 1)
+
+
+@pytest.fixture(scope="module")
+def small(tsm_mod):
+    wl = W.WORKLOADS[1]
+    return Case(tsm_mod, wl.dims, wl.eps, wl.gauge_seed, wl.kappa, wl.mu, -1, max_nrhs=4)
+
+
+@pytest.fixture(scope="module")
+def ragged(tsm_mod):
+    # extents that are not multiples of anything convenient: V_h = 6*10*4*6/2 = 720 sites
+    return Case(tsm_mod, (6, 10, 4, 6), 0.6, 77, 0.157, 0.02, +1, max_nrhs=12)
+
+
+@pytest.fixture(scope="module")
+def medium(tsm_mod):
+    wl = W.WORKLOADS[2]
+    return Case(tsm_mod, wl.dims, wl.eps, wl.gauge_seed, wl.kappa, wl.mu, -1, max_nrhs=4)
+
+
+# ---------------------------------------------------------------- H1/H3: indexing and noise, bit-exact
+@pytest.mark.parametrize("kind", [0, 1])
+def test_noise_bit_exact(small, ragged, kind):
+    for c in (small, ragged):
+        for sid in (0, 5, 4000000000):
+            seed = 0x1211012600000001
+            got = c.t.noise(seed, sid, kind)
+            want = oracle.noise(c.dims, seed, sid, kind)
+            assert np.array_equal(got, want)
+
+
+def test_pack_unpack_round_trip_is_exact(ragged):
+    c = ragged
+    psi = W.random_spinor(c.dims, 5, nrhs=3)
+    buf = c.t.pack(F64, psi)
+    assert np.array_equal(c.t.unpack(F64, 3, buf), psi)
+    # fp32 / bf16 storage round the values once, nothing else
+    assert np.array_equal(c.t.unpack(F32, 3, c.t.pack(F32, psi)), psi.astype(np.complex64).astype(np.complex128))
+    b = c.t.unpack(BF16, 3, c.t.pack(BF16, psi))
+    assert rel(b, psi) < 2 ** -8
+
+
+def test_gauge_ingest_reports_unitarity(small, tsm_mod):
+    assert small.dev < 1e-13
+    bad = small.U.copy()
+    bad[2, 17] *= 1.001
+    t = tsm_mod.Tsm(small.dims, max_nrhs=1)
+    assert abs(t.set_gauge(bad, 18) - 0.003) < 1e-3       # accepted with 18 reals, deviation reported
+    with pytest.raises(tsm_mod.TsmError) as e:
+        t.set_gauge(bad, 12)
+    assert e.value.code == tsm_mod.ENOTUNITARY
+    t.close()
+
+
+# ---------------------------------------------------------------- H5: the stencil
+def _oracle_op(c, op, psi):
+    """psi: full-lattice [V][4][3]; returns the full-lattice oracle result of operator `op`."""
+    e = (c.par == 0)[:, None, None]
+    if op == 0:
+        return oracle.hop(c.dims, c.theta, c.U, psi * ~e, 0)
+    if op == 1:
+        return oracle.hop(c.dims, c.theta, c.U, psi * e, 1)
+    if op == 2:
+        return oracle.apply_Mhat(c.dims, c.theta, c.kappa, c.mu, c.U, psi * e)
+    if op == 3:
+        return oracle.apply_Mhat_dag(c.dims, c.theta, c.kappa, c.mu, c.U, psi * e)
+    return oracle.apply_M(c.dims, c.theta, c.kappa, c.mu, c.U, psi)
+
+
+def _gpu_op(c, op, prec, psi):
+    """psi: [nrhs][V][4][3].  Packs, applies, unpacks; unused parities come back as zeros."""
+    nrhs = psi.shape[0]
+    t = c.t
+    fb = t.field_bytes(prec, nrhs)
+    full_in = t.pack(prec, psi)
+    full_out = t.alloc_field(prec, nrhs, full=True)
+    if op == 4:
+        t.dslash(op, prec, nrhs, full_in, full_out)
+    else:
+        in_par = {0: 1, 1: 0, 2: 0, 3: 0}[op]
+        out_par = {0: 0, 1: 1, 2: 0, 3: 0}[op]
+        t.dslash(op, prec, nrhs, full_in[in_par * fb:(in_par + 1) * fb], full_out[out_par * fb:(out_par + 1) * fb])
+    return t.unpack(prec, nrhs, full_out)
+
+
+@pytest.mark.parametrize("op", [0, 1, 2, 3, 4])
+def test_dslash_fp64_parity(small, ragged, medium, op):
+    for c in (small, ragged, medium):
+        psi = W.random_spinor(c.dims, 100 + op, nrhs=1)
+        got = _gpu_op(c, op, F64, psi)[0]
+        want = _oracle_op(c, op, psi[0])
+        assert rel(got, want) < 1e-12, (c.dims, op)
+
+
+@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("op", [0, 1, 2, 3, 4])
+def test_dslash_fp32_parity(tsm_mod, op, recon):
+    for dims, theta in [((4, 4, 4, 8), -1), ((6, 10, 4, 6), +1)]:
+        c = Case(tsm_mod, dims, 0.6, 81, 0.157, 0.02, theta, max_nrhs=2, recon=recon)
+        psi = W.random_spinor(dims, 200 + op, nrhs=1)
+        got = _gpu_op(c, op, F32, psi)[0]
+        # the oracle sees the same fp32-rounded input (links stay fp64 on its side)
+        want = _oracle_op(c, op, psi[0].astype(np.complex64).astype(np.complex128))
+        assert rel(got, want) < 1e-5, (dims, op, recon)
+        c.t.close()
+
+
+@pytest.mark.parametrize("op", [0, 3, 4])
+def test_dslash_bf16_storage_parity(ragged, op):
+    c = ragged
+    psi = W.random_spinor(c.dims, 300 + op, nrhs=1)
+    rounded = c.t.unpack(BF16, 1, c.t.pack(BF16, psi))
+    got = _gpu_op(c, op, BF16, psi)[0]
+    want = _oracle_op(c, op, rounded[0])
+    assert rel_l2(got, want) < 1e-2
+
+
+@pytest.mark.parametrize("nrhs", [2, 3, 4, 12])
+@pytest.mark.parametrize("prec,tol", [(F64, 1e-12), (F32, 1e-5)])
+def test_dslash_multi_rhs(ragged, nrhs, prec, tol):
+    c = ragged
+    psi = W.random_spinor(c.dims, 400 + nrhs, nrhs=nrhs)
+    for op in (0, 2, 4):
+        got = _gpu_op(c, op, prec, psi)
+        for j in range(nrhs):
+            src = psi[j] if prec == F64 else psi[j].astype(np.complex64).astype(np.complex128)
+            assert rel(got[j], _oracle_op(c, op, src)) < tol, (op, j)
+
+
+# ---------------------------------------------------------------- H4/H6/H7: solves
+def test_hp_solve_matches_oracle(small, medium, tsm_mod):
+    for c, seed in ((small, W.WORKLOADS[1].noise_seed), (medium, W.WORKLOADS[2].noise_seed)):
+        eta = oracle.noise(c.dims, seed, 1)
+        s_ref, info_ref = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, 1e-10, 2000)
+        rc, info = c.t.solve(seed, [1], F64, 1e-10, 2000, slot=0, want_true_resid=True)
+        assert rc == 0 and info[0]["status"] == 0
+        assert info[0]["iters"] == info_ref["iters"]
+        assert np.isclose(info[0]["rel_resid_rec"], info_ref["rel_resid_rec"], rtol=1e-6)
+        s = c.t.get_solution(0, 0)
+        rho = oracle.true_residual(c.dims, c.theta, c.kappa, c.mu, c.U, eta, s)
+        assert rho <= 1.5e-10                                              # A16(iii)
+        assert np.isclose(info[0]["rel_resid_true"], rho, rtol=1e-3)
+        assert rel(s, s_ref) < 1e-11
+        # same fixed iteration count: identical recurrences, rounding-order differences only (A16(ii))
+        k = info_ref["iters"]
+        s_fix_ref, _ = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, 0.0, k)
+        rc, info = c.t.solve(seed, [1], F64, 0.0, k, slot=1)
+        assert rc == 0 and info[0]["iters"] == k
+        assert rel(c.t.get_solution(1, 0), s_fix_ref) < 1e-12
+
+
+def test_truncated_solves_match_oracle_iterates(small):
+    """fp64 LP (config 1): same recurrences, so the truncated iterate itself matches."""
+    c = small
+    seed = W.WORKLOADS[1].noise_seed
+    eta = oracle.noise(c.dims, seed, 3)
+    for tol, k in ((1e-2, 1000), (0.0, 1), (0.0, 2), (0.0, 5)):
+        s_ref, info_ref = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, tol, k)
+        rc, info = c.t.solve(seed, [3], F64, tol, k, slot=0)
+        assert rc == 0
+        assert info[0]["iters"] == info_ref["iters"]
+        assert rel(c.t.get_solution(0, 0), s_ref) < 1e-12
+    # tolerance not reached: flagged, iterate kept (8(b))
+    rc, info = c.t.solve(seed, [3], F64, 1e-12, 3, slot=0)
+    assert rc == -6 and info[0]["status"] == -6 and info[0]["iters"] == 3
+    s_ref, _ = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, 0.0, 3)
+    assert rel(c.t.get_solution(0, 0), s_ref) < 1e-12
+
+
+def test_fp32_lp_solves_by_true_residual(medium):
+    """A17: residual mode rho <= 2 tol and |iters - oracle| <= 1; fixed-k mode rho <= max(2 rho_oracle, 100 eps)."""
+    c = medium
+    wl = W.WORKLOADS[2]
+    for sid in (0, 7):
+        eta = oracle.noise(c.dims, wl.noise_seed, sid)
+        _, info_ref = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, wl.lp_tol, 1000)
+        rc, info = c.t.solve(wl.noise_seed, [sid], F32, wl.lp_tol, 1000, slot=1, want_true_resid=True)
+        assert rc == 0
+        assert abs(info[0]["iters"] - info_ref["iters"]) <= 1
+        s = c.t.get_solution(1, 0)
+        rho = oracle.true_residual(c.dims, c.theta, c.kappa, c.mu, c.U, eta, s)
+        assert rho <= 2 * wl.lp_tol
+        assert np.isclose(info[0]["rel_resid_true"], rho, rtol=1e-3)
+        for k in (5, 20, 60):
+            s_ref, info_ref = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, 0.0, k)
+            rc, info = c.t.solve(wl.noise_seed, [sid], F32, 0.0, k, slot=1)
+            assert rc == 0 and info[0]["iters"] == k
+            s = c.t.get_solution(1, 0)
+            rho = oracle.true_residual(c.dims, c.theta, c.kappa, c.mu, c.U, eta, s)
+            assert rho <= max(2 * info_ref["rel_resid_true"], 100 * 6e-8)
+            if k == 5:   # equal iteration count, early iterate: elementwise to fp32 accuracy
+                assert rel(s, s_ref) < 2e-5
+
+
+def test_batched_solve_is_independent_of_batch_composition(medium):
+    """A14: batched, not block, CG: each source gets the iterate it would get alone."""
+    c = medium
+    seed = W.WORKLOADS[2].noise_seed
+    rc, info = c.t.solve(seed, [4, 9, 2, 11], F64, 1e-6, 500, slot=0)
+    assert rc == 0
+    batch = [c.t.get_solution(0, j) for j in range(4)]
+    for j, sid in enumerate([4, 9, 2, 11]):
+        rc, single = c.t.solve(seed, [sid], F64, 1e-6, 500, slot=1)
+        assert single[0]["iters"] == info[j]["iters"]
+        assert np.array_equal(c.t.get_solution(1, 0), batch[j])
+    assert len({i["iters"] for i in info}) >= 1
+
+
+# ---------------------------------------------------------------- H8/H9: contractions
+@pytest.mark.parametrize("deriv", [False, True])
+def test_contraction_parity_on_the_oracle_solution(small, ragged, deriv):
+    """A16(i): feed the oracle's s to the GPU contraction; 1e-12 relative to the largest loop."""
+    for c in (small, ragged):
+        seed = 99
+        c.t.loops_reset(deriv)
+        rc, _ = c.t.solve(seed, [2, 6], F64, 0.0, 1, slot=0)     # registers the source ids of the slot
+        for j, sid in enumerate((2, 6)):
+            eta = oracle.noise(c.dims, seed, sid)
+            s, _ = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, 1e-10, 2000)
+            c.t.set_solution(0, j, s)
+            want = oracle.all_loops(c.dims, c.theta, c.U, eta, s, deriv)
+            got = c.t.loops_source(0, j)
+            assert got.shape == want.shape
+            assert rel(got, want) < 1e-12
+
+
+def test_contraction_fp32_slot(ragged):
+    c = ragged
+    c.t.loops_reset(True)
+    rc, _ = c.t.solve(5, [1], F32, 0.0, 30, slot=1)
+    s = c.t.get_solution(1, 0)
+    eta = oracle.noise(c.dims, 5, 1)
+    want = oracle.all_loops(c.dims, c.theta, c.U, eta, s, True)
+    assert rel(c.t.loops_source(1, 0), want) < 1e-5
+
+
+# ---------------------------------------------------------------- H10: Eq. 2.4
+def test_tsm_loop_set_config1(small):
+    """Config 1 in full: fp64 throughout, N_HP=2, N_LP=4, LP at 1e-2 (A11: 6 sources)."""
+    c = small
+    wl = W.WORKLOADS[1]
+    per = {}
+    want = oracle.tsm_loops(c.dims, c.theta, c.kappa, c.mu, c.U, wl.noise_seed, wl.n_hp, wl.n_lp,
+                            wl.hp_tol, 2000, wl.lp_tol, wl.lp_iters, with_derivative=True, per_source=per)
+    got, secs, rc = c.t.run_loop_set(wl.noise_seed, wl.n_hp, wl.n_lp, F64, wl.lp_tol, wl.lp_iters,
+                                     hp_tol=wl.hp_tol, hp_max_iter=2000, nrhs=1, with_derivative=True)
+    assert rc == 0 and secs > 0
+    # HP solves stop at 1e-10, so HP loops agree to ~cond*tol (A16(iii)); LP iterates agree to rounding
+    assert rel(got, want) < 1e-8
+    # batching must not change anything: same set with 2 sources per batch
+    got2, _, _ = c.t.run_loop_set(wl.noise_seed, wl.n_hp, wl.n_lp, F64, wl.lp_tol, wl.lp_iters,
+                                  hp_tol=wl.hp_tol, hp_max_iter=2000, nrhs=2, with_derivative=True)
+    assert np.array_equal(got, got2)
+    # LP == HP: the correction vanishes identically and Eq. 2.4 is Eq. 2.2 over the LP set (P11)
+    got3, _, _ = c.t.run_loop_set(wl.noise_seed, 2, 3, F64, 1e-9, 2000, hp_tol=1e-9, hp_max_iter=2000, nrhs=1)
+    corr, lp, n_hp, n_lp = c.t.loops_get_state()
+    assert n_hp == 2 and n_lp == 3 and not corr.any()
+    assert np.array_equal(got3, lp / 3)
+
+
+def test_tsm_manual_accumulation_and_state(small):
+    c = small
+    seed = 31
+    c.t.loops_reset(False)
+    c.t.solve(seed, [0, 1], F64, 1e-10, 2000, slot=0)
+    c.t.solve(seed, [0, 1], F64, 0.0, 3, slot=1)
+    l_hp = [c.t.loops_source(0, j) for j in range(2)]
+    l_lp = [c.t.loops_source(1, j) for j in range(2)]
+    c.t.loops_add_correction(0, 1)
+    c.t.solve(seed, [2, 3, 4], F64, 0.0, 3, slot=1)
+    l_lp2 = [c.t.loops_source(1, j) for j in range(3)]
+    c.t.loops_add_lp(1)
+    got = c.t.loops_finalize()
+    want = (l_hp[0] - l_lp[0] + l_hp[1] - l_lp[1]) / 2 + sum(l_lp2) / 3
+    assert rel(got, want) < 1e-14
+    corr, lp, n_hp, n_lp = c.t.loops_get_state()
+    assert (n_hp, n_lp) == (2, 3)
+    c.t.loops_reset(False)
+    c.t.loops_set_state(corr, lp, n_hp, n_lp)           # resume
+    assert np.array_equal(c.t.loops_finalize(), got)
+    # Eq. 2.4 needs the same eta_j on both sides
+    c.t.solve(seed, [5, 6, 7], F64, 0.0, 3, slot=0)
+    c.t.solve(seed, [5, 6, 8], F64, 0.0, 3, slot=1)
+    with pytest.raises(Exception):
+        c.t.loops_add_correction(0, 1)
+
+
+# ---------------------------------------------------------------- error behaviour (8(b))
+def test_state_and_argument_errors(tsm_mod):
+    t = tsm_mod.Tsm((4, 4, 4, 4), max_nrhs=2)
+    with pytest.raises(tsm_mod.TsmError) as e:
+        t.solve(1, [0], F64, 1e-6, 10)
+    assert e.value.code == tsm_mod.ESTATE                # no gauge / params yet
+    t.set_gauge(W.unit_links((4, 4, 4, 4)))
+    with pytest.raises(tsm_mod.TsmError) as e:
+        t.solve(1, [0], F64, 1e-6, 10)
+    assert e.value.code == tsm_mod.ESTATE
+    t.set_params(0.12, 0.1)
+    with pytest.raises(tsm_mod.TsmError) as e:
+        t.solve(1, [0, 1, 2], F64, 1e-6, 10)             # nrhs > max_nrhs
+    assert e.value.code == tsm_mod.EINVAL
+    with pytest.raises(tsm_mod.TsmError) as e:
+        t.get_solution(1, 0)                             # empty slot
+    assert e.value.code == tsm_mod.ESTATE
+    rc, info = t.solve(1, [0], F64, 1e-8, 200)
+    assert rc == 0
+    with pytest.raises(tsm_mod.TsmError):
+        tsm_mod.Tsm((4, 4, 5, 4))
+    t.close()
