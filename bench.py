@@ -1,0 +1,360 @@
+#!/usr/bin/env python
+"""bench.py -- the hot path of the TSM loop estimator on B200, one JSON line on stdout.
+
+A "step" is one pass of the whole hot path over one batch of noise sources of the
+32^3 x 64 workload (BASELINE.json configs[4], the one `metric` is quoted on): generate
+12 Z4 sources on the device, source preparation, 100 fixed iterations of fp32 even-odd CG
+on Mhat^dag Mhat (4 stencil launches + 2 fused BLAS launches each), reconstruction, local
+and one-derivative loop contractions, accumulation into the Eq. 2.4 sums.
+
+  value     = LP CG solves/s with the gauge field resident in HBM (device-timed, CUDA events)
+  e2e       = the same through the public API with HOST buffers: every step uploads the gauge
+              configuration from pinned host memory (tsm_set_gauge), solves, contracts, and
+              reads the loops back to the host
+  roofline  = the stencil kernels inside the timed steps: algorithmic bytes / CUDA-event time
+  cpu_baseline = the oracle timed on this box's host cores on a bounded sample
+
+python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload 1..5]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1211_0126_b200 import workloads as W  # noqa: E402
+
+METRIC = "lp_cg_solves_per_s"
+UNIT = "solves/s"
+PRECS = {"f64": 0, "f32": 1, "bf16": 2}
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ----------------------------------------------------------------------------- algorithmic bytes
+def stencil_bytes_per_site(prec: str, recon: int, nrhs: int, kind: int) -> float:
+    """SURVEY.md 8(d) / DESIGN.md: compulsory bytes per output site per source of one stencil
+    launch: 8 neighbour spinors are each read once per field (24 reals in, 24 out = 48 w_s),
+    8 links of n_g reals shared by the nrhs sources of a batch, +24 w_s for the x term (kind 1),
+    +24 w_s more for the vector of the fused <p,q> reduction (kind 2)."""
+    w_s = {"f64": 8, "f32": 4, "bf16": 2}[prec]
+    w_g, n_g = (8, 18) if prec == "f64" else (4, recon)
+    return (48 + 24 * kind) * w_s + 8.0 * n_g * w_g / nrhs
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device: int):
+        self.device = device
+        self.rows = []
+        self.proc = None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.device), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc is not None:
+            time.sleep(0.15)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+                for k, n in enumerate(names):
+                    if r[3 + k].lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ----------------------------------------------------------------------------- the oracle legs
+def oracle_sample(wl, U, sid: int = 0):
+    """Bounded sample of one step on the host cores, with the oracle as it stands: one source,
+    source preparation + 1 and 3 CG iterations + reconstruction (+ residual check), and one
+    pass of the loop contractions; the full lp_iters-iteration solve is extrapolated linearly
+    in the iteration count.  Returns (seconds per solve incl. contraction, detail dict)."""
+    import oracle
+    eta = oracle.noise(wl.dims, wl.noise_seed, sid)
+    t0 = time.perf_counter()
+    s1, _ = oracle.solve(wl.dims, wl.t_boundary, wl.kappa, wl.mu, U, eta, 0.0, 1)
+    t1 = time.perf_counter()
+    s3, _ = oracle.solve(wl.dims, wl.t_boundary, wl.kappa, wl.mu, U, eta, 0.0, 3)
+    t3 = time.perf_counter()
+    oracle.all_loops(wl.dims, wl.t_boundary, U, eta, s3, wl.derivative)
+    tl = time.perf_counter()
+    t_iter = ((t3 - t1) - (t1 - t0)) / 2.0
+    iters = wl.lp_iters if wl.lp_tol == 0 else 10
+    t_solve = (t1 - t0) + (iters - 1) * t_iter + (tl - t3)
+    detail = {"t_1iter_solve_s": t1 - t0, "t_per_cg_iteration_s": t_iter, "t_contract_s": tl - t3,
+              "iterations_extrapolated_to": iters}
+    return t_solve, detail
+
+
+def run_reference(args, wl):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+    oracle.build()
+    U = wl.links()
+    times = []
+    detail = {}
+    for k in range(args.warmup + args.steps):
+        t, detail = oracle_sample(wl, U, sid=k)
+        if k >= args.warmup:
+            times.append(t)
+    t = float(np.mean(times))
+    value = 1.0 / t
+    cores = oracle.n_threads()
+    sample = ("per step: 1 source of the workload; source preparation, 1- and 3-iteration CG solves, "
+              "reconstruction, fp64 residual and one contraction pass run in full, the "
+              f"{detail['iterations_extrapolated_to']}-iteration solve extrapolated linearly")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "lattice": list(wl.dims), "lp_iters": wl.lp_iters, "lp_tol": wl.lp_tol,
+                       "derivative_loops": wl.derivative},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                             "detail": detail},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------- our arm
+def run_ours(args, wl):
+    import torch
+    import torch.distributed as dist
+    from paper_1211_0126_b200 import tsm
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (there is no CPU fallback for the product path)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    peak, peak_src = measured_peaks()
+    prec_name = wl.lp_prec if wl.lp_prec != "bf16" else "f32"   # bf16 solver not built yet: see DESIGN.md
+    prec = PRECS[prec_name]
+    nrhs = wl.nrhs
+    tol, iters = wl.lp_tol, wl.lp_iters
+
+    t0 = time.perf_counter()
+    U = wl.links()
+    log(f"[bench] rank {rank}: links {wl.name} generated in {time.perf_counter() - t0:.1f} s")
+    links_host = torch.from_numpy(U.view(np.float64).reshape(-1)).pin_memory()
+    stream = torch.cuda.current_stream()
+    t = tsm.Tsm(wl.dims, t_boundary=wl.t_boundary, device=local, max_nrhs=nrhs, stream=stream)
+    t.set_params(wl.kappa, wl.mu)
+    dev = t.set_gauge(links_host, wl.reconstruct)
+    log(f"[bench] unitarity deviation {dev:.2e}; workspace {t.workspace.numel() / 2**30:.1f} GiB")
+    t.loops_reset(wl.derivative)
+    # replicas only: every rank works on its own, disjoint source ids
+    next_id = [rank * 1_000_000]
+
+    def step():
+        ids = list(range(next_id[0], next_id[0] + nrhs))
+        next_id[0] += nrhs
+        rc, info = t.solve(wl.noise_seed, ids, prec, tol, iters, slot=1)
+        t.loops_add_lp(1)
+        return info
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        info = step()
+    # ---- timed region: resident inputs
+    t.profile(True)
+    barrier()
+    l0 = t.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        e0.record(stream)
+        for _ in range(args.steps):
+            info = step()
+        e1.record(stream)
+        barrier()
+    ms = e0.elapsed_time(e1)
+    launches = t.launch_count() - l0
+    t.profile(False)
+    prof = {k: t.profile_read(prec, k, nrhs) for k in range(5)}
+    if world > 1:
+        tt = torch.tensor([ms], device=f"cuda:{local}", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms = float(tt.item())
+    value = world * nrhs * args.steps / (ms * 1e-3)
+
+    # ---- roofline of the stencil kernels inside the timed steps
+    Vh = wl.V // 2
+    alg_bytes = sum(stencil_bytes_per_site(prec_name, wl.reconstruct, nrhs, k) * Vh * nrhs * prof[k][1] for k in range(3))
+    st_ms = sum(prof[k][0] for k in range(3))
+    st_n = sum(prof[k][1] for k in range(3))
+    achieved = alg_bytes / (st_ms * 1e-3) / 1e9 if st_ms > 0 else 0.0
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src, "kernel": f"k_dslash<{prec_name}, recon {wl.reconstruct}> x {nrhs} sources",
+                "launches_timed": st_n, "avg_launch_us": st_ms * 1e3 / max(st_n, 1),
+                "algorithmic_bytes_per_launch": alg_bytes / max(st_n, 1),
+                "share_of_step": {"stencil": st_ms / ms, "cg_update_xr": prof[3][0] / ms, "cg_update_p": prof[4][0] / ms},
+                "gflops_at_1320_per_site": 1320.0 * Vh * nrhs * st_n / (st_ms * 1e-3) / 1e9 if st_ms > 0 else 0.0}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": prec_name, "data": "synthetic",
+            "config": {"workload": wl.name, "lattice": list(wl.dims), "kappa": wl.kappa, "mu": wl.mu, "links_eps": wl.eps,
+                       "nrhs_per_batch": nrhs, "lp_iters": iters, "lp_tol": tol, "reconstruct": wl.reconstruct,
+                       "derivative_loops": wl.derivative, "parallelism": f"replicas x{world}",
+                       "l2": "inputs larger than L2 (links 604 MB + 12 x 101 MB vectors per pass)"},
+            "gpu_launches": int(launches), "clocks": clk.summary(), "roofline": roofline,
+            "lp_iters_done": [i["iters"] for i in info]}
+
+    if rank == 0 and not args.skip_extras:
+        line.update(extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U))
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    t.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U):
+    """e2e through the host-buffer API, single-launch stencil table, full loop set, oracle baseline."""
+    out = {}
+    nrhs = wl.nrhs
+    stream = torch.cuda.current_stream()
+    # ---- e2e: host gauge field in, host loops out, every step
+    n_e2e = max(1, min(args.steps, 3))
+    torch.cuda.synchronize()
+    w0 = time.perf_counter()
+    for k in range(n_e2e):
+        t.set_gauge(links_host, wl.reconstruct)          # H2D of the configuration + reorder kernels
+        t.loops_reset(wl.derivative)
+        step()
+        loops = t.loops_finalize()                       # D2H of the [n_ops][T] loops
+    torch.cuda.synchronize()
+    w1 = time.perf_counter()
+    out["e2e"] = {"value": nrhs * n_e2e / (w1 - w0), "unit": UNIT, "h2d_bytes_per_step": int(links_host.numel() * 8),
+                  "d2h_bytes_per_step": int(loops.nbytes), "steps": n_e2e,
+                  "note": "every step re-uploads the gauge configuration from pinned host memory; in production one upload serves N_HP+N_LP solves"}
+
+    # ---- single-launch stencil table (north_star: >= 70 % of HBM peak on single-RHS fp32 / fp64)
+    table = {}
+    for pname, n in (("f32", 1), ("f64", 1), ("f32", nrhs), ("bf16", 1)):
+        p = PRECS[pname]
+        a = t.alloc_field(p, n)
+        b = t.alloc_field(p, n)
+        a.view(torch.int16)[:] = 0x3C00 if pname == "bf16" else 0
+        if pname != "bf16":
+            (a.view(torch.float32) if pname == "f32" else a.view(torch.float64)).normal_()
+        reps = 50
+        for _ in range(5):
+            t.dslash(tsm.OP_D_EO, p, n, a, b)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            t.dslash(tsm.OP_D_EO, p, n, a, b)
+            t.dslash(tsm.OP_D_OE, p, n, b, a)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        us = e0.elapsed_time(e1) * 1e3 / (2 * reps)
+        by = stencil_bytes_per_site(pname, wl.reconstruct, n, 0) * (wl.V // 2) * n
+        table[f"{pname}_nrhs{n}"] = {"us": us, "algorithmic_GBs": by / us / 1e3, "frac_of_measured_peak": by / us / 1e3 / peak,
+                                     "frac_of_8000": by / us / 1e3 / 8000.0, "gflops": 1320.0 * (wl.V // 2) * n / us / 1e3}
+        del a, b
+    out["dslash"] = table
+
+    # ---- the whole of Eq. 2.4 for this configuration (reading A23)
+    if not args.no_full_set:
+        loops, secs, rc = t.run_loop_set(wl.noise_seed, wl.n_hp, wl.n_lp, prec, wl.lp_tol, wl.lp_iters, hp_tol=wl.hp_tol,
+                                         hp_max_iter=5000, nrhs=nrhs, with_derivative=wl.derivative)
+        out["tsm_loop_set"] = {"seconds": secs, "n_hp": wl.n_hp, "n_lp": wl.n_lp, "rc": rc,
+                               "finite": bool(np.isfinite(loops.view(np.float64)).all())}
+        rc, info = t.solve(wl.noise_seed, list(range(min(nrhs, wl.n_hp))), tsm.F64, wl.hp_tol, 5000, slot=0, want_true_resid=True)
+        out["hp_solve"] = {"iters": [i["iters"] for i in info], "secs_batch": info[0]["secs"],
+                           "true_resid_max": max(i["rel_resid_true"] for i in info)}
+
+    # ---- the oracle on this box's host cores, bounded sample
+    if not args.no_cpu_baseline:
+        import oracle
+        oracle.build()
+        tcpu, detail = oracle_sample(wl, U)
+        out["cpu_baseline"] = {"value": 1.0 / tcpu, "unit": UNIT, "cores": oracle.n_threads(), "kind": "oracle",
+                               "sample": ("1 source: source preparation, 1- and 3-iteration CG solves, reconstruction, residual and one "
+                                          f"contraction pass run in full; the {detail['iterations_extrapolated_to']}-iteration solve "
+                                          "extrapolated linearly in the iteration count"),
+                               "detail": detail}
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", type=int, default=5)
+    ap.add_argument("--skip-extras", action="store_true", help="only the timed steps (no e2e/table/full set/oracle)")
+    ap.add_argument("--no-full-set", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    wl = W.WORKLOADS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, wl)
+    else:
+        run_ours(args, wl)
+
+
+if __name__ == "__main__":
+    main()

@@ -151,6 +151,15 @@ int tsm_run_loop_set(tsm_ctx* ctx, uint64_t seed, int kind, int n_hp, int n_lp, 
 /* Number of kernels this library has launched on the context since creation. */
 long long tsm_launch_count(const tsm_ctx* ctx);
 
+/* Measurement aid: with profiling enabled every stencil and CG
+ * BLAS launch is bracketed by CUDA events on the library's stream.  tsm_profile_read
+ * synchronises, returns the summed duration (ms) and the number of launches recorded so far
+ * for one class and forgets them.  prec: TSM_F64/F32/BF16; kind: 0 stencil (H5), 1 stencil
+ * with the x term, 2 stencil with x term and the <p,q> reduction, 3 x/r update, 4 p update;
+ * nrhs <= 0 matches any batch size. */
+int tsm_profile(tsm_ctx* ctx, int enable);
+int tsm_profile_read(tsm_ctx* ctx, int prec, int kind, int nrhs, double* total_ms, long long* count);
+
 #ifdef __cplusplus
 }
 #endif

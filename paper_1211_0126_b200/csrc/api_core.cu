@@ -84,6 +84,7 @@ int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
     ctx->with_deriv = 0;
     ctx->n_hp = ctx->n_lp = 0;
     ctx->launches = 0;
+    ctx->prof_on = false;
     ctx->cg = nullptr; ctx->cg_host = nullptr; ctx->host_small = nullptr; ctx->ids_dev = nullptr;
     for (int s = 0; s < 2; s++) { ctx->slot_prec[s] = -1; ctx->slot_nrhs[s] = 0; }
     build_gamma_table(ctx->gam);
@@ -111,6 +112,8 @@ int tsm_destroy(tsm_ctx* ctx)
     if (ctx->cg_host) cudaFreeHost(ctx->cg_host);
     if (ctx->host_small) cudaFreeHost(ctx->host_small);
     if (ctx->ids_dev) cudaFree(ctx->ids_dev);
+    for (ProfRec& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (cudaEvent_t e : ctx->prof_pool) cudaEventDestroy(e);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;
@@ -120,6 +123,37 @@ int tsm_destroy(tsm_ctx* ctx)
 const char* tsm_last_error(const tsm_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 
 long long tsm_launch_count(const tsm_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int tsm_profile(tsm_ctx* ctx, int enable)
+{
+    if (!ctx) return TSM_EINVAL;
+    ctx->prof_on = enable != 0;
+    return TSM_OK;
+}
+
+int tsm_profile_read(tsm_ctx* ctx, int prec, int kind, int nrhs, double* total_ms, long long* count)
+{
+    if (!ctx || !total_ms || !count) return TSM_EINVAL;
+    TSM_CUDA(ctx, cudaSetDevice(ctx->device));
+    TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    double tot = 0;
+    long long n = 0;
+    std::vector<ProfRec> keep;
+    for (ProfRec& r : ctx->prof) {
+        if (r.prec == prec && r.kind == kind && (nrhs <= 0 || r.nrhs == nrhs)) {
+            float ms = 0;
+            if (cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess) { tot += ms; n++; }
+            ctx->prof_pool.push_back(r.a);
+            ctx->prof_pool.push_back(r.b);
+        } else {
+            keep.push_back(r);
+        }
+    }
+    ctx->prof.swap(keep);
+    *total_ms = tot;
+    *count = n;
+    return TSM_OK;
+}
 
 size_t tsm_field_bytes(const tsm_ctx* ctx, int prec, int nrhs)
 {

@@ -40,10 +40,9 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_init(const int Vh, const int nrh
     const double tot = block_sum_all(sum, smem);
     if (threadIdx.x == 0) partials[(size_t)rhs * gridDim.x + blockIdx.x] = tot;
     if (last_block_arrive(&cg->ticket)) {
-        int all = 1;
-        for (int j = 0; j < nrhs; j++) {
-            const double v = sum_partials(partials, j, gridDim.x, smem);
-            if (threadIdx.x == 0) {
+        for (int j = threadIdx.x >> 5; j < nrhs; j += BLAS_BS / 32) {
+            const double v = sum_partials_warp(partials, j, gridDim.x);
+            if ((threadIdx.x & 31) == 0) {
                 cg->rr[j] = v;
                 cg->bb[j] = v;
                 cg->pq[j] = 0;
@@ -51,10 +50,14 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_init(const int Vh, const int nrh
                 cg->iters[j] = 0;
                 cg->status[j] = TSM_OK;
                 cg->done[j] = !(v > 0);
-                all &= cg->done[j];
             }
         }
-        if (threadIdx.x == 0) cg->all_done = all;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int all = 1;
+            for (int j = 0; j < nrhs; j++) all &= cg->done[j];
+            cg->all_done = all;
+        }
     }
 }
 
@@ -100,10 +103,9 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_update_xr(const int Vh, const in
     const double tot = block_sum_all(sum, smem);
     if (threadIdx.x == 0) partials[(size_t)rhs * gridDim.x + blockIdx.x] = tot;
     if (last_block_arrive(&cg->ticket)) {
-        int all = 1;
-        for (int j = 0; j < nrhs; j++) {
-            const double v = sum_partials(partials, j, gridDim.x, smem);
-            if (threadIdx.x == 0) {
+        for (int j = threadIdx.x >> 5; j < nrhs; j += BLAS_BS / 32) {
+            const double v = sum_partials_warp(partials, j, gridDim.x);
+            if ((threadIdx.x & 31) == 0) {
                 if (!cg->done[j]) {
                     const double rr_j = cg->rr[j], pq_j = cg->pq[j];
                     if (!(pq_j > 0) || !isfinite(pq_j) || !(rr_j > 0) || !isfinite(rr_j)) {
@@ -116,10 +118,14 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_update_xr(const int Vh, const in
                         if (tol > 0 && sqrt(v / cg->bb[j]) <= tol) cg->done[j] = 1;
                     }
                 }
-                all &= cg->done[j];
             }
         }
-        if (threadIdx.x == 0) cg->all_done = all;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int all = 1;
+            for (int j = 0; j < nrhs; j++) all &= cg->done[j];
+            cg->all_done = all;
+        }
     }
 }
 
@@ -149,9 +155,9 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_update_p(const int Vh, void* __r
 
 inline dim3 blas_grid(const tsm_ctx* ctx, int nrhs)
 {
+    // the x grid does not depend on nrhs: same thread->element map and reduction tree in any batch (A14)
     long long gx = (3LL * ctx->g.Vh + BLAS_BS - 1) / BLAS_BS;
-    long long cap = (long long)ctx->nsm * 8 / nrhs;
-    if (cap < ctx->nsm) cap = ctx->nsm;
+    const long long cap = (long long)ctx->nsm * 4;
     if (gx > cap) gx = cap;
     return dim3((unsigned)gx, (unsigned)nrhs);
 }
@@ -182,7 +188,9 @@ int launch_cg_update_xr(tsm_ctx* ctx, int prec, int nrhs, void* x, const void* p
 {
     const dim3 grid = blas_grid(ctx, nrhs);
     if ((size_t)grid.x * nrhs > ctx->partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
+    const int pi = prof_begin(ctx, prec, 3, nrhs);
     BLAS_SWITCH(prec, (k_cg_update_xr<PV, PP><<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, nrhs, x, p, r, q, tol, ctx->partials, ctx->cg)));
+    prof_end(ctx, pi);
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;
@@ -191,7 +199,9 @@ int launch_cg_update_xr(tsm_ctx* ctx, int prec, int nrhs, void* x, const void* p
 int launch_cg_update_p(tsm_ctx* ctx, int prec, int nrhs, void* p, const void* r)
 {
     const dim3 grid = blas_grid(ctx, nrhs);
+    const int pi = prof_begin(ctx, prec, 4, nrhs);
     BLAS_SWITCH(prec, (k_cg_update_p<PV, PP><<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, p, r, ctx->cg)));
+    prof_end(ctx, pi);
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;
@@ -216,9 +226,9 @@ __global__ void __launch_bounds__(BLAS_BS) k_diff_norm2(const int Vh, const int 
     const double tot = block_sum_all(sum, smem);
     if (threadIdx.x == 0) partials[(size_t)rhs * gridDim.x + blockIdx.x] = tot;
     if (last_block_arrive(&cg->ticket)) {
-        for (int j = 0; j < nrhs; j++) {
-            const double v = sum_partials(partials, j, gridDim.x, smem);
-            if (threadIdx.x == 0) cg->pq[j] = v;
+        for (int j = threadIdx.x >> 5; j < nrhs; j += BLAS_BS / 32) {
+            const double v = sum_partials_warp(partials, j, gridDim.x);
+            if ((threadIdx.x & 31) == 0) cg->pq[j] = v;
         }
     }
 }

@@ -94,12 +94,12 @@ __device__ __forceinline__ void hop_direction(const void* pack, const void* in, 
 }
 
 template <int PREC> struct DslashCfg {
-    static constexpr int MINB = (PREC == TSM_F64) ? 2 : 4;   // 128-thread blocks per SM the register budget allows
+    static constexpr int MAXT = (PREC == TSM_F64) ? 256 : 512;   // threads per block: 255 regs (fp64) / 128 regs (fp32)
 };
 
 // DOT: 0 none, 1: partial sums of Re<y, out>, last block leaves the totals in cg->pq[rhs].
 template <int PREC, int RECON, bool DAGGER, bool XPAY, int DOT>
-__global__ void __launch_bounds__(128, DslashCfg<PREC>::MINB)
+__global__ void __launch_bounds__(DslashCfg<PREC>::MAXT, 1)
 k_dslash(const Geom g, const int par, const int nrhs, const void* __restrict__ pack, const void* __restrict__ in_,
          const void* __restrict__ x_, void* __restrict__ out_, const DslashCoef cf, const void* __restrict__ y_,
          double* __restrict__ partials, CgScalars* __restrict__ cg, const int check_done)
@@ -162,9 +162,10 @@ k_dslash(const Geom g, const int par, const int nrhs, const void* __restrict__ p
         const double tot = block_row_sum(dot, smem);
         if (threadIdx.x == 0 && rhs < nrhs) partials[(size_t)rhs * gridDim.x + blockIdx.x] = tot;
         if (last_block_arrive(&cg->ticket)) {
-            for (int r = 0; r < nrhs; r++) {
-                const double v = sum_partials(partials, r, gridDim.x, smem);
-                if (threadIdx.x == 0 && threadIdx.y == 0) cg->pq[r] = v;
+            const int flat = threadIdx.y * blockDim.x + threadIdx.x, nwarp = (blockDim.x * blockDim.y) >> 5;
+            for (int r = flat >> 5; r < nrhs; r += nwarp) {
+                const double v = sum_partials_warp(partials, r, gridDim.x);
+                if ((flat & 31) == 0) cg->pq[r] = v;
             }
         }
     }
@@ -174,20 +175,24 @@ template <int PREC, int RECON, bool DAGGER, bool XPAY, int DOT>
 int launch_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void* in, const void* x, void* out,
              const DslashCoef& c, const void* y, int check_done)
 {
-    const int BS = 128;
+    // 128 sites x RY sources per block.  The x extent and the x grid do not depend on the batch,
+    // so every source sees the same thread->site map and the same reduction tree in any batch.
+    const int bs = 128;
+    const int max_ry = (PREC == TSM_F64) ? 2 : 4;     // register file: 512 x 128 regs (fp32), 256 x 255 (fp64)
     int ry = 1;
-    if (nrhs >= 4 && nrhs % 4 == 0) ry = 4;          // 4 sources share each link fetch through L1
+    if (nrhs % 4 == 0 && max_ry >= 4) ry = 4;          // RY sources share each link fetch through L1
     else if (nrhs % 2 == 0) ry = 2;
-    const int bs = BS / ry;
     dim3 block(bs, ry);
     const int gy = nrhs / ry;
     int gx = (ctx->g.Vh + bs - 1) / bs;
-    const int cap = ctx->nsm * 16;                    // grid-stride beyond this; keeps the partial count small
+    const int cap = ctx->nsm * 8;                     // grid-stride beyond this; keeps the partial count small
     if (gx > cap) gx = cap;
     dim3 grid(gx, gy);
     if (DOT && (size_t)gx * nrhs > ctx->partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
+    const int pi = prof_begin(ctx, PREC, DOT ? 2 : (XPAY ? 1 : 0), nrhs);
     k_dslash<PREC, RECON, DAGGER, XPAY, DOT><<<grid, block, 0, ctx->stream>>>(ctx->g, par, nrhs, pack, in, x, out, c, y,
                                                                              ctx->partials, ctx->cg, check_done);
+    prof_end(ctx, pi);
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;

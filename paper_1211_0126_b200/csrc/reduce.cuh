@@ -38,11 +38,14 @@ __device__ __forceinline__ bool last_block_arrive(unsigned* ticket)
     return is_last != 0;
 }
 
-// In the last block: total of partials[rhs * nblk + 0 .. nblk) in a fixed order; valid in flat thread 0.
-__device__ __forceinline__ double sum_partials(const double* partials, int rhs, int nblk, double* smem)
+// In the last block: total of partials[rhs * nblk + 0 .. nblk), summed by ONE warp (lane-strided,
+// then the fixed shuffle tree), so the order depends on nblk only -- not on the block shape or on
+// how many sources are in the batch (A14: a source's iterate is bit-identical in any batch).
+// Call with all 32 lanes of the warp; result valid in lane 0.
+__device__ __forceinline__ double sum_partials_warp(const double* partials, int rhs, int nblk)
 {
-    const int tid = threadIdx.y * blockDim.x + threadIdx.x, nt = blockDim.x * blockDim.y;
+    const int lane = (threadIdx.y * blockDim.x + threadIdx.x) & 31;
     double v = 0;
-    for (int k = tid; k < nblk; k += nt) v += __ldcg(partials + (size_t)rhs * nblk + k);
-    return block_sum_all(v, smem);
+    for (int k = lane; k < nblk; k += 32) v += __ldcg(partials + (size_t)rhs * nblk + k);
+    return warp_sum(v);
 }

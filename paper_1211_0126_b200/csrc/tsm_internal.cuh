@@ -7,6 +7,7 @@
 #include <cuda_bf16.h>
 #include <stdint.h>
 #include <string>
+#include <vector>
 
 #include "../../include/tsm.h"
 
@@ -294,6 +295,10 @@ struct GammaTable {          // Gamma_{alpha, col[alpha]} = i^ph[alpha], all oth
     int ph[16][4];
 };
 
+// Optional per-launch timing (tsm_profile): CUDA events on the library's stream around each
+// stencil / BLAS launch.  kind: 0 stencil, 1 stencil+xpay, 2 stencil+xpay+dot, 3 update_xr, 4 update_p.
+struct ProfRec { int prec, kind, nrhs; cudaEvent_t a, b; };
+
 struct tsm_ctx {
     Geom g;
     int device;
@@ -329,6 +334,9 @@ struct tsm_ctx {
     GammaTable gam;
     int n_ops, with_deriv, n_hp, n_lp;
     long long launches;
+    bool prof_on;
+    std::vector<ProfRec> prof;
+    std::vector<cudaEvent_t> prof_pool;
     cudaEvent_t ev0, ev1;
     std::string err;
 };
@@ -341,6 +349,23 @@ struct tsm_ctx {
             return TSM_ECUDA;                                                                    \
         }                                                                                        \
     } while (0)
+
+inline int prof_begin(tsm_ctx* ctx, int prec, int kind, int nrhs)
+{
+    if (!ctx->prof_on) return -1;
+    ProfRec r{prec, kind, nrhs, nullptr, nullptr};
+    for (cudaEvent_t* e : {&r.a, &r.b}) {
+        if (!ctx->prof_pool.empty()) { *e = ctx->prof_pool.back(); ctx->prof_pool.pop_back(); }
+        else if (cudaEventCreate(e) != cudaSuccess) return -1;
+    }
+    cudaEventRecord(r.a, ctx->stream);
+    ctx->prof.push_back(r);
+    return (int)ctx->prof.size() - 1;
+}
+inline void prof_end(tsm_ctx* ctx, int idx)
+{
+    if (idx >= 0) cudaEventRecord(ctx->prof[idx].b, ctx->stream);
+}
 
 inline int tsm_fail(tsm_ctx* ctx, int code, const char* msg)
 {

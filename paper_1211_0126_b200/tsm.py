@@ -28,7 +28,7 @@ EXPORTS = [
     "tsm_pack", "tsm_unpack", "tsm_dslash", "tsm_solve", "tsm_get_solution", "tsm_set_solution",
     "tsm_loops_reset", "tsm_loops_add_correction", "tsm_loops_add_lp", "tsm_loops_source",
     "tsm_loops_finalize", "tsm_loops_get_state", "tsm_loops_set_state", "tsm_run_loop_set",
-    "tsm_launch_count",
+    "tsm_launch_count", "tsm_profile", "tsm_profile_read",
 ]
 
 
@@ -86,6 +86,8 @@ def load_library():
     lib.tsm_run_loop_set.argtypes = [vp, u64, i, i, i, i, ctypes.c_double, i, ctypes.c_double, i, i, i, dp, dp]
     lib.tsm_launch_count.argtypes = [vp]
     lib.tsm_launch_count.restype = ctypes.c_longlong
+    lib.tsm_profile.argtypes = [vp, i]
+    lib.tsm_profile_read.argtypes = [vp, i, i, i, dp, ctypes.POINTER(ctypes.c_longlong)]
     _lib = lib
     return lib
 
@@ -152,6 +154,15 @@ class Tsm:
 
     def launch_count(self) -> int:
         return int(self.lib.tsm_launch_count(self._h))
+
+    def profile(self, enable: bool):
+        self._check(self.lib.tsm_profile(self._h, int(enable)))
+
+    def profile_read(self, prec: int, kind: int, nrhs: int = 0):
+        """(total ms, launches) recorded for one kernel class since the last read."""
+        ms, n = ctypes.c_double(), ctypes.c_longlong()
+        self._check(self.lib.tsm_profile_read(self._h, prec, kind, nrhs, ctypes.byref(ms), ctypes.byref(n)))
+        return ms.value, n.value
 
     def field_bytes(self, prec: int, nrhs: int = 1) -> int:
         return int(self.lib.tsm_field_bytes(self._h, prec, nrhs))

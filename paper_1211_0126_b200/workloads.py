@@ -12,6 +12,8 @@ DESIGN.md "Input recipe").
 """
 from __future__ import annotations
 
+import os
+from concurrent.futures import ThreadPoolExecutor
 from dataclasses import dataclass, field
 
 import numpy as np
@@ -37,7 +39,7 @@ def volume(dims) -> int:
     return int(dims[0]) * int(dims[1]) * int(dims[2]) * int(dims[3])
 
 
-def random_su3_links(dims, eps: float, seed: int, chunk: int = 1 << 18) -> np.ndarray:
+def random_su3_links(dims, eps: float, seed: int, chunk: int = 1 << 16) -> np.ndarray:
     """Seeded weak-field SU(3) links U = exp(i*eps*H).
 
     H = sum_a c_a lambda_a / 2 with c_a uniform in [-1, 1) (reading A21), drawn
@@ -47,15 +49,27 @@ def random_su3_links(dims, eps: float, seed: int, chunk: int = 1 << 18) -> np.nd
     """
     V = volume(dims)
     rng = np.random.Generator(np.random.PCG64(seed))
-    out = np.empty((4 * V, 3, 3), dtype=np.complex128)
     n = 4 * V
-    for lo in range(0, n, chunk):
+    out = np.empty((n, 3, 3), dtype=np.complex128)
+    gm = _GELL_MANN.reshape(8, 9)
+    # the random stream is drawn serially in [mu][lex][a] order; only the per-matrix
+    # eigendecompositions run on a thread pool, so the result does not depend on the pool size
+    coef = rng.random((n, 8)) * 2.0 - 1.0
+
+    def work(lo):
         hi = min(n, lo + chunk)
-        c = rng.random((hi - lo, 8)) * 2.0 - 1.0
-        H = np.einsum("na,aij->nij", c, _GELL_MANN) * 0.5
+        H = (coef[lo:hi] @ gm).reshape(hi - lo, 3, 3) * 0.5
         w, v = np.linalg.eigh(H)
-        ph = np.exp(1j * eps * w)
-        out[lo:hi] = np.einsum("nik,nk,njk->nij", v, ph, v.conj())
+        out[lo:hi] = (v * np.exp(1j * eps * w)[:, None, :]) @ v.conj().transpose(0, 2, 1)
+
+    starts = range(0, n, chunk)
+    nthreads = min(len(os.sched_getaffinity(0)), 16, len(starts))
+    if nthreads > 1:
+        with ThreadPoolExecutor(nthreads) as ex:
+            list(ex.map(work, starts))
+    else:
+        for lo in starts:
+            work(lo)
     return out.reshape(4, V, 3, 3)
 
 
