@@ -211,9 +211,8 @@ int tsm_loops_add_correction(tsm_ctx* ctx, int slot_hp, int slot_lp)
         memcmp(ctx->slot_ids[slot_hp], ctx->slot_ids[slot_lp], nrhs * sizeof(uint32_t)) != 0)
         return tsm_fail(ctx, TSM_ESTATE, "HP and LP slots hold different sources (Eq. 2.4 needs the same eta_j)");
     if ((rc = launch_contract(ctx, slot_hp))) return rc;
-    if ((rc = launch_accumulate(ctx, ctx->acc_corr, ctx->loops_src[slot_hp], nrhs, +1.0))) return rc;
     if ((rc = launch_contract(ctx, slot_lp))) return rc;
-    if ((rc = launch_accumulate(ctx, ctx->acc_corr, ctx->loops_src[slot_lp], nrhs, -1.0))) return rc;
+    if ((rc = launch_accumulate(ctx, ctx->acc_corr, ctx->loops_src[slot_hp], ctx->loops_src[slot_lp], nrhs))) return rc;
     ctx->n_hp += nrhs;
     return TSM_OK;
 }
@@ -225,7 +224,7 @@ int tsm_loops_add_lp(tsm_ctx* ctx, int slot_lp)
     if ((rc = check_slot(ctx, slot_lp, 0))) return rc;
     const int nrhs = ctx->slot_nrhs[slot_lp];
     if ((rc = launch_contract(ctx, slot_lp))) return rc;
-    if ((rc = launch_accumulate(ctx, ctx->acc_lp, ctx->loops_src[slot_lp], nrhs, +1.0))) return rc;
+    if ((rc = launch_accumulate(ctx, ctx->acc_lp, ctx->loops_src[slot_lp], nullptr, nrhs))) return rc;
     ctx->n_lp += nrhs;
     return TSM_OK;
 }

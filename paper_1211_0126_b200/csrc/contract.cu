@@ -129,13 +129,15 @@ __global__ void k_contract_finish(const int Lt, const int nblk, const int n_ops,
     }
 }
 
-__global__ void k_accumulate(const int n, const int nrhs, double* __restrict__ acc, const double* __restrict__ src, const double sign)
+// acc += a[r] - b[r] source by source, in source order: the sums of Eq. 2.4 come out bit-identical
+// however the sources were batched (b == nullptr: acc += a[r]).
+__global__ void k_accumulate(const int n, const int nrhs, double* __restrict__ acc, const double* __restrict__ a, const double* __restrict__ b)
 {
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= n) return;
-    double s = 0;
-    for (int r = 0; r < nrhs; r++) s += src[(size_t)r * n + idx];
-    acc[idx] += sign * s;
+    double s = acc[idx];
+    for (int r = 0; r < nrhs; r++) s += b ? (a[(size_t)r * n + idx] - b[(size_t)r * n + idx]) : a[(size_t)r * n + idx];
+    acc[idx] = s;
 }
 
 __global__ void k_finalize(const int n, const double* __restrict__ corr, const double* __restrict__ lp, const double w_hp,
@@ -214,10 +216,10 @@ int launch_contract(tsm_ctx* ctx, int slot)
     return TSM_OK;
 }
 
-int launch_accumulate(tsm_ctx* ctx, double* acc, const double* src, int nrhs, double sign)
+int launch_accumulate(tsm_ctx* ctx, double* acc, const double* a, const double* b, int nrhs)
 {
     const int n = ctx->n_ops * ctx->g.L[3] * 2;
-    k_accumulate<<<(n + 255) / 256, 256, 0, ctx->stream>>>(n, nrhs, acc, src, sign);
+    k_accumulate<<<(n + 255) / 256, 256, 0, ctx->stream>>>(n, nrhs, acc, a, b);
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;

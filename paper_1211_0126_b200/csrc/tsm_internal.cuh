@@ -386,7 +386,7 @@ int launch_cg_update_xr(tsm_ctx* ctx, int prec, int nrhs, void* x, const void* p
 int launch_cg_update_p(tsm_ctx* ctx, int prec, int nrhs, void* p, const void* r);
 int launch_convert(tsm_ctx* ctx, int prec_in, int prec_out, int nrhs_fields, const void* in, void* out);
 int launch_contract(tsm_ctx* ctx, int slot);
-int launch_accumulate(tsm_ctx* ctx, double* acc, const double* src, int nrhs, double sign);
+int launch_accumulate(tsm_ctx* ctx, double* acc, const double* a, const double* b, int nrhs);
 int launch_finalize(tsm_ctx* ctx);
 void build_gamma_table(GammaTable& t);
 int ctx_enter(tsm_ctx* ctx, bool need_ws, bool need_gauge, bool need_params);
