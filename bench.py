@@ -55,11 +55,11 @@ def measured_peaks():
 def stencil_bytes_per_site(prec: str, recon: int, nrhs: int, kind: int) -> float:
     """SURVEY.md 8(d) / DESIGN.md: compulsory bytes per output site per source of one stencil
     launch: 8 neighbour spinors are each read once per field (24 reals in, 24 out = 48 w_s),
-    8 links of n_g reals shared by the nrhs sources of a batch, +24 w_s for the x term (kind 1),
-    +24 w_s more for the vector of the fused <p,q> reduction (kind 2)."""
+    8 links of n_g reals shared by the nrhs sources of a batch, +24 w_s for the x term (kinds 1, 2;
+    kind 2 also leaves |out|^2 per tile, which moves no extra field)."""
     w_s = {"f64": 8, "f32": 4, "bf16": 2}[prec]
     w_g, n_g = (8, 18) if prec == "f64" else (4, recon)
-    return (48 + 24 * kind) * w_s + 8.0 * n_g * w_g / nrhs
+    return (48 + (24 if kind else 0)) * w_s + 8.0 * n_g * w_g / nrhs
 
 
 class ClockSampler:

@@ -34,6 +34,8 @@ size_t carve_workspace(tsm_ctx* ctx, int max_nrhs, char* base)
     const size_t pc2 = (size_t)max_nrhs * 5 * g.L[3] * 2 * 8 * 32;
     if (pc2 > pc) pc = pc2;
     { size_t o = c.take(pc * sizeof(double)); if (base) { ctx->partials = (double*)at(o); ctx->partials_count = pc; } }
+    const size_t npc = (size_t)max_nrhs * ((g.Vh + 127) / 128);
+    { size_t o = c.take(npc * sizeof(double)); if (base) { ctx->norm_partials = (double*)at(o); ctx->norm_partials_count = npc; } }
     const size_t lb = (size_t)(TSM_N_LOCAL_OPS + TSM_N_DERIV_OPS) * g.L[3] * 2 * sizeof(double);
     for (int s = 0; s < 2; s++) { size_t o = c.take(lb * max_nrhs); if (base) ctx->loops_src[s] = (double*)at(o); }
     { size_t o = c.take(lb); if (base) ctx->acc_corr = (double*)at(o); }
@@ -75,6 +77,15 @@ int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
     ctx->g.V = V;
     ctx->g.Vh = (int)(V / 2);
     ctx->g.theta = t_boundary;
+    {   // traversal slabs: the largest divisor of Lz that is <= 8 z-planes
+        Geom& g = ctx->g;
+        g.S = g.Lxh * dims[1];
+        g.bz = 1;
+        for (int b = 1; b <= 8 && b <= dims[2]; b++)
+            if (dims[2] % b == 0) g.bz = b;
+        g.dLxh = make_fastdiv(g.Lxh); g.dLy = make_fastdiv(dims[1]); g.dLz = make_fastdiv(dims[2]);
+        g.dS = make_fastdiv(g.S); g.dSB = make_fastdiv(g.bz * g.S); g.dLt = make_fastdiv(dims[3]);
+    }
     ctx->device = device;
     ctx->stream = 0;
     ctx->have_params = ctx->have_gauge = ctx->have_ws = false;
@@ -270,23 +281,23 @@ int tsm_dslash(tsm_ctx* ctx, int op, int prec, int nrhs, const void* dev_in, voi
     const TwistCoef R = {1, a, 1, -a}, Rinv = {n, -a * n, n, a * n}, Rb = {1, -a, 1, a}, Rbinv = {n, a * n, n, -a * n};
     const TwistCoef mk2 = {-k * k, 0, -k * k, 0}, mk = {-k, 0, -k, 0};
     switch (op) {
-        case TSM_OP_D_EO: return launch_dslash(ctx, prec, 0, false, nrhs, dev_in, nullptr, dev_out, {zero, one}, nullptr, 0);
-        case TSM_OP_D_OE: return launch_dslash(ctx, prec, 1, false, nrhs, dev_in, nullptr, dev_out, {zero, one}, nullptr, 0);
+        case TSM_OP_D_EO: return launch_dslash(ctx, prec, 0, false, nrhs, dev_in, nullptr, dev_out, {zero, one}, 0);
+        case TSM_OP_D_OE: return launch_dslash(ctx, prec, 1, false, nrhs, dev_in, nullptr, dev_out, {zero, one}, 0);
         case TSM_OP_MHAT:
-            rc = launch_dslash(ctx, prec, 1, false, nrhs, dev_in, nullptr, ctx->vec[4], {zero, Rinv}, nullptr, 0);
+            rc = launch_dslash(ctx, prec, 1, false, nrhs, dev_in, nullptr, ctx->vec[4], {zero, Rinv}, 0);
             if (rc) return rc;
-            return launch_dslash(ctx, prec, 0, false, nrhs, ctx->vec[4], dev_in, dev_out, {R, mk2}, nullptr, 0);
+            return launch_dslash(ctx, prec, 0, false, nrhs, ctx->vec[4], dev_in, dev_out, {R, mk2}, 0);
         case TSM_OP_MHAT_DAG:
-            rc = launch_dslash(ctx, prec, 1, true, nrhs, dev_in, nullptr, ctx->vec[4], {zero, Rbinv}, nullptr, 0);
+            rc = launch_dslash(ctx, prec, 1, true, nrhs, dev_in, nullptr, ctx->vec[4], {zero, Rbinv}, 0);
             if (rc) return rc;
-            return launch_dslash(ctx, prec, 0, true, nrhs, ctx->vec[4], dev_in, dev_out, {Rb, mk2}, nullptr, 0);
+            return launch_dslash(ctx, prec, 0, true, nrhs, ctx->vec[4], dev_in, dev_out, {Rb, mk2}, 0);
         case TSM_OP_M_FULL: {
             const size_t fp = field_bytes(prec, ctx->g.Vh, nrhs);
             const char* in_e = (const char*)dev_in; const char* in_o = in_e + fp;
             char* out_e = (char*)dev_out; char* out_o = out_e + fp;
-            rc = launch_dslash(ctx, prec, 0, false, nrhs, in_o, in_e, out_e, {R, mk}, nullptr, 0);
+            rc = launch_dslash(ctx, prec, 0, false, nrhs, in_o, in_e, out_e, {R, mk}, 0);
             if (rc) return rc;
-            return launch_dslash(ctx, prec, 1, false, nrhs, in_e, in_o, out_o, {R, mk}, nullptr, 0);
+            return launch_dslash(ctx, prec, 1, false, nrhs, in_e, in_o, out_o, {R, mk}, 0);
         }
         default: return tsm_fail(ctx, TSM_EINVAL, "bad dslash op");
     }

@@ -28,13 +28,15 @@ Twists make_twists(const tsm_ctx* ctx)
 }
 
 // One CG iteration on Mhat^dag Mhat (O5): four stencil launches and two fused BLAS launches.
+// Re<p,q> = <p, Mhat^dag Mhat p> is taken as |Mhat p|^2 = |w|^2 from the epilogue of the second
+// stencil launch (same number up to rounding; saves re-reading p), summed in k_cg_update_xr.
 int cg_iteration(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, void* r, void* p, void* q, void* w, void* t, double tol)
 {
     int rc;
-    if ((rc = launch_dslash(ctx, prec, 1, false, nrhs, p, nullptr, t, {tw.zero, tw.Rinv}, nullptr, 2))) return rc;   // t = R^-1 D_oe p
-    if ((rc = launch_dslash(ctx, prec, 0, false, nrhs, t, p, w, {tw.R, tw.mk2}, nullptr, 2))) return rc;             // w = Mhat p
-    if ((rc = launch_dslash(ctx, prec, 1, true, nrhs, w, nullptr, t, {tw.zero, tw.Rbinv}, nullptr, 2))) return rc;   // t = Rb^-1 D_oe^dag w
-    if ((rc = launch_dslash(ctx, prec, 0, true, nrhs, t, w, q, {tw.Rb, tw.mk2}, p, 3))) return rc;                   // q = Mhat^dag w; <p,q>
+    if ((rc = launch_dslash(ctx, prec, 1, false, nrhs, p, nullptr, t, {tw.zero, tw.Rinv}, 2))) return rc;   // t = R^-1 D_oe p
+    if ((rc = launch_dslash(ctx, prec, 0, false, nrhs, t, p, w, {tw.R, tw.mk2}, 3))) return rc;             // w = Mhat p; |w|^2 per tile
+    if ((rc = launch_dslash(ctx, prec, 1, true, nrhs, w, nullptr, t, {tw.zero, tw.Rbinv}, 2))) return rc;   // t = Rb^-1 D_oe^dag w
+    if ((rc = launch_dslash(ctx, prec, 0, true, nrhs, t, w, q, {tw.Rb, tw.mk2}, 2))) return rc;             // q = Mhat^dag w
     if ((rc = launch_cg_update_xr(ctx, prec, nrhs, x, p, r, q, tol))) return rc;
     return launch_cg_update_p(ctx, prec, nrhs, p, r);
 }
@@ -61,8 +63,8 @@ int true_residuals(tsm_ctx* ctx, int slot, double* out)
     if ((rc = launch_noise(ctx, TSM_F64, nrhs, ctx->slot_seed[slot], ctx->ids_dev + slot * TSM_MAX_NRHS, ctx->slot_kind[slot], eta))) return rc;
     const Twists tw = make_twists(ctx);
     const TwistCoef mk = {-ctx->kappa, 0, -ctx->kappa, 0};
-    if ((rc = launch_dslash(ctx, TSM_F64, 0, false, nrhs, s64 + fb, s64, ms, {tw.R, mk}, nullptr, 0))) return rc;
-    if ((rc = launch_dslash(ctx, TSM_F64, 1, false, nrhs, s64, s64 + fb, ms + fb, {tw.R, mk}, nullptr, 0))) return rc;
+    if ((rc = launch_dslash(ctx, TSM_F64, 0, false, nrhs, s64 + fb, s64, ms, {tw.R, mk}, 0))) return rc;
+    if ((rc = launch_dslash(ctx, TSM_F64, 1, false, nrhs, s64, s64 + fb, ms + fb, {tw.R, mk}, 0))) return rc;
     if ((rc = launch_diff_norm2(ctx, nrhs, eta, ms))) return rc;
     if ((rc = fetch_scalars(ctx))) return rc;
     const double eta2 = 12.0 * (double)ctx->g.V;   // |eta_{alpha c}(x)| = 1 for Z4 and Z2
@@ -110,9 +112,9 @@ int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs,
     if ((rc = launch_noise(ctx, sp, nrhs, seed, ids_dev, kind, s_e))) return rc;
     // H4: bhat = eta_e + kappa D_eo R^-1 eta_o (into w);  b' = Mhat^dag bhat (into r)
     if ((rc = launch_twist(ctx, sp, nrhs, s_o, aux, tw.Rinv))) return rc;
-    if ((rc = launch_dslash(ctx, sp, 0, false, nrhs, aux, s_e, w, {tw.one, tw.k}, nullptr, 0))) return rc;
-    if ((rc = launch_dslash(ctx, sp, 1, true, nrhs, w, nullptr, t, {tw.zero, tw.Rbinv}, nullptr, 0))) return rc;
-    if ((rc = launch_dslash(ctx, sp, 0, true, nrhs, t, w, r, {tw.Rb, tw.mk2}, nullptr, 0))) return rc;
+    if ((rc = launch_dslash(ctx, sp, 0, false, nrhs, aux, s_e, w, {tw.one, tw.k}, 0))) return rc;
+    if ((rc = launch_dslash(ctx, sp, 1, true, nrhs, w, nullptr, t, {tw.zero, tw.Rbinv}, 0))) return rc;
+    if ((rc = launch_dslash(ctx, sp, 0, true, nrhs, t, w, r, {tw.Rb, tw.mk2}, 0))) return rc;
     // O5: x0 = 0 (x lives in the slot's even half), r0 = p0 = b'
     void* x = s_e;
     if ((rc = launch_cg_init(ctx, prec, nrhs, r, p, x))) return rc;
@@ -126,7 +128,7 @@ int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs,
         }
     }
     // H7: s_e = x, s_o = R^-1 (eta_o + kappa D_oe x)
-    if ((rc = launch_dslash(ctx, sp, 1, false, nrhs, x, s_o, aux, {tw.Rinv, tw.kRinv}, nullptr, 0))) return rc;
+    if ((rc = launch_dslash(ctx, sp, 1, false, nrhs, x, s_o, aux, {tw.Rinv, tw.kRinv}, 0))) return rc;
     TSM_CUDA(ctx, cudaMemcpyAsync(s_o, aux, field_bytes(sp, Vh, nrhs), cudaMemcpyDeviceToDevice, ctx->stream));
     TSM_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
     if ((rc = fetch_scalars(ctx))) return rc;

@@ -64,13 +64,25 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_init(const int Vh, const int nrh
 template <int PV, int PP>
 __global__ void __launch_bounds__(BLAS_BS) k_cg_update_xr(const int Vh, const int nrhs, void* __restrict__ x_, const void* __restrict__ p_,
                                                           void* __restrict__ r_, const void* __restrict__ q_, const double tol,
+                                                          const double* __restrict__ norm_partials, const int ntiles,
                                                           double* __restrict__ partials, CgScalars* cg)
 {
     using TV = typename PT<PV>::real;
     using TP = typename PT<PP>::real;
     if (cg->all_done) return;
     const int rhs = blockIdx.y;
-    const double rr = cg->rr[rhs], pq = cg->pq[rhs];
+    __shared__ double smem[32];
+    __shared__ double pq_s;
+    // Re<p,q> = |Mhat p|^2: every block sums the stencil's per-tile partials of its source in the same
+    // fixed order (the partials sit in L2), so all blocks -- and any batch composition -- agree bit for bit.
+    {
+        double v = 0;
+        for (int k = threadIdx.x; k < ntiles; k += BLAS_BS) v += __ldcg(norm_partials + (size_t)rhs * ntiles + k);
+        v = block_sum_all(v, smem);
+        if (threadIdx.x == 0) { pq_s = v; if (blockIdx.x == 0) cg->pq[rhs] = v; }
+        __syncthreads();
+    }
+    const double rr = cg->rr[rhs], pq = pq_s;
     const bool frozen = cg->done[rhs] != 0;
     const bool breakdown = !(pq > 0) || !isfinite(pq) || !(rr > 0) || !isfinite(rr);   // A13
     double sum = 0;
@@ -99,7 +111,6 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_update_xr(const int Vh, const in
             store8<PV>(r, Vh, i, k8, rv);
         }
     }
-    __shared__ double smem[32];
     const double tot = block_sum_all(sum, smem);
     if (threadIdx.x == 0) partials[(size_t)rhs * gridDim.x + blockIdx.x] = tot;
     if (last_block_arrive(&cg->ticket)) {
@@ -189,7 +200,7 @@ int launch_cg_update_xr(tsm_ctx* ctx, int prec, int nrhs, void* x, const void* p
     const dim3 grid = blas_grid(ctx, nrhs);
     if ((size_t)grid.x * nrhs > ctx->partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
     const int pi = prof_begin(ctx, prec, 3, nrhs);
-    BLAS_SWITCH(prec, (k_cg_update_xr<PV, PP><<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, nrhs, x, p, r, q, tol, ctx->partials, ctx->cg)));
+    BLAS_SWITCH(prec, (k_cg_update_xr<PV, PP><<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, nrhs, x, p, r, q, tol, ctx->norm_partials, ctx->norm_ntiles, ctx->partials, ctx->cg)));
     prof_end(ctx, pi);
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());

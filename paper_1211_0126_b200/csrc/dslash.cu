@@ -8,10 +8,10 @@
 // 1 + 2 i kappa mu gamma5 is never a separate pass).  Spin projection to 2 spin x 3 colour happens
 // before the SU(3) multiply (C3); the time-boundary phase is applied in-kernel (A22).
 //
-// One thread owns one output site of one source.  blockDim = (BS sites, RY sources): the warps
+// One thread owns one output site of one source.  blockDim = (128 sites, RY sources): the warps
 // of a block that differ only in the source index read the same link vectors, so links are
-// fetched from HBM once per block and served from L1 for the other sources.
-#include "reduce.cuh"
+// fetched once per block and served from L1 for the other sources.
+#include "tsm_internal.cuh"
 
 namespace {
 
@@ -97,29 +97,37 @@ template <int PREC> struct DslashCfg {
     static constexpr int MAXT = (PREC == TSM_F64) ? 256 : 512;   // threads per block: 255 regs (fp64) / 128 regs (fp32)
 };
 
-// DOT: 0 none, 1: partial sums of Re<y, out>, last block leaves the totals in cg->pq[rhs].
-template <int PREC, int RECON, bool DAGGER, bool XPAY, int DOT>
+constexpr int TILE = 128;   // sites per tile = blockDim.x
+
+// Persistent kernel: gridDim.x resident blocks sweep the work items w = tile * gy + group in order,
+// so the whole chip works on one narrow front of the traversal (tiles) and the gy source groups of a
+// tile run next to each other in time (their link fetches meet in L2).  gridDim.x is a multiple of gy.
+// NORM: the block also leaves sum |out|^2 of its tile, per source, in partials[rhs * ntiles + tile]
+// (fixed tree, no atomics: the same value whatever the batch composition, A14/A19).
+template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM>
 __global__ void __launch_bounds__(DslashCfg<PREC>::MAXT, 1)
-k_dslash(const Geom g, const int par, const int nrhs, const void* __restrict__ pack, const void* __restrict__ in_,
-         const void* __restrict__ x_, void* __restrict__ out_, const DslashCoef cf, const void* __restrict__ y_,
-         double* __restrict__ partials, CgScalars* __restrict__ cg, const int check_done)
+k_dslash(const Geom g, const int par, const int gy, const int ntiles, const void* __restrict__ pack,
+         const void* __restrict__ in_, const void* __restrict__ x_, void* __restrict__ out_, const DslashCoef cf,
+         double* __restrict__ partials, const CgScalars* __restrict__ cg, const int check_done)
 {
     using T = typename PT<PREC>::real;
     if (check_done && cg->all_done) return;
-    const int rhs = blockIdx.y * blockDim.y + threadIdx.y;
     const int Vh = g.Vh;
     const size_t fb = field_bytes(PREC, Vh, 1);
-    const char* in = (const char*)in_ + fb * rhs;
-    const char* xin = XPAY ? (const char*)x_ + fb * rhs : nullptr;
-    const char* yin = DOT ? (const char*)y_ + fb * rhs : nullptr;
-    char* out = (char*)out_ + fb * rhs;
     const T cxur = (T)cf.x.up_re, cxui = (T)cf.x.up_im, cxlr = (T)cf.x.lo_re, cxli = (T)cf.x.lo_im;
     const T cdur = (T)cf.d.up_re, cdui = (T)cf.d.up_im, cdlr = (T)cf.d.lo_re, cdli = (T)cf.d.lo_im;
-    double dot = 0.0;
+    __shared__ double smem[NORM ? 32 * 4 : 1];
 
-    if (rhs < nrhs) {
-        for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < Vh; i += gridDim.x * blockDim.x) {
-            const SiteCoord s = decode_site(g, i, par);
+    for (int w = blockIdx.x; w < ntiles * gy; w += gridDim.x) {
+        const int tile = w / gy, group = w - tile * gy;
+        const int rhs = group * blockDim.y + threadIdx.y;
+        const char* in = (const char*)in_ + fb * rhs;
+        char* out = (char*)out_ + fb * rhs;
+        const int v = tile * TILE + threadIdx.x;
+        double nrm = 0.0;
+        if (v < Vh) {
+            SiteCoord s;
+            const int i = traverse_site(g, v, par, s);
             int nb[8];
             neighbours(g, i, s, nb);
             const T ph_f = (s.t == g.L[3] - 1) ? (T)g.theta : (T)1;
@@ -140,7 +148,7 @@ k_dslash(const Geom g, const int par, const int nrhs, const void* __restrict__ p
             }
             if (XPAY) {
                 T xv[24];
-                load_spinor<PREC>(xin, Vh, i, xv);
+                load_spinor<PREC>((const char*)x_ + fb * rhs, Vh, i, xv);
 #pragma unroll
                 for (int q = 0; q < 12; q++) {
                     const T cr = (q < 6) ? cxur : cxlr, ci = (q < 6) ? cxui : cxli;
@@ -149,90 +157,100 @@ k_dslash(const Geom g, const int par, const int nrhs, const void* __restrict__ p
                 }
             }
             store_spinor<PREC>(out, Vh, i, o);
-            if (DOT) {
-                T yv[24];
-                load_spinor<PREC>(yin, Vh, i, yv);
+            if (NORM) {
+                if (PREC == TSM_BF16) {   // the norm of what was stored, i.e. of the vector the solver uses
+                    T ob[24];
 #pragma unroll
-                for (int k = 0; k < 24; k++) dot += (double)yv[k] * (double)o[k];
+                    for (int k8 = 0; k8 < 3; k8++) { const uint4 pk = float_to_bf16x8((const float*)(o + 8 * k8)); bf16x8_to_float(pk, (float*)(ob + 8 * k8)); }
+#pragma unroll
+                    for (int k = 0; k < 24; k++) nrm += (double)ob[k] * (double)ob[k];
+                } else {
+#pragma unroll
+                    for (int k = 0; k < 24; k++) nrm += (double)o[k] * (double)o[k];
+                }
             }
         }
-    }
-    if (DOT) {
-        __shared__ double smem[32 * 8];
-        const double tot = block_row_sum(dot, smem);
-        if (threadIdx.x == 0 && rhs < nrhs) partials[(size_t)rhs * gridDim.x + blockIdx.x] = tot;
-        if (last_block_arrive(&cg->ticket)) {
-            const int flat = threadIdx.y * blockDim.x + threadIdx.x, nwarp = (blockDim.x * blockDim.y) >> 5;
-            for (int r = flat >> 5; r < nrhs; r += nwarp) {
-                const double v = sum_partials_warp(partials, r, gridDim.x);
-                if ((flat & 31) == 0) cg->pq[r] = v;
-            }
+        if (NORM) {
+            const double tot = block_row_sum(nrm, smem);
+            if (threadIdx.x == 0) partials[(size_t)rhs * ntiles + tile] = tot;
         }
     }
 }
 
-template <int PREC, int RECON, bool DAGGER, bool XPAY, int DOT>
-int launch_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void* in, const void* x, void* out,
-             const DslashCoef& c, const void* y, int check_done)
+// resident blocks per SM of each instantiation, queried once
+template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM> int resident_blocks(int threads)
 {
-    // 128 sites x RY sources per block.  The x extent and the x grid do not depend on the batch,
-    // so every source sees the same thread->site map and the same reduction tree in any batch.
-    const int bs = 128;
+    static int cache[5] = {0, 0, 0, 0, 0};   // indexed by blockDim.y
+    const int ry = threads / TILE;
+    if (cache[ry] == 0) {
+        int nb = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_dslash<PREC, RECON, DAGGER, XPAY, NORM>, threads, 0) != cudaSuccess || nb < 1) nb = 1;
+        cache[ry] = nb;
+    }
+    return cache[ry];
+}
+
+template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM>
+int launch_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void* in, const void* x, void* out,
+             const DslashCoef& c, int check_done)
+{
+    // 128 sites x RY sources per block: the RY warps rows read the same link vectors (L1 hits).
     const int max_ry = (PREC == TSM_F64) ? 2 : 4;     // register file: 512 x 128 regs (fp32), 256 x 255 (fp64)
     int ry = 1;
-    if (nrhs % 4 == 0 && max_ry >= 4) ry = 4;          // RY sources share each link fetch through L1
+    if (nrhs % 4 == 0 && max_ry >= 4) ry = 4;
     else if (nrhs % 2 == 0) ry = 2;
-    dim3 block(bs, ry);
+    dim3 block(TILE, ry);
     const int gy = nrhs / ry;
-    int gx = (ctx->g.Vh + bs - 1) / bs;
-    const int cap = ctx->nsm * 8;                     // grid-stride beyond this; keeps the partial count small
-    if (gx > cap) gx = cap;
-    dim3 grid(gx, gy);
-    if (DOT && (size_t)gx * nrhs > ctx->partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
-    const int pi = prof_begin(ctx, PREC, DOT ? 2 : (XPAY ? 1 : 0), nrhs);
-    k_dslash<PREC, RECON, DAGGER, XPAY, DOT><<<grid, block, 0, ctx->stream>>>(ctx->g, par, nrhs, pack, in, x, out, c, y,
-                                                                             ctx->partials, ctx->cg, check_done);
+    const int ntiles = (ctx->g.Vh + TILE - 1) / TILE;
+    long long grid = (long long)ctx->nsm * resident_blocks<PREC, RECON, DAGGER, XPAY, NORM>(TILE * ry);
+    grid -= grid % gy;
+    if (grid < gy) grid = gy;
+    if (grid > (long long)ntiles * gy) grid = (long long)ntiles * gy;
+    if (NORM && (size_t)ntiles * nrhs > ctx->norm_partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
+    const int pi = prof_begin(ctx, PREC, NORM ? 2 : (XPAY ? 1 : 0), nrhs);
+    k_dslash<PREC, RECON, DAGGER, XPAY, NORM><<<(unsigned)grid, block, 0, ctx->stream>>>(ctx->g, par, gy, ntiles, pack, in, x, out, c,
+                                                                                         ctx->norm_partials, ctx->cg, check_done);
     prof_end(ctx, pi);
     ctx->launches++;
+    ctx->norm_ntiles = ntiles;
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;
 }
 
 template <int PREC, int RECON>
 int launch_p(tsm_ctx* ctx, int par, bool dagger, int nrhs, const void* pack, const void* in, const void* x, void* out,
-             const DslashCoef& c, const void* y, int dot_mode, int check_done)
+             const DslashCoef& c, int norm, int check_done)
 {
     const bool xpay = x != nullptr;
-    const int dot = dot_mode != 0;
-#define GO(DG, XP, DT) return launch_t<PREC, RECON, DG, XP, DT>(ctx, par, nrhs, pack, in, x, out, c, y, check_done)
-    if (!dagger && !xpay && !dot) GO(false, false, 0);
-    if (!dagger && xpay && !dot) GO(false, true, 0);
-    if (dagger && !xpay && !dot) GO(true, false, 0);
-    if (dagger && xpay && !dot) GO(true, true, 0);
-    if (dagger && xpay && dot) GO(true, true, 1);
-    if (!dagger && xpay && dot) GO(false, true, 1);
+#define GO(DG, XP, NM) return launch_t<PREC, RECON, DG, XP, NM>(ctx, par, nrhs, pack, in, x, out, c, check_done)
+    if (!dagger && !xpay && !norm) GO(false, false, false);
+    if (!dagger && xpay && !norm) GO(false, true, false);
+    if (dagger && !xpay && !norm) GO(true, false, false);
+    if (dagger && xpay && !norm) GO(true, true, false);
+    if (!dagger && xpay && norm) GO(false, true, true);
 #undef GO
     return tsm_fail(ctx, TSM_EINVAL, "unsupported dslash variant");
 }
 
 }  // namespace
 
-// dot_mode bit 0: Re<dot_y, out> into cg->pq; bit 1: early exit when cg->all_done.
+// mode bit 0: leave per-tile sums of |out|^2 in ctx->partials (the CG's <p, Mhat^dag Mhat p> = |Mhat p|^2);
+// bit 1: early exit when cg->all_done.
 int launch_dslash(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs, const void* in, const void* x,
-                  void* out, const DslashCoef& c, const void* dot_y, int dot_mode)
+                  void* out, const DslashCoef& c, int mode)
 {
-    const int dm = dot_mode & 1, chk = (dot_mode >> 1) & 1;
+    const int nm = mode & 1, chk = (mode >> 1) & 1;
     if (prec == TSM_F64)
-        return launch_p<TSM_F64, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge64[out_parity], in, x, out, c, dot_y, dm, chk);
+        return launch_p<TSM_F64, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge64[out_parity], in, x, out, c, nm, chk);
     if (prec == TSM_F32) {
         if (ctx->recon == 18)
-            return launch_p<TSM_F32, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, dot_y, dm, chk);
-        return launch_p<TSM_F32, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, dot_y, dm, chk);
+            return launch_p<TSM_F32, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
+        return launch_p<TSM_F32, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
     }
     if (prec == TSM_BF16) {
         if (ctx->recon == 18)
-            return launch_p<TSM_BF16, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, dot_y, dm, chk);
-        return launch_p<TSM_BF16, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, dot_y, dm, chk);
+            return launch_p<TSM_BF16, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
+        return launch_p<TSM_BF16, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
     }
     return tsm_fail(ctx, TSM_EINVAL, "bad precision");
 }

@@ -12,6 +12,35 @@
 #include "../../include/tsm.h"
 
 // ------------------------------------------------------------------ geometry (H1)
+// Division by a run-time lattice extent with a precomputed magic number (Granlund-Montgomery,
+// exact for every 32-bit numerator): q = (t + ((n - t) >> 1)) >> (l - 1), t = umulhi(n, m).
+struct FastDiv {
+    unsigned m, l, d;
+#ifdef __CUDACC__
+    __device__ __forceinline__ unsigned div(unsigned n) const
+    {
+        if (l == 0) return n;
+        const unsigned t = __umulhi(n, m);
+        return (t + ((n - t) >> 1)) >> (l - 1);
+    }
+    __device__ __forceinline__ void divmod(unsigned n, unsigned& q, unsigned& r) const
+    {
+        q = div(n);
+        r = n - q * d;
+    }
+#endif
+};
+inline FastDiv make_fastdiv(unsigned d)
+{
+    FastDiv f;
+    f.d = d;
+    unsigned l = 0;
+    while ((1ull << l) < d) l++;
+    f.l = l;
+    f.m = l == 0 ? 0u : (unsigned)(((1ull << 32) * ((1ull << l) - d)) / d + 1);
+    return f;
+}
+
 struct Geom {
     int L[4];      // Lx, Ly, Lz, Lt (all even)
     int Lxh;       // Lx / 2
@@ -19,6 +48,10 @@ struct Geom {
     int Vh;        // V / 2
     long long V;
     int theta;     // time boundary phase, +1 or -1 (A3)
+    // stencil traversal order: z-slabs of bz planes, t sweeping inside a slab
+    int bz;        // z planes per slab (divides Lz)
+    int S;         // Lxh * Ly: cb sites per z plane
+    FastDiv dLxh, dLy, dLz, dS, dSB, dLt;   // SB = bz * S
 };
 
 struct SiteCoord { int xh, y, z, t, rowpar; };
@@ -27,14 +60,29 @@ struct SiteCoord { int xh, y, z, t, rowpar; };
 __device__ __forceinline__ SiteCoord decode_site(const Geom& g, int i, int par)
 {
     SiteCoord s;
-    s.xh = i % g.Lxh;
-    int r = i / g.Lxh;
-    s.y = r % g.L[1];
-    r /= g.L[1];
-    s.z = r % g.L[2];
-    s.t = r / g.L[2];
+    unsigned r, xh, y, z, t;
+    g.dLxh.divmod((unsigned)i, r, xh);
+    g.dLy.divmod(r, r, y);
+    g.dLz.divmod(r, t, z);
+    s.xh = (int)xh; s.y = (int)y; s.z = (int)z; s.t = (int)t;
     s.rowpar = (s.y + s.z + s.t + par) & 1;
     return s;
+}
+
+// Traversal index v in [0, Vh) -> cb index i.  v runs over (z-slab, t, z in slab, y, xh): the sweep
+// goes through all timeslices of one slab of bz z-planes before moving to the next slab, so the
+// +-t neighbours of a site are only bz*S sites away in traversal order (the reuse window that has
+// to stay in L2 is 2*bz*S sites instead of 2*Vsh).  Also returns the coordinates.
+__device__ __forceinline__ int traverse_site(const Geom& g, int v, int par, SiteCoord& s)
+{
+    unsigned q1, r, zb, t, zi, rest, y, xh;
+    g.dSB.divmod((unsigned)v, q1, r);
+    g.dLt.divmod(q1, zb, t);
+    g.dS.divmod(r, zi, rest);
+    g.dLxh.divmod(rest, y, xh);
+    s.xh = (int)xh; s.y = (int)y; s.z = (int)(zb * g.bz + zi); s.t = (int)t;
+    s.rowpar = (s.y + s.z + s.t + par) & 1;
+    return (int)(t * g.Vsh + s.z * g.S + rest);
 }
 
 __device__ __forceinline__ long long lex_of_site(const Geom& g, const SiteCoord& s)
@@ -296,7 +344,7 @@ struct GammaTable {          // Gamma_{alpha, col[alpha]} = i^ph[alpha], all oth
 };
 
 // Optional per-launch timing (tsm_profile): CUDA events on the library's stream around each
-// stencil / BLAS launch.  kind: 0 stencil, 1 stencil+xpay, 2 stencil+xpay+dot, 3 update_xr, 4 update_p.
+// stencil / BLAS launch.  kind: 0 stencil, 1 stencil+xpay, 2 stencil+xpay+norm, 3 update_xr, 4 update_p.
 struct ProfRec { int prec, kind, nrhs; cudaEvent_t a, b; };
 
 struct tsm_ctx {
@@ -320,8 +368,11 @@ struct tsm_ctx {
     int slot_prec[2], slot_nrhs[2], slot_kind[2];
     uint64_t slot_seed[2];
     uint32_t slot_ids[2][TSM_MAX_NRHS];
-    double* partials;                // reduction scratch
+    double* partials;                // reduction scratch of the BLAS / contraction kernels
     size_t partials_count;
+    double* norm_partials;           // [rhs][tile] sums of |out|^2 left by the stencil's NORM epilogue
+    size_t norm_partials_count;
+    int norm_ntiles;
     double* loops_src[2];            // per-source loops of a slot [rhs][n_ops][T][2]
     double* acc_corr;                // [n_ops][T][2]
     double* acc_lp;
@@ -375,7 +426,7 @@ inline int tsm_fail(tsm_ctx* ctx, int code, const char* msg)
 
 // ------------------------------------------------------------------ launchers (defined in the .cu files)
 int launch_dslash(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs, const void* in, const void* x,
-                  void* out, const DslashCoef& c, const void* dot_y, int dot_mode);
+                  void* out, const DslashCoef& c, int mode);
 int launch_twist(tsm_ctx* ctx, int prec, int nrhs, const void* in, void* out, const TwistCoef& c);
 int launch_gauge_pack(tsm_ctx* ctx, double* max_dev_out);
 int launch_pack_spinor(tsm_ctx* ctx, int prec, int nrhs, const double* dev_lex, void* dev_native);
