@@ -28,9 +28,10 @@
  *     default stream).  Calls that return host scalars or arrays synchronise that stream
  *     before returning; calls that only take dev_* pointers are asynchronous.
  *   - "Native layout" of a single-parity spinor field with V_h = V/2 sites, nrhs sources:
- *       [rhs][chunk][cb] of 16-byte vectors; fp64: 12 chunks of double2 (one complex each,
- *       q = 3*alpha + c); fp32: 6 chunks of float4 (complex q = 2*chunk, 2*chunk+1);
- *       bf16: 3 chunks of 8 x bf16 (complex q = 4*chunk .. 4*chunk+3);
+ *       [rhs][block of 32 cb sites][chunk][site in block] of 16-byte vectors (V_h is padded up
+ *       to a multiple of 32; the padding is never read or written); fp64: 12 chunks of double2
+ *       (one complex each, q = 3*alpha + c); fp32: 6 chunks of float4 (complex q = 2*chunk,
+ *       2*chunk+1); bf16: 3 chunks of 8 x bf16 (complex q = 4*chunk .. 4*chunk+3);
  *       cb = lex >> 1 is the checkerboard index, parity = (x+y+z+t) & 1 (H1).
  *       A full-lattice field is [parity 0,1] of those.  tsm_field_bytes() gives sizes.
  *   - Error behaviour: wrong-state calls (no workspace / gauge / params yet) -> TSM_ESTATE;
@@ -94,7 +95,7 @@ int tsm_set_gauge(tsm_ctx* ctx, const double* host_links, int reconstruct, doubl
  * (parity-test hook; the solver generates its sources itself). */
 int tsm_noise(tsm_ctx* ctx, uint64_t seed, uint32_t source_id, int kind, double* host_out);
 
-/* Host lex fp64 [nrhs][V][4][3][2]  <->  device native full-lattice field [parity][rhs][chunk][cb]. */
+/* Host lex fp64 [nrhs][V][4][3][2]  <->  device native full-lattice field [parity][rhs][block][chunk][site]. */
 int tsm_pack(tsm_ctx* ctx, int prec, int nrhs, const double* host_lex, void* dev_native);
 int tsm_unpack(tsm_ctx* ctx, int prec, int nrhs, const void* dev_native, double* host_lex);
 

@@ -25,16 +25,17 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_init(const int Vh, const int nrh
     char* x = (char*)x_ + field_bytes(PV, Vh, 1) * rhs;
     char* p = (char*)p_ + field_bytes(PP, Vh, 1) * rhs;
     double sum = 0;
-    const int n = 3 * Vh;
+    const int n = 3 * (int)padded_sites(Vh);
     for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += gridDim.x * blockDim.x) {
-        const int k8 = idx / Vh, i = idx - k8 * Vh;
+        const int k8 = (idx >> 5) % 3, i = (idx >> 5) / 3 * LB + (idx & 31);   // (layout block, k8, site in block)
+        if (i >= Vh) continue;
         TV rv[8], z[8];
         TP pv[8];
-        load8<PV>(r, Vh, i, k8, rv);
+        load8<PV>(r, i, k8, rv);
 #pragma unroll
         for (int k = 0; k < 8; k++) { sum += (double)rv[k] * (double)rv[k]; pv[k] = (TP)rv[k]; z[k] = 0; }
-        store8<PP>(p, Vh, i, k8, pv);
-        store8<PV>(x, Vh, i, k8, z);
+        store8<PP>(p, i, k8, pv);
+        store8<PV>(x, i, k8, z);
     }
     __shared__ double smem[32];
     const double tot = block_sum_all(sum, smem);
@@ -92,23 +93,24 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_update_xr(const int Vh, const in
         char* r = (char*)r_ + field_bytes(PV, Vh, 1) * rhs;
         const char* q = (const char*)q_ + field_bytes(PV, Vh, 1) * rhs;
         const char* p = (const char*)p_ + field_bytes(PP, Vh, 1) * rhs;
-        const int n = 3 * Vh;
+        const int n = 3 * (int)padded_sites(Vh);
         for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += gridDim.x * blockDim.x) {
-            const int k8 = idx / Vh, i = idx - k8 * Vh;
+            const int k8 = (idx >> 5) % 3, i = (idx >> 5) / 3 * LB + (idx & 31);
+            if (i >= Vh) continue;
             TV xv[8], rv[8], qv[8];
             TP pv[8];
-            load8<PV>(x, Vh, i, k8, xv);
-            load8<PP>(p, Vh, i, k8, pv);
-            load8<PV>(r, Vh, i, k8, rv);
-            load8<PV>(q, Vh, i, k8, qv);
+            load8<PV>(x, i, k8, xv);
+            load8<PP>(p, i, k8, pv);
+            load8<PV>(r, i, k8, rv);
+            load8<PV>(q, i, k8, qv);
 #pragma unroll
             for (int k = 0; k < 8; k++) {
                 xv[k] += alpha * (TV)pv[k];
                 rv[k] -= alpha * qv[k];
                 sum += (double)rv[k] * (double)rv[k];
             }
-            store8<PV>(x, Vh, i, k8, xv);
-            store8<PV>(r, Vh, i, k8, rv);
+            store8<PV>(x, i, k8, xv);
+            store8<PV>(r, i, k8, rv);
         }
     }
     const double tot = block_sum_all(sum, smem);
@@ -151,23 +153,24 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_update_p(const int Vh, void* __r
     const TV beta = (TV)cg->beta[rhs];
     char* p = (char*)p_ + field_bytes(PP, Vh, 1) * rhs;
     const char* r = (const char*)r_ + field_bytes(PV, Vh, 1) * rhs;
-    const int n = 3 * Vh;
+    const int n = 3 * (int)padded_sites(Vh);
     for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += gridDim.x * blockDim.x) {
-        const int k8 = idx / Vh, i = idx - k8 * Vh;
+        const int k8 = (idx >> 5) % 3, i = (idx >> 5) / 3 * LB + (idx & 31);   // (layout block, k8, site in block)
+        if (i >= Vh) continue;
         TV rv[8];
         TP pv[8];
-        load8<PV>(r, Vh, i, k8, rv);
-        load8<PP>(p, Vh, i, k8, pv);
+        load8<PV>(r, i, k8, rv);
+        load8<PP>(p, i, k8, pv);
 #pragma unroll
         for (int k = 0; k < 8; k++) pv[k] = (TP)(rv[k] + beta * (TV)pv[k]);
-        store8<PP>(p, Vh, i, k8, pv);
+        store8<PP>(p, i, k8, pv);
     }
 }
 
 inline dim3 blas_grid(const tsm_ctx* ctx, int nrhs)
 {
     // the x grid does not depend on nrhs: same thread->element map and reduction tree in any batch (A14)
-    long long gx = (3LL * ctx->g.Vh + BLAS_BS - 1) / BLAS_BS;
+    long long gx = (3LL * padded_sites(ctx->g.Vh) + BLAS_BS - 1) / BLAS_BS;
     const long long cap = (long long)ctx->nsm * 4;
     if (gx > cap) gx = cap;
     return dim3((unsigned)gx, (unsigned)nrhs);
@@ -219,18 +222,23 @@ int launch_cg_update_p(tsm_ctx* ctx, int prec, int nrhs, void* p, const void* r)
 }
 
 namespace {
-// full-lattice fp64 fields [parity][rhs][12][cb] double2; one block row per source
-__global__ void __launch_bounds__(BLAS_BS) k_diff_norm2(const int Vh, const int nrhs, const double2* __restrict__ a,
-                                                        const double2* __restrict__ b, double* __restrict__ partials, CgScalars* cg)
+// |a - b|^2 per source over full-lattice fp64 native fields [parity][rhs]; one block row per source
+__global__ void __launch_bounds__(BLAS_BS) k_diff_norm2(const int Vh, const int nrhs, const void* __restrict__ a,
+                                                        const void* __restrict__ b, double* __restrict__ partials, CgScalars* cg)
 {
     const int rhs = blockIdx.y;
-    const size_t n = (size_t)12 * Vh;
+    const int n = 3 * (int)padded_sites(Vh);
     double sum = 0;
     for (int par = 0; par < 2; par++) {
-        const size_t base = ((size_t)par * nrhs + rhs) * n;
-        for (size_t idx = blockIdx.x * (size_t)blockDim.x + threadIdx.x; idx < n; idx += (size_t)gridDim.x * blockDim.x) {
-            const double2 u = a[base + idx], v = b[base + idx];
-            sum += (u.x - v.x) * (u.x - v.x) + (u.y - v.y) * (u.y - v.y);
+        const size_t off = field_bytes(TSM_F64, Vh, nrhs) * par + field_bytes(TSM_F64, Vh, 1) * rhs;
+        for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += gridDim.x * blockDim.x) {
+            const int k8 = (idx >> 5) % 3, i = (idx >> 5) / 3 * LB + (idx & 31);
+            if (i >= Vh) continue;
+            double u[8], v[8];
+            load8<TSM_F64>((const char*)a + off, i, k8, u);
+            load8<TSM_F64>((const char*)b + off, i, k8, v);
+#pragma unroll
+            for (int k = 0; k < 8; k++) sum += (u[k] - v[k]) * (u[k] - v[k]);
         }
     }
     __shared__ double smem[32];
@@ -248,7 +256,7 @@ __global__ void __launch_bounds__(BLAS_BS) k_diff_norm2(const int Vh, const int 
 int launch_diff_norm2(tsm_ctx* ctx, int nrhs, const void* a, const void* b)
 {
     const dim3 grid = blas_grid(ctx, nrhs);
-    k_diff_norm2<<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, nrhs, (const double2*)a, (const double2*)b, ctx->partials, ctx->cg);
+    k_diff_norm2<<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, nrhs, a, b, ctx->partials, ctx->cg);
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;

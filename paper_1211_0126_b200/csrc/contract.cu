@@ -43,20 +43,20 @@ __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs
         const uint32_t bits = noise_bits(lex_of_site(g, sc), seed, sid, kind);
         T v[24];
         if (!DERIV) {
-            load_spinor<PREC>(s_same, Vh, i, v);
+            load_spinor<PREC>(s_same, i, v);
         } else {
             int nb[8];
             neighbours(g, i, sc, nb);
             T uf[18], ub[18], sf[24], sb[24], a[6], b[6];
             // runtime mu: the four directions are four block groups of the same launch
             switch (mu) {
-                case 0: load_link_pair<PREC, RECON>(pack, Vh, i, 0, uf, ub); break;
-                case 1: load_link_pair<PREC, RECON>(pack, Vh, i, 1, uf, ub); break;
-                case 2: load_link_pair<PREC, RECON>(pack, Vh, i, 2, uf, ub); break;
-                default: load_link_pair<PREC, RECON>(pack, Vh, i, 3, uf, ub); break;
+                case 0: load_link_pair<PREC, RECON>(pack, i, 0, uf, ub); break;
+                case 1: load_link_pair<PREC, RECON>(pack, i, 1, uf, ub); break;
+                case 2: load_link_pair<PREC, RECON>(pack, i, 2, uf, ub); break;
+                default: load_link_pair<PREC, RECON>(pack, i, 3, uf, ub); break;
             }
-            load_spinor<PREC>(s_other, Vh, nb[2 * mu], sf);
-            load_spinor<PREC>(s_other, Vh, nb[2 * mu + 1], sb);
+            load_spinor<PREC>(s_other, nb[2 * mu], sf);
+            load_spinor<PREC>(s_other, nb[2 * mu + 1], sb);
             const T ph_f = (mu == 3 && sc.t == g.L[3] - 1) ? (T)g.theta : (T)1;
             const T ph_b = (mu == 3 && sc.t == 0) ? (T)g.theta : (T)1;
 #pragma unroll

@@ -65,15 +65,15 @@ template <typename T, int MU, int SGN> __device__ __forceinline__ void accumulat
 }
 
 template <int PREC, int RECON, bool DAGGER, int MU>
-__device__ __forceinline__ void hop_direction(const void* pack, const void* in, int Vh, int i, const int* nb,
+__device__ __forceinline__ void hop_direction(const void* pack, const void* in, int i, const int* nb,
                                               typename PT<PREC>::real ph_f, typename PT<PREC>::real ph_b,
                                               typename PT<PREC>::real* acc)
 {
     using T = typename PT<PREC>::real;
     constexpr int SF = DAGGER ? +1 : -1;   // forward hop carries (1 - g_mu), dagger swaps
     T uf[18], ub[18], psi[24], h[12], gq[12];
-    load_link_pair<PREC, RECON>(pack, Vh, i, MU, uf, ub);
-    load_spinor<PREC>(in, Vh, nb[2 * MU], psi);
+    load_link_pair<PREC, RECON>(pack, i, MU, uf, ub);
+    load_spinor<PREC>(in, nb[2 * MU], psi);
     project<T, MU, SF>(psi, h);
     if (MU == 3) {
 #pragma unroll
@@ -82,7 +82,7 @@ __device__ __forceinline__ void hop_direction(const void* pack, const void* in, 
     su3_mul(uf, h, gq);
     su3_mul(uf, h + 6, gq + 6);
     accumulate<T, MU, SF>(gq, acc);
-    load_spinor<PREC>(in, Vh, nb[2 * MU + 1], psi);
+    load_spinor<PREC>(in, nb[2 * MU + 1], psi);
     project<T, MU, -SF>(psi, h);
     if (MU == 3) {
 #pragma unroll
@@ -135,10 +135,10 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const void
             T acc[24];
 #pragma unroll
             for (int k = 0; k < 24; k++) acc[k] = 0;
-            hop_direction<PREC, RECON, DAGGER, 0>(pack, in, Vh, i, nb, ph_f, ph_b, acc);
-            hop_direction<PREC, RECON, DAGGER, 1>(pack, in, Vh, i, nb, ph_f, ph_b, acc);
-            hop_direction<PREC, RECON, DAGGER, 2>(pack, in, Vh, i, nb, ph_f, ph_b, acc);
-            hop_direction<PREC, RECON, DAGGER, 3>(pack, in, Vh, i, nb, ph_f, ph_b, acc);
+            hop_direction<PREC, RECON, DAGGER, 0>(pack, in, i, nb, ph_f, ph_b, acc);
+            hop_direction<PREC, RECON, DAGGER, 1>(pack, in, i, nb, ph_f, ph_b, acc);
+            hop_direction<PREC, RECON, DAGGER, 2>(pack, in, i, nb, ph_f, ph_b, acc);
+            hop_direction<PREC, RECON, DAGGER, 3>(pack, in, i, nb, ph_f, ph_b, acc);
             T o[24];
 #pragma unroll
             for (int q = 0; q < 12; q++) {
@@ -148,7 +148,7 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const void
             }
             if (XPAY) {
                 T xv[24];
-                load_spinor<PREC>((const char*)x_ + fb * rhs, Vh, i, xv);
+                load_spinor<PREC>((const char*)x_ + fb * rhs, i, xv);
 #pragma unroll
                 for (int q = 0; q < 12; q++) {
                     const T cr = (q < 6) ? cxur : cxlr, ci = (q < 6) ? cxui : cxli;
@@ -156,7 +156,7 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const void
                     o[2 * q + 1] += cr * xv[2 * q + 1] + ci * xv[2 * q];
                 }
             }
-            store_spinor<PREC>(out, Vh, i, o);
+            store_spinor<PREC>(out, i, o);
             if (NORM) {
                 if (PREC == TSM_BF16) {   // the norm of what was stored, i.e. of the vector the solver uses
                     T ob[24];

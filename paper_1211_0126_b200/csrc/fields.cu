@@ -52,8 +52,8 @@ __global__ void k_gauge_pack(const Geom g, const int recon, const double* __rest
         const SiteCoord s = decode_site(g, i, par);
         const long long lex = lex_of_site(g, s);
         const int x[4] = {2 * s.xh + s.rowpar, s.y, s.z, s.t};
-        double2* p64 = reinterpret_cast<double2*>(par ? pack64_1 : pack64_0);
-        float4* p32 = reinterpret_cast<float4*>(par ? pack32_1 : pack32_0);
+        char* p64 = site_ptr<72>(par ? pack64_1 : pack64_0, i);
+        char* p32 = recon == 18 ? site_ptr<36>(par ? pack32_1 : pack32_0, i) : site_ptr<24>(par ? pack32_1 : pack32_0, i);
         for (int mu = 0; mu < 4; mu++) {
             int xm[4] = {x[0], x[1], x[2], x[3]};
             xm[mu] = (x[mu] + g.L[mu] - 1) % g.L[mu];
@@ -69,18 +69,18 @@ __global__ void k_gauge_pack(const Geom g, const int recon, const double* __rest
                 }
             dev = fmax(dev, unitarity_dev(f));
             for (int j = 0; j < 9; j++) {
-                p64[(size_t)(18 * mu + j) * Vh + i] = make_double2(f[2 * j], f[2 * j + 1]);
-                p64[(size_t)(18 * mu + 9 + j) * Vh + i] = make_double2(b[2 * j], b[2 * j + 1]);
+                *reinterpret_cast<double2*>(p64 + (18 * mu + j) * LB_ROW) = make_double2(f[2 * j], f[2 * j + 1]);
+                *reinterpret_cast<double2*>(p64 + (18 * mu + 9 + j) * LB_ROW) = make_double2(b[2 * j], b[2 * j + 1]);
             }
             if (recon == 18) {
                 float l[36];
                 for (int k = 0; k < 18; k++) { l[k] = (float)f[k]; l[18 + k] = (float)b[k]; }
                 for (int j = 0; j < 9; j++)
-                    p32[(size_t)(9 * mu + j) * Vh + i] = make_float4(l[4 * j], l[4 * j + 1], l[4 * j + 2], l[4 * j + 3]);
+                    *reinterpret_cast<float4*>(p32 + (9 * mu + j) * LB_ROW) = make_float4(l[4 * j], l[4 * j + 1], l[4 * j + 2], l[4 * j + 3]);
             } else {
                 for (int j = 0; j < 3; j++) {
-                    p32[(size_t)(6 * mu + j) * Vh + i] = make_float4((float)f[4 * j], (float)f[4 * j + 1], (float)f[4 * j + 2], (float)f[4 * j + 3]);
-                    p32[(size_t)(6 * mu + 3 + j) * Vh + i] = make_float4((float)b[4 * j], (float)b[4 * j + 1], (float)b[4 * j + 2], (float)b[4 * j + 3]);
+                    *reinterpret_cast<float4*>(p32 + (6 * mu + j) * LB_ROW) = make_float4((float)f[4 * j], (float)f[4 * j + 1], (float)f[4 * j + 2], (float)f[4 * j + 3]);
+                    *reinterpret_cast<float4*>(p32 + (6 * mu + 3 + j) * LB_ROW) = make_float4((float)b[4 * j], (float)b[4 * j + 1], (float)b[4 * j + 2], (float)b[4 * j + 3]);
                 }
             }
         }
@@ -104,7 +104,7 @@ __global__ void k_pack_spinor(const Geom g, const int nrhs, const double* __rest
 #pragma unroll
         for (int k = 0; k < 24; k++) v[k] = (T)src[k];
         char* dst = (char*)native + field_bytes(PREC, Vh, nrhs) * par + field_bytes(PREC, Vh, 1) * rhs;
-        store_spinor<PREC>(dst, Vh, i, v);
+        store_spinor<PREC>(dst, i, v);
     }
 }
 
@@ -121,7 +121,7 @@ __global__ void k_unpack_spinor(const Geom g, const int nrhs, const void* __rest
         const SiteCoord s = decode_site(g, i, par);
         const char* src = (const char*)native + field_bytes(PREC, Vh, nrhs) * par + field_bytes(PREC, Vh, 1) * rhs;
         T v[24];
-        load_spinor<PREC>(src, Vh, i, v);
+        load_spinor<PREC>(src, i, v);
         double* dst = lexf + ((size_t)rhs * g.V + lex_of_site(g, s)) * 24;
 #pragma unroll
         for (int k = 0; k < 24; k++) dst[k] = (double)v[k];
@@ -150,7 +150,7 @@ __global__ void k_noise(const Geom g, const int nrhs, const uint64_t seed, const
             v[2 * q + 1] = (T)im;
         }
         char* dst = (char*)native + field_bytes(PREC, Vh, nrhs) * par + field_bytes(PREC, Vh, 1) * rhs;
-        store_spinor<PREC>(dst, Vh, i, v);
+        store_spinor<PREC>(dst, i, v);
     }
 }
 
@@ -166,7 +166,7 @@ __global__ void k_twist(const int Vh, const int nrhs, const void* __restrict__ i
         const int rhs = (int)(tid / (3LL * Vh));
         const size_t off = field_bytes(PREC, Vh, 1) * rhs;
         T v[8], o[8];
-        load8<PREC>((const char*)in + off, Vh, i, k8, v);
+        load8<PREC>((const char*)in + off, i, k8, v);
 #pragma unroll
         for (int j = 0; j < 4; j++) {
             const int q = 4 * k8 + j;
@@ -174,7 +174,7 @@ __global__ void k_twist(const int Vh, const int nrhs, const void* __restrict__ i
             o[2 * j] = cr * v[2 * j] - ci * v[2 * j + 1];
             o[2 * j + 1] = cr * v[2 * j + 1] + ci * v[2 * j];
         }
-        store8<PREC>((char*)out + off, Vh, i, k8, o);
+        store8<PREC>((char*)out + off, i, k8, o);
     }
 }
 
@@ -188,10 +188,10 @@ __global__ void k_convert(const int Vh, const int nfields, const void* __restric
         const int f = (int)(tid / (3LL * Vh));
         typename PT<PIN>::real v[8];
         typename PT<POUT>::real o[8];
-        load8<PIN>((const char*)in + field_bytes(PIN, Vh, 1) * f, Vh, i, k8, v);
+        load8<PIN>((const char*)in + field_bytes(PIN, Vh, 1) * f, i, k8, v);
 #pragma unroll
         for (int k = 0; k < 8; k++) o[k] = (typename PT<POUT>::real)v[k];
-        store8<POUT>((char*)out + field_bytes(POUT, Vh, 1) * f, Vh, i, k8, o);
+        store8<POUT>((char*)out + field_bytes(POUT, Vh, 1) * f, i, k8, o);
     }
 }
 

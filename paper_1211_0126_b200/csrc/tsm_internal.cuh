@@ -124,10 +124,27 @@ template <> struct PT<TSM_BF16> {
     static constexpr int GAUGE_F64 = 0;
 };
 
+// Storage is blocked: 32 consecutive cb sites form a block, inside a block the 16-byte vectors are
+// ordered [chunk][site in block].  A warp still reads 512 contiguous bytes per chunk, a site's
+// chunks sit at COMPILE-TIME offsets (k * 512 B) from one base address (one address computation per
+// site instead of one per vector), and a block is one contiguous piece of memory.  Fields are
+// padded to a whole number of blocks; kernels never touch the padding.
+constexpr int LB = 32;            // sites per layout block
+constexpr int LB_ROW = LB * 16;   // bytes of one chunk row of a block
+__host__ __device__ inline long long padded_sites(long long Vh) { return (Vh + LB - 1) / LB * LB; }
 __host__ __device__ inline size_t field_bytes(int prec, long long Vh, int nrhs)
 {
     const size_t per_site = prec == TSM_F64 ? 192 : (prec == TSM_F32 ? 96 : 48);
-    return per_site * (size_t)Vh * (size_t)nrhs;
+    return per_site * (size_t)padded_sites(Vh) * (size_t)nrhs;
+}
+// address of chunk 0 of site i in a field (or link pack) with NCH chunks per site
+template <int NCH> __device__ __forceinline__ const char* site_ptr(const void* f, int i)
+{
+    return (const char*)f + (size_t)(i >> 5) * (size_t)(NCH * LB_ROW) + (size_t)((i & 31) * 16);
+}
+template <int NCH> __device__ __forceinline__ char* site_ptr(void* f, int i)
+{
+    return (char*)f + (size_t)(i >> 5) * (size_t)(NCH * LB_ROW) + (size_t)((i & 31) * 16);
 }
 __host__ __device__ inline int nchunk_of(int prec) { return prec == TSM_F64 ? 12 : (prec == TSM_F32 ? 6 : 3); }
 
@@ -152,55 +169,55 @@ __device__ __forceinline__ uint4 float_to_bf16x8(const float* o)
 }
 
 // Load / store 8 consecutive reals (reals 8*k8 .. 8*k8+7 of site i) of a field.
-template <int PREC> __device__ __forceinline__ void load8(const void* f, int Vh, int i, int k8, typename PT<PREC>::real* o)
+template <int PREC> __device__ __forceinline__ void load8(const void* f, int i, int k8, typename PT<PREC>::real* o)
 {
+    const char* p = site_ptr<PT<PREC>::NCHUNK>(f, i);
     if constexpr (PREC == TSM_F64) {
-        const double2* p = reinterpret_cast<const double2*>(f) + (size_t)(4 * k8) * Vh + i;
 #pragma unroll
-        for (int j = 0; j < 4; j++) { const double2 v = __ldg(p + (size_t)j * Vh); o[2 * j] = v.x; o[2 * j + 1] = v.y; }
+        for (int j = 0; j < 4; j++) { const double2 v = __ldg(reinterpret_cast<const double2*>(p + (4 * k8 + j) * LB_ROW)); o[2 * j] = v.x; o[2 * j + 1] = v.y; }
     } else if constexpr (PREC == TSM_F32) {
-        const float4* p = reinterpret_cast<const float4*>(f) + (size_t)(2 * k8) * Vh + i;
 #pragma unroll
-        for (int j = 0; j < 2; j++) { const float4 v = __ldg(p + (size_t)j * Vh); o[4 * j] = v.x; o[4 * j + 1] = v.y; o[4 * j + 2] = v.z; o[4 * j + 3] = v.w; }
+        for (int j = 0; j < 2; j++) { const float4 v = __ldg(reinterpret_cast<const float4*>(p + (2 * k8 + j) * LB_ROW)); o[4 * j] = v.x; o[4 * j + 1] = v.y; o[4 * j + 2] = v.z; o[4 * j + 3] = v.w; }
     } else {
-        const uint4 v = __ldg(reinterpret_cast<const uint4*>(f) + (size_t)k8 * Vh + i);
+        const uint4 v = __ldg(reinterpret_cast<const uint4*>(p + k8 * LB_ROW));
         bf16x8_to_float(v, o);
     }
 }
-template <int PREC> __device__ __forceinline__ void store8(void* f, int Vh, int i, int k8, const typename PT<PREC>::real* o)
+template <int PREC> __device__ __forceinline__ void store8(void* f, int i, int k8, const typename PT<PREC>::real* o)
 {
+    char* p = site_ptr<PT<PREC>::NCHUNK>(f, i);
     if constexpr (PREC == TSM_F64) {
-        double2* p = reinterpret_cast<double2*>(f) + (size_t)(4 * k8) * Vh + i;
 #pragma unroll
-        for (int j = 0; j < 4; j++) p[(size_t)j * Vh] = make_double2(o[2 * j], o[2 * j + 1]);
+        for (int j = 0; j < 4; j++) *reinterpret_cast<double2*>(p + (4 * k8 + j) * LB_ROW) = make_double2(o[2 * j], o[2 * j + 1]);
     } else if constexpr (PREC == TSM_F32) {
-        float4* p = reinterpret_cast<float4*>(f) + (size_t)(2 * k8) * Vh + i;
 #pragma unroll
-        for (int j = 0; j < 2; j++) p[(size_t)j * Vh] = make_float4(o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
+        for (int j = 0; j < 2; j++) *reinterpret_cast<float4*>(p + (2 * k8 + j) * LB_ROW) = make_float4(o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
     } else {
-        reinterpret_cast<uint4*>(f)[(size_t)k8 * Vh + i] = float_to_bf16x8(o);
+        *reinterpret_cast<uint4*>(p + k8 * LB_ROW) = float_to_bf16x8(o);
     }
 }
-template <int PREC> __device__ __forceinline__ void load_spinor(const void* f, int Vh, int i, typename PT<PREC>::real* s)
+template <int PREC> __device__ __forceinline__ void load_spinor(const void* f, int i, typename PT<PREC>::real* s)
 {
 #pragma unroll
-    for (int k = 0; k < 3; k++) load8<PREC>(f, Vh, i, k, s + 8 * k);
+    for (int k = 0; k < 3; k++) load8<PREC>(f, i, k, s + 8 * k);
 }
-template <int PREC> __device__ __forceinline__ void store_spinor(void* f, int Vh, int i, const typename PT<PREC>::real* s)
+template <int PREC> __device__ __forceinline__ void store_spinor(void* f, int i, const typename PT<PREC>::real* s)
 {
 #pragma unroll
-    for (int k = 0; k < 3; k++) store8<PREC>(f, Vh, i, k, s + 8 * k);
+    for (int k = 0; k < 3; k++) store8<PREC>(f, i, k, s + 8 * k);
 }
 
 // ------------------------------------------------------------------ gauge packs (H2)
 // For output parity p and cb site i the pack holds 8 matrices, d = 2*mu + b:
 //   b = 0: U_mu(x)          (forward hop)      b = 1: U_mu(x - mu)^dagger (backward hop, stored daggered)
-// fp64: [72][Vh] double2, link d = chunks 9d .. 9d+8 (row-major complex entries).
-// fp32, 18 reals: [36][Vh] float4, direction mu = chunks 9mu .. 9mu+8 = 36 floats (fwd 18, bwd 18).
-// fp32, 12 reals: [24][Vh] float4, link d = chunks 3d .. 3d+2 (rows 0,1; row 2 = conj(row0 x row1)).
+// Same blocked storage as the fields ([block of 32 sites][chunk][site in block] of 16-byte vectors):
+// fp64: 72 chunks of double2, link d = chunks 9d .. 9d+8 (row-major complex entries).
+// fp32, 18 reals: 36 chunks of float4, direction mu = chunks 9mu .. 9mu+8 = 36 floats (fwd 18, bwd 18).
+// fp32, 12 reals: 24 chunks of float4, link d = chunks 3d .. 3d+2 (rows 0,1; row 2 = conj(row0 x row1)).
+__host__ __device__ inline int gauge_nchunk(int f64, int recon) { return f64 ? 72 : (recon == 18 ? 36 : 24); }
 __host__ __device__ inline size_t gauge_pack_bytes(int f64, int recon, long long Vh)
 {
-    return (size_t)Vh * 8 * (f64 ? 18 * 8 : recon * 4);
+    return (size_t)padded_sites(Vh) * 16 * gauge_nchunk(f64, recon);
 }
 
 template <typename T> __device__ __forceinline__ void reconstruct_row2(T* u)
@@ -217,44 +234,54 @@ template <typename T> __device__ __forceinline__ void reconstruct_row2(T* u)
 }
 
 // Loads both links of direction mu for site i: uf = U_mu(x), ub = U_mu(x-mu)^dagger (18 reals each).
-template <int PREC, int RECON> __device__ __forceinline__ void load_link_pair(const void* pack, int Vh, int i, int mu,
+template <int PREC, int RECON> __device__ __forceinline__ void load_link_pair(const void* pack, int i, int mu,
                                                                              typename PT<PREC>::real* uf, typename PT<PREC>::real* ub)
 {
     if constexpr (PT<PREC>::GAUGE_F64) {
-        const double2* p = reinterpret_cast<const double2*>(pack) + (size_t)(18 * mu) * Vh + i;
+        const char* p = site_ptr<72>(pack, i) + (18 * mu) * LB_ROW;
 #pragma unroll
-        for (int j = 0; j < 9; j++) { const double2 v = __ldcs(p + (size_t)j * Vh); uf[2 * j] = v.x; uf[2 * j + 1] = v.y; }
+        for (int j = 0; j < 9; j++) { const double2 v = __ldcs(reinterpret_cast<const double2*>(p + j * LB_ROW)); uf[2 * j] = v.x; uf[2 * j + 1] = v.y; }
 #pragma unroll
-        for (int j = 0; j < 9; j++) { const double2 v = __ldcs(p + (size_t)(9 + j) * Vh); ub[2 * j] = v.x; ub[2 * j + 1] = v.y; }
+        for (int j = 0; j < 9; j++) { const double2 v = __ldcs(reinterpret_cast<const double2*>(p + (9 + j) * LB_ROW)); ub[2 * j] = v.x; ub[2 * j + 1] = v.y; }
     } else if constexpr (RECON == 18) {
-        const float4* p = reinterpret_cast<const float4*>(pack) + (size_t)(9 * mu) * Vh + i;
+        const char* p = site_ptr<36>(pack, i) + (9 * mu) * LB_ROW;
         float l[36];
 #pragma unroll
-        for (int j = 0; j < 9; j++) { const float4 v = __ldcs(p + (size_t)j * Vh); l[4 * j] = v.x; l[4 * j + 1] = v.y; l[4 * j + 2] = v.z; l[4 * j + 3] = v.w; }
+        for (int j = 0; j < 9; j++) { const float4 v = __ldcs(reinterpret_cast<const float4*>(p + j * LB_ROW)); l[4 * j] = v.x; l[4 * j + 1] = v.y; l[4 * j + 2] = v.z; l[4 * j + 3] = v.w; }
 #pragma unroll
         for (int j = 0; j < 18; j++) { uf[j] = l[j]; ub[j] = l[18 + j]; }
     } else {
-        const float4* p = reinterpret_cast<const float4*>(pack) + (size_t)(6 * mu) * Vh + i;
+        const char* p = site_ptr<24>(pack, i) + (6 * mu) * LB_ROW;
 #pragma unroll
-        for (int j = 0; j < 3; j++) { const float4 v = __ldcs(p + (size_t)j * Vh); uf[4 * j] = v.x; uf[4 * j + 1] = v.y; uf[4 * j + 2] = v.z; uf[4 * j + 3] = v.w; }
+        for (int j = 0; j < 3; j++) { const float4 v = __ldcs(reinterpret_cast<const float4*>(p + j * LB_ROW)); uf[4 * j] = v.x; uf[4 * j + 1] = v.y; uf[4 * j + 2] = v.z; uf[4 * j + 3] = v.w; }
 #pragma unroll
-        for (int j = 0; j < 3; j++) { const float4 v = __ldcs(p + (size_t)(3 + j) * Vh); ub[4 * j] = v.x; ub[4 * j + 1] = v.y; ub[4 * j + 2] = v.z; ub[4 * j + 3] = v.w; }
+        for (int j = 0; j < 3; j++) { const float4 v = __ldcs(reinterpret_cast<const float4*>(p + (3 + j) * LB_ROW)); ub[4 * j] = v.x; ub[4 * j + 1] = v.y; ub[4 * j + 2] = v.z; ub[4 * j + 3] = v.w; }
         reconstruct_row2(uf);
         reconstruct_row2(ub);
     }
 }
 
-// out[c] (+)= sum_c' U[c][c'] h[c'] for one spin row (3 complex), U 18 reals row-major.
+__device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
+
+// o[c] = sum_c' U[c][c'] h[c'] for one spin row (3 complex), U 18 reals row-major; explicit FMA
+// chains (12 per complex output: the compiler does not contract "x += a*b - c*d" into two FMAs).
 template <typename T> __device__ __forceinline__ void su3_mul(const T* u, const T* h, T* o)
 {
 #pragma unroll
     for (int c = 0; c < 3; c++) {
-        T re = u[6 * c] * h[0] - u[6 * c + 1] * h[1];
-        T im = u[6 * c] * h[1] + u[6 * c + 1] * h[0];
-        re += u[6 * c + 2] * h[2] - u[6 * c + 3] * h[3];
-        im += u[6 * c + 2] * h[3] + u[6 * c + 3] * h[2];
-        re += u[6 * c + 4] * h[4] - u[6 * c + 5] * h[5];
-        im += u[6 * c + 4] * h[5] + u[6 * c + 5] * h[4];
+        T re = u[6 * c] * h[0];
+        T im = u[6 * c] * h[1];
+        re = fma_(-u[6 * c + 1], h[1], re);
+        im = fma_(u[6 * c + 1], h[0], im);
+        re = fma_(u[6 * c + 2], h[2], re);
+        im = fma_(u[6 * c + 2], h[3], im);
+        re = fma_(-u[6 * c + 3], h[3], re);
+        im = fma_(u[6 * c + 3], h[2], im);
+        re = fma_(u[6 * c + 4], h[4], re);
+        im = fma_(u[6 * c + 4], h[5], im);
+        re = fma_(-u[6 * c + 5], h[5], re);
+        im = fma_(u[6 * c + 5], h[4], im);
         o[2 * c] = re;
         o[2 * c + 1] = im;
     }
