@@ -185,7 +185,7 @@ def run_ours(args, wl):
     peak, peak_src = measured_peaks()
     prec_name = wl.lp_prec if wl.lp_prec != "bf16" else "f32"   # bf16 solver not built yet: see DESIGN.md
     prec = PRECS[prec_name]
-    nrhs = wl.nrhs
+    nrhs = args.nrhs if args.nrhs > 0 else wl.nrhs
     tol, iters = wl.lp_tol, wl.lp_iters
 
     t0 = time.perf_counter()
@@ -272,7 +272,7 @@ def run_ours(args, wl):
 def extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U):
     """e2e through the host-buffer API, single-launch stencil table, full loop set, oracle baseline."""
     out = {}
-    nrhs = wl.nrhs
+    nrhs = args.nrhs if args.nrhs > 0 else wl.nrhs
     stream = torch.cuda.current_stream()
     # ---- e2e: host gauge field in, host loops out, every step
     n_e2e = max(1, min(args.steps, 3))
@@ -345,6 +345,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", type=int, default=5)
+    ap.add_argument("--nrhs", type=int, default=0, help="sources per batch (default: the workload's; other values are profiling aids, not the headline)")
     ap.add_argument("--skip-extras", action="store_true", help="only the timed steps (no e2e/table/full set/oracle)")
     ap.add_argument("--no-full-set", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
