@@ -11,58 +11,11 @@
 // One thread owns one output site of one source.  blockDim = (128 sites, RY sources): the warps
 // of a block that differ only in the source index read the same link vectors, so links are
 // fetched once per block and served from L1 for the other sources.
-#include "tsm_internal.cuh"
+#include <cstdlib>
+
+#include "dslash_common.cuh"
 
 namespace {
-
-template <typename T, int MU, int SGN> __device__ __forceinline__ void project(const T* p, T* h)
-{
-    // h = psi_up + SGN * a_mu psi_low, gamma_mu = [[0, a_mu], [a_mu^dag, 0]] (C3)
-    constexpr T s = (T)SGN;
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-        const T p0r = p[2 * c], p0i = p[2 * c + 1], p1r = p[6 + 2 * c], p1i = p[6 + 2 * c + 1];
-        const T p2r = p[12 + 2 * c], p2i = p[12 + 2 * c + 1], p3r = p[18 + 2 * c], p3i = p[18 + 2 * c + 1];
-        if (MU == 0) {          // a_0 = -i sigma_x
-            h[2 * c] = p0r + s * p3i;      h[2 * c + 1] = p0i - s * p3r;
-            h[6 + 2 * c] = p1r + s * p2i;  h[6 + 2 * c + 1] = p1i - s * p2r;
-        } else if (MU == 1) {   // a_1 = -i sigma_y = [[0,-1],[1,0]]
-            h[2 * c] = p0r - s * p3r;      h[2 * c + 1] = p0i - s * p3i;
-            h[6 + 2 * c] = p1r + s * p2r;  h[6 + 2 * c + 1] = p1i + s * p2i;
-        } else if (MU == 2) {   // a_2 = -i sigma_z = diag(-i, i)
-            h[2 * c] = p0r + s * p2i;      h[2 * c + 1] = p0i - s * p2r;
-            h[6 + 2 * c] = p1r - s * p3i;  h[6 + 2 * c + 1] = p1i + s * p3r;
-        } else {                // a_3 = 1
-            h[2 * c] = p0r + s * p2r;      h[2 * c + 1] = p0i + s * p2i;
-            h[6 + 2 * c] = p1r + s * p3r;  h[6 + 2 * c + 1] = p1i + s * p3i;
-        }
-    }
-}
-
-template <typename T, int MU, int SGN> __device__ __forceinline__ void accumulate(const T* g, T* acc)
-{
-    // acc_up += g, acc_low += SGN * a_mu^dag g
-    constexpr T s = (T)SGN;
-#pragma unroll
-    for (int k = 0; k < 12; k++) acc[k] += g[k];
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-        const T g0r = g[2 * c], g0i = g[2 * c + 1], g1r = g[6 + 2 * c], g1i = g[6 + 2 * c + 1];
-        if (MU == 0) {          // a_0^dag = i sigma_x
-            acc[12 + 2 * c] -= s * g1i;  acc[12 + 2 * c + 1] += s * g1r;
-            acc[18 + 2 * c] -= s * g0i;  acc[18 + 2 * c + 1] += s * g0r;
-        } else if (MU == 1) {   // a_1^dag = [[0,1],[-1,0]]
-            acc[12 + 2 * c] += s * g1r;  acc[12 + 2 * c + 1] += s * g1i;
-            acc[18 + 2 * c] -= s * g0r;  acc[18 + 2 * c + 1] -= s * g0i;
-        } else if (MU == 2) {   // a_2^dag = diag(i, -i)
-            acc[12 + 2 * c] -= s * g0i;  acc[12 + 2 * c + 1] += s * g0r;
-            acc[18 + 2 * c] += s * g1i;  acc[18 + 2 * c + 1] -= s * g1r;
-        } else {
-            acc[12 + 2 * c] += s * g0r;  acc[12 + 2 * c + 1] += s * g0i;
-            acc[18 + 2 * c] += s * g1r;  acc[18 + 2 * c + 1] += s * g1i;
-        }
-    }
-}
 
 template <int PREC, int RECON, bool DAGGER, int MU>
 __device__ __forceinline__ void hop_direction(const void* pack, const void* in, int i, const int* nb,
@@ -104,7 +57,9 @@ constexpr int TILE = 128;   // sites per tile = blockDim.x
 // tile run next to each other in time (their link fetches meet in L2).  gridDim.x is a multiple of gy.
 // NORM: the block also leaves sum |out|^2 of its tile, per source, in partials[rhs * ntiles + tile]
 // (fixed tree, no atomics: the same value whatever the batch composition, A14/A19).
-template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM>
+// POUT: storage precision of `out` (differs from PREC only for the last stencil of a bf16 CG
+// iteration, whose result q is kept in fp32).
+template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM, int POUT>
 __global__ void __launch_bounds__(DslashCfg<PREC>::MAXT, 1)
 k_dslash(const Geom g, const int par, const int gy, const int ntiles, const void* __restrict__ pack,
          const void* __restrict__ in_, const void* __restrict__ x_, void* __restrict__ out_, const DslashCoef cf,
@@ -113,7 +68,7 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const void
     using T = typename PT<PREC>::real;
     if (check_done && cg->all_done) return;
     const int Vh = g.Vh;
-    const size_t fb = field_bytes(PREC, Vh, 1);
+    const size_t fb = field_bytes(PREC, Vh, 1), fbo = field_bytes(POUT, Vh, 1);
     const T cxur = (T)cf.x.up_re, cxui = (T)cf.x.up_im, cxlr = (T)cf.x.lo_re, cxli = (T)cf.x.lo_im;
     const T cdur = (T)cf.d.up_re, cdui = (T)cf.d.up_im, cdlr = (T)cf.d.lo_re, cdli = (T)cf.d.lo_im;
     __shared__ double smem[NORM ? 32 * 4 : 1];
@@ -122,7 +77,7 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const void
         const int tile = w / gy, group = w - tile * gy;
         const int rhs = group * blockDim.y + threadIdx.y;
         const char* in = (const char*)in_ + fb * rhs;
-        char* out = (char*)out_ + fb * rhs;
+        char* out = (char*)out_ + fbo * rhs;
         const int v = tile * TILE + threadIdx.x;
         double nrm = 0.0;
         if (v < Vh) {
@@ -156,9 +111,9 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const void
                     o[2 * q + 1] += cr * xv[2 * q + 1] + ci * xv[2 * q];
                 }
             }
-            store_spinor<PREC>(out, i, o);
+            store_spinor<POUT>(out, i, o);
             if (NORM) {
-                if (PREC == TSM_BF16) {   // the norm of what was stored, i.e. of the vector the solver uses
+                if (POUT == TSM_BF16) {   // the norm of what was stored, i.e. of the vector the solver uses
                     T ob[24];
 #pragma unroll
                     for (int k8 = 0; k8 < 3; k8++) { const uint4 pk = float_to_bf16x8((const float*)(o + 8 * k8)); bf16x8_to_float(pk, (float*)(ob + 8 * k8)); }
@@ -178,19 +133,19 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const void
 }
 
 // resident blocks per SM of each instantiation, queried once
-template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM> int resident_blocks(int threads)
+template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM, int POUT> int resident_blocks(int threads)
 {
     static int cache[5] = {0, 0, 0, 0, 0};   // indexed by blockDim.y
     const int ry = threads / TILE;
     if (cache[ry] == 0) {
         int nb = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_dslash<PREC, RECON, DAGGER, XPAY, NORM>, threads, 0) != cudaSuccess || nb < 1) nb = 1;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_dslash<PREC, RECON, DAGGER, XPAY, NORM, POUT>, threads, 0) != cudaSuccess || nb < 1) nb = 1;
         cache[ry] = nb;
     }
     return cache[ry];
 }
 
-template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM>
+template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM, int POUT>
 int launch_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void* in, const void* x, void* out,
              const DslashCoef& c, int check_done)
 {
@@ -202,13 +157,13 @@ int launch_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void* in, 
     dim3 block(TILE, ry);
     const int gy = nrhs / ry;
     const int ntiles = (ctx->g.Vh + TILE - 1) / TILE;
-    long long grid = (long long)ctx->nsm * resident_blocks<PREC, RECON, DAGGER, XPAY, NORM>(TILE * ry);
+    long long grid = (long long)ctx->nsm * resident_blocks<PREC, RECON, DAGGER, XPAY, NORM, POUT>(TILE * ry);
     grid -= grid % gy;
     if (grid < gy) grid = gy;
     if (grid > (long long)ntiles * gy) grid = (long long)ntiles * gy;
     if (NORM && (size_t)ntiles * nrhs > ctx->norm_partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
     const int pi = prof_begin(ctx, PREC, NORM ? 2 : (XPAY ? 1 : 0), nrhs);
-    k_dslash<PREC, RECON, DAGGER, XPAY, NORM><<<(unsigned)grid, block, 0, ctx->stream>>>(ctx->g, par, gy, ntiles, pack, in, x, out, c,
+    k_dslash<PREC, RECON, DAGGER, XPAY, NORM, POUT><<<(unsigned)grid, block, 0, ctx->stream>>>(ctx->g, par, gy, ntiles, pack, in, x, out, c,
                                                                                          ctx->norm_partials, ctx->cg, check_done);
     prof_end(ctx, pi);
     ctx->launches++;
@@ -219,10 +174,16 @@ int launch_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void* in, 
 
 template <int PREC, int RECON>
 int launch_p(tsm_ctx* ctx, int par, bool dagger, int nrhs, const void* pack, const void* in, const void* x, void* out,
-             const DslashCoef& c, int norm, int check_done)
+             const DslashCoef& c, int norm, int check_done, int out32)
 {
     const bool xpay = x != nullptr;
-#define GO(DG, XP, NM) return launch_t<PREC, RECON, DG, XP, NM>(ctx, par, nrhs, pack, in, x, out, c, check_done)
+    if constexpr (PREC == TSM_BF16) {
+        if (out32) {
+            if (dagger && xpay && !norm) return launch_t<PREC, RECON, true, true, false, TSM_F32>(ctx, par, nrhs, pack, in, x, out, c, check_done);
+            return tsm_fail(ctx, TSM_EINVAL, "unsupported dslash variant (fp32 output)");
+        }
+    }
+#define GO(DG, XP, NM) return launch_t<PREC, RECON, DG, XP, NM, PREC>(ctx, par, nrhs, pack, in, x, out, c, check_done)
     if (!dagger && !xpay && !norm) GO(false, false, false);
     if (!dagger && xpay && !norm) GO(false, true, false);
     if (dagger && !xpay && !norm) GO(true, false, false);
@@ -234,23 +195,33 @@ int launch_p(tsm_ctx* ctx, int par, bool dagger, int nrhs, const void* pack, con
 
 }  // namespace
 
+// Which fp32 batches go to the shared-memory-staged kernel of dslash_tile.cu (TSM_TILE=0 turns it off,
+// TSM_TILE=2 sends single sources there as well: tuning aids).
+static bool tile_stencil_enabled(int nrhs)
+{
+    const char* e = getenv("TSM_TILE");   // TUNING: read on every call
+    const int mode = e ? atoi(e) : 1;
+    return mode == 2 || (mode == 1 && nrhs >= 2);
+}
+
 // mode bit 0: leave per-tile sums of |out|^2 in ctx->partials (the CG's <p, Mhat^dag Mhat p> = |Mhat p|^2);
-// bit 1: early exit when cg->all_done.
+// bit 1: early exit when cg->all_done; bit 2 (bf16 storage only): `out` is an fp32 field.
 int launch_dslash(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs, const void* in, const void* x,
                   void* out, const DslashCoef& c, int mode)
 {
-    const int nm = mode & 1, chk = (mode >> 1) & 1;
+    const int nm = mode & 1, chk = (mode >> 1) & 1, o32 = (mode >> 2) & 1;
+    if ((prec == TSM_F32 || prec == TSM_BF16) && tile_stencil_enabled(nrhs)) return launch_dslash_tile(ctx, prec, out_parity, dagger, nrhs, in, x, out, c, mode);
     if (prec == TSM_F64)
-        return launch_p<TSM_F64, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge64[out_parity], in, x, out, c, nm, chk);
+        return launch_p<TSM_F64, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge64[out_parity], in, x, out, c, nm, chk, o32);
     if (prec == TSM_F32) {
         if (ctx->recon == 18)
-            return launch_p<TSM_F32, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
-        return launch_p<TSM_F32, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
+            return launch_p<TSM_F32, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk, o32);
+        return launch_p<TSM_F32, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk, o32);
     }
     if (prec == TSM_BF16) {
         if (ctx->recon == 18)
-            return launch_p<TSM_BF16, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
-        return launch_p<TSM_BF16, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
+            return launch_p<TSM_BF16, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk, o32);
+        return launch_p<TSM_BF16, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk, o32);
     }
     return tsm_fail(ctx, TSM_EINVAL, "bad precision");
 }

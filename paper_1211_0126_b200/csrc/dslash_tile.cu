@@ -1,0 +1,344 @@
+// dslash_tile.cu -- H5 for batches of sources (fp32 and bf16 storage): the stencil of dslash.cu with
+// the links of a tile staged in shared memory by bulk asynchronous copies (TMA, cp.async.bulk).
+//
+// A persistent CTA owns one tile of 128 output sites at a time and applies the stencil to ALL
+// sources of the batch before it moves on.  The 8 links of the tile's sites are one contiguous
+// piece of the link pack (4 layout blocks x NCH chunks x 512 B = 72 KB with 18 reals, 48 KB with
+// 12): a single cp.async.bulk brings it into shared memory, completion is signalled on an
+// mbarrier, and the copy for the CTA's NEXT tile is issued before the current tile is computed
+// (two buffers), so the only loads that come straight from DRAM are never waited for by the
+// arithmetic.  Every link is then read from HBM/L2 once per tile whatever the batch size, and
+// R sources are handled per thread with the link pair held in registers (R x fewer shared-memory
+// reads, R independent dependency chains).  blockDim = (128 sites, RY source rows); a CTA loops over
+// G = ceil(nrhs / (RY * R)) groups of sources.  Neighbour spinors come through L1/L2 (ld.global.nc).
+//
+// Arithmetic per source is the same sequence of operations as in dslash.cu (same projection,
+// same FMA chains, same accumulation order over mu), so a source's result does not depend on the
+// batch it is in (reading A14).
+#include <cstdlib>
+
+#include "dslash_common.cuh"
+
+namespace {
+
+constexpr int TT = 128;   // sites per tile = blockDim.x = 4 layout blocks
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+// global -> shared bulk copy (TMA engine, SASS UBLKCP); bytes a multiple of 16, both addresses 16-byte aligned
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// both links of direction MU of the thread's site from the staged tile (same layout as the pack)
+template <int RECON, int MU> __device__ __forceinline__ void lds_link_pair(const char* tile_links, int tx, float* uf, float* ub)
+{
+    constexpr int NCH = RECON == 18 ? 36 : 24;
+    const char* p = tile_links + (tx >> 5) * (NCH * LB_ROW) + (tx & 31) * 16;
+    if constexpr (RECON == 18) {
+        float l[36];
+#pragma unroll
+        for (int j = 0; j < 9; j++) {
+            const float4 v = *reinterpret_cast<const float4*>(p + (9 * MU + j) * LB_ROW);
+            l[4 * j] = v.x; l[4 * j + 1] = v.y; l[4 * j + 2] = v.z; l[4 * j + 3] = v.w;
+        }
+#pragma unroll
+        for (int j = 0; j < 18; j++) { uf[j] = l[j]; ub[j] = l[18 + j]; }
+    } else {
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            const float4 v = *reinterpret_cast<const float4*>(p + (6 * MU + j) * LB_ROW);
+            uf[4 * j] = v.x; uf[4 * j + 1] = v.y; uf[4 * j + 2] = v.z; uf[4 * j + 3] = v.w;
+        }
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            const float4 v = *reinterpret_cast<const float4*>(p + (6 * MU + 3 + j) * LB_ROW);
+            ub[4 * j] = v.x; ub[4 * j + 1] = v.y; ub[4 * j + 2] = v.z; ub[4 * j + 3] = v.w;
+        }
+        reconstruct_row2(uf);
+        reconstruct_row2(ub);
+    }
+}
+
+// one direction, R sources: links once, then the forward and the backward hop of every source
+template <int PREC, int RECON, bool DAGGER, int MU, int R>
+__device__ __forceinline__ void hop_direction_r(const char* tile_links, int tx, const char* in, size_t fb, const int* nb, float ph_f,
+                                                float ph_b, float (*acc)[24])
+{
+    constexpr int SF = DAGGER ? +1 : -1;   // forward hop carries (1 - g_mu), dagger swaps
+    float uf[18], ub[18];
+    lds_link_pair<RECON, MU>(tile_links, tx, uf, ub);
+#pragma unroll
+    for (int r = 0; r < R; r++) {
+        float psi[24], h[12], gq[12];
+        load_spinor<PREC>(in + fb * r, nb[2 * MU], psi);
+        project<float, MU, SF>(psi, h);
+        if (MU == 3) {
+#pragma unroll
+            for (int k = 0; k < 12; k++) h[k] *= ph_f;
+        }
+        su3_mul(uf, h, gq);
+        su3_mul(uf, h + 6, gq + 6);
+        accumulate<float, MU, SF>(gq, acc[r]);
+    }
+#pragma unroll
+    for (int r = 0; r < R; r++) {
+        float psi[24], h[12], gq[12];
+        load_spinor<PREC>(in + fb * r, nb[2 * MU + 1], psi);
+        project<float, MU, -SF>(psi, h);
+        if (MU == 3) {
+#pragma unroll
+            for (int k = 0; k < 12; k++) h[k] *= ph_b;
+        }
+        su3_mul(ub, h, gq);
+        su3_mul(ub, h + 6, gq + 6);
+        accumulate<float, MU, -SF>(gq, acc[r]);
+    }
+}
+
+// cb index of the first site of tile `tile`.  With slab traversal (S a multiple of 128) the tiles
+// follow the z-slab / t order of dslash.cu's traverse_site; otherwise plain cb order.  Either way a
+// tile is 128 consecutive cb sites starting at a multiple of 128 (4 whole layout blocks).
+__device__ __forceinline__ int tile_base(const Geom& g, int tile, int slab)
+{
+    const int v0 = tile * TT;
+    if (!slab) return v0;
+    unsigned q1, r, zb, t, zi, rest;
+    g.dSB.divmod((unsigned)v0, q1, r);
+    g.dLt.divmod(q1, zb, t);
+    g.dS.divmod(r, zi, rest);
+    return (int)(t * g.Vsh + (zb * g.bz + zi) * g.S + rest);
+}
+
+template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM, int POUT, int RY, int R>
+__global__ void __launch_bounds__(TT * RY, 1)
+k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, const int slab, const void* __restrict__ pack,
+              const void* __restrict__ in_, const void* __restrict__ x_, void* __restrict__ out_, const DslashCoef cf,
+              double* __restrict__ partials, const CgScalars* __restrict__ cg, const int check_done)
+{
+    constexpr int NCH = RECON == 18 ? 36 : 24;
+    constexpr unsigned TILE_BYTES = 4 * NCH * LB_ROW;
+    extern __shared__ __align__(128) char smem[];
+    __shared__ __align__(8) uint64_t bar[2];
+    __shared__ double red[NORM ? 32 * RY : 1];
+    if (check_done && cg->all_done) return;
+    const int Vh = g.Vh;
+    const int nblocks = (int)(padded_sites(Vh) / LB);
+    const size_t fb = field_bytes(PREC, Vh, 1), fbo = field_bytes(POUT, Vh, 1);
+    const float cxur = (float)cf.x.up_re, cxui = (float)cf.x.up_im, cxlr = (float)cf.x.lo_re, cxli = (float)cf.x.lo_im;
+    const float cdur = (float)cf.d.up_re, cdui = (float)cf.d.up_im, cdlr = (float)cf.d.lo_re, cdli = (float)cf.d.lo_im;
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const bool leader = (tx == 0 && ty == 0);
+
+    auto issue = [&](int tile, int b) {
+        const int i0 = tile_base(g, tile, slab);
+        int nb_ = nblocks - (i0 >> 5);
+        if (nb_ > 4) nb_ = 4;
+        const unsigned bytes = (unsigned)nb_ * NCH * LB_ROW;
+        mbar_expect_tx(&bar[b], bytes);
+        bulk_g2s(smem + (size_t)b * TILE_BYTES, (const char*)pack + (size_t)(i0 >> 5) * (NCH * LB_ROW), bytes, &bar[b]);
+    };
+
+    if (leader) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (leader && (int)blockIdx.x < ntiles) issue(blockIdx.x, 0);
+
+    int it = 0;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
+        const int b = it & 1;
+        // buffer b^1 was last read in iteration it-1, which ended with __syncthreads()
+        if (leader && tile + (int)gridDim.x < ntiles) issue(tile + gridDim.x, b ^ 1);
+        const int i = tile_base(g, tile, slab) + tx;
+        const bool live = i < Vh;
+        SiteCoord s = decode_site(g, live ? i : 0, par);
+        int nb[8];
+        neighbours(g, live ? i : 0, s, nb);
+        const float ph_f = (s.t == g.L[3] - 1) ? (float)g.theta : 1.f;
+        const float ph_b = (s.t == 0) ? (float)g.theta : 1.f;
+        mbar_wait(&bar[b], (unsigned)((it >> 1) & 1));
+        const char* links = smem + (size_t)b * TILE_BYTES;
+
+        for (int grp = 0; grp * RY * R < nrhs; grp++) {
+            const int rhs0 = (grp * RY + ty) * R;
+            const bool act = live && rhs0 < nrhs;      // R divides nrhs: a row is wholly inside or outside
+            double nrm[R];
+#pragma unroll
+            for (int r = 0; r < R; r++) nrm[r] = 0.0;
+            if (act) {
+                const char* in = (const char*)in_ + fb * rhs0;
+                float acc[R][24];
+#pragma unroll
+                for (int r = 0; r < R; r++)
+#pragma unroll
+                    for (int k = 0; k < 24; k++) acc[r][k] = 0.f;
+                hop_direction_r<PREC, RECON, DAGGER, 0, R>(links, tx, in, fb, nb, ph_f, ph_b, acc);
+                hop_direction_r<PREC, RECON, DAGGER, 1, R>(links, tx, in, fb, nb, ph_f, ph_b, acc);
+                hop_direction_r<PREC, RECON, DAGGER, 2, R>(links, tx, in, fb, nb, ph_f, ph_b, acc);
+                hop_direction_r<PREC, RECON, DAGGER, 3, R>(links, tx, in, fb, nb, ph_f, ph_b, acc);
+#pragma unroll
+                for (int r = 0; r < R; r++) {
+                    float o[24];
+#pragma unroll
+                    for (int q = 0; q < 12; q++) {
+                        const float cr = (q < 6) ? cdur : cdlr, ci = (q < 6) ? cdui : cdli;
+                        o[2 * q] = cr * acc[r][2 * q] - ci * acc[r][2 * q + 1];
+                        o[2 * q + 1] = cr * acc[r][2 * q + 1] + ci * acc[r][2 * q];
+                    }
+                    if (XPAY) {
+                        float xv[24];
+                        load_spinor<PREC>((const char*)x_ + fb * (rhs0 + r), i, xv);
+#pragma unroll
+                        for (int q = 0; q < 12; q++) {
+                            const float cr = (q < 6) ? cxur : cxlr, ci = (q < 6) ? cxui : cxli;
+                            o[2 * q] += cr * xv[2 * q] - ci * xv[2 * q + 1];
+                            o[2 * q + 1] += cr * xv[2 * q + 1] + ci * xv[2 * q];
+                        }
+                    }
+                    store_spinor<POUT>((char*)out_ + fbo * (rhs0 + r), i, o);
+                    if (NORM) {
+                        if (POUT == TSM_BF16) {   // the norm of what was stored, i.e. of the vector the solver uses
+                            float ob[24];
+#pragma unroll
+                            for (int k8 = 0; k8 < 3; k8++) { const uint4 pk = float_to_bf16x8(o + 8 * k8); bf16x8_to_float(pk, ob + 8 * k8); }
+#pragma unroll
+                            for (int k = 0; k < 24; k++) nrm[r] += (double)ob[k] * (double)ob[k];
+                        } else {
+#pragma unroll
+                            for (int k = 0; k < 24; k++) nrm[r] += (double)o[k] * (double)o[k];
+                        }
+                    }
+                }
+            }
+            if (NORM) {
+#pragma unroll
+                for (int r = 0; r < R; r++) {
+                    const double tot = block_row_sum(nrm[r], red);
+                    if (tx == 0 && rhs0 < nrhs) partials[(size_t)(rhs0 + r) * ntiles + tile] = tot;
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM, int POUT, int RY, int R>
+int launch_tile_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void* in, const void* x, void* out, const DslashCoef& c,
+                  int check_done)
+{
+    constexpr int NCH = RECON == 18 ? 36 : 24;
+    constexpr size_t SMEM = 2 * 4 * NCH * LB_ROW;
+    auto kern = k_dslash_tile<PREC, RECON, DAGGER, XPAY, NORM, POUT, RY, R>;
+    static unsigned long long attr_done = 0;   // per device
+    if (!((attr_done >> (ctx->device & 63)) & 1ull)) {
+        TSM_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
+        attr_done |= 1ull << (ctx->device & 63);
+    }
+    const Geom& g = ctx->g;
+    const int ntiles = (g.Vh + TT - 1) / TT;
+    const int slab = (g.S % TT == 0) ? 1 : 0;
+    int grid = ctx->nsm;            // one CTA per SM (shared memory: two link buffers)
+    if (grid > ntiles) grid = ntiles;
+    if (NORM && (size_t)ntiles * nrhs > ctx->norm_partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
+    const int pi = prof_begin(ctx, PREC, NORM ? 2 : (XPAY ? 1 : 0), nrhs);
+    kern<<<grid, dim3(TT, RY), SMEM, ctx->stream>>>(g, par, nrhs, ntiles, slab, pack, in, x, out, c, ctx->norm_partials, ctx->cg, check_done);
+    prof_end(ctx, pi);
+    ctx->launches++;
+    ctx->norm_ntiles = ntiles;
+    TSM_CUDA(ctx, cudaGetLastError());
+    return TSM_OK;
+}
+
+template <int PREC, int RECON, int RY, int R>
+int launch_tile_v(tsm_ctx* ctx, int par, bool dagger, int nrhs, const void* pack, const void* in, const void* x, void* out,
+                  const DslashCoef& c, int norm, int check_done, int out32)
+{
+    const bool xpay = x != nullptr;
+    if constexpr (PREC == TSM_BF16) {
+        if (out32) {
+            if (dagger && xpay && !norm)
+                return launch_tile_t<PREC, RECON, true, true, false, TSM_F32, RY, R>(ctx, par, nrhs, pack, in, x, out, c, check_done);
+            return tsm_fail(ctx, TSM_EINVAL, "unsupported dslash variant (fp32 output)");
+        }
+    }
+#define GO(DG, XP, NM) return launch_tile_t<PREC, RECON, DG, XP, NM, PREC, RY, R>(ctx, par, nrhs, pack, in, x, out, c, check_done)
+    if (!dagger && !xpay && !norm) GO(false, false, false);
+    if (!dagger && xpay && !norm) GO(false, true, false);
+    if (dagger && !xpay && !norm) GO(true, false, false);
+    if (dagger && xpay && !norm) GO(true, true, false);
+    if (!dagger && xpay && norm) GO(false, true, true);
+#undef GO
+    return tsm_fail(ctx, TSM_EINVAL, "unsupported dslash variant");
+}
+
+template <int PREC, int RECON>
+int launch_tile_s(tsm_ctx* ctx, int ry, int r, int par, bool dagger, int nrhs, const void* pack, const void* in, const void* x,
+                  void* out, const DslashCoef& c, int norm, int check_done, int out32)
+{
+#define SHAPE(RY_, R_) if (ry == RY_ && r == R_) return launch_tile_v<PREC, RECON, RY_, R_>(ctx, par, dagger, nrhs, pack, in, x, out, c, norm, check_done, out32)
+    SHAPE(4, 1);
+    SHAPE(2, 1);
+    SHAPE(1, 1);
+#undef SHAPE
+    return tsm_fail(ctx, TSM_EINVAL, "unsupported tile shape");
+}
+
+}  // namespace
+
+// Shape of the CTA for a batch of nrhs sources: RY source rows x R sources per thread; R divides nrhs.
+void tile_shape(int nrhs, int& ry, int& r)
+{
+    const char* a = getenv("TSM_TILE_RY");   // TUNING: read on every call while the shapes are being explored
+    const char* b = getenv("TSM_TILE_R");
+    const int env_ry = a ? atoi(a) : 0, env_r = b ? atoi(b) : 0;
+    if (env_ry > 0 && env_r > 0 && nrhs % env_r == 0) { ry = env_ry; r = env_r; return; }
+    if (nrhs == 1) { ry = 1; r = 1; return; }
+    if (nrhs == 2) { ry = 2; r = 1; return; }
+    ry = 4; r = 1;
+}
+
+// fp32 / bf16 storage, any nrhs >= 1.  mode bits as in launch_dslash.
+int launch_dslash_tile(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs, const void* in, const void* x, void* out,
+                       const DslashCoef& c, int mode)
+{
+    const int nm = mode & 1, chk = (mode >> 1) & 1, o32 = (mode >> 2) & 1;
+    int ry, r;
+    tile_shape(nrhs, ry, r);
+    const void* pack = ctx->gauge32[out_parity];
+    if (prec == TSM_F32) {
+        if (ctx->recon == 18) return launch_tile_s<TSM_F32, 18>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk, o32);
+        return launch_tile_s<TSM_F32, 12>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk, o32);
+    }
+    if (prec == TSM_BF16) {
+        if (ctx->recon == 18) return launch_tile_s<TSM_BF16, 18>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk, o32);
+        return launch_tile_s<TSM_BF16, 12>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk, o32);
+    }
+    return tsm_fail(ctx, TSM_EINVAL, "tile stencil: unsupported precision");
+}

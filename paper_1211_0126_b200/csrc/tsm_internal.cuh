@@ -454,6 +454,8 @@ inline int tsm_fail(tsm_ctx* ctx, int code, const char* msg)
 // ------------------------------------------------------------------ launchers (defined in the .cu files)
 int launch_dslash(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs, const void* in, const void* x,
                   void* out, const DslashCoef& c, int mode);
+int launch_dslash_tile(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs, const void* in, const void* x,
+                       void* out, const DslashCoef& c, int mode);
 int launch_twist(tsm_ctx* ctx, int prec, int nrhs, const void* in, void* out, const TwistCoef& c);
 int launch_gauge_pack(tsm_ctx* ctx, double* max_dev_out);
 int launch_pack_spinor(tsm_ctx* ctx, int prec, int nrhs, const double* dev_lex, void* dev_native);
