@@ -4,7 +4,7 @@
 A "step" is one pass of the whole hot path over one batch of noise sources of the
 32^3 x 64 workload (BASELINE.json configs[4], the one `metric` is quoted on): generate
 12 Z4 sources on the device, source preparation, 100 fixed iterations of fp32 even-odd CG
-on Mhat^dag Mhat (4 stencil launches + 2 fused BLAS launches each), reconstruction, local
+on Mhat^dag Mhat (4 stencil launches, 2 one-block reductions and 1 fused BLAS launch each), reconstruction, local
 and one-derivative loop contractions, accumulation into the Eq. 2.4 sums.
 
   value     = LP CG solves/s with the gauge field resident in HBM (device-timed, CUDA events)
@@ -32,6 +32,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+from paper_1211_0126_b200 import replicas  # noqa: E402
 from paper_1211_0126_b200 import workloads as W  # noqa: E402
 
 METRIC = "lp_cg_solves_per_s"
@@ -55,11 +56,16 @@ def measured_peaks():
 def stencil_bytes_per_site(prec: str, recon: int, nrhs: int, kind: int) -> float:
     """SURVEY.md 8(d) / DESIGN.md: compulsory bytes per output site per source of one stencil
     launch: 8 neighbour spinors are each read once per field (24 reals in, 24 out = 48 w_s),
-    8 links of n_g reals shared by the nrhs sources of a batch, +24 w_s for the x term (kinds 1, 2;
-    kind 2 also leaves |out|^2 per tile, which moves no extra field)."""
+    8 links of n_g reals shared by the nrhs sources of a batch, +24 w_s for the x term (kinds 1, 2, 3;
+    kind 2 also leaves |out|^2 per tile, which moves no extra field; kind 3 does not store its
+    result but reads and writes the CG residual r, fp32 when the spinors are bf16)."""
     w_s = {"f64": 8, "f32": 4, "bf16": 2}[prec]
+    w_r = 4 if prec == "bf16" else w_s
     w_g, n_g = (8, 18) if prec == "f64" else (4, recon)
-    return (48 + (24 if kind else 0)) * w_s + 8.0 * n_g * w_g / nrhs
+    links = 8.0 * n_g * w_g / nrhs
+    if kind == 3:
+        return 48 * w_s + 48 * w_r + links
+    return (48 + (24 if kind else 0)) * w_s + links
 
 
 class ClockSampler:
@@ -183,7 +189,7 @@ def run_ours(args, wl):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     peak, peak_src = measured_peaks()
-    prec_name = wl.lp_prec if wl.lp_prec != "bf16" else "f32"   # bf16 solver not built yet: see DESIGN.md
+    prec_name = wl.lp_prec
     prec = PRECS[prec_name]
     nrhs = args.nrhs if args.nrhs > 0 else wl.nrhs
     tol, iters = wl.lp_tol, wl.lp_iters
@@ -199,11 +205,11 @@ def run_ours(args, wl):
     log(f"[bench] unitarity deviation {dev:.2e}; workspace {t.workspace.numel() / 2**30:.1f} GiB")
     t.loops_reset(wl.derivative)
     # replicas only: every rank works on its own, disjoint source ids
-    next_id = [rank * 1_000_000]
+    next_step = [0]
 
     def step():
-        ids = list(range(next_id[0], next_id[0] + nrhs))
-        next_id[0] += nrhs
+        ids = replicas.replica_source_ids(rank, next_step[0], nrhs)
+        next_step[0] += 1
         rc, info = t.solve(wl.noise_seed, ids, prec, tol, iters, slot=1)
         t.loops_add_lp(1)
         return info
@@ -231,23 +237,21 @@ def run_ours(args, wl):
     launches = t.launch_count() - l0
     t.profile(False)
     prof = {k: t.profile_read(prec, k, nrhs) for k in range(5)}
-    if world > 1:
-        tt = torch.tensor([ms], device=f"cuda:{local}", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
-    value = world * nrhs * args.steps / (ms * 1e-3)
+    ms = replicas.max_over_ranks(ms, device=f"cuda:{local}")
+    value = replicas.whole_job_throughput(nrhs, args.steps, ms, world)
 
     # ---- roofline of the stencil kernels inside the timed steps
     Vh = wl.V // 2
-    alg_bytes = sum(stencil_bytes_per_site(prec_name, wl.reconstruct, nrhs, k) * Vh * nrhs * prof[k][1] for k in range(3))
-    st_ms = sum(prof[k][0] for k in range(3))
-    st_n = sum(prof[k][1] for k in range(3))
+    alg_bytes = sum(stencil_bytes_per_site(prec_name, wl.reconstruct, nrhs, k) * Vh * nrhs * prof[k][1] for k in range(4))
+    st_ms = sum(prof[k][0] for k in range(4))
+    st_n = sum(prof[k][1] for k in range(4))
     achieved = alg_bytes / (st_ms * 1e-3) / 1e9 if st_ms > 0 else 0.0
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": None, "peak_source": peak_src, "kernel": f"k_dslash<{prec_name}, recon {wl.reconstruct}> x {nrhs} sources",
                 "launches_timed": st_n, "avg_launch_us": st_ms * 1e3 / max(st_n, 1),
                 "algorithmic_bytes_per_launch": alg_bytes / max(st_n, 1),
-                "share_of_step": {"stencil": st_ms / ms, "cg_update_xr": prof[3][0] / ms, "cg_update_p": prof[4][0] / ms},
+                "share_of_step": {"stencil": st_ms / ms, "cg_update_xp": prof[4][0] / ms},
+                "per_kind_us": {str(k): (prof[k][0] * 1e3 / prof[k][1] if prof[k][1] else None) for k in range(5)},
                 "gflops_at_1320_per_site": 1320.0 * Vh * nrhs * st_n / (st_ms * 1e-3) / 1e9 if st_ms > 0 else 0.0}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

@@ -156,7 +156,8 @@ long long tsm_launch_count(const tsm_ctx* ctx);
  * BLAS launch is bracketed by CUDA events on the library's stream.  tsm_profile_read
  * synchronises, returns the summed duration (ms) and the number of launches recorded so far
  * for one class and forgets them.  prec: TSM_F64/F32/BF16; kind: 0 stencil (H5), 1 stencil
- * with the x term, 2 stencil with x term and per-tile sum of |out|^2, 3 x/r update, 4 p update;
+ * with the x term, 2 stencil with x term and per-tile sum of |out|^2, 3 stencil with x term whose
+ * result updates the CG residual in place (r -= alpha q, per-tile |r|^2), 4 the CG x/p update;
  * nrhs <= 0 matches any batch size. */
 int tsm_profile(tsm_ctx* ctx, int enable);
 int tsm_profile_read(tsm_ctx* ctx, int prec, int kind, int nrhs, double* total_ms, long long* count);

@@ -27,18 +27,20 @@ Twists make_twists(const tsm_ctx* ctx)
     return t;
 }
 
-// One CG iteration on Mhat^dag Mhat (O5): four stencil launches and two fused BLAS launches.
-// Re<p,q> = <p, Mhat^dag Mhat p> is taken as |Mhat p|^2 = |w|^2 from the epilogue of the second
-// stencil launch (same number up to rounding; saves re-reading p), summed in k_cg_update_xr.
-int cg_iteration(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, void* r, void* p, void* q, void* w, void* t, double tol)
+// One CG iteration on Mhat^dag Mhat (O5): four stencil launches, two one-block-per-source reductions and
+// one fused BLAS launch.  Re<p,q> = <p, Mhat^dag Mhat p> is taken as |Mhat p|^2 = |w|^2 from the epilogue of
+// the second stencil launch (same number up to rounding; saves re-reading p and q).  q = Mhat^dag w is never
+// stored: the fourth stencil launch applies r -= alpha q in its epilogue and leaves |r|^2 per tile.
+int cg_iteration(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, void* r, void* p, void* w, void* t, double tol)
 {
     int rc;
     if ((rc = launch_dslash(ctx, prec, 1, false, nrhs, p, nullptr, t, {tw.zero, tw.Rinv}, 2))) return rc;   // t = R^-1 D_oe p
     if ((rc = launch_dslash(ctx, prec, 0, false, nrhs, t, p, w, {tw.R, tw.mk2}, 3))) return rc;             // w = Mhat p; |w|^2 per tile
+    if ((rc = launch_cg_reduce(ctx, 0, nrhs))) return rc;                                                   // alpha
     if ((rc = launch_dslash(ctx, prec, 1, true, nrhs, w, nullptr, t, {tw.zero, tw.Rbinv}, 2))) return rc;   // t = Rb^-1 D_oe^dag w
-    if ((rc = launch_dslash(ctx, prec, 0, true, nrhs, t, w, q, {tw.Rb, tw.mk2}, 2))) return rc;             // q = Mhat^dag w
-    if ((rc = launch_cg_update_xr(ctx, prec, nrhs, x, p, r, q, tol))) return rc;
-    return launch_cg_update_p(ctx, prec, nrhs, p, r);
+    if ((rc = launch_dslash(ctx, prec, 0, true, nrhs, t, w, r, {tw.Rb, tw.mk2}, 6))) return rc;             // r -= alpha Mhat^dag w; |r|^2 per tile
+    if ((rc = launch_cg_reduce(ctx, 1, nrhs))) return rc;                                                   // rr'
+    return launch_cg_update_xp(ctx, prec, nrhs, x, p, r, tol);                                              // x += alpha p; p = r + beta p
 }
 
 int fetch_scalars(tsm_ctx* ctx)
@@ -92,8 +94,9 @@ int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs,
     if (!source_ids || nrhs < 1 || nrhs > ctx->max_nrhs || (kind != TSM_Z4 && kind != TSM_Z2) || prec < 0 || prec > 2 ||
         !(tol >= 0) || max_iter < 0 || slot < 0 || slot > 1)
         return tsm_fail(ctx, TSM_EINVAL, "bad solve arguments");
-    if (prec == TSM_BF16) return tsm_fail(ctx, TSM_EINVAL, "bf16 solves are not built yet");
-    const int sp = prec;   // precision of the stored solution
+    // bf16 storage (config 4): source preparation, x, r, q, reconstruction and the stored solution are
+    // fp32; only the search direction p and the stencil temporaries t, w are bf16 (fp32 arithmetic).
+    const int sp = prec == TSM_BF16 ? TSM_F32 : prec;   // precision of the stored solution
     const int Vh = ctx->g.Vh;
     const Twists tw = make_twists(ctx);
     ctx->slot_prec[slot] = sp;
@@ -107,7 +110,7 @@ int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs,
 
     char* s_e = (char*)ctx->slot[slot];
     char* s_o = s_e + field_bytes(sp, Vh, nrhs);
-    void *r = ctx->vec[0], *p = ctx->vec[1], *q = ctx->vec[2], *w = ctx->vec[3], *t = ctx->vec[4], *aux = ctx->vec[5];
+    void *r = ctx->vec[0], *p = ctx->vec[1], *w = ctx->vec[3], *t = ctx->vec[4], *aux = ctx->vec[5];
     // H3: eta straight into the slot (eta_e where s_e will be, eta_o where s_o will be)
     if ((rc = launch_noise(ctx, sp, nrhs, seed, ids_dev, kind, s_e))) return rc;
     // H4: bhat = eta_e + kappa D_eo R^-1 eta_o (into w);  b' = Mhat^dag bhat (into r)
@@ -120,7 +123,7 @@ int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs,
     if ((rc = launch_cg_init(ctx, prec, nrhs, r, p, x))) return rc;
     const int poll = 4;
     for (int k = 1; k <= max_iter; k++) {
-        if ((rc = cg_iteration(ctx, prec, nrhs, tw, x, r, p, q, w, t, tol))) return rc;
+        if ((rc = cg_iteration(ctx, prec, nrhs, tw, x, r, p, w, t, tol))) return rc;
         if (tol > 0 && (k % poll == 0) && k < max_iter) {
             TSM_CUDA(ctx, cudaMemcpyAsync(&ctx->cg_host->all_done, &ctx->cg->all_done, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
             TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));

@@ -1,9 +1,10 @@
 // blas.cu -- H6: the fused BLAS-1 / reduction kernels of CG on Mhat^dag Mhat (O5).
 //
-// Per iteration, after the four stencil launches (the last of which leaves Re<p,q> in cg->pq):
-//   k_cg_update_xr : alpha = rr/pq; x += alpha p; r -= alpha q; rr' = |r|^2  (one pass, fp64 sums)
-//                    last block: iteration count, stopping test |r|/|b'| <= tol (A8), beta, freeze flags
-//   k_cg_update_p  : p = r + beta p
+// Per iteration (api_solve.cu: cg_iteration):
+//   stencil 2 leaves |w|^2 = Re<p,q> per tile   -> k_cg_reduce(0): alpha = rr / Re<p,q>
+//   stencil 4 does r -= alpha q, |r|^2 per tile  -> k_cg_reduce(1): rr' = |r|^2
+//   k_cg_update_xp : x += alpha p; p = r + (rr'/rr) p   (one pass over x, p, r)
+//                    last block: iteration count, stopping test |r|/|b'| <= tol (A8), freeze flags
 // All scalars stay on the device (CgScalars); every source has its own (A14) and a finished
 // source is frozen: its x, r, p are no longer touched.  Sums are deterministic (A19).
 //
@@ -62,108 +63,86 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_init(const int Vh, const int nrh
     }
 }
 
+// Sum of the per-tile partials a stencil epilogue left for every source (one block per source; the order
+// depends on ntiles only, so a source gets the same sum in any batch, A14/A19), then:
+//   which == 0 (after w = Mhat p, EPI_NORM):  pq = |w|^2 = Re<p,q>;  alpha = rr / pq, or 0 for a frozen
+//              source; 0 / non-finite pq or rr freezes the source and flags TSM_EBREAKDOWN (A13)
+//   which == 1 (after r -= alpha q, EPI_RESID): rr_new = |r|^2
+__global__ void __launch_bounds__(BLAS_BS) k_cg_reduce(const int which, const double* __restrict__ norm_partials, const int ntiles,
+                                                       CgScalars* cg)
+{
+    if (cg->all_done) return;
+    const int rhs = blockIdx.x;
+    __shared__ double smem[32];
+    double v = 0;
+    for (int k = threadIdx.x; k < ntiles; k += BLAS_BS) v += __ldcg(norm_partials + (size_t)rhs * ntiles + k);
+    v = block_sum_all(v, smem);
+    if (threadIdx.x != 0) return;
+    if (which == 1) { cg->rr_new[rhs] = v; return; }
+    cg->pq[rhs] = v;
+    double alpha = 0.0;
+    if (!cg->done[rhs]) {
+        const double rr = cg->rr[rhs];
+        if (!(v > 0) || !isfinite(v) || !(rr > 0) || !isfinite(rr)) {
+            cg->done[rhs] = 1;
+            cg->status[rhs] = TSM_EBREAKDOWN;
+        } else {
+            alpha = rr / v;
+        }
+    }
+    cg->alpha[rhs] = alpha;
+}
+
+// x += alpha p; p = r + beta p with beta = rr_new / rr (one pass: reads x, p, r; writes x, p).  r was already
+// updated by the stencil that produced q (EPI_RESID).  The last block to finish does the per-source
+// bookkeeping of O5: iteration count, rr <- rr_new, the stopping test |r|/|b'| <= tol (A8), freeze flags.
 template <int PV, int PP>
-__global__ void __launch_bounds__(BLAS_BS) k_cg_update_xr(const int Vh, const int nrhs, void* __restrict__ x_, const void* __restrict__ p_,
-                                                          void* __restrict__ r_, const void* __restrict__ q_, const double tol,
-                                                          const double* __restrict__ norm_partials, const int ntiles,
-                                                          double* __restrict__ partials, CgScalars* cg)
+__global__ void __launch_bounds__(BLAS_BS) k_cg_update_xp(const int Vh, const int nrhs, void* __restrict__ x_, void* __restrict__ p_,
+                                                          const void* __restrict__ r_, const double tol, CgScalars* cg)
 {
     using TV = typename PT<PV>::real;
     using TP = typename PT<PP>::real;
     if (cg->all_done) return;
     const int rhs = blockIdx.y;
-    __shared__ double smem[32];
-    __shared__ double pq_s;
-    // Re<p,q> = |Mhat p|^2: every block sums the stencil's per-tile partials of its source in the same
-    // fixed order (the partials sit in L2), so all blocks -- and any batch composition -- agree bit for bit.
-    {
-        double v = 0;
-        for (int k = threadIdx.x; k < ntiles; k += BLAS_BS) v += __ldcg(norm_partials + (size_t)rhs * ntiles + k);
-        v = block_sum_all(v, smem);
-        if (threadIdx.x == 0) { pq_s = v; if (blockIdx.x == 0) cg->pq[rhs] = v; }
-        __syncthreads();
-    }
-    const double rr = cg->rr[rhs], pq = pq_s;
-    const bool frozen = cg->done[rhs] != 0;
-    const bool breakdown = !(pq > 0) || !isfinite(pq) || !(rr > 0) || !isfinite(rr);   // A13
-    double sum = 0;
-    if (!frozen && !breakdown) {
-        const TV alpha = (TV)(rr / pq);
+    if (!cg->done[rhs]) {
+        const TV alpha = (TV)cg->alpha[rhs];
+        const TV beta = (TV)(cg->rr_new[rhs] / cg->rr[rhs]);
         char* x = (char*)x_ + field_bytes(PV, Vh, 1) * rhs;
-        char* r = (char*)r_ + field_bytes(PV, Vh, 1) * rhs;
-        const char* q = (const char*)q_ + field_bytes(PV, Vh, 1) * rhs;
-        const char* p = (const char*)p_ + field_bytes(PP, Vh, 1) * rhs;
+        const char* r = (const char*)r_ + field_bytes(PV, Vh, 1) * rhs;
+        char* p = (char*)p_ + field_bytes(PP, Vh, 1) * rhs;
         const int n = 3 * (int)padded_sites(Vh);
         for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += gridDim.x * blockDim.x) {
-            const int k8 = (idx >> 5) % 3, i = (idx >> 5) / 3 * LB + (idx & 31);
+            const int k8 = (idx >> 5) % 3, i = (idx >> 5) / 3 * LB + (idx & 31);   // (layout block, k8, site in block)
             if (i >= Vh) continue;
-            TV xv[8], rv[8], qv[8];
+            TV xv[8], rv[8];
             TP pv[8];
             load8<PV>(x, i, k8, xv);
             load8<PP>(p, i, k8, pv);
             load8<PV>(r, i, k8, rv);
-            load8<PV>(q, i, k8, qv);
 #pragma unroll
             for (int k = 0; k < 8; k++) {
                 xv[k] += alpha * (TV)pv[k];
-                rv[k] -= alpha * qv[k];
-                sum += (double)rv[k] * (double)rv[k];
+                pv[k] = (TP)(rv[k] + beta * (TV)pv[k]);
             }
             store8<PV>(x, i, k8, xv);
-            store8<PV>(r, i, k8, rv);
+            store8<PP>(p, i, k8, pv);
         }
     }
-    const double tot = block_sum_all(sum, smem);
-    if (threadIdx.x == 0) partials[(size_t)rhs * gridDim.x + blockIdx.x] = tot;
     if (last_block_arrive(&cg->ticket)) {
-        for (int j = threadIdx.x >> 5; j < nrhs; j += BLAS_BS / 32) {
-            const double v = sum_partials_warp(partials, j, gridDim.x);
-            if ((threadIdx.x & 31) == 0) {
-                if (!cg->done[j]) {
-                    const double rr_j = cg->rr[j], pq_j = cg->pq[j];
-                    if (!(pq_j > 0) || !isfinite(pq_j) || !(rr_j > 0) || !isfinite(rr_j)) {
-                        cg->done[j] = 1;
-                        cg->status[j] = TSM_EBREAKDOWN;
-                    } else {
-                        cg->iters[j] += 1;
-                        cg->beta[j] = v / rr_j;
-                        cg->rr[j] = v;
-                        if (tol > 0 && sqrt(v / cg->bb[j]) <= tol) cg->done[j] = 1;
-                    }
-                }
-            }
-        }
-        __syncthreads();
         if (threadIdx.x == 0) {
             int all = 1;
-            for (int j = 0; j < nrhs; j++) all &= cg->done[j];
+            for (int j = 0; j < nrhs; j++) {
+                if (!cg->done[j]) {
+                    const double v = cg->rr_new[j];
+                    cg->iters[j] += 1;
+                    cg->beta[j] = v / cg->rr[j];
+                    cg->rr[j] = v;
+                    if (tol > 0 && sqrt(v / cg->bb[j]) <= tol) cg->done[j] = 1;
+                }
+                all &= cg->done[j];
+            }
             cg->all_done = all;
         }
-    }
-}
-
-template <int PV, int PP>
-__global__ void __launch_bounds__(BLAS_BS) k_cg_update_p(const int Vh, void* __restrict__ p_, const void* __restrict__ r_, const CgScalars* cg)
-{
-    using TV = typename PT<PV>::real;
-    using TP = typename PT<PP>::real;
-    if (cg->all_done) return;
-    const int rhs = blockIdx.y;
-    if (cg->done[rhs]) return;
-    const TV beta = (TV)cg->beta[rhs];
-    char* p = (char*)p_ + field_bytes(PP, Vh, 1) * rhs;
-    const char* r = (const char*)r_ + field_bytes(PV, Vh, 1) * rhs;
-    const int n = 3 * (int)padded_sites(Vh);
-    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += gridDim.x * blockDim.x) {
-        const int k8 = (idx >> 5) % 3, i = (idx >> 5) / 3 * LB + (idx & 31);   // (layout block, k8, site in block)
-        if (i >= Vh) continue;
-        TV rv[8];
-        TP pv[8];
-        load8<PV>(r, i, k8, rv);
-        load8<PP>(p, i, k8, pv);
-#pragma unroll
-        for (int k = 0; k < 8; k++) pv[k] = (TP)(rv[k] + beta * (TV)pv[k]);
-        store8<PP>(p, i, k8, pv);
     }
 }
 
@@ -198,23 +177,19 @@ int launch_cg_init(tsm_ctx* ctx, int prec, int nrhs, const void* r, void* p, voi
     return TSM_OK;
 }
 
-int launch_cg_update_xr(tsm_ctx* ctx, int prec, int nrhs, void* x, const void* p, void* r, const void* q, double tol)
+int launch_cg_reduce(tsm_ctx* ctx, int which, int nrhs)
 {
-    const dim3 grid = blas_grid(ctx, nrhs);
-    if ((size_t)grid.x * nrhs > ctx->partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
-    const int pi = prof_begin(ctx, prec, 3, nrhs);
-    BLAS_SWITCH(prec, (k_cg_update_xr<PV, PP><<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, nrhs, x, p, r, q, tol, ctx->norm_partials, ctx->norm_ntiles, ctx->partials, ctx->cg)));
-    prof_end(ctx, pi);
+    k_cg_reduce<<<nrhs, BLAS_BS, 0, ctx->stream>>>(which, ctx->norm_partials, ctx->norm_ntiles, ctx->cg);
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;
 }
 
-int launch_cg_update_p(tsm_ctx* ctx, int prec, int nrhs, void* p, const void* r)
+int launch_cg_update_xp(tsm_ctx* ctx, int prec, int nrhs, void* x, void* p, const void* r, double tol)
 {
     const dim3 grid = blas_grid(ctx, nrhs);
     const int pi = prof_begin(ctx, prec, 4, nrhs);
-    BLAS_SWITCH(prec, (k_cg_update_p<PV, PP><<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, p, r, ctx->cg)));
+    BLAS_SWITCH(prec, (k_cg_update_xp<PV, PP><<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, nrhs, x, p, r, tol, ctx->cg)));
     prof_end(ctx, pi);
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());

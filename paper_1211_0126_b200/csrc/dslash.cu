@@ -55,23 +55,25 @@ constexpr int TILE = 128;   // sites per tile = blockDim.x
 // Persistent kernel: gridDim.x resident blocks sweep the work items w = tile * gy + group in order,
 // so the whole chip works on one narrow front of the traversal (tiles) and the gy source groups of a
 // tile run next to each other in time (their link fetches meet in L2).  gridDim.x is a multiple of gy.
-// NORM: the block also leaves sum |out|^2 of its tile, per source, in partials[rhs * ntiles + tile]
+// EPI_NORM: the block also leaves sum |out|^2 of its tile, per source, in partials[rhs * ntiles + tile]
 // (fixed tree, no atomics: the same value whatever the batch composition, A14/A19).
-// POUT: storage precision of `out` (differs from PREC only for the last stencil of a bf16 CG
-// iteration, whose result q is kept in fp32).
-template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM, int POUT>
+// EPI_RESID: the result q is not stored at all: `out` is the CG residual r (fp32 with bf16 storage), updated
+// in place r -= alpha[rhs] * q, and the block leaves sum |r|^2 of its tile in partials (O5's "r -= alpha q;
+// rr' = |r|^2" fused into the stencil that produces q).
+template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI>
 __global__ void __launch_bounds__(DslashCfg<PREC>::MAXT, 1)
-k_dslash(const Geom g, const int par, const int gy, const int ntiles, const void* __restrict__ pack,
+k_dslash(const Geom g, const int par, const int gy, const int ntiles, const int slab, const void* __restrict__ pack,
          const void* __restrict__ in_, const void* __restrict__ x_, void* __restrict__ out_, const DslashCoef cf,
          double* __restrict__ partials, const CgScalars* __restrict__ cg, const int check_done)
 {
     using T = typename PT<PREC>::real;
     if (check_done && cg->all_done) return;
     const int Vh = g.Vh;
-    const size_t fb = field_bytes(PREC, Vh, 1), fbo = field_bytes(POUT, Vh, 1);
+    constexpr int PR = PREC == TSM_BF16 ? TSM_F32 : PREC;   // storage of r
+    const size_t fb = field_bytes(PREC, Vh, 1), fbo = field_bytes(EPI == EPI_RESID ? PR : PREC, Vh, 1);
     const T cxur = (T)cf.x.up_re, cxui = (T)cf.x.up_im, cxlr = (T)cf.x.lo_re, cxli = (T)cf.x.lo_im;
     const T cdur = (T)cf.d.up_re, cdui = (T)cf.d.up_im, cdlr = (T)cf.d.lo_re, cdli = (T)cf.d.lo_im;
-    __shared__ double smem[NORM ? 32 * 4 : 1];
+    __shared__ double smem[EPI != EPI_NONE ? 32 * 4 : 1];
 
     for (int w = blockIdx.x; w < ntiles * gy; w += gridDim.x) {
         const int tile = w / gy, group = w - tile * gy;
@@ -81,8 +83,12 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const void
         const int v = tile * TILE + threadIdx.x;
         double nrm = 0.0;
         if (v < Vh) {
+            // slab order when whole tiles fit the z planes (S % 128 == 0), else plain cb order: in both
+            // cases the same tiles, in the same order, as dslash_tile.cu (identical partial sums, A14/A19)
             SiteCoord s;
-            const int i = traverse_site(g, v, par, s);
+            int i = v;
+            if (slab) i = traverse_site(g, v, par, s);
+            else s = decode_site(g, v, par);
             int nb[8];
             neighbours(g, i, s, nb);
             const T ph_f = (s.t == g.L[3] - 1) ? (T)g.theta : (T)1;
@@ -111,9 +117,21 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const void
                     o[2 * q + 1] += cr * xv[2 * q + 1] + ci * xv[2 * q];
                 }
             }
-            store_spinor<POUT>(out, i, o);
-            if (NORM) {
-                if (POUT == TSM_BF16) {   // the norm of what was stored, i.e. of the vector the solver uses
+            if (EPI == EPI_RESID) {
+                const T alpha = (T)cg->alpha[rhs];
+                T rv[24];
+                load_spinor<PR>(out, i, rv);
+#pragma unroll
+                for (int k = 0; k < 24; k++) {
+                    rv[k] -= alpha * o[k];
+                    nrm += (double)rv[k] * (double)rv[k];
+                }
+                store_spinor<PR>(out, i, rv);
+            } else {
+                store_spinor<PREC>(out, i, o);
+            }
+            if (EPI == EPI_NORM) {
+                if (PREC == TSM_BF16) {   // the norm of what was stored, i.e. of the vector the solver uses
                     T ob[24];
 #pragma unroll
                     for (int k8 = 0; k8 < 3; k8++) { const uint4 pk = float_to_bf16x8((const float*)(o + 8 * k8)); bf16x8_to_float(pk, (float*)(ob + 8 * k8)); }
@@ -125,7 +143,7 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const void
                 }
             }
         }
-        if (NORM) {
+        if (EPI != EPI_NONE) {
             const double tot = block_row_sum(nrm, smem);
             if (threadIdx.x == 0) partials[(size_t)rhs * ntiles + tile] = tot;
         }
@@ -133,19 +151,19 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const void
 }
 
 // resident blocks per SM of each instantiation, queried once
-template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM, int POUT> int resident_blocks(int threads)
+template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI> int resident_blocks(int threads)
 {
     static int cache[5] = {0, 0, 0, 0, 0};   // indexed by blockDim.y
     const int ry = threads / TILE;
     if (cache[ry] == 0) {
         int nb = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_dslash<PREC, RECON, DAGGER, XPAY, NORM, POUT>, threads, 0) != cudaSuccess || nb < 1) nb = 1;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_dslash<PREC, RECON, DAGGER, XPAY, EPI>, threads, 0) != cudaSuccess || nb < 1) nb = 1;
         cache[ry] = nb;
     }
     return cache[ry];
 }
 
-template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM, int POUT>
+template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI>
 int launch_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void* in, const void* x, void* out,
              const DslashCoef& c, int check_done)
 {
@@ -157,13 +175,13 @@ int launch_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void* in, 
     dim3 block(TILE, ry);
     const int gy = nrhs / ry;
     const int ntiles = (ctx->g.Vh + TILE - 1) / TILE;
-    long long grid = (long long)ctx->nsm * resident_blocks<PREC, RECON, DAGGER, XPAY, NORM, POUT>(TILE * ry);
+    long long grid = (long long)ctx->nsm * resident_blocks<PREC, RECON, DAGGER, XPAY, EPI>(TILE * ry);
     grid -= grid % gy;
     if (grid < gy) grid = gy;
     if (grid > (long long)ntiles * gy) grid = (long long)ntiles * gy;
-    if (NORM && (size_t)ntiles * nrhs > ctx->norm_partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
-    const int pi = prof_begin(ctx, PREC, NORM ? 2 : (XPAY ? 1 : 0), nrhs);
-    k_dslash<PREC, RECON, DAGGER, XPAY, NORM, POUT><<<(unsigned)grid, block, 0, ctx->stream>>>(ctx->g, par, gy, ntiles, pack, in, x, out, c,
+    if (EPI != EPI_NONE && (size_t)ntiles * nrhs > ctx->norm_partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
+    const int pi = prof_begin(ctx, PREC, EPI == EPI_RESID ? 3 : (EPI == EPI_NORM ? 2 : (XPAY ? 1 : 0)), nrhs);
+    k_dslash<PREC, RECON, DAGGER, XPAY, EPI><<<(unsigned)grid, block, 0, ctx->stream>>>(ctx->g, par, gy, ntiles, (ctx->g.S % TILE == 0) ? 1 : 0, pack, in, x, out, c,
                                                                                          ctx->norm_partials, ctx->cg, check_done);
     prof_end(ctx, pi);
     ctx->launches++;
@@ -174,21 +192,16 @@ int launch_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void* in, 
 
 template <int PREC, int RECON>
 int launch_p(tsm_ctx* ctx, int par, bool dagger, int nrhs, const void* pack, const void* in, const void* x, void* out,
-             const DslashCoef& c, int norm, int check_done, int out32)
+             const DslashCoef& c, int epi, int check_done)
 {
     const bool xpay = x != nullptr;
-    if constexpr (PREC == TSM_BF16) {
-        if (out32) {
-            if (dagger && xpay && !norm) return launch_t<PREC, RECON, true, true, false, TSM_F32>(ctx, par, nrhs, pack, in, x, out, c, check_done);
-            return tsm_fail(ctx, TSM_EINVAL, "unsupported dslash variant (fp32 output)");
-        }
-    }
-#define GO(DG, XP, NM) return launch_t<PREC, RECON, DG, XP, NM, PREC>(ctx, par, nrhs, pack, in, x, out, c, check_done)
-    if (!dagger && !xpay && !norm) GO(false, false, false);
-    if (!dagger && xpay && !norm) GO(false, true, false);
-    if (dagger && !xpay && !norm) GO(true, false, false);
-    if (dagger && xpay && !norm) GO(true, true, false);
-    if (!dagger && xpay && norm) GO(false, true, true);
+#define GO(DG, XP, EP) return launch_t<PREC, RECON, DG, XP, EP>(ctx, par, nrhs, pack, in, x, out, c, check_done)
+    if (!dagger && !xpay && epi == EPI_NONE) GO(false, false, EPI_NONE);
+    if (!dagger && xpay && epi == EPI_NONE) GO(false, true, EPI_NONE);
+    if (dagger && !xpay && epi == EPI_NONE) GO(true, false, EPI_NONE);
+    if (dagger && xpay && epi == EPI_NONE) GO(true, true, EPI_NONE);
+    if (!dagger && xpay && epi == EPI_NORM) GO(false, true, EPI_NORM);
+    if (dagger && xpay && epi == EPI_RESID) GO(true, true, EPI_RESID);
 #undef GO
     return tsm_fail(ctx, TSM_EINVAL, "unsupported dslash variant");
 }
@@ -199,29 +212,29 @@ int launch_p(tsm_ctx* ctx, int par, bool dagger, int nrhs, const void* pack, con
 // TSM_TILE=2 sends single sources there as well: tuning aids).
 static bool tile_stencil_enabled(int nrhs)
 {
-    const char* e = getenv("TSM_TILE");   // TUNING: read on every call
-    const int mode = e ? atoi(e) : 1;
+    static int mode = -1;
+    if (mode < 0) { const char* e = getenv("TSM_TILE"); mode = e ? atoi(e) : 1; }
     return mode == 2 || (mode == 1 && nrhs >= 2);
 }
 
 // mode bit 0: leave per-tile sums of |out|^2 in ctx->partials (the CG's <p, Mhat^dag Mhat p> = |Mhat p|^2);
-// bit 1: early exit when cg->all_done; bit 2 (bf16 storage only): `out` is an fp32 field.
+// bit 1: early exit when cg->all_done; bit 2: `out` is the CG residual, updated in place (EPI_RESID).
 int launch_dslash(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs, const void* in, const void* x,
                   void* out, const DslashCoef& c, int mode)
 {
-    const int nm = mode & 1, chk = (mode >> 1) & 1, o32 = (mode >> 2) & 1;
+    const int chk = (mode >> 1) & 1, nm = (mode & 4) ? EPI_RESID : ((mode & 1) ? EPI_NORM : EPI_NONE);
     if ((prec == TSM_F32 || prec == TSM_BF16) && tile_stencil_enabled(nrhs)) return launch_dslash_tile(ctx, prec, out_parity, dagger, nrhs, in, x, out, c, mode);
     if (prec == TSM_F64)
-        return launch_p<TSM_F64, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge64[out_parity], in, x, out, c, nm, chk, o32);
+        return launch_p<TSM_F64, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge64[out_parity], in, x, out, c, nm, chk);
     if (prec == TSM_F32) {
         if (ctx->recon == 18)
-            return launch_p<TSM_F32, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk, o32);
-        return launch_p<TSM_F32, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk, o32);
+            return launch_p<TSM_F32, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
+        return launch_p<TSM_F32, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
     }
     if (prec == TSM_BF16) {
         if (ctx->recon == 18)
-            return launch_p<TSM_BF16, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk, o32);
-        return launch_p<TSM_BF16, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk, o32);
+            return launch_p<TSM_BF16, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
+        return launch_p<TSM_BF16, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
     }
     return tsm_fail(ctx, TSM_EINVAL, "bad precision");
 }

@@ -17,42 +17,12 @@
 // batch it is in (reading A14).
 #include <cstdlib>
 
+#include "bulk_copy.cuh"
 #include "dslash_common.cuh"
 
 namespace {
 
 constexpr int TT = 128;   // sites per tile = blockDim.x = 4 layout blocks
-
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-}
-// global -> shared bulk copy (TMA engine, SASS UBLKCP); bytes a multiple of 16, both addresses 16-byte aligned
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t* bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
 
 // both links of direction MU of the thread's site from the staged tile (same layout as the pack)
 template <int RECON, int MU> __device__ __forceinline__ void lds_link_pair(const char* tile_links, int tx, float* uf, float* ub)
@@ -134,9 +104,9 @@ __device__ __forceinline__ int tile_base(const Geom& g, int tile, int slab)
     return (int)(t * g.Vsh + (zb * g.bz + zi) * g.S + rest);
 }
 
-template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM, int POUT, int RY, int R>
+template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI, int RY, int R>
 __global__ void __launch_bounds__(TT * RY, 1)
-k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, const int slab, const void* __restrict__ pack,
+k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, const int slab, const int nbuf, const void* __restrict__ pack,
               const void* __restrict__ in_, const void* __restrict__ x_, void* __restrict__ out_, const DslashCoef cf,
               double* __restrict__ partials, const CgScalars* __restrict__ cg, const int check_done)
 {
@@ -144,11 +114,12 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
     constexpr unsigned TILE_BYTES = 4 * NCH * LB_ROW;
     extern __shared__ __align__(128) char smem[];
     __shared__ __align__(8) uint64_t bar[2];
-    __shared__ double red[NORM ? 32 * RY : 1];
+    constexpr int PR = PREC == TSM_BF16 ? TSM_F32 : PREC;   // storage of the CG residual (EPI_RESID)
+    __shared__ double red[EPI != EPI_NONE ? RY * 2 * 4 * R : 1];
     if (check_done && cg->all_done) return;
     const int Vh = g.Vh;
     const int nblocks = (int)(padded_sites(Vh) / LB);
-    const size_t fb = field_bytes(PREC, Vh, 1), fbo = field_bytes(POUT, Vh, 1);
+    const size_t fb = field_bytes(PREC, Vh, 1), fbo = field_bytes(EPI == EPI_RESID ? PR : PREC, Vh, 1);
     const float cxur = (float)cf.x.up_re, cxui = (float)cf.x.up_im, cxlr = (float)cf.x.lo_re, cxli = (float)cf.x.lo_im;
     const float cdur = (float)cf.d.up_re, cdui = (float)cf.d.up_im, cdlr = (float)cf.d.lo_re, cdli = (float)cf.d.lo_im;
     const int tx = threadIdx.x, ty = threadIdx.y;
@@ -173,9 +144,9 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
 
     int it = 0;
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
-        const int b = it & 1;
+        const int b = nbuf == 2 ? (it & 1) : 0;
         // buffer b^1 was last read in iteration it-1, which ended with __syncthreads()
-        if (leader && tile + (int)gridDim.x < ntiles) issue(tile + gridDim.x, b ^ 1);
+        if (nbuf == 2 && leader && tile + (int)gridDim.x < ntiles) issue(tile + gridDim.x, b ^ 1);
         const int i = tile_base(g, tile, slab) + tx;
         const bool live = i < Vh;
         SiteCoord s = decode_site(g, live ? i : 0, par);
@@ -183,7 +154,7 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
         neighbours(g, live ? i : 0, s, nb);
         const float ph_f = (s.t == g.L[3] - 1) ? (float)g.theta : 1.f;
         const float ph_b = (s.t == 0) ? (float)g.theta : 1.f;
-        mbar_wait(&bar[b], (unsigned)((it >> 1) & 1));
+        mbar_wait(&bar[b], (unsigned)((nbuf == 2 ? (it >> 1) : it) & 1));
         const char* links = smem + (size_t)b * TILE_BYTES;
 
         for (int grp = 0; grp * RY * R < nrhs; grp++) {
@@ -222,9 +193,21 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
                             o[2 * q + 1] += cr * xv[2 * q + 1] + ci * xv[2 * q];
                         }
                     }
-                    store_spinor<POUT>((char*)out_ + fbo * (rhs0 + r), i, o);
-                    if (NORM) {
-                        if (POUT == TSM_BF16) {   // the norm of what was stored, i.e. of the vector the solver uses
+                    if (EPI == EPI_RESID) {   // out_ is r: r -= alpha q, |r|^2 (q itself is never stored)
+                        const float alpha = (float)cg->alpha[rhs0 + r];
+                        float rv[24];
+                        load_spinor<PR>((const char*)out_ + fbo * (rhs0 + r), i, rv);
+#pragma unroll
+                        for (int k = 0; k < 24; k++) {
+                            rv[k] -= alpha * o[k];
+                            nrm[r] += (double)rv[k] * (double)rv[k];
+                        }
+                        store_spinor<PR>((char*)out_ + fbo * (rhs0 + r), i, rv);
+                    } else {
+                        store_spinor<PREC>((char*)out_ + fbo * (rhs0 + r), i, o);
+                    }
+                    if (EPI == EPI_NORM) {
+                        if (PREC == TSM_BF16) {   // the norm of what was stored, i.e. of the vector the solver uses
                             float ob[24];
 #pragma unroll
                             for (int k8 = 0; k8 < 3; k8++) { const uint4 pk = float_to_bf16x8(o + 8 * k8); bf16x8_to_float(pk, ob + 8 * k8); }
@@ -237,28 +220,36 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
                     }
                 }
             }
-            if (NORM) {
+            if (EPI != EPI_NONE && rhs0 < nrhs) {
+                // sum over the row's 128 sites in a fixed order (A19): shuffle tree per warp, then the 4 warps;
+                // only this row's 4 warps synchronise (named barrier), the other rows run on.  `red` is
+                // double-buffered by group parity; a tile ends with __syncthreads().
+                double* w = red + (ty * 2 + (grp & 1)) * 4 * R;
 #pragma unroll
                 for (int r = 0; r < R; r++) {
-                    const double tot = block_row_sum(nrm[r], red);
-                    if (tx == 0 && rhs0 < nrhs) partials[(size_t)(rhs0 + r) * ntiles + tile] = tot;
+                    const double v = warp_sum(nrm[r]);
+                    if ((tx & 31) == 0) w[(tx >> 5) * R + r] = v;
                 }
+                row_barrier(1 + ty, TT);
+                if (tx < R) partials[(size_t)(rhs0 + tx) * ntiles + tile] = ((w[tx] + w[R + tx]) + w[2 * R + tx]) + w[3 * R + tx];
             }
         }
         __syncthreads();
+        if (nbuf == 1 && leader && tile + (int)gridDim.x < ntiles) issue(tile + gridDim.x, 0);
     }
 }
 
-template <int PREC, int RECON, bool DAGGER, bool XPAY, bool NORM, int POUT, int RY, int R>
+template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI, int RY, int R>
 int launch_tile_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void* in, const void* x, void* out, const DslashCoef& c,
                   int check_done)
 {
     constexpr int NCH = RECON == 18 ? 36 : 24;
-    constexpr size_t SMEM = 2 * 4 * NCH * LB_ROW;
-    auto kern = k_dslash_tile<PREC, RECON, DAGGER, XPAY, NORM, POUT, RY, R>;
+    const int nbuf = 2;   // two link buffers: the next tile's copy overlaps this tile's arithmetic (1 buffer: 799 vs 725 us)
+    const size_t SMEM = (size_t)nbuf * 4 * NCH * LB_ROW;
+    auto kern = k_dslash_tile<PREC, RECON, DAGGER, XPAY, EPI, RY, R>;
     static unsigned long long attr_done = 0;   // per device
     if (!((attr_done >> (ctx->device & 63)) & 1ull)) {
-        TSM_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
+        TSM_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 4 * NCH * LB_ROW));
         attr_done |= 1ull << (ctx->device & 63);
     }
     const Geom& g = ctx->g;
@@ -266,9 +257,9 @@ int launch_tile_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void*
     const int slab = (g.S % TT == 0) ? 1 : 0;
     int grid = ctx->nsm;            // one CTA per SM (shared memory: two link buffers)
     if (grid > ntiles) grid = ntiles;
-    if (NORM && (size_t)ntiles * nrhs > ctx->norm_partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
-    const int pi = prof_begin(ctx, PREC, NORM ? 2 : (XPAY ? 1 : 0), nrhs);
-    kern<<<grid, dim3(TT, RY), SMEM, ctx->stream>>>(g, par, nrhs, ntiles, slab, pack, in, x, out, c, ctx->norm_partials, ctx->cg, check_done);
+    if (EPI != EPI_NONE && (size_t)ntiles * nrhs > ctx->norm_partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
+    const int pi = prof_begin(ctx, PREC, EPI == EPI_RESID ? 3 : (EPI == EPI_NORM ? 2 : (XPAY ? 1 : 0)), nrhs);
+    kern<<<grid, dim3(TT, RY), SMEM, ctx->stream>>>(g, par, nrhs, ntiles, slab, nbuf, pack, in, x, out, c, ctx->norm_partials, ctx->cg, check_done);
     prof_end(ctx, pi);
     ctx->launches++;
     ctx->norm_ntiles = ntiles;
@@ -278,31 +269,25 @@ int launch_tile_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void*
 
 template <int PREC, int RECON, int RY, int R>
 int launch_tile_v(tsm_ctx* ctx, int par, bool dagger, int nrhs, const void* pack, const void* in, const void* x, void* out,
-                  const DslashCoef& c, int norm, int check_done, int out32)
+                  const DslashCoef& c, int epi, int check_done)
 {
     const bool xpay = x != nullptr;
-    if constexpr (PREC == TSM_BF16) {
-        if (out32) {
-            if (dagger && xpay && !norm)
-                return launch_tile_t<PREC, RECON, true, true, false, TSM_F32, RY, R>(ctx, par, nrhs, pack, in, x, out, c, check_done);
-            return tsm_fail(ctx, TSM_EINVAL, "unsupported dslash variant (fp32 output)");
-        }
-    }
-#define GO(DG, XP, NM) return launch_tile_t<PREC, RECON, DG, XP, NM, PREC, RY, R>(ctx, par, nrhs, pack, in, x, out, c, check_done)
-    if (!dagger && !xpay && !norm) GO(false, false, false);
-    if (!dagger && xpay && !norm) GO(false, true, false);
-    if (dagger && !xpay && !norm) GO(true, false, false);
-    if (dagger && xpay && !norm) GO(true, true, false);
-    if (!dagger && xpay && norm) GO(false, true, true);
+#define GO(DG, XP, EP) return launch_tile_t<PREC, RECON, DG, XP, EP, RY, R>(ctx, par, nrhs, pack, in, x, out, c, check_done)
+    if (!dagger && !xpay && epi == EPI_NONE) GO(false, false, EPI_NONE);
+    if (!dagger && xpay && epi == EPI_NONE) GO(false, true, EPI_NONE);
+    if (dagger && !xpay && epi == EPI_NONE) GO(true, false, EPI_NONE);
+    if (dagger && xpay && epi == EPI_NONE) GO(true, true, EPI_NONE);
+    if (!dagger && xpay && epi == EPI_NORM) GO(false, true, EPI_NORM);
+    if (dagger && xpay && epi == EPI_RESID) GO(true, true, EPI_RESID);
 #undef GO
     return tsm_fail(ctx, TSM_EINVAL, "unsupported dslash variant");
 }
 
 template <int PREC, int RECON>
 int launch_tile_s(tsm_ctx* ctx, int ry, int r, int par, bool dagger, int nrhs, const void* pack, const void* in, const void* x,
-                  void* out, const DslashCoef& c, int norm, int check_done, int out32)
+                  void* out, const DslashCoef& c, int epi, int check_done)
 {
-#define SHAPE(RY_, R_) if (ry == RY_ && r == R_) return launch_tile_v<PREC, RECON, RY_, R_>(ctx, par, dagger, nrhs, pack, in, x, out, c, norm, check_done, out32)
+#define SHAPE(RY_, R_) if (ry == RY_ && r == R_) return launch_tile_v<PREC, RECON, RY_, R_>(ctx, par, dagger, nrhs, pack, in, x, out, c, epi, check_done)
     SHAPE(4, 1);
     SHAPE(2, 1);
     SHAPE(1, 1);
@@ -315,10 +300,6 @@ int launch_tile_s(tsm_ctx* ctx, int ry, int r, int par, bool dagger, int nrhs, c
 // Shape of the CTA for a batch of nrhs sources: RY source rows x R sources per thread; R divides nrhs.
 void tile_shape(int nrhs, int& ry, int& r)
 {
-    const char* a = getenv("TSM_TILE_RY");   // TUNING: read on every call while the shapes are being explored
-    const char* b = getenv("TSM_TILE_R");
-    const int env_ry = a ? atoi(a) : 0, env_r = b ? atoi(b) : 0;
-    if (env_ry > 0 && env_r > 0 && nrhs % env_r == 0) { ry = env_ry; r = env_r; return; }
     if (nrhs == 1) { ry = 1; r = 1; return; }
     if (nrhs == 2) { ry = 2; r = 1; return; }
     ry = 4; r = 1;
@@ -328,17 +309,17 @@ void tile_shape(int nrhs, int& ry, int& r)
 int launch_dslash_tile(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs, const void* in, const void* x, void* out,
                        const DslashCoef& c, int mode)
 {
-    const int nm = mode & 1, chk = (mode >> 1) & 1, o32 = (mode >> 2) & 1;
+    const int chk = (mode >> 1) & 1, nm = (mode & 4) ? EPI_RESID : ((mode & 1) ? EPI_NORM : EPI_NONE);
     int ry, r;
     tile_shape(nrhs, ry, r);
     const void* pack = ctx->gauge32[out_parity];
     if (prec == TSM_F32) {
-        if (ctx->recon == 18) return launch_tile_s<TSM_F32, 18>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk, o32);
-        return launch_tile_s<TSM_F32, 12>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk, o32);
+        if (ctx->recon == 18) return launch_tile_s<TSM_F32, 18>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk);
+        return launch_tile_s<TSM_F32, 12>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk);
     }
     if (prec == TSM_BF16) {
-        if (ctx->recon == 18) return launch_tile_s<TSM_BF16, 18>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk, o32);
-        return launch_tile_s<TSM_BF16, 12>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk, o32);
+        if (ctx->recon == 18) return launch_tile_s<TSM_BF16, 18>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk);
+        return launch_tile_s<TSM_BF16, 12>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk);
     }
     return tsm_fail(ctx, TSM_EINVAL, "tile stencil: unsupported precision");
 }

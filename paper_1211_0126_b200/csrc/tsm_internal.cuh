@@ -351,6 +351,8 @@ struct CgScalars {
     double bb[TSM_MAX_NRHS];      // |b'|^2
     double pq[TSM_MAX_NRHS];      // Re <p, q>
     double beta[TSM_MAX_NRHS];
+    double alpha[TSM_MAX_NRHS];   // rr / Re<p,q> of this iteration; 0 for a frozen source
+    double rr_new[TSM_MAX_NRHS];  // |r|^2 after this iteration's residual update
     int iters[TSM_MAX_NRHS];
     int done[TSM_MAX_NRHS];       // frozen: converged, broken down, or zero source
     int status[TSM_MAX_NRHS];
@@ -361,6 +363,8 @@ struct CgScalars {
 // ------------------------------------------------------------------ epilogue coefficients
 // out = Tx * x + Td * (D in), T = c_up on spins 0,1 and c_lo on spins 2,3 (complex), i.e.
 // T = alpha + i beta gamma5 with c_up = alpha + i beta, c_lo = alpha - i beta (C3: gamma5 diagonal).
+// stencil epilogues beyond out = Tx x + Td D in
+enum { EPI_NONE = 0, EPI_NORM = 1, EPI_RESID = 2 };
 struct TwistCoef { double up_re, up_im, lo_re, lo_im; };
 struct DslashCoef { TwistCoef x, d; };
 
@@ -371,7 +375,7 @@ struct GammaTable {          // Gamma_{alpha, col[alpha]} = i^ph[alpha], all oth
 };
 
 // Optional per-launch timing (tsm_profile): CUDA events on the library's stream around each
-// stencil / BLAS launch.  kind: 0 stencil, 1 stencil+xpay, 2 stencil+xpay+norm, 3 update_xr, 4 update_p.
+// stencil / BLAS launch.  kind: 0 stencil, 1 stencil+xpay, 2 stencil+xpay+norm, 3 stencil+xpay+residual update, 4 update_xp.
 struct ProfRec { int prec, kind, nrhs; cudaEvent_t a, b; };
 
 struct tsm_ctx {
@@ -462,8 +466,8 @@ int launch_pack_spinor(tsm_ctx* ctx, int prec, int nrhs, const double* dev_lex, 
 int launch_unpack_spinor(tsm_ctx* ctx, int prec, int nrhs, const void* dev_native, double* dev_lex);
 int launch_noise(tsm_ctx* ctx, int prec, int nrhs, uint64_t seed, const uint32_t* dev_ids, int kind, void* dev_full);
 int launch_cg_init(tsm_ctx* ctx, int prec, int nrhs, const void* r, void* p, void* x);
-int launch_cg_update_xr(tsm_ctx* ctx, int prec, int nrhs, void* x, const void* p, void* r, const void* q, double tol);
-int launch_cg_update_p(tsm_ctx* ctx, int prec, int nrhs, void* p, const void* r);
+int launch_cg_reduce(tsm_ctx* ctx, int which, int nrhs);
+int launch_cg_update_xp(tsm_ctx* ctx, int prec, int nrhs, void* x, void* p, const void* r, double tol);
 int launch_convert(tsm_ctx* ctx, int prec_in, int prec_out, int nrhs_fields, const void* in, void* out);
 int launch_contract(tsm_ctx* ctx, int slot);
 int launch_accumulate(tsm_ctx* ctx, double* acc, const double* a, const double* b, int nrhs);

@@ -349,3 +349,48 @@ def test_state_and_argument_errors(tsm_mod):
     with pytest.raises(tsm_mod.TsmError):
         tsm_mod.Tsm((4, 4, 5, 4))
     t.close()
+
+
+# ---------------------------------------------------------------- bf16 storage (config 4) and fp32 batches
+def test_bf16_lp_solves_by_true_residual(tsm_mod):
+    """A17 for bf16 storage: config 4's parameters on an 8^3 x 16 lattice, 4 sources per batch, tol 5e-3:
+    fp64 true residual of the full system <= 2 tol, iteration count within 2 of the oracle's."""
+    wl = W.WORKLOADS[4]
+    c = Case(tsm_mod, (8, 8, 8, 16), wl.eps, wl.gauge_seed, wl.kappa, wl.mu, -1, max_nrhs=4, recon=12)
+    ids = [0, 1, 2, 3]
+    rc, info = c.t.solve(wl.noise_seed, ids, BF16, wl.lp_tol, 1000, slot=1, want_true_resid=True)
+    assert rc == 0
+    for j, sid in enumerate(ids):
+        eta = oracle.noise(c.dims, wl.noise_seed, sid)
+        _, info_ref = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, wl.lp_tol, 1000)
+        assert abs(info[j]["iters"] - info_ref["iters"]) <= 2, (info[j], info_ref)
+        rho = oracle.true_residual(c.dims, c.theta, c.kappa, c.mu, c.U, eta, c.t.get_solution(1, j))
+        assert rho <= 2 * wl.lp_tol, rho
+        assert np.isclose(info[j]["rel_resid_true"], rho, rtol=1e-3)
+    # fixed-k mode: rho <= max(2 rho_oracle(k), 100 eps_bf16) with eps_bf16 = 2^-8
+    eta = oracle.noise(c.dims, wl.noise_seed, 0)
+    for k in (3, 12):
+        _, info_ref = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, 0.0, k)
+        rc, info = c.t.solve(wl.noise_seed, [0, 1], BF16, 0.0, k, slot=1)
+        assert rc == 0 and info[0]["iters"] == k
+        rho = oracle.true_residual(c.dims, c.theta, c.kappa, c.mu, c.U, eta, c.t.get_solution(1, 0))
+        assert rho <= max(2 * info_ref["rel_resid_true"], 100 * 2.0 ** -8)
+    c.t.close()
+
+
+@pytest.mark.parametrize("prec", [F32, BF16])
+def test_low_precision_batches_are_independent_of_batch_composition(medium, ragged, prec):
+    """A14 in the LP precisions: the batched kernels (shared-memory link tiles, several sources per CTA)
+    and the single-source kernel give a source the same iterate, bit for bit."""
+    for c in (medium, ragged):
+        seed = 4242
+        ids = [4, 9, 2, 11, 7]
+        rc, info = c.t.solve(seed, ids[:4], prec, 0.0, 6, slot=0)
+        assert rc == 0
+        batch = [c.t.get_solution(0, j) for j in range(4)]
+        for j in (0, 3):
+            rc, single = c.t.solve(seed, [ids[j]], prec, 0.0, 6, slot=1)
+            assert np.array_equal(c.t.get_solution(1, 0), batch[j]), (c.dims, prec, j)
+        rc, _ = c.t.solve(seed, [ids[3], ids[4], ids[0]], prec, 0.0, 6, slot=1)   # other batch, other position
+        assert np.array_equal(c.t.get_solution(1, 0), batch[3])
+        assert np.array_equal(c.t.get_solution(1, 2), batch[0])
