@@ -68,6 +68,15 @@ def stencil_bytes_per_site(prec: str, recon: int, nrhs: int, kind: int) -> float
     return (48 + (24 if kind else 0)) * w_s + links
 
 
+# DRAM traffic per stencil launch from ncu (dram__bytes_read.sum + dram__bytes_write.sum, mean of the four
+# stencil launches of one CG iteration), keyed by (workload, precision, sources per batch); the capture and
+# its command are in profiles/r01_dslash_r12_tile.md and profiles/r01_dslash_r1.md.  None when not captured.
+NCU_TRAFFIC_BYTES = {
+    ("cfg5_32x32x32x64", "f32", 12): (4.628e9 + 3.369e9 + 5.838e9 + 3.377e9) / 4,
+    ("cfg5_32x32x32x64", "f32", 1): (0.906e9 + 0.789e9 + 0.905e9 + 0.789e9) / 4,
+}
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -247,7 +256,8 @@ def run_ours(args, wl):
     st_n = sum(prof[k][1] for k in range(4))
     achieved = alg_bytes / (st_ms * 1e-3) / 1e9 if st_ms > 0 else 0.0
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src, "kernel": f"k_dslash<{prec_name}, recon {wl.reconstruct}> x {nrhs} sources",
+                "traffic": NCU_TRAFFIC_BYTES.get((wl.name, prec_name, nrhs)), "traffic_unit": "bytes per launch (ncu, profiles/)",
+                "peak_source": peak_src, "kernel": f"{'k_dslash_tile' if nrhs > 1 and prec_name != 'f64' else 'k_dslash'}<{prec_name}, recon {wl.reconstruct}> x {nrhs} sources (the 4 stencil launches of a CG iteration)",
                 "launches_timed": st_n, "avg_launch_us": st_ms * 1e3 / max(st_n, 1),
                 "algorithmic_bytes_per_launch": alg_bytes / max(st_n, 1),
                 "share_of_step": {"stencil": st_ms / ms, "cg_update_xp": prof[4][0] / ms},
