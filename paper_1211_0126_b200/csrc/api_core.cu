@@ -56,6 +56,12 @@ int ctx_enter(tsm_ctx* ctx, bool need_ws, bool need_gauge, bool need_params)
     return TSM_OK;
 }
 
+void ctx_drop_graphs(tsm_ctx* ctx)
+{
+    for (CgGraph& g : ctx->graphs) cudaGraphExecDestroy(g.exec);
+    ctx->graphs.clear();
+}
+
 extern "C" {
 
 int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
@@ -88,6 +94,7 @@ int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
     }
     ctx->device = device;
     ctx->stream = 0;
+    ctx->own_stream = nullptr;
     ctx->have_params = ctx->have_gauge = ctx->have_ws = false;
     ctx->recon = 18;
     ctx->max_nrhs = 0;
@@ -110,6 +117,8 @@ int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
     ok = ok && cudaMallocHost(&ctx->host_small, hs) == cudaSuccess;
     ok = ok && cudaMalloc(&ctx->ids_dev, 2 * TSM_MAX_NRHS * sizeof(uint32_t)) == cudaSuccess;
     ok = ok && cudaEventCreate(&ctx->ev0) == cudaSuccess && cudaEventCreate(&ctx->ev1) == cudaSuccess;
+    ok = ok && cudaStreamCreate(&ctx->own_stream) == cudaSuccess;   // blocking: ordered with the legacy default stream
+    ctx->stream = ctx->own_stream;
     if (!ok) { tsm_destroy(ctx); return TSM_ECUDA; }
     *out = ctx;
     return TSM_OK;
@@ -119,6 +128,8 @@ int tsm_destroy(tsm_ctx* ctx)
 {
     if (!ctx) return TSM_EINVAL;
     cudaSetDevice(ctx->device);
+    ctx_drop_graphs(ctx);
+    if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->cg) cudaFree(ctx->cg);
     if (ctx->cg_host) cudaFreeHost(ctx->cg_host);
     if (ctx->host_small) cudaFreeHost(ctx->host_small);
@@ -190,6 +201,7 @@ int tsm_set_workspace(tsm_ctx* ctx, void* dev_ptr, size_t bytes, int max_nrhs)
     carve_workspace(ctx, max_nrhs, ctx->ws);
     ctx->have_ws = true;
     ctx->have_gauge = false;
+    ctx_drop_graphs(ctx);
     for (int s = 0; s < 2; s++) { ctx->slot_prec[s] = -1; ctx->slot_nrhs[s] = 0; }
     return TSM_OK;
 }
@@ -197,7 +209,9 @@ int tsm_set_workspace(tsm_ctx* ctx, void* dev_ptr, size_t bytes, int max_nrhs)
 int tsm_set_stream(tsm_ctx* ctx, void* cuda_stream)
 {
     if (!ctx) return TSM_EINVAL;
-    ctx->stream = (cudaStream_t)cuda_stream;
+    // the legacy default stream (NULL) cannot be captured into a CUDA graph: the library then uses its own
+    // blocking stream, which keeps the legacy stream's ordering with the caller's default-stream work
+    ctx->stream = cuda_stream ? (cudaStream_t)cuda_stream : ctx->own_stream;
     return TSM_OK;
 }
 
@@ -205,6 +219,7 @@ int tsm_set_params(tsm_ctx* ctx, double kappa, double mu)
 {
     if (!ctx) return TSM_EINVAL;
     if (!std::isfinite(kappa) || !std::isfinite(mu) || kappa == 0.0) return tsm_fail(ctx, TSM_EINVAL, "bad kappa/mu");
+    ctx_drop_graphs(ctx);
     ctx->kappa = kappa;
     ctx->mu = mu;
     ctx->have_params = true;
@@ -217,6 +232,7 @@ int tsm_set_gauge(tsm_ctx* ctx, const double* host_links, int reconstruct, doubl
     if (rc) return rc;
     if (!host_links || (reconstruct != 18 && reconstruct != 12)) return tsm_fail(ctx, TSM_EINVAL, "bad gauge arguments");
     ctx->have_gauge = false;
+    if (reconstruct != ctx->recon) ctx_drop_graphs(ctx);   // other kernel variants; same pointers otherwise
     ctx->recon = reconstruct;
     const size_t bytes = (size_t)4 * ctx->g.V * 18 * sizeof(double);
     TSM_CUDA(ctx, cudaMemcpyAsync(ctx->staging, host_links, bytes, cudaMemcpyHostToDevice, ctx->stream));

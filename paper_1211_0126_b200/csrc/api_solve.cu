@@ -1,6 +1,7 @@
 // api_solve.cu -- C ABI (include/tsm.h): the solver driver (H3, H4, H6, H7), the loop
 // accumulators (H8-H10) and the whole-configuration TSM driver (Eq. 2.4).
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 #include "tsm_internal.cuh"
@@ -41,6 +42,44 @@ int cg_iteration(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, vo
     if ((rc = launch_dslash(ctx, prec, 0, true, nrhs, t, w, r, {tw.Rb, tw.mk2}, 6))) return rc;             // r -= alpha Mhat^dag w; |r|^2 per tile
     if ((rc = launch_cg_reduce(ctx, 1, nrhs))) return rc;                                                   // rr'
     return launch_cg_update_xp(ctx, prec, nrhs, x, p, r, tol);                                              // x += alpha p; p = r + beta p
+}
+
+// `iters` CG iterations as ONE CUDA graph launch (captured once per argument set and cached): on small
+// lattices an iteration is 7 launches of a few microseconds each and the solve is launch-bound otherwise.
+// TSM_GRAPH=0 turns it off.  Not used while per-launch profiling is on (events between the launches).
+bool graphs_enabled(const tsm_ctx* ctx)
+{
+    static int on = -1;
+    if (on < 0) { const char* e = getenv("TSM_GRAPH"); on = e ? atoi(e) : 1; }
+    return on != 0 && !ctx->prof_on && ctx->stream != nullptr && ctx->stream != cudaStreamLegacy && ctx->stream != cudaStreamPerThread;
+}
+
+int cg_iterations_graph(tsm_ctx* ctx, int prec, int nrhs, int iters, const Twists& tw, void* x, void* r, void* p, void* w, void* t, double tol)
+{
+    for (const CgGraph& g : ctx->graphs)
+        if (g.prec == prec && g.nrhs == nrhs && g.iters == iters && g.x == x && g.r == r && g.p == p && g.w == w && g.t == t && g.tol == tol) {
+            TSM_CUDA(ctx, cudaGraphLaunch(g.exec, ctx->stream));
+            ctx->launches += 7LL * iters;
+            return TSM_OK;
+        }
+    const long long l0 = ctx->launches;
+    TSM_CUDA(ctx, cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeRelaxed));
+    int rc = TSM_OK;
+    for (int k = 0; k < iters && rc == TSM_OK; k++) rc = cg_iteration(ctx, prec, nrhs, tw, x, r, p, w, t, tol);
+    cudaGraph_t graph = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(ctx->stream, &graph);
+    ctx->launches = l0;
+    if (rc != TSM_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+    TSM_CUDA(ctx, e);
+    CgGraph g{prec, nrhs, iters, x, r, p, w, t, tol, nullptr};
+    const cudaError_t ei = cudaGraphInstantiate(&g.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    TSM_CUDA(ctx, ei);
+    if (ctx->graphs.size() >= 16) { cudaGraphExecDestroy(ctx->graphs.front().exec); ctx->graphs.erase(ctx->graphs.begin()); }
+    ctx->graphs.push_back(g);
+    TSM_CUDA(ctx, cudaGraphLaunch(g.exec, ctx->stream));
+    ctx->launches += 7LL * iters;
+    return TSM_OK;
 }
 
 int fetch_scalars(tsm_ctx* ctx)
@@ -121,10 +160,22 @@ int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs,
     // O5: x0 = 0 (x lives in the slot's even half), r0 = p0 = b'
     void* x = s_e;
     if ((rc = launch_cg_init(ctx, prec, nrhs, r, p, x))) return rc;
+    // iterations run in chunks of `poll`; in residual mode the host reads the all-done flag after each chunk
+    // (a finished batch makes every later kernel return at once), in fixed-iteration mode it never does.
+    // The first chunk is launched kernel by kernel (it also sets up the kernels' attributes), full later
+    // chunks as one cached CUDA graph.
     const int poll = 4;
-    for (int k = 1; k <= max_iter; k++) {
-        if ((rc = cg_iteration(ctx, prec, nrhs, tw, x, r, p, w, t, tol))) return rc;
-        if (tol > 0 && (k % poll == 0) && k < max_iter) {
+    const bool use_graph = graphs_enabled(ctx);
+    for (int k = 0; k < max_iter;) {
+        const int chunk = max_iter - k < poll ? max_iter - k : poll;
+        if (use_graph && k > 0 && chunk == poll) {
+            if ((rc = cg_iterations_graph(ctx, prec, nrhs, chunk, tw, x, r, p, w, t, tol))) return rc;
+        } else {
+            for (int j = 0; j < chunk; j++)
+                if ((rc = cg_iteration(ctx, prec, nrhs, tw, x, r, p, w, t, tol))) return rc;
+        }
+        k += chunk;
+        if (tol > 0 && k < max_iter) {
             TSM_CUDA(ctx, cudaMemcpyAsync(&ctx->cg_host->all_done, &ctx->cg->all_done, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
             TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
             if (ctx->cg_host->all_done) break;

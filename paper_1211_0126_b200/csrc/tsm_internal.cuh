@@ -378,10 +378,20 @@ struct GammaTable {          // Gamma_{alpha, col[alpha]} = i^ph[alpha], all oth
 // stencil / BLAS launch.  kind: 0 stencil, 1 stencil+xpay, 2 stencil+xpay+norm, 3 stencil+xpay+residual update, 4 update_xp.
 struct ProfRec { int prec, kind, nrhs; cudaEvent_t a, b; };
 
+// A captured run of CG iterations (CUDA graph), keyed by everything the captured launches depend on.
+struct CgGraph {
+    int prec, nrhs, iters;
+    void *x, *r, *p, *w, *t;
+    double tol;
+    cudaGraphExec_t exec;
+};
+
 struct tsm_ctx {
     Geom g;
     int device;
-    cudaStream_t stream;
+    cudaStream_t stream;             // where work is enqueued: the caller's stream or own_stream
+    cudaStream_t own_stream;         // library-owned BLOCKING stream (serialises with the legacy default stream)
+    std::vector<CgGraph> graphs;     // cleared whenever kappa/mu, the gauge storage or the workspace change
     double kappa, mu;
     bool have_params, have_gauge, have_ws;
     int recon;                       // storage of the fp32 link copy (18 / 12)
@@ -474,5 +484,6 @@ int launch_accumulate(tsm_ctx* ctx, double* acc, const double* a, const double* 
 int launch_finalize(tsm_ctx* ctx);
 void build_gamma_table(GammaTable& t);
 int ctx_enter(tsm_ctx* ctx, bool need_ws, bool need_gauge, bool need_params);
+void ctx_drop_graphs(tsm_ctx* ctx);
 // |a - b|^2 per source over full-lattice fp64 fields, left in cg->pq[rhs] (true-residual helper)
 int launch_diff_norm2(tsm_ctx* ctx, int nrhs, const void* a, const void* b);

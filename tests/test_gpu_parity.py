@@ -394,3 +394,25 @@ def test_low_precision_batches_are_independent_of_batch_composition(medium, ragg
         rc, _ = c.t.solve(seed, [ids[3], ids[4], ids[0]], prec, 0.0, 6, slot=1)   # other batch, other position
         assert np.array_equal(c.t.get_solution(1, 0), batch[3])
         assert np.array_equal(c.t.get_solution(1, 2), batch[0])
+
+
+def test_cuda_graph_chunks_equal_kernel_by_kernel_launches(medium):
+    """Later chunks of 4 CG iterations run as one cached CUDA graph; with per-launch profiling on the same
+    iterations are launched kernel by kernel.  Same kernels, same order: bit-identical iterates."""
+    c = medium
+    seed = 777
+    for prec, tol, k in ((F64, 1e-10, 2000), (F32, 0.0, 23), (BF16, 0.0, 9)):
+        c.t.profile(False)
+        rc, info_g = c.t.solve(seed, [3, 8], prec, tol, k, slot=0)
+        a = [c.t.get_solution(0, j) for j in range(2)]
+        c.t.profile(True)
+        rc, info_d = c.t.solve(seed, [3, 8], prec, tol, k, slot=1)
+        c.t.profile(False)
+        for kind in range(5):
+            c.t.profile_read(prec, kind)
+        assert [i["iters"] for i in info_g] == [i["iters"] for i in info_d]
+        for j in range(2):
+            assert np.array_equal(a[j], c.t.get_solution(1, j)), (prec, j)
+    n0 = c.t.launch_count()
+    c.t.solve(seed, [3], F32, 0.0, 12, slot=0)
+    assert c.t.launch_count() - n0 == 6 + 7 * 12 + 1      # noise, twist, 3 stencils, init; 7 per iteration; reconstruction
