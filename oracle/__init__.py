@@ -159,13 +159,23 @@ def loops_deriv(dims, theta, U, eta, s) -> np.ndarray:
     return out
 
 
-def all_loops(dims, theta, U, eta, s, with_derivative: bool) -> np.ndarray:
-    """[n_ops][Lt]: the 16 local loops, then (if asked) [mu][Gamma] derivative loops (O6b order)."""
-    loc = loops(dims, eta, s)
-    if not with_derivative:
-        return loc
-    der = loops_deriv(dims, theta, U, eta, s).reshape(64, dims[3])
-    return np.concatenate([loc, der], axis=0)
+def loops_one_end(dims, kappa, mu, s) -> np.ndarray:
+    """Eq. 2.5: per-source one-end loops -2ia sum_x s^dag gamma5 Gamma s, [16][Lt]."""
+    s = _c128(s)
+    out = np.empty((16, dims[3]), dtype=np.complex128)
+    lib().oracle_loops_one_end(_c_int4(*dims), ctypes.c_double(kappa), ctypes.c_double(mu), _d(s), _d(out))
+    return out
+
+
+def all_loops(dims, theta, U, eta, s, with_derivative: bool, one_end=None) -> np.ndarray:
+    """[n_ops][Lt]: the 16 local loops, then (if asked) [mu][Gamma] derivative loops (O6b order), then
+    (if one_end=(kappa, mu) is given) the 16 one-end loops of Eq. 2.5."""
+    parts = [loops(dims, eta, s)]
+    if with_derivative:
+        parts.append(loops_deriv(dims, theta, U, eta, s).reshape(64, dims[3]))
+    if one_end is not None:
+        parts.append(loops_one_end(dims, one_end[0], one_end[1], s))
+    return parts[0] if len(parts) == 1 else np.concatenate(parts, axis=0)
 
 
 def tsm_loops(dims, theta, kappa, mu, U, seed, n_hp, n_lp, hp_tol, hp_max_iter,

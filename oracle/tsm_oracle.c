@@ -18,6 +18,7 @@
  * algebra, P6 gauge covariance, P7 dense brute force, P8 estimator statistics,
  * P9 free-field loops, P10 one-end identity, P11 TSM algebra, P12 Philox known
  * answers, P13 CG Krylov optimality, P14 derivative, P15 delta-source stencil.
+ * P16 one-end trick (Eq. 2.5) against dense M(mu)^-1 - M(-mu)^-1.
  * Parity unpinned (defined only by the algorithm O5): the values of truncated LP
  * iterates beyond P13's Krylov-minimiser check.
  *
@@ -502,4 +503,51 @@ void oracle_loops_deriv(const int L[4], int theta, const double *U, const double
         oracle_loops(L, eta, d, out + (long)mu * 16 * T * 2);
     }
     free(d);
+}
+
+/* ------------------------------------------------------------------------- */
+/* N1: the one-end trick, Eq. 2.5.             */
+/*   (2 i mu a / N) sum_r <s_r gamma5 X s_r> = Tr(M_u^-1 X) - Tr(M_d^-1 X)    */
+/* from M_u - M_d = 2 i mu a gamma5.  In the kappa-normalised   */
+/* operator of O2 the identity reads M(mu) - M(-mu) = 2 i a gamma5, a = 2     */
+/* kappa mu, and M(-mu) = gamma5 M(mu)^dag gamma5, hence                      */
+/*   M_u^-1 - M_d^-1 = -2 i a M_u^-1 gamma5 M_d^-1,                           */
+/*   E_eta[ s^dag gamma5 X s ] = Tr[X M_u^-1 gamma5 M_d^-1]  for s = M_u^-1 eta */
+/* so the per-source, per-timeslice one-end loop whose noise average is       */
+/* sum_{x in t} tr[Gamma (M_u^-1 - M_d^-1)(x,x)] is (reading A24: the sign is */
+/* fixed by the right-hand side of Eq. 2.5 with s solving the mu > 0 flavour) */
+/*   L1_Gamma(t; s) = -2 i a sum_{x in t} sum_{alpha beta c}                  */
+/*                    conj(s_{alpha c}(x)) (gamma5 Gamma)_{alpha beta} s_{beta c}(x). */
+/* out is [16][Lt][2].                                                        */
+/* ------------------------------------------------------------------------- */
+void oracle_loops_one_end(const int L[4], double kappa, double mu, const double *s_, double *out_)
+{
+    const cplx *s = (const cplx *)s_;
+    cplx *out = (cplx *)out_;
+    const long Vs = (long)L[0] * L[1] * L[2];
+    const int T = L[3];
+    const double a = 2.0 * kappa * mu;
+    cplx g[5][4][4];
+    build_gamma(g);
+    for (int G = 0; G < 16; G++) {
+        double gm[32];
+        cplx Gam[4][4], g5G[4][4];
+        oracle_gamma(G, gm);
+        for (int i = 0; i < 4; i++)
+            for (int j = 0; j < 4; j++) Gam[i][j] = gm[2 * (4 * i + j)] + I * gm[2 * (4 * i + j) + 1];
+        mat4_mul(g[4], Gam, g5G);
+        for (int t = 0; t < T; t++) {
+            cplx acc = 0;
+            for (long sx = 0; sx < Vs; sx++) {
+                const long st = (long)t * Vs + sx;
+                for (int al = 0; al < NS; al++)
+                    for (int be = 0; be < NS; be++) {
+                        if (g5G[al][be] == 0) continue;
+                        for (int c = 0; c < NC; c++)
+                            acc += conj(s[(st * NS + al) * NC + c]) * g5G[al][be] * s[(st * NS + be) * NC + c];
+                    }
+            }
+            out[(long)G * T + t] = -2.0 * I * a * acc;
+        }
+    }
 }

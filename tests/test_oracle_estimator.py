@@ -289,3 +289,59 @@ def test_p11_tsm_unbiased_with_crude_lp(tiny):
         lp_err = np.sqrt(lps.var(axis=0).real[G] / n_lp)
         biased |= bool((np.abs(lp_only - exact) > 6 * lp_err).any())
     assert biased, "a 2-iteration LP estimate should be visibly biased without the correction"
+
+
+# ---------------------------------------------------------------- P16 one-end loops (Eq. 2.5, N1)
+def test_p16_one_end_loops_sum_over_a_complete_basis_is_the_flavour_difference(tiny):
+    """Eq. 2.5 with the noise average done exactly: summing the oracle's per-source one-end
+    loops over the complete basis eta = e_k (E[eta eta^dag] = 1 replaced by sum_k e_k e_k^dag = 1) must give
+    sum_{x in t} tr[Gamma (M_u^-1 - M_d^-1)(x,x)] from the two dense inverses -- sign, factor 2 i a, gamma5,
+    timeslice and Gamma index all pinned, with nothing stochastic."""
+    d = tiny
+    dims, V = d["dims"], d["V"]
+    Md = dense_from_apply(lambda v: oracle.apply_M(dims, d["theta"], d["kappa"], -d["mu"], d["U"], v), V)
+    diff = d["Minv"] - np.linalg.inv(Md)
+    total = np.zeros((16, dims[3]), dtype=np.complex128)
+    for k in range(12 * V):
+        s_k = d["Minv"][:, k].reshape(V, 4, 3)
+        total += oracle.loops_one_end(dims, d["kappa"], d["mu"], s_k)
+    for G in range(16):
+        want = timeslice_projector_trace(dims, oracle.gamma(G), diff)
+        assert np.allclose(total[G], want, atol=1e-10), G
+    # a dropped gamma5 or a wrong sign would fail: the gamma5 loop is purely imaginary-difference
+    assert np.abs(total[1]).max() > 1e-3
+
+
+def test_p16_one_end_estimator_is_unbiased_and_less_noisy(tiny):
+    """With Z4 noise the one-end estimator of tr[g5 (M_u^-1 - M_d^-1)] is unbiased and has a
+    smaller variance than the difference of two standard estimators at the same number of solves."""
+    d = tiny
+    dims, V = d["dims"], d["V"]
+    Md = dense_from_apply(lambda v: oracle.apply_M(dims, d["theta"], d["kappa"], -d["mu"], d["U"], v), V)
+    Mdinv = np.linalg.inv(Md)
+    exact = timeslice_projector_trace(dims, oracle.gamma(1), d["Minv"] - Mdinv).sum()
+    N = 200
+    one_end, std = [], []
+    for j in range(N):
+        eta = oracle.noise(dims, 2024, j)
+        s_u = (d["Minv"] @ eta.reshape(-1)).reshape(eta.shape)
+        s_d = (Mdinv @ eta.reshape(-1)).reshape(eta.shape)
+        one_end.append(oracle.loops_one_end(dims, d["kappa"], d["mu"], s_u)[1].sum())
+        std.append(oracle.loops(dims, eta, s_u)[1].sum() - oracle.loops(dims, eta, s_d)[1].sum())
+    one_end, std = np.array(one_end), np.array(std)
+    err = one_end.std(ddof=1) / np.sqrt(N)
+    assert abs(one_end.mean() - exact) < 5 * err
+    assert one_end.std() < std.std()
+
+
+def test_one_end_loops_match_plain_einsum():
+    dims = (2, 4, 2, 4)
+    s = W.random_spinor(dims, 8)
+    kappa, mu = 0.15, 0.3
+    got = oracle.loops_one_end(dims, kappa, mu, s)
+    Vs = volume(dims) // dims[3]
+    st = s.reshape(dims[3], Vs, 4, 3)
+    for G in range(16):
+        g5G = G5 @ oracle.gamma(G)
+        want = -2j * (2 * kappa * mu) * np.einsum("txac,ab,txbc->t", st.conj(), g5G, st)
+        assert np.allclose(got[G], want, atol=1e-12)
