@@ -345,6 +345,29 @@ def extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U):
         del a, b
     out["dslash"] = table
 
+    # ---- contraction kernels (H8, H9 and the one-end loops of Eq. 2.5, N1) on the slot the timed steps left
+    t.loops_reset(wl.derivative, one_end=True)
+    t.profile(True)
+    for _ in range(3):
+        t.loops_add_lp(1)
+    t.profile(False)
+    sp = PRECS["f32" if prec_name == "bf16" else prec_name]
+    w_sol = 8 if prec_name == "f64" else 4
+    names = {5: "local_16_gamma", 6: "derivative_4_directions", 7: "one_end_eq_2_5"}
+    # algorithmic bytes per site of the full lattice and source: s once (eta is regenerated, never read);
+    # derivative: s once + the 8 links of the site
+    n_g = 18 if prec_name == "f64" else wl.reconstruct
+    by_site = {5: 24 * w_sol, 6: 24 * w_sol + 8 * n_g * (8 if prec_name == "f64" else 4), 7: 24 * w_sol}
+    ct = {}
+    for k in (5, 6, 7):
+        ms_k, n_k = t.profile_read(sp, k, nrhs)
+        if n_k:
+            us = ms_k * 1e3 / n_k
+            gb = by_site[k] * wl.V * nrhs / us / 1e3
+            ct[names[k]] = {"us": us, "algorithmic_GBs": gb, "frac_of_measured_peak": gb / peak}
+    out["contraction"] = ct
+    t.loops_reset(wl.derivative)
+
     # ---- the whole of Eq. 2.4 for this configuration (reading A23)
     if not args.no_full_set:
         loops, secs, rc = t.run_loop_set(wl.noise_seed, wl.n_hp, wl.n_lp, prec, wl.lp_tol, wl.lp_iters, hp_tol=wl.hp_tol,
@@ -360,6 +383,9 @@ def extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U):
         import oracle
         oracle.build()
         tcpu, detail = oracle_sample(wl, U)
+        t0 = time.perf_counter()
+        oracle.loops_one_end(wl.dims, wl.kappa, wl.mu, oracle.noise(wl.dims, wl.noise_seed, 0))
+        detail["t_one_end_contract_s"] = time.perf_counter() - t0
         out["cpu_baseline"] = {"value": 1.0 / tcpu, "unit": UNIT, "cores": oracle.n_threads(), "kind": "oracle",
                                "sample": ("1 source: source preparation, 1- and 3-iteration CG solves, reconstruction, residual and one "
                                           f"contraction pass run in full; the {detail['iterations_extrapolated_to']}-iteration solve "

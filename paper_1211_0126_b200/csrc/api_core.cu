@@ -31,12 +31,12 @@ size_t carve_workspace(tsm_ctx* ctx, int max_nrhs, char* base)
     { size_t o = c.take(6 * fb); if (base) for (int k = 0; k < 6; k++) ctx->vec[k] = at(o + k * fb); }
     for (int s = 0; s < 2; s++) { size_t o = c.take(2 * fb); if (base) ctx->slot[s] = at(o); }
     size_t pc = (size_t)ctx->nsm * 16 * max_nrhs;
-    const size_t pc2 = (size_t)max_nrhs * 5 * g.L[3] * 2 * 8 * 32;
+    const size_t pc2 = (size_t)max_nrhs * 6 * g.L[3] * 2 * 8 * 32;
     if (pc2 > pc) pc = pc2;
     { size_t o = c.take(pc * sizeof(double)); if (base) { ctx->partials = (double*)at(o); ctx->partials_count = pc; } }
     const size_t npc = (size_t)max_nrhs * ((g.Vh + 127) / 128);
     { size_t o = c.take(npc * sizeof(double)); if (base) { ctx->norm_partials = (double*)at(o); ctx->norm_partials_count = npc; } }
-    const size_t lb = (size_t)(TSM_N_LOCAL_OPS + TSM_N_DERIV_OPS) * g.L[3] * 2 * sizeof(double);
+    const size_t lb = (size_t)TSM_MAX_OPS * g.L[3] * 2 * sizeof(double);
     for (int s = 0; s < 2; s++) { size_t o = c.take(lb * max_nrhs); if (base) ctx->loops_src[s] = (double*)at(o); }
     { size_t o = c.take(lb); if (base) ctx->acc_corr = (double*)at(o); }
     { size_t o = c.take(lb); if (base) ctx->acc_lp = (double*)at(o); }
@@ -100,6 +100,7 @@ int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
     ctx->max_nrhs = 0;
     ctx->n_ops = TSM_N_LOCAL_OPS;
     ctx->with_deriv = 0;
+    ctx->with_one_end = 0;
     ctx->n_hp = ctx->n_lp = 0;
     ctx->launches = 0;
     ctx->prof_on = false;
@@ -113,7 +114,7 @@ int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
     ok = ok && cudaMalloc(&ctx->cg, sizeof(CgScalars)) == cudaSuccess;
     ok = ok && cudaMemset(ctx->cg, 0, sizeof(CgScalars)) == cudaSuccess;
     ok = ok && cudaMallocHost(&ctx->cg_host, sizeof(CgScalars)) == cudaSuccess;
-    const size_t hs = (size_t)(TSM_N_LOCAL_OPS + TSM_N_DERIV_OPS) * dims[3] * 2 * sizeof(double) * 2 + 256;
+    const size_t hs = (size_t)TSM_MAX_OPS * dims[3] * 2 * sizeof(double) * 2 + 256;
     ok = ok && cudaMallocHost(&ctx->host_small, hs) == cudaSuccess;
     ok = ok && cudaMalloc(&ctx->ids_dev, 2 * TSM_MAX_NRHS * sizeof(uint32_t)) == cudaSuccess;
     ok = ok && cudaEventCreate(&ctx->ev0) == cudaSuccess && cudaEventCreate(&ctx->ev1) == cudaSuccess;

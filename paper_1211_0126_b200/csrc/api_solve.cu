@@ -242,12 +242,14 @@ int tsm_set_solution(tsm_ctx* ctx, int slot, int rhs, const double* host_in)
     return TSM_OK;
 }
 
-int tsm_loops_reset(tsm_ctx* ctx, int with_derivative)
+int tsm_loops_reset(tsm_ctx* ctx, int ops)
 {
     int rc = ctx_enter(ctx, true, false, false);
     if (rc) return rc;
-    ctx->with_deriv = with_derivative ? 1 : 0;
-    ctx->n_ops = TSM_N_LOCAL_OPS + (with_derivative ? TSM_N_DERIV_OPS : 0);
+    if (ops < 0 || ops > (TSM_OPS_DERIVATIVE | TSM_OPS_ONE_END)) return tsm_fail(ctx, TSM_EINVAL, "bad loop operator set");
+    ctx->with_deriv = (ops & TSM_OPS_DERIVATIVE) ? 1 : 0;
+    ctx->with_one_end = (ops & TSM_OPS_ONE_END) ? 1 : 0;
+    ctx->n_ops = TSM_N_LOCAL_OPS + (ctx->with_deriv ? TSM_N_DERIV_OPS : 0) + (ctx->with_one_end ? TSM_N_ONE_END_OPS : 0);
     ctx->n_hp = ctx->n_lp = 0;
     const size_t lb = (size_t)ctx->n_ops * ctx->g.L[3] * 2 * sizeof(double);
     TSM_CUDA(ctx, cudaMemsetAsync(ctx->acc_corr, 0, lb, ctx->stream));
@@ -341,7 +343,7 @@ int tsm_loops_set_state(tsm_ctx* ctx, const double* host_corr, const double* hos
 }
 
 int tsm_run_loop_set(tsm_ctx* ctx, uint64_t seed, int kind, int n_hp, int n_lp, int lp_prec, double lp_tol, int lp_iters,
-                     double hp_tol, int hp_max_iter, int nrhs, int with_derivative, double* host_out, double* secs_out)
+                     double hp_tol, int hp_max_iter, int nrhs, int ops, double* host_out, double* secs_out)
 {
     int rc = ctx_enter(ctx, true, true, true);
     if (rc) return rc;
@@ -351,7 +353,7 @@ int tsm_run_loop_set(tsm_ctx* ctx, uint64_t seed, int kind, int n_hp, int n_lp, 
     TSM_CUDA(ctx, cudaEventCreate(&e1));
     TSM_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
     int worst = TSM_OK;
-    if ((rc = tsm_loops_reset(ctx, with_derivative))) goto fail;
+    if ((rc = tsm_loops_reset(ctx, ops))) goto fail;
     for (int j0 = 0; j0 < n_hp + n_lp;) {
         const bool hp = j0 < n_hp;
         const int end = hp ? n_hp : n_hp + n_lp;

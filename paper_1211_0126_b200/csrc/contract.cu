@@ -6,6 +6,10 @@
 //     for mu = 0..3 (reading A18; O6b).
 // eta is never read from memory: it is regenerated from the Philox counter (PAPER.md:80,
 // "noise sources were generated on-the-fly").  Sums are fp64 with a fixed tree (A19).
+// N1  one-end trick (Eq. 2.5; reading A24): the same 4x4 spin matrix with eta replaced by s
+//     itself, C'_{ab}(t) = sum_{x in t, c} conj(s_{ac}(x)) s_{bc}(x), then
+//     L1_Gamma(t) = -2 i a sum_{ab} (gamma5 Gamma)_{ab} C'_{ab}(t), a = 2 kappa mu, whose noise average is
+//     sum_{x in t} tr[Gamma (M_u^-1 - M_d^-1)(x,x)].
 // H10 Eq. 2.4 accumulators (O7).
 #include "reduce.cuh"
 
@@ -14,9 +18,11 @@ namespace {
 constexpr int CT_BS = 128;
 constexpr int CT_MAXBLK = 8;   // blocks per (timeslice, parity)
 
-// grid = (nblk * ngroup_in_launch, Lt, nrhs * 2); GROUP0 = 0: local; GROUP0 = 1: derivative, mu = blockIdx.x / nblk.
-// partials: [rhs][group 0..4][t][par][blk][32]
-template <int PREC, int RECON, bool DERIV>
+// grid = (nblk * ngroup_in_launch, Lt, nrhs * 2); MODE 0: local; 1: derivative, mu = blockIdx.x / nblk; 2: one-end.
+// partials: [rhs][group 0..5][t][par][blk][32], group 0 local, 1..4 derivative mu, 5 one-end
+constexpr int CT_NGROUP = 6;
+enum { CT_LOCAL = 0, CT_DERIV = 1, CT_ONE_END = 2 };
+template <int PREC, int RECON, int MODE>
 __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs, const int nblk, const void* __restrict__ sol,
                                                     const void* __restrict__ pack0, const void* __restrict__ pack1,
                                                     const uint64_t seed, const uint32_t* __restrict__ ids, const int kind,
@@ -40,9 +46,10 @@ __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs
     for (int j = blk * CT_BS + threadIdx.x; j < g.Vsh; j += nblk * CT_BS) {
         const int i = t * g.Vsh + j;
         const SiteCoord sc = decode_site(g, i, par);
-        const uint32_t bits = noise_bits(lex_of_site(g, sc), seed, sid, kind);
+        uint32_t bits = 0;
+        if (MODE != CT_ONE_END) bits = noise_bits(lex_of_site(g, sc), seed, sid, kind);
         T v[24];
-        if (!DERIV) {
+        if (MODE != CT_DERIV) {
             load_spinor<PREC>(s_same, i, v);
         } else {
             int nb[8];
@@ -71,9 +78,16 @@ __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs
         for (int al = 0; al < 4; al++)
 #pragma unroll
             for (int c = 0; c < 3; c++) {
-                float er, ei;
-                noise_value((bits >> (2 * (3 * al + c))) & 3, kind, er, ei);
-                const double cr = er, ci = -ei;   // conj(eta)
+                double cr, ci;
+                if (MODE == CT_ONE_END) {   // conj(s) in place of conj(eta)
+                    cr = (double)v[2 * (3 * al + c)];
+                    ci = -(double)v[2 * (3 * al + c) + 1];
+                } else {
+                    float er, ei;
+                    noise_value((bits >> (2 * (3 * al + c))) & 3, kind, er, ei);
+                    cr = er;
+                    ci = -ei;   // conj(eta)
+                }
 #pragma unroll
                 for (int be = 0; be < 4; be++) {
                     const double sr = (double)v[2 * (3 * be + c)], si = (double)v[2 * (3 * be + c) + 1];
@@ -94,21 +108,24 @@ __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs
     if (threadIdx.x < 32) {
         double tot = 0;
         for (int ww = 0; ww < CT_BS / 32; ww++) tot += sm[ww][threadIdx.x];
-        const int group = DERIV ? 1 + mu : 0;
-        const size_t o = ((((size_t)rhs * 5 + group) * g.L[3] + t) * 2 + par) * nblk + blk;
+        const int group = MODE == CT_DERIV ? 1 + mu : (MODE == CT_ONE_END ? 5 : 0);
+        const size_t o = ((((size_t)rhs * CT_NGROUP + group) * g.L[3] + t) * 2 + par) * nblk + blk;
         partials[o * 32 + threadIdx.x] = tot;
     }
 }
 
-// grid = (Lt, ngroups, nrhs), 32 threads: finish the sums and apply the 16 Gamma.
-__global__ void k_contract_finish(const int Lt, const int nblk, const int n_ops, const GammaTable gt,
-                                  const double* __restrict__ partials, double* __restrict__ loops)
+// grid = (Lt, 6, nrhs), 32 threads: finish the sums and apply the 16 Gamma.  op_base[group] is the first op
+// index of the group, or -1 if the group is not computed; two_a = 2 * (2 kappa mu) for the one-end group.
+struct OpBase { int v[CT_NGROUP]; };
+__global__ void k_contract_finish(const int Lt, const int nblk, const int n_ops, const GammaTable gt, const OpBase ob,
+                                  const double two_a, const double* __restrict__ partials, double* __restrict__ loops)
 {
     const int t = blockIdx.x, group = blockIdx.y, rhs = blockIdx.z, k = threadIdx.x;
+    if (ob.v[group] < 0) return;
     __shared__ double C[32];
     double tot = 0;
     for (int pb = 0; pb < 2 * nblk; pb++) {
-        const size_t o = (((size_t)rhs * 5 + group) * Lt + t) * 2 * nblk + pb;
+        const size_t o = (((size_t)rhs * CT_NGROUP + group) * Lt + t) * 2 * nblk + pb;
         tot += partials[o * 32 + k];
     }
     C[k] = tot;
@@ -116,16 +133,22 @@ __global__ void k_contract_finish(const int Lt, const int nblk, const int n_ops,
     if (k < 16) {
         double re = 0, im = 0;
         for (int al = 0; al < 4; al++) {
-            const int be = gt.col[k][al], ph = gt.ph[k][al] & 3;
+            const int be = gt.col[k][al];
+            // one-end: (gamma5 Gamma)_{al,be} = +-Gamma_{al,be} (gamma5 = diag(1,1,-1,-1): phase + 2 on rows 2,3)
+            const int ph = (gt.ph[k][al] + ((group == 5 && al >= 2) ? 2 : 0)) & 3;
             const double cr = C[2 * (4 * al + be)], ci = C[2 * (4 * al + be) + 1];
             // multiply by i^ph
             re += (ph == 0) ? cr : (ph == 1) ? -ci : (ph == 2) ? -cr : ci;
             im += (ph == 0) ? ci : (ph == 1) ? cr : (ph == 2) ? -ci : -cr;
         }
-        const int op = (group == 0) ? k : 16 + 16 * (group - 1) + k;
-        double* dst = loops + (((size_t)rhs * n_ops + op) * Lt + t) * 2;
-        dst[0] = re;
-        dst[1] = im;
+        double* dst = loops + (((size_t)rhs * n_ops + ob.v[group] + k) * Lt + t) * 2;
+        if (group == 5) {   // times -2 i a:  -2ia (re + i im) = 2a im - i 2a re
+            dst[0] = two_a * im;
+            dst[1] = -two_a * re;
+        } else {
+            dst[0] = re;
+            dst[1] = im;
+        }
     }
 }
 
@@ -185,7 +208,7 @@ int launch_contract(tsm_ctx* ctx, int slot)
     const int nrhs = ctx->slot_nrhs[slot], prec = ctx->slot_prec[slot];
     int nblk = (g.Vsh + CT_BS - 1) / CT_BS;
     if (nblk > CT_MAXBLK) nblk = CT_MAXBLK;
-    const size_t need = (size_t)nrhs * 5 * g.L[3] * 2 * nblk * 32;
+    const size_t need = (size_t)nrhs * CT_NGROUP * g.L[3] * 2 * nblk * 32;
     if (need > ctx->partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
     const uint32_t* ids = ctx->ids_dev + slot * TSM_MAX_NRHS;
     const uint64_t seed = ctx->slot_seed[slot];
@@ -196,10 +219,20 @@ int launch_contract(tsm_ctx* ctx, int slot)
     do {                                                                                                                     \
         const void* p0 = (P == TSM_F64) ? ctx->gauge64[0] : ctx->gauge32[0];                                                 \
         const void* p1 = (P == TSM_F64) ? ctx->gauge64[1] : ctx->gauge32[1];                                                 \
-        k_contract<P, R, false><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, p0, p1, seed, ids, kind, ctx->partials); \
+        int pi = prof_begin(ctx, P, 5, nrhs);                                                                                \
+        k_contract<P, R, CT_LOCAL><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, p0, p1, seed, ids, kind, ctx->partials); \
+        prof_end(ctx, pi);                                                                                                   \
         ctx->launches++;                                                                                                     \
         if (ctx->with_deriv) {                                                                                               \
-            k_contract<P, R, true><<<grid_d, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, p0, p1, seed, ids, kind, ctx->partials); \
+            pi = prof_begin(ctx, P, 6, nrhs);                                                                                \
+            k_contract<P, R, CT_DERIV><<<grid_d, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, p0, p1, seed, ids, kind, ctx->partials); \
+            prof_end(ctx, pi);                                                                                               \
+            ctx->launches++;                                                                                                 \
+        }                                                                                                                    \
+        if (ctx->with_one_end) {                                                                                             \
+            pi = prof_begin(ctx, P, 7, nrhs);                                                                                \
+            k_contract<P, R, CT_ONE_END><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, p0, p1, seed, ids, kind, ctx->partials); \
+            prof_end(ctx, pi);                                                                                               \
             ctx->launches++;                                                                                                 \
         }                                                                                                                    \
     } while (0)
@@ -209,8 +242,14 @@ int launch_contract(tsm_ctx* ctx, int slot)
     else return tsm_fail(ctx, TSM_ESTATE, "slot holds no fp64/fp32 solution");
 #undef CT
     TSM_CUDA(ctx, cudaGetLastError());
-    const dim3 grid_f(g.L[3], ctx->with_deriv ? 5 : 1, nrhs);
-    k_contract_finish<<<grid_f, 32, 0, ctx->stream>>>(g.L[3], nblk, ctx->n_ops, ctx->gam, ctx->partials, ctx->loops_src[slot]);
+    OpBase ob;
+    ob.v[0] = 0;
+    for (int m = 0; m < 4; m++) ob.v[1 + m] = ctx->with_deriv ? TSM_N_LOCAL_OPS + 16 * m : -1;
+    ob.v[5] = ctx->with_one_end ? TSM_N_LOCAL_OPS + (ctx->with_deriv ? TSM_N_DERIV_OPS : 0) : -1;
+    if (ctx->with_one_end && !ctx->have_params) return tsm_fail(ctx, TSM_ESTATE, "one-end loops need kappa/mu (tsm_set_params)");
+    const dim3 grid_f(g.L[3], CT_NGROUP, nrhs);
+    k_contract_finish<<<grid_f, 32, 0, ctx->stream>>>(g.L[3], nblk, ctx->n_ops, ctx->gam, ob, 2.0 * (2.0 * ctx->kappa * ctx->mu),
+                                                      ctx->partials, ctx->loops_src[slot]);
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;

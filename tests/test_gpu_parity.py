@@ -416,3 +416,56 @@ def test_cuda_graph_chunks_equal_kernel_by_kernel_launches(medium):
     n0 = c.t.launch_count()
     c.t.solve(seed, [3], F32, 0.0, 12, slot=0)
     assert c.t.launch_count() - n0 == 6 + 7 * 12 + 1      # noise, twist, 3 stencils, init; 7 per iteration; reconstruction
+
+
+# ---------------------------------------------------------------- N1: one-end trick loops (Eq. 2.5)
+@pytest.mark.parametrize("deriv", [False, True])
+def test_one_end_loops_parity_on_the_oracle_solution(small, ragged, deriv):
+    """The 16 one-end loops -2ia sum_x s^dag gamma5 Gamma s (appended after the other ops), on the oracle's own
+    s: 1e-12 relative to the largest loop; the other ops are unchanged by asking for them."""
+    for c in (small, ragged):
+        seed = 123
+        c.t.loops_reset(deriv, one_end=True)
+        rc, _ = c.t.solve(seed, [1, 4], F64, 0.0, 1, slot=0)
+        for j, sid in enumerate((1, 4)):
+            eta = oracle.noise(c.dims, seed, sid)
+            s, _ = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, 1e-10, 2000)
+            c.t.set_solution(0, j, s)
+            want = oracle.all_loops(c.dims, c.theta, c.U, eta, s, deriv, one_end=(c.kappa, c.mu))
+            got = c.t.loops_source(0, j)
+            assert got.shape == want.shape == (16 + (64 if deriv else 0) + 16, c.dims[3])
+            assert rel(got[-16:], want[-16:]) < 1e-12
+            assert rel(got[:-16], want[:-16]) < 1e-12
+        c.t.loops_reset(False)
+
+
+def test_one_end_loops_through_eq_2_4(small):
+    """Eq. 2.4 on the one-end loops: correction L1(s_HP) - L1(s_LP) plus the LP average, against the oracle's pieces."""
+    c = small
+    wl = W.WORKLOADS[1]
+    got, secs, rc = c.t.run_loop_set(wl.noise_seed, 2, 3, F64, 0.0, 4, hp_tol=1e-10, hp_max_iter=2000, nrhs=2, one_end=True)
+    assert rc == 0 and got.shape == (32, c.dims[3])
+    corr = np.zeros((32, c.dims[3]), dtype=np.complex128)
+    lp = np.zeros_like(corr)
+    for j in range(5):
+        eta = oracle.noise(c.dims, wl.noise_seed, j)
+        s_lp, _ = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, 0.0, 4)
+        l_lp = oracle.all_loops(c.dims, c.theta, c.U, eta, s_lp, False, one_end=(c.kappa, c.mu))
+        if j < 2:
+            s_hp, _ = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, 1e-10, 2000)
+            corr += oracle.all_loops(c.dims, c.theta, c.U, eta, s_hp, False, one_end=(c.kappa, c.mu)) - l_lp
+        else:
+            lp += l_lp
+    want = corr / 2 + lp / 3
+    assert rel(got[16:], want[16:]) < 1e-8 and rel(got[:16], want[:16]) < 1e-8
+    c.t.loops_reset(False)
+
+
+def test_one_end_fp32_slot(ragged):
+    c = ragged
+    c.t.loops_reset(False, one_end=True)
+    rc, _ = c.t.solve(6, [2, 3], F32, 0.0, 25, slot=1)
+    s = c.t.get_solution(1, 1)
+    want = oracle.loops_one_end(c.dims, c.kappa, c.mu, s)
+    assert rel(c.t.loops_source(1, 1)[16:], want) < 1e-5
+    c.t.loops_reset(False)
