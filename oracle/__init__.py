@@ -167,14 +167,26 @@ def loops_one_end(dims, kappa, mu, s) -> np.ndarray:
     return out
 
 
-def all_loops(dims, theta, U, eta, s, with_derivative: bool, one_end=None) -> np.ndarray:
+def loops_gen_one_end(dims, theta, kappa, U, s) -> np.ndarray:
+    """Eq. 2.6: per-source generalised one-end loops 2 sum_x s^dag g5 Gamma g5 D_W s, [16][Lt]."""
+    U = _c128(U)
+    s = _c128(s)
+    out = np.empty((16, dims[3]), dtype=np.complex128)
+    lib().oracle_loops_gen_one_end(_c_int4(*dims), ctypes.c_int(theta), ctypes.c_double(kappa), _d(U), _d(s), _d(out))
+    return out
+
+
+def all_loops(dims, theta, U, eta, s, with_derivative: bool, one_end=None, gen_one_end=None) -> np.ndarray:
     """[n_ops][Lt]: the 16 local loops, then (if asked) [mu][Gamma] derivative loops (O6b order), then
-    (if one_end=(kappa, mu) is given) the 16 one-end loops of Eq. 2.5."""
+    (if one_end=(kappa, mu) is given) the 16 one-end loops of Eq. 2.5, then (if gen_one_end=kappa is given)
+    the 16 generalised one-end loops of Eq. 2.6."""
     parts = [loops(dims, eta, s)]
     if with_derivative:
         parts.append(loops_deriv(dims, theta, U, eta, s).reshape(64, dims[3]))
     if one_end is not None:
         parts.append(loops_one_end(dims, one_end[0], one_end[1], s))
+    if gen_one_end is not None:
+        parts.append(loops_gen_one_end(dims, theta, gen_one_end, U, s))
     return parts[0] if len(parts) == 1 else np.concatenate(parts, axis=0)
 
 

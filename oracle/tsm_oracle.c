@@ -18,7 +18,8 @@
  * algebra, P6 gauge covariance, P7 dense brute force, P8 estimator statistics,
  * P9 free-field loops, P10 one-end identity, P11 TSM algebra, P12 Philox known
  * answers, P13 CG Krylov optimality, P14 derivative, P15 delta-source stencil.
- * P16 one-end trick (Eq. 2.5) against dense M(mu)^-1 - M(-mu)^-1.
+ * P16 one-end trick (Eq. 2.5) against dense M(mu)^-1 - M(-mu)^-1, P17 generalised one-end
+ * trick (Eq. 2.6) against dense M(mu)^-1 + M(-mu)^-1.
  * Parity unpinned (defined only by the algorithm O5): the values of truncated LP
  * iterates beyond P13's Krylov-minimiser check.
  *
@@ -550,4 +551,49 @@ void oracle_loops_one_end(const int L[4], double kappa, double mu, const double 
             out[(long)G * T + t] = -2.0 * I * a * acc;
         }
     }
+}
+
+/* ------------------------------------------------------------------------- */
+/* N2: the generalised one-end trick, Eq. 2.6. */
+/*   (2 / N) sum_r <s_r gamma5 X gamma5 D_W s_r> = Tr(M_u^-1 X) + Tr(M_d^-1 X) */
+/* from M_u + M_d = 2 D_W, "D_W the Dirac-Wilson operator without a twisted   */
+/* mass term": in the kappa-normalised operator of O2 that is   */
+/* D_W = M(mu = 0) = 1 - kappa D_hop.  Per source and timeslice, as written:  */
+/*   L2_Gamma(t; s) = 2 sum_{x in t} sum_{alpha beta c}                       */
+/*        conj(s_{alpha c}(x)) (gamma5 Gamma gamma5)_{alpha beta} (D_W s)_{beta c}(x). */
+/* out is [16][Lt][2].                                                        */
+/* ------------------------------------------------------------------------- */
+void oracle_loops_gen_one_end(const int L[4], int theta, double kappa, const double *U, const double *s_, double *out_)
+{
+    const cplx *s = (const cplx *)s_;
+    cplx *out = (cplx *)out_;
+    const long V = vol(L), Vs = (long)L[0] * L[1] * L[2];
+    const int T = L[3];
+    cplx *y = malloc(V * SPINOR * sizeof(cplx));
+    oracle_apply_M(L, theta, kappa, 0.0, U, s_, (double *)y);   /* D_W s */
+    cplx g[5][4][4];
+    build_gamma(g);
+    for (int G = 0; G < 16; G++) {
+        double gm[32];
+        cplx Gam[4][4], t1[4][4], X5[4][4];
+        oracle_gamma(G, gm);
+        for (int i = 0; i < 4; i++)
+            for (int j = 0; j < 4; j++) Gam[i][j] = gm[2 * (4 * i + j)] + I * gm[2 * (4 * i + j) + 1];
+        mat4_mul(g[4], Gam, t1);
+        mat4_mul(t1, g[4], X5);   /* gamma5 Gamma gamma5 */
+        for (int t = 0; t < T; t++) {
+            cplx acc = 0;
+            for (long sx = 0; sx < Vs; sx++) {
+                const long st = (long)t * Vs + sx;
+                for (int al = 0; al < NS; al++)
+                    for (int be = 0; be < NS; be++) {
+                        if (X5[al][be] == 0) continue;
+                        for (int c = 0; c < NC; c++)
+                            acc += conj(s[(st * NS + al) * NC + c]) * X5[al][be] * y[(st * NS + be) * NC + c];
+                    }
+            }
+            out[(long)G * T + t] = 2.0 * acc;
+        }
+    }
+    free(y);
 }

@@ -345,3 +345,38 @@ def test_one_end_loops_match_plain_einsum():
         g5G = G5 @ oracle.gamma(G)
         want = -2j * (2 * kappa * mu) * np.einsum("txac,ab,txbc->t", st.conj(), g5G, st)
         assert np.allclose(got[G], want, atol=1e-12)
+
+
+# ---------------------------------------------------------------- P17 generalised one-end loops (Eq. 2.6, N2)
+def test_p17_gen_one_end_loops_sum_over_a_complete_basis_is_the_flavour_sum(tiny):
+    """Eq. 2.6, noise average done exactly over the complete basis eta = e_k: the oracle's
+    per-source loops 2 s^dag g5 Gamma g5 D_W s must sum to sum_{x in t} tr[Gamma (M_u^-1 + M_d^-1)(x,x)]."""
+    d = tiny
+    dims, V = d["dims"], d["V"]
+    Md = dense_from_apply(lambda v: oracle.apply_M(dims, d["theta"], d["kappa"], -d["mu"], d["U"], v), V)
+    DW = dense_from_apply(lambda v: oracle.apply_M(dims, d["theta"], d["kappa"], 0.0, d["U"], v), V)
+    assert np.allclose(d["M"] + Md, 2 * DW, atol=1e-14)            # PAPER.md:64: M_u + M_d = 2 D_W
+    summ = d["Minv"] + np.linalg.inv(Md)
+    total = np.zeros((16, dims[3]), dtype=np.complex128)
+    for k in range(12 * V):
+        s_k = d["Minv"][:, k].reshape(V, 4, 3)
+        total += oracle.loops_gen_one_end(dims, d["theta"], d["kappa"], d["U"], s_k)
+    for G in range(16):
+        want = timeslice_projector_trace(dims, oracle.gamma(G), summ)
+        assert np.allclose(total[G], want, atol=1e-9), G
+    assert np.abs(total[0]).max() > 1.0 and np.abs(total[9]).max() > 1e-3
+
+
+def test_gen_one_end_loops_match_plain_einsum():
+    dims = (2, 4, 2, 4)
+    U = W.random_su3_links(dims, 0.5, 3)
+    s = W.random_spinor(dims, 9)
+    kappa = 0.15
+    got = oracle.loops_gen_one_end(dims, +1, kappa, U, s)
+    y = oracle.apply_M(dims, +1, kappa, 0.0, U, s)
+    Vs = volume(dims) // dims[3]
+    st, yt = s.reshape(dims[3], Vs, 4, 3), y.reshape(dims[3], Vs, 4, 3)
+    for G in range(16):
+        X5 = G5 @ oracle.gamma(G) @ G5
+        want = 2 * np.einsum("txac,ab,txbc->t", st.conj(), X5, yt)
+        assert np.allclose(got[G], want, atol=1e-12)
