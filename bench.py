@@ -345,21 +345,22 @@ def extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U):
         del a, b
     out["dslash"] = table
 
-    # ---- contraction kernels (H8, H9 and the one-end loops of Eq. 2.5, N1) on the slot the timed steps left
-    t.loops_reset(wl.derivative, one_end=True)
+    # ---- contraction kernels (H8, H9, the one-end loops of Eq. 2.5 (N1) and of Eq. 2.6 (N2; its two D_W stencil
+    # launches are counted with the stencils, not here) on the slot the timed steps left
+    t.loops_reset(wl.derivative, one_end=True, gen_one_end=True)
     t.profile(True)
     for _ in range(3):
         t.loops_add_lp(1)
     t.profile(False)
     sp = PRECS["f32" if prec_name == "bf16" else prec_name]
     w_sol = 8 if prec_name == "f64" else 4
-    names = {5: "local_16_gamma", 6: "derivative_4_directions", 7: "one_end_eq_2_5"}
+    names = {5: "local_16_gamma", 6: "derivative_4_directions", 7: "one_end_eq_2_5", 8: "gen_one_end_eq_2_6_contraction_only"}
     # algorithmic bytes per site of the full lattice and source: s once (eta is regenerated, never read);
     # derivative: s once + the 8 links of the site
     n_g = 18 if prec_name == "f64" else wl.reconstruct
-    by_site = {5: 24 * w_sol, 6: 24 * w_sol + 8 * n_g * (8 if prec_name == "f64" else 4), 7: 24 * w_sol}
+    by_site = {5: 24 * w_sol, 6: 24 * w_sol + 8 * n_g * (8 if prec_name == "f64" else 4), 7: 24 * w_sol, 8: 48 * w_sol}
     ct = {}
-    for k in (5, 6, 7):
+    for k in (5, 6, 7, 8):
         ms_k, n_k = t.profile_read(sp, k, nrhs)
         if n_k:
             us = ms_k * 1e3 / n_k
@@ -386,6 +387,9 @@ def extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U):
         t0 = time.perf_counter()
         oracle.loops_one_end(wl.dims, wl.kappa, wl.mu, oracle.noise(wl.dims, wl.noise_seed, 0))
         detail["t_one_end_contract_s"] = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        oracle.loops_gen_one_end(wl.dims, wl.t_boundary, wl.kappa, U, oracle.noise(wl.dims, wl.noise_seed, 0))
+        detail["t_gen_one_end_contract_s"] = time.perf_counter() - t0
         out["cpu_baseline"] = {"value": 1.0 / tcpu, "unit": UNIT, "cores": oracle.n_threads(), "kind": "oracle",
                                "sample": ("1 source: source preparation, 1- and 3-iteration CG solves, reconstruction, residual and one "
                                           f"contraction pass run in full; the {detail['iterations_extrapolated_to']}-iteration solve "

@@ -22,7 +22,9 @@
  *               sigma_01,02,03,12,13,23), then (TSM_OPS_DERIVATIVE) 16 + 16*mu + Gamma for the derivative
  *               loops, then (TSM_OPS_ONE_END) 16 more: the one-end loops of Eq. 2.5,
  *               L1_Gamma(t) = -2 i (2 kappa mu) sum_{x in t} s^dag gamma5 Gamma s, whose noise average is
- *               sum_{x in t} tr[Gamma (M_u^-1 - M_d^-1)(x,x)] (kappa-normalised operators).
+ *               sum_{x in t} tr[Gamma (M_u^-1 - M_d^-1)(x,x)] (kappa-normalised operators), then
+ *               (TSM_OPS_GEN_ONE_END) 16 more: Eq. 2.6, L2_Gamma(t) = 2 sum_{x in t} s^dag gamma5 Gamma gamma5 D_W s,
+ *               D_W = 1 - kappa D_hop, noise average sum_{x in t} tr[Gamma (M_u^-1 + M_d^-1)(x,x)].
  *   - The library allocates no large device memory.  All of it (link copies, solver
  *     vectors, solution slots, reduction scratch) lives in ONE caller-provided workspace
  *     (a torch tensor's data_ptr()), sized by tsm_workspace_bytes().  The context owns
@@ -65,10 +67,12 @@ enum { TSM_OP_D_EO = 0,      /* out_e = D_eo in_o                         (H5)  
 #define TSM_N_LOCAL_OPS 16
 #define TSM_N_DERIV_OPS 64
 #define TSM_N_ONE_END_OPS 16
-#define TSM_MAX_OPS (TSM_N_LOCAL_OPS + TSM_N_DERIV_OPS + TSM_N_ONE_END_OPS)
+#define TSM_N_GEN_ONE_END_OPS 16
+#define TSM_MAX_OPS (TSM_N_LOCAL_OPS + TSM_N_DERIV_OPS + TSM_N_ONE_END_OPS + TSM_N_GEN_ONE_END_OPS)
 /* which loops are computed besides the 16 local ones (bit mask `ops` of tsm_loops_reset / tsm_run_loop_set) */
 enum { TSM_OPS_DERIVATIVE = 1,   /* one-derivative loops, 4 directions (O6b)                 */
-       TSM_OPS_ONE_END = 2 };    /* one-end-trick loops of Eq. 2.5; need tsm_set_params   */
+       TSM_OPS_ONE_END = 2,      /* one-end-trick loops of Eq. 2.5; need tsm_set_params   */
+       TSM_OPS_GEN_ONE_END = 4 };/* generalised one-end-trick loops of Eq. 2.6; same      */
 
 /* Geometry (H1).  dims = (Lx,Ly,Lz,Lt), every extent even and >= 4.  t_boundary = +1
  * periodic or -1 antiperiodic in time (A3).  device = CUDA ordinal. */
@@ -139,7 +143,7 @@ int tsm_get_solution(tsm_ctx* ctx, int slot, int rhs, double* host_out /* [V][4]
 int tsm_set_solution(tsm_ctx* ctx, int slot, int rhs, const double* host_in /* [V][4][3][2] */);
 
 /* H8-H10: per-timeslice loops and the TSM accumulators (Eq. 2.4, O6, O6b, O7).  `ops` is a bit mask of
- * TSM_OPS_*: n_ops = 16 [+ 64] [+ 16].  The one-end loops are bilinear in s, and Eq. 2.4 is applied to them
+ * TSM_OPS_*: n_ops = 16 [+ 64] [+ 16] [+ 16].  The one-end loops are bilinear in s, and Eq. 2.4 is applied to them
  * exactly as to the others: correction = L1(s_HP) - L1(s_LP), biased estimate = L1(s_LP). */
 int tsm_loops_reset(tsm_ctx* ctx, int ops);
 int tsm_loops_add_correction(tsm_ctx* ctx, int slot_hp, int slot_lp); /* += L(HP)-L(LP); N_HP += nrhs */
@@ -168,7 +172,7 @@ long long tsm_launch_count(const tsm_ctx* ctx);
  * for one class and forgets them.  prec: TSM_F64/F32/BF16; kind: 0 stencil (H5), 1 stencil
  * with the x term, 2 stencil with x term and per-tile sum of |out|^2, 3 stencil with x term whose
  * result updates the CG residual in place (r -= alpha q, per-tile |r|^2), 4 the CG x/p update,
- * 5 / 6 / 7 the local / derivative / one-end contraction (prec = that of the slot);
+ * 5 / 6 / 7 / 8 the local / derivative / one-end / generalised one-end contraction (prec = that of the slot);
  * nrhs <= 0 matches any batch size. */
 int tsm_profile(tsm_ctx* ctx, int enable);
 int tsm_profile_read(tsm_ctx* ctx, int prec, int kind, int nrhs, double* total_ms, long long* count);

@@ -246,10 +246,12 @@ int tsm_loops_reset(tsm_ctx* ctx, int ops)
 {
     int rc = ctx_enter(ctx, true, false, false);
     if (rc) return rc;
-    if (ops < 0 || ops > (TSM_OPS_DERIVATIVE | TSM_OPS_ONE_END)) return tsm_fail(ctx, TSM_EINVAL, "bad loop operator set");
+    if (ops < 0 || ops > (TSM_OPS_DERIVATIVE | TSM_OPS_ONE_END | TSM_OPS_GEN_ONE_END)) return tsm_fail(ctx, TSM_EINVAL, "bad loop operator set");
     ctx->with_deriv = (ops & TSM_OPS_DERIVATIVE) ? 1 : 0;
     ctx->with_one_end = (ops & TSM_OPS_ONE_END) ? 1 : 0;
-    ctx->n_ops = TSM_N_LOCAL_OPS + (ctx->with_deriv ? TSM_N_DERIV_OPS : 0) + (ctx->with_one_end ? TSM_N_ONE_END_OPS : 0);
+    ctx->with_gen_one_end = (ops & TSM_OPS_GEN_ONE_END) ? 1 : 0;
+    ctx->n_ops = TSM_N_LOCAL_OPS + (ctx->with_deriv ? TSM_N_DERIV_OPS : 0) + (ctx->with_one_end ? TSM_N_ONE_END_OPS : 0) +
+                 (ctx->with_gen_one_end ? TSM_N_GEN_ONE_END_OPS : 0);
     ctx->n_hp = ctx->n_lp = 0;
     const size_t lb = (size_t)ctx->n_ops * ctx->g.L[3] * 2 * sizeof(double);
     TSM_CUDA(ctx, cudaMemsetAsync(ctx->acc_corr, 0, lb, ctx->stream));

@@ -10,6 +10,10 @@
 //     itself, C'_{ab}(t) = sum_{x in t, c} conj(s_{ac}(x)) s_{bc}(x), then
 //     L1_Gamma(t) = -2 i a sum_{ab} (gamma5 Gamma)_{ab} C'_{ab}(t), a = 2 kappa mu, whose noise average is
 //     sum_{x in t} tr[Gamma (M_u^-1 - M_d^-1)(x,x)].
+// N2  generalised one-end trick (Eq. 2.6): y = D_W s with D_W = M(mu = 0) = 1 - kappa D_hop
+//     (two stencil launches into a scratch field), C''_{ab}(t) = sum conj(s_{ac}) y_{bc},
+//     L2_Gamma(t) = 2 sum_{ab} (gamma5 Gamma gamma5)_{ab} C''_{ab}(t); noise average
+//     sum_{x in t} tr[Gamma (M_u^-1 + M_d^-1)(x,x)].
 // H10 Eq. 2.4 accumulators (O7).
 #include "reduce.cuh"
 
@@ -18,13 +22,14 @@ namespace {
 constexpr int CT_BS = 128;
 constexpr int CT_MAXBLK = 8;   // blocks per (timeslice, parity)
 
-// grid = (nblk * ngroup_in_launch, Lt, nrhs * 2); MODE 0: local; 1: derivative, mu = blockIdx.x / nblk; 2: one-end.
-// partials: [rhs][group 0..5][t][par][blk][32], group 0 local, 1..4 derivative mu, 5 one-end
-constexpr int CT_NGROUP = 6;
-enum { CT_LOCAL = 0, CT_DERIV = 1, CT_ONE_END = 2 };
+// grid = (nblk * ngroup_in_launch, Lt, nrhs * 2); MODE 0: local; 1: derivative, mu = blockIdx.x / nblk; 2: one-end;
+// 3: generalised one-end (second = D_W s, same [parity][rhs] layout as sol).
+// partials: [rhs][group 0..6][t][par][blk][32], group 0 local, 1..4 derivative mu, 5 one-end, 6 generalised one-end
+constexpr int CT_NGROUP = 7;
+enum { CT_LOCAL = 0, CT_DERIV = 1, CT_ONE_END = 2, CT_GEN_ONE_END = 3 };
 template <int PREC, int RECON, int MODE>
 __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs, const int nblk, const void* __restrict__ sol,
-                                                    const void* __restrict__ pack0, const void* __restrict__ pack1,
+                                                    const void* __restrict__ second, const void* __restrict__ pack0, const void* __restrict__ pack1,
                                                     const uint64_t seed, const uint32_t* __restrict__ ids, const int kind,
                                                     double* __restrict__ partials)
 {
@@ -47,9 +52,12 @@ __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs
         const int i = t * g.Vsh + j;
         const SiteCoord sc = decode_site(g, i, par);
         uint32_t bits = 0;
-        if (MODE != CT_ONE_END) bits = noise_bits(lex_of_site(g, sc), seed, sid, kind);
-        T v[24];
-        if (MODE != CT_DERIV) {
+        if (MODE == CT_LOCAL || MODE == CT_DERIV) bits = noise_bits(lex_of_site(g, sc), seed, sid, kind);
+        T v[24], sv[24];
+        if (MODE == CT_GEN_ONE_END) {
+            load_spinor<PREC>(s_same, i, sv);
+            load_spinor<PREC>((const char*)second + fpar * par + frhs * rhs, i, v);
+        } else if (MODE != CT_DERIV) {
             load_spinor<PREC>(s_same, i, v);
         } else {
             int nb[8];
@@ -82,6 +90,9 @@ __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs
                 if (MODE == CT_ONE_END) {   // conj(s) in place of conj(eta)
                     cr = (double)v[2 * (3 * al + c)];
                     ci = -(double)v[2 * (3 * al + c) + 1];
+                } else if (MODE == CT_GEN_ONE_END) {
+                    cr = (double)sv[2 * (3 * al + c)];
+                    ci = -(double)sv[2 * (3 * al + c) + 1];
                 } else {
                     float er, ei;
                     noise_value((bits >> (2 * (3 * al + c))) & 3, kind, er, ei);
@@ -108,7 +119,7 @@ __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs
     if (threadIdx.x < 32) {
         double tot = 0;
         for (int ww = 0; ww < CT_BS / 32; ww++) tot += sm[ww][threadIdx.x];
-        const int group = MODE == CT_DERIV ? 1 + mu : (MODE == CT_ONE_END ? 5 : 0);
+        const int group = MODE == CT_DERIV ? 1 + mu : (MODE == CT_ONE_END ? 5 : (MODE == CT_GEN_ONE_END ? 6 : 0));
         const size_t o = ((((size_t)rhs * CT_NGROUP + group) * g.L[3] + t) * 2 + par) * nblk + blk;
         partials[o * 32 + threadIdx.x] = tot;
     }
@@ -135,7 +146,8 @@ __global__ void k_contract_finish(const int Lt, const int nblk, const int n_ops,
         for (int al = 0; al < 4; al++) {
             const int be = gt.col[k][al];
             // one-end: (gamma5 Gamma)_{al,be} = +-Gamma_{al,be} (gamma5 = diag(1,1,-1,-1): phase + 2 on rows 2,3)
-            const int ph = (gt.ph[k][al] + ((group == 5 && al >= 2) ? 2 : 0)) & 3;
+            // generalised one-end: (gamma5 Gamma gamma5)_{al,be}: one more sign when be is a lower spin
+            const int ph = (gt.ph[k][al] + ((group >= 5 && al >= 2) ? 2 : 0) + ((group == 6 && be >= 2) ? 2 : 0)) & 3;
             const double cr = C[2 * (4 * al + be)], ci = C[2 * (4 * al + be) + 1];
             // multiply by i^ph
             re += (ph == 0) ? cr : (ph == 1) ? -ci : (ph == 2) ? -cr : ci;
@@ -145,6 +157,9 @@ __global__ void k_contract_finish(const int Lt, const int nblk, const int n_ops,
         if (group == 5) {   // times -2 i a:  -2ia (re + i im) = 2a im - i 2a re
             dst[0] = two_a * im;
             dst[1] = -two_a * re;
+        } else if (group == 6) {   // times 2 (Eq. 2.6)
+            dst[0] = 2.0 * re;
+            dst[1] = 2.0 * im;
         } else {
             dst[0] = re;
             dst[1] = im;
@@ -215,23 +230,40 @@ int launch_contract(tsm_ctx* ctx, int slot)
     const int kind = ctx->slot_kind[slot];
     const dim3 grid_l(nblk, g.L[3], nrhs * 2), grid_d(nblk * 4, g.L[3], nrhs * 2);
     const void* sol = ctx->slot[slot];
+    // N2: second = D_W s = (1 - kappa D_hop) s on the full lattice, into the (idle) solver vectors
+    void* second = ctx->vec[0];
+    if (ctx->with_gen_one_end) {
+        if (!ctx->have_params) return tsm_fail(ctx, TSM_ESTATE, "generalised one-end loops need kappa (tsm_set_params)");
+        const size_t fp = field_bytes(prec, g.Vh, nrhs);
+        const TwistCoef one = {1, 0, 1, 0}, mk = {-ctx->kappa, 0, -ctx->kappa, 0};
+        const char* s_e = (const char*)sol; const char* s_o = s_e + fp;
+        int rc;
+        if ((rc = launch_dslash(ctx, prec, 0, false, nrhs, s_o, s_e, second, {one, mk}, 0))) return rc;
+        if ((rc = launch_dslash(ctx, prec, 1, false, nrhs, s_e, s_o, (char*)second + fp, {one, mk}, 0))) return rc;
+    }
 #define CT(P, R)                                                                                                             \
     do {                                                                                                                     \
         const void* p0 = (P == TSM_F64) ? ctx->gauge64[0] : ctx->gauge32[0];                                                 \
         const void* p1 = (P == TSM_F64) ? ctx->gauge64[1] : ctx->gauge32[1];                                                 \
         int pi = prof_begin(ctx, P, 5, nrhs);                                                                                \
-        k_contract<P, R, CT_LOCAL><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, p0, p1, seed, ids, kind, ctx->partials); \
+        k_contract<P, R, CT_LOCAL><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials); \
         prof_end(ctx, pi);                                                                                                   \
         ctx->launches++;                                                                                                     \
         if (ctx->with_deriv) {                                                                                               \
             pi = prof_begin(ctx, P, 6, nrhs);                                                                                \
-            k_contract<P, R, CT_DERIV><<<grid_d, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, p0, p1, seed, ids, kind, ctx->partials); \
+            k_contract<P, R, CT_DERIV><<<grid_d, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials); \
+            prof_end(ctx, pi);                                                                                               \
+            ctx->launches++;                                                                                                 \
+        }                                                                                                                    \
+        if (ctx->with_gen_one_end) {                                                                                         \
+            pi = prof_begin(ctx, P, 8, nrhs);                                                                                \
+            k_contract<P, R, CT_GEN_ONE_END><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials); \
             prof_end(ctx, pi);                                                                                               \
             ctx->launches++;                                                                                                 \
         }                                                                                                                    \
         if (ctx->with_one_end) {                                                                                             \
             pi = prof_begin(ctx, P, 7, nrhs);                                                                                \
-            k_contract<P, R, CT_ONE_END><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, p0, p1, seed, ids, kind, ctx->partials); \
+            k_contract<P, R, CT_ONE_END><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials); \
             prof_end(ctx, pi);                                                                                               \
             ctx->launches++;                                                                                                 \
         }                                                                                                                    \
@@ -246,6 +278,7 @@ int launch_contract(tsm_ctx* ctx, int slot)
     ob.v[0] = 0;
     for (int m = 0; m < 4; m++) ob.v[1 + m] = ctx->with_deriv ? TSM_N_LOCAL_OPS + 16 * m : -1;
     ob.v[5] = ctx->with_one_end ? TSM_N_LOCAL_OPS + (ctx->with_deriv ? TSM_N_DERIV_OPS : 0) : -1;
+    ob.v[6] = ctx->with_gen_one_end ? TSM_N_LOCAL_OPS + (ctx->with_deriv ? TSM_N_DERIV_OPS : 0) + (ctx->with_one_end ? TSM_N_ONE_END_OPS : 0) : -1;
     if (ctx->with_one_end && !ctx->have_params) return tsm_fail(ctx, TSM_ESTATE, "one-end loops need kappa/mu (tsm_set_params)");
     const dim3 grid_f(g.L[3], CT_NGROUP, nrhs);
     k_contract_finish<<<grid_f, 32, 0, ctx->stream>>>(g.L[3], nblk, ctx->n_ops, ctx->gam, ob, 2.0 * (2.0 * ctx->kappa * ctx->mu),

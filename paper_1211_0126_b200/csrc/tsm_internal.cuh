@@ -424,7 +424,7 @@ struct tsm_ctx {
     double* host_small;              // pinned scratch (loops, unitarity)
     uint32_t* ids_dev;               // [2][TSM_MAX_NRHS]
     GammaTable gam;
-    int n_ops, with_deriv, with_one_end, n_hp, n_lp;
+    int n_ops, with_deriv, with_one_end, with_gen_one_end, n_hp, n_lp;
     long long launches;
     bool prof_on;
     std::vector<ProfRec> prof;

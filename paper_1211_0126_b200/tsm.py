@@ -20,7 +20,7 @@ F64, F32, BF16 = 0, 1, 2
 Z4, Z2 = 0, 1
 OP_D_EO, OP_D_OE, OP_MHAT, OP_MHAT_DAG, OP_M_FULL = 0, 1, 2, 3, 4
 MAX_NRHS = 16
-OPS_DERIVATIVE, OPS_ONE_END = 1, 2
+OPS_DERIVATIVE, OPS_ONE_END, OPS_GEN_ONE_END = 1, 2, 4
 PREC = {"f64": F64, "f32": F32, "bf16": BF16}
 
 EXPORTS = [
@@ -236,13 +236,14 @@ class Tsm:
         self._check(self.lib.tsm_set_solution(self._h, slot, rhs, _dptr(a)))
 
     @staticmethod
-    def _ops(with_derivative: bool, one_end: bool) -> int:
-        return (OPS_DERIVATIVE if with_derivative else 0) | (OPS_ONE_END if one_end else 0)
+    def _ops(with_derivative: bool, one_end: bool, gen_one_end: bool = False) -> int:
+        return ((OPS_DERIVATIVE if with_derivative else 0) | (OPS_ONE_END if one_end else 0)
+                | (OPS_GEN_ONE_END if gen_one_end else 0))
 
-    def loops_reset(self, with_derivative: bool = False, one_end: bool = False):
-        """n_ops = 16 local [+ 64 derivative] [+ 16 one-end (Eq. 2.5)] loops, in that order."""
-        self.n_ops = 16 + (64 if with_derivative else 0) + (16 if one_end else 0)
-        self._check(self.lib.tsm_loops_reset(self._h, self._ops(with_derivative, one_end)))
+    def loops_reset(self, with_derivative: bool = False, one_end: bool = False, gen_one_end: bool = False):
+        """n_ops = 16 local [+ 64 derivative] [+ 16 one-end (Eq. 2.5)] [+ 16 generalised one-end (Eq. 2.6)]."""
+        self.n_ops = 16 + (64 if with_derivative else 0) + (16 if one_end else 0) + (16 if gen_one_end else 0)
+        self._check(self.lib.tsm_loops_reset(self._h, self._ops(with_derivative, one_end, gen_one_end)))
 
     def loops_add_correction(self, slot_hp: int, slot_lp: int):
         self._check(self.lib.tsm_loops_add_correction(self._h, slot_hp, slot_lp))
@@ -274,12 +275,12 @@ class Tsm:
 
     def run_loop_set(self, seed: int, n_hp: int, n_lp: int, lp_prec: int, lp_tol: float, lp_iters: int,
                      hp_tol: float = 1e-10, hp_max_iter: int = 5000, nrhs: int = 1,
-                     with_derivative: bool = False, kind: int = Z4, one_end: bool = False):
+                     with_derivative: bool = False, kind: int = Z4, one_end: bool = False, gen_one_end: bool = False):
         """Eq. 2.4 for one configuration.  Returns (loops [n_ops][Lt], device seconds, rc)."""
-        self.n_ops = 16 + (64 if with_derivative else 0) + (16 if one_end else 0)
+        self.n_ops = 16 + (64 if with_derivative else 0) + (16 if one_end else 0) + (16 if gen_one_end else 0)
         out = np.empty((self.n_ops, self.Lt), dtype=np.complex128)
         secs = ctypes.c_double(0.0)
         rc = self.lib.tsm_run_loop_set(self._h, seed, kind, n_hp, n_lp, lp_prec, lp_tol, lp_iters, hp_tol,
-                                       hp_max_iter, nrhs, self._ops(with_derivative, one_end), _dptr(out), ctypes.byref(secs))
+                                       hp_max_iter, nrhs, self._ops(with_derivative, one_end, gen_one_end), _dptr(out), ctypes.byref(secs))
         self._check(rc, allow=(EBREAKDOWN, ENOCONV))
         return out, secs.value, rc

@@ -469,3 +469,38 @@ def test_one_end_fp32_slot(ragged):
     want = oracle.loops_one_end(c.dims, c.kappa, c.mu, s)
     assert rel(c.t.loops_source(1, 1)[16:], want) < 1e-5
     c.t.loops_reset(False)
+
+
+# ---------------------------------------------------------------- N2: generalised one-end trick loops (Eq. 2.6)
+def test_gen_one_end_loops_parity_on_the_oracle_solution(small, ragged):
+    """All four operator groups at once (16 local + 64 derivative + 16 one-end + 16 generalised one-end), on the
+    oracle's own s: 1e-12 relative to the largest loop of each group."""
+    for c in (small, ragged):
+        seed = 321
+        c.t.loops_reset(True, one_end=True, gen_one_end=True)
+        rc, _ = c.t.solve(seed, [0, 5, 9], F64, 0.0, 1, slot=0)
+        for j, sid in enumerate((0, 5, 9)):
+            eta = oracle.noise(c.dims, seed, sid)
+            s, _ = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, 1e-10, 2000)
+            c.t.set_solution(0, j, s)
+        for j, sid in enumerate((0, 5, 9)):
+            eta = oracle.noise(c.dims, seed, sid)
+            s = c.t.get_solution(0, j)
+            want = oracle.all_loops(c.dims, c.theta, c.U, eta, s, True, one_end=(c.kappa, c.mu), gen_one_end=c.kappa)
+            got = c.t.loops_source(0, j)
+            assert got.shape == want.shape == (112, c.dims[3])
+            for lo, hi in ((0, 16), (16, 80), (80, 96), (96, 112)):
+                assert rel(got[lo:hi], want[lo:hi]) < 1e-12, (c.dims, j, lo)
+        c.t.loops_reset(False)
+
+
+def test_gen_one_end_alone_and_fp32(ragged):
+    c = ragged
+    c.t.loops_reset(False, gen_one_end=True)
+    rc, _ = c.t.solve(7, [2, 3], F32, 0.0, 25, slot=1)
+    s = c.t.get_solution(1, 0)
+    want = oracle.loops_gen_one_end(c.dims, c.theta, c.kappa, c.U, s)
+    got = c.t.loops_source(1, 0)
+    assert got.shape == (32, c.dims[3])
+    assert rel(got[16:], want) < 1e-5
+    c.t.loops_reset(False)
