@@ -176,10 +176,22 @@ def loops_gen_one_end(dims, theta, kappa, U, s) -> np.ndarray:
     return out
 
 
-def all_loops(dims, theta, U, eta, s, with_derivative: bool, one_end=None, gen_one_end=None) -> np.ndarray:
+def loops_momentum(dims, eta, s, momenta) -> np.ndarray:
+    """Reading A25: L_Gamma(t, p) = sum_x exp(+i p.x) eta^dag Gamma s, p_i = 2 pi n_i / L_i; [nmom][16][Lt]."""
+    eta = _c128(eta)
+    s = _c128(s)
+    mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+    out = np.empty((mom.shape[0], 16, dims[3]), dtype=np.complex128)
+    lib().oracle_loops_momentum(_c_int4(*dims), _d(eta), _d(s), ctypes.c_int(mom.shape[0]),
+                                mom.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), _d(out))
+    return out
+
+
+def all_loops(dims, theta, U, eta, s, with_derivative: bool, one_end=None, gen_one_end=None, momenta=None) -> np.ndarray:
     """[n_ops][Lt]: the 16 local loops, then (if asked) [mu][Gamma] derivative loops (O6b order), then
     (if one_end=(kappa, mu) is given) the 16 one-end loops of Eq. 2.5, then (if gen_one_end=kappa is given)
-    the 16 generalised one-end loops of Eq. 2.6."""
+    the 16 generalised one-end loops of Eq. 2.6, then (if momenta [nmom][3] are given) 16 momentum-projected
+    local loops per momentum (reading A25)."""
     parts = [loops(dims, eta, s)]
     if with_derivative:
         parts.append(loops_deriv(dims, theta, U, eta, s).reshape(64, dims[3]))
@@ -187,6 +199,8 @@ def all_loops(dims, theta, U, eta, s, with_derivative: bool, one_end=None, gen_o
         parts.append(loops_one_end(dims, one_end[0], one_end[1], s))
     if gen_one_end is not None:
         parts.append(loops_gen_one_end(dims, theta, gen_one_end, U, s))
+    if momenta is not None:
+        parts.append(loops_momentum(dims, eta, s, momenta).reshape(-1, dims[3]))
     return parts[0] if len(parts) == 1 else np.concatenate(parts, axis=0)
 
 

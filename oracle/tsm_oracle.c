@@ -19,7 +19,7 @@
  * P9 free-field loops, P10 one-end identity, P11 TSM algebra, P12 Philox known
  * answers, P13 CG Krylov optimality, P14 derivative, P15 delta-source stencil.
  * P16 one-end trick (Eq. 2.5) against dense M(mu)^-1 - M(-mu)^-1, P17 generalised one-end
- * trick (Eq. 2.6) against dense M(mu)^-1 + M(-mu)^-1.
+ * trick (Eq. 2.6) against dense M(mu)^-1 + M(-mu)^-1, P18 momentum-projected loops against numpy's FFT.
  * Parity unpinned (defined only by the algorithm O5): the values of truncated LP
  * iterates beyond P13's Krylov-minimiser check.
  *
@@ -596,4 +596,48 @@ void oracle_loops_gen_one_end(const int L[4], int theta, double kappa, const dou
         }
     }
     free(y);
+}
+
+/* ------------------------------------------------------------------------- */
+/* N3: Fourier transform of the loops ("the CUFFT  */
+/* library" is used for it; the paper gives no formula).  Reading A25: for    */
+/* integer triples n, spatial momentum p_i = 2 pi n_i / L_i, the plain        */
+/* definition                                                                 */
+/*   L_Gamma(t, p) = sum_{x in t} exp(+i p.x) sum_{alpha beta c}              */
+/*        conj(eta_{alpha c}(x)) Gamma_{alpha beta} s_{beta c}(x)             */
+/* (n = 0 is O6).  mom is [nmom][3], out is [nmom][16][Lt][2].                */
+/* ------------------------------------------------------------------------- */
+void oracle_loops_momentum(const int L[4], const double *eta_, const double *s_, int nmom, const int *mom, double *out_)
+{
+    const cplx *eta = (const cplx *)eta_, *s = (const cplx *)s_;
+    cplx *out = (cplx *)out_;
+    const long Vs = (long)L[0] * L[1] * L[2];
+    const int T = L[3];
+    const double twopi = 6.283185307179586476925286766559;
+    for (int m = 0; m < nmom; m++)
+        for (int G = 0; G < 16; G++) {
+            double gm[32];
+            oracle_gamma(G, gm);
+            for (int t = 0; t < T; t++) {
+                cplx acc = 0;
+                for (long sx = 0; sx < Vs; sx++) {
+                    const long st = (long)t * Vs + sx;
+                    int x[4];
+                    coords_of(L, st, x);
+                    const double px = twopi * ((double)mom[3 * m] * x[0] / L[0] + (double)mom[3 * m + 1] * x[1] / L[1] +
+                                               (double)mom[3 * m + 2] * x[2] / L[2]);
+                    const cplx ph = cos(px) + I * sin(px);
+                    cplx d = 0;
+                    for (int a = 0; a < NS; a++)
+                        for (int b = 0; b < NS; b++) {
+                            const cplx gab = gm[2 * (4 * a + b)] + I * gm[2 * (4 * a + b) + 1];
+                            if (gab == 0) continue;
+                            for (int c = 0; c < NC; c++)
+                                d += conj(eta[(st * NS + a) * NC + c]) * gab * s[(st * NS + b) * NC + c];
+                        }
+                    acc += ph * d;
+                }
+                out[((long)m * 16 + G) * T + t] = acc;
+            }
+        }
 }

@@ -380,3 +380,25 @@ def test_gen_one_end_loops_match_plain_einsum():
         X5 = G5 @ oracle.gamma(G) @ G5
         want = 2 * np.einsum("txac,ab,txbc->t", st.conj(), X5, yt)
         assert np.allclose(got[G], want, atol=1e-12)
+
+
+# ---------------------------------------------------------------- P18 momentum-projected loops (N3)
+def test_p18_momentum_loops_against_numpy_fft():
+    """Reading A25 pinned by a library FFT: the per-site density d_Gamma(x) = eta^dag Gamma s, transformed by
+    numpy.fft over the three spatial axes (kernel exp(-2 pi i n.x/L)), equals the oracle's loops at -n."""
+    dims = (4, 6, 2, 4)
+    eta = oracle.noise(dims, 5, 3)
+    s = W.random_spinor(dims, 10)
+    Lx, Ly, Lz, Lt = dims
+    moms = [(0, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1), (-1, 2, 1), (3, -2, 0)]
+    got = oracle.loops_momentum(dims, eta, s, moms)
+    assert np.allclose(got[0], oracle.loops(dims, eta, s), atol=1e-12)           # n = 0 is O6
+    for G in (0, 1, 4, 9, 13):
+        dens = np.einsum("xac,ab,xbc->x", eta.conj(), oracle.gamma(G), s).reshape(Lt, Lz, Ly, Lx)
+        ft = np.fft.fftn(dens, axes=(1, 2, 3))                                   # indexed [t][nz][ny][nx]
+        for m, (nx, ny, nz) in enumerate(moms):
+            want = ft[:, (-nz) % Lz, (-ny) % Ly, (-nx) % Lx]
+            assert np.allclose(got[m, G], want, atol=1e-10), (G, m)
+    # n and n + L are the same momentum
+    again = oracle.loops_momentum(dims, eta, s, [(1 + Lx, 0, 0), (-1, 2 - Ly, 1 + 3 * Lz)])
+    assert np.allclose(again[0], got[1], atol=1e-10) and np.allclose(again[1], got[4], atol=1e-10)
