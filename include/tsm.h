@@ -68,11 +68,13 @@ enum { TSM_OP_D_EO = 0,      /* out_e = D_eo in_o                         (H5)  
 #define TSM_N_DERIV_OPS 64
 #define TSM_N_ONE_END_OPS 16
 #define TSM_N_GEN_ONE_END_OPS 16
-#define TSM_MAX_OPS (TSM_N_LOCAL_OPS + TSM_N_DERIV_OPS + TSM_N_ONE_END_OPS + TSM_N_GEN_ONE_END_OPS)
+#define TSM_MAX_MOMENTA 16
+#define TSM_MAX_OPS (TSM_N_LOCAL_OPS + TSM_N_DERIV_OPS + TSM_N_ONE_END_OPS + TSM_N_GEN_ONE_END_OPS + 16 * TSM_MAX_MOMENTA)
 /* which loops are computed besides the 16 local ones (bit mask `ops` of tsm_loops_reset / tsm_run_loop_set) */
 enum { TSM_OPS_DERIVATIVE = 1,   /* one-derivative loops, 4 directions (O6b)                 */
        TSM_OPS_ONE_END = 2,      /* one-end-trick loops of Eq. 2.5; need tsm_set_params   */
-       TSM_OPS_GEN_ONE_END = 4 };/* generalised one-end-trick loops of Eq. 2.6; same      */
+       TSM_OPS_GEN_ONE_END = 4,  /* generalised one-end-trick loops of Eq. 2.6; same      */
+       TSM_OPS_MOMENTA = 8 };    /* momentum-projected local loops for the list of tsm_loops_set_momenta   */
 
 /* Geometry (H1).  dims = (Lx,Ly,Lz,Lt), every extent even and >= 4.  t_boundary = +1
  * periodic or -1 antiperiodic in time (A3).  device = CUDA ordinal. */
@@ -143,9 +145,14 @@ int tsm_get_solution(tsm_ctx* ctx, int slot, int rhs, double* host_out /* [V][4]
 int tsm_set_solution(tsm_ctx* ctx, int slot, int rhs, const double* host_in /* [V][4][3][2] */);
 
 /* H8-H10: per-timeslice loops and the TSM accumulators (Eq. 2.4, O6, O6b, O7).  `ops` is a bit mask of
- * TSM_OPS_*: n_ops = 16 [+ 64] [+ 16] [+ 16].  The one-end loops are bilinear in s, and Eq. 2.4 is applied to them
+ * TSM_OPS_*: n_ops = 16 [+ 64] [+ 16] [+ 16] [+ 16 nmom].  The one-end loops are bilinear in s, and Eq. 2.4 is applied to them
  * exactly as to the others: correction = L1(s_HP) - L1(s_LP), biased estimate = L1(s_LP). */
 int tsm_loops_reset(tsm_ctx* ctx, int ops);
+/* Momenta of the projected loops (Fourier transform of the loops; reading A25): n is [nmom][3]
+ * integers, p_i = 2 pi n_i / L_i, nmom <= TSM_MAX_MOMENTA.  With TSM_OPS_MOMENTA in `ops` the op list ends with
+ * 16 loops per momentum, op = base + 16*m + Gamma: sum_{x in t} exp(+i p.x) eta^dag Gamma s.  Call it before
+ * tsm_loops_reset (which fixes n_ops). */
+int tsm_loops_set_momenta(tsm_ctx* ctx, int nmom, const int* n);
 int tsm_loops_add_correction(tsm_ctx* ctx, int slot_hp, int slot_lp); /* += L(HP)-L(LP); N_HP += nrhs */
 int tsm_loops_add_lp(tsm_ctx* ctx, int slot_lp);                   /* += L(LP); N_LP += nrhs  */
 int tsm_loops_source(tsm_ctx* ctx, int slot, int rhs, double* host_out /* [n_ops][Lt][2] */);
@@ -172,7 +179,7 @@ long long tsm_launch_count(const tsm_ctx* ctx);
  * for one class and forgets them.  prec: TSM_F64/F32/BF16; kind: 0 stencil (H5), 1 stencil
  * with the x term, 2 stencil with x term and per-tile sum of |out|^2, 3 stencil with x term whose
  * result updates the CG residual in place (r -= alpha q, per-tile |r|^2), 4 the CG x/p update,
- * 5 / 6 / 7 / 8 the local / derivative / one-end / generalised one-end contraction (prec = that of the slot);
+ * 5 / 6 / 7 / 8 / 9 the local / derivative / one-end / generalised one-end / momentum contraction (prec = that of the slot);
  * nrhs <= 0 matches any batch size. */
 int tsm_profile(tsm_ctx* ctx, int enable);
 int tsm_profile_read(tsm_ctx* ctx, int prec, int kind, int nrhs, double* total_ms, long long* count);

@@ -31,7 +31,7 @@ size_t carve_workspace(tsm_ctx* ctx, int max_nrhs, char* base)
     { size_t o = c.take(6 * fb); if (base) for (int k = 0; k < 6; k++) ctx->vec[k] = at(o + k * fb); }
     for (int s = 0; s < 2; s++) { size_t o = c.take(2 * fb); if (base) ctx->slot[s] = at(o); }
     size_t pc = (size_t)ctx->nsm * 16 * max_nrhs;
-    const size_t pc2 = (size_t)max_nrhs * 7 * g.L[3] * 2 * 8 * 32;
+    const size_t pc2 = (size_t)max_nrhs * (7 + TSM_MAX_MOMENTA) * g.L[3] * 2 * 8 * 32;
     if (pc2 > pc) pc = pc2;
     { size_t o = c.take(pc * sizeof(double)); if (base) { ctx->partials = (double*)at(o); ctx->partials_count = pc; } }
     const size_t npc = (size_t)max_nrhs * ((g.Vh + 127) / 128);
@@ -102,6 +102,8 @@ int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
     ctx->with_deriv = 0;
     ctx->with_one_end = 0;
     ctx->with_gen_one_end = 0;
+    ctx->with_momenta = 0;
+    ctx->n_mom = 0;
     ctx->n_hp = ctx->n_lp = 0;
     ctx->launches = 0;
     ctx->prof_on = false;

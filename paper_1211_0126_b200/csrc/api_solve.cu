@@ -246,16 +246,29 @@ int tsm_loops_reset(tsm_ctx* ctx, int ops)
 {
     int rc = ctx_enter(ctx, true, false, false);
     if (rc) return rc;
-    if (ops < 0 || ops > (TSM_OPS_DERIVATIVE | TSM_OPS_ONE_END | TSM_OPS_GEN_ONE_END)) return tsm_fail(ctx, TSM_EINVAL, "bad loop operator set");
+    if (ops < 0 || ops > (TSM_OPS_DERIVATIVE | TSM_OPS_ONE_END | TSM_OPS_GEN_ONE_END | TSM_OPS_MOMENTA))
+        return tsm_fail(ctx, TSM_EINVAL, "bad loop operator set");
     ctx->with_deriv = (ops & TSM_OPS_DERIVATIVE) ? 1 : 0;
     ctx->with_one_end = (ops & TSM_OPS_ONE_END) ? 1 : 0;
     ctx->with_gen_one_end = (ops & TSM_OPS_GEN_ONE_END) ? 1 : 0;
     ctx->n_ops = TSM_N_LOCAL_OPS + (ctx->with_deriv ? TSM_N_DERIV_OPS : 0) + (ctx->with_one_end ? TSM_N_ONE_END_OPS : 0) +
                  (ctx->with_gen_one_end ? TSM_N_GEN_ONE_END_OPS : 0);
+    ctx->with_momenta = (ops & TSM_OPS_MOMENTA) ? 1 : 0;
+    if (ctx->with_momenta) ctx->n_ops += 16 * ctx->n_mom;
     ctx->n_hp = ctx->n_lp = 0;
     const size_t lb = (size_t)ctx->n_ops * ctx->g.L[3] * 2 * sizeof(double);
     TSM_CUDA(ctx, cudaMemsetAsync(ctx->acc_corr, 0, lb, ctx->stream));
     TSM_CUDA(ctx, cudaMemsetAsync(ctx->acc_lp, 0, lb, ctx->stream));
+    return TSM_OK;
+}
+
+int tsm_loops_set_momenta(tsm_ctx* ctx, int nmom, const int* n)
+{
+    if (!ctx) return TSM_EINVAL;
+    if (nmom < 0 || nmom > TSM_MAX_MOMENTA || (nmom > 0 && !n)) return tsm_fail(ctx, TSM_EINVAL, "bad momentum list");
+    ctx->n_mom = nmom;
+    for (int m = 0; m < nmom; m++)
+        for (int k = 0; k < 3; k++) ctx->mom[m][k] = n[3 * m + k];
     return TSM_OK;
 }
 

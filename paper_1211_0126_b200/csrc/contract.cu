@@ -14,6 +14,9 @@
 //     (two stencil launches into a scratch field), C''_{ab}(t) = sum conj(s_{ac}) y_{bc},
 //     L2_Gamma(t) = 2 sum_{ab} (gamma5 Gamma gamma5)_{ab} C''_{ab}(t); noise average
 //     sum_{x in t} tr[Gamma (M_u^-1 + M_d^-1)(x,x)].
+// N3  momentum-projected local loops (PAPER.md:72 uses cuFFT for the Fourier transform; reading A25): for a
+//     short list of integer momenta n, L_Gamma(t, p) = sum_{x in t} exp(+2 pi i n.x/L) eta^dag Gamma s, as one
+//     more block group per momentum (a direct phase sum: a handful of momenta, not a full FFT).
 // H10 Eq. 2.4 accumulators (O7).
 #include "reduce.cuh"
 
@@ -24,14 +27,17 @@ constexpr int CT_MAXBLK = 8;   // blocks per (timeslice, parity)
 
 // grid = (nblk * ngroup_in_launch, Lt, nrhs * 2); MODE 0: local; 1: derivative, mu = blockIdx.x / nblk; 2: one-end;
 // 3: generalised one-end (second = D_W s, same [parity][rhs] layout as sol).
-// partials: [rhs][group 0..6][t][par][blk][32], group 0 local, 1..4 derivative mu, 5 one-end, 6 generalised one-end
-constexpr int CT_NGROUP = 7;
-enum { CT_LOCAL = 0, CT_DERIV = 1, CT_ONE_END = 2, CT_GEN_ONE_END = 3 };
+// 4: momentum-projected local, momentum index = blockIdx.x / nblk.
+// partials: [rhs][group][t][par][blk][32], group 0 local, 1..4 derivative mu, 5 one-end, 6 generalised one-end,
+// 7 + m momentum m
+constexpr int CT_NGROUP = 7 + TSM_MAX_MOMENTA;
+enum { CT_LOCAL = 0, CT_DERIV = 1, CT_ONE_END = 2, CT_GEN_ONE_END = 3, CT_MOMENTUM = 4 };
+struct Momenta { int n[TSM_MAX_MOMENTA][3]; };
 template <int PREC, int RECON, int MODE>
 __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs, const int nblk, const void* __restrict__ sol,
                                                     const void* __restrict__ second, const void* __restrict__ pack0, const void* __restrict__ pack1,
                                                     const uint64_t seed, const uint32_t* __restrict__ ids, const int kind,
-                                                    double* __restrict__ partials)
+                                                    double* __restrict__ partials, const Momenta mom)
 {
     using T = typename PT<PREC>::real;
     const int Vh = g.Vh;
@@ -52,7 +58,7 @@ __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs
         const int i = t * g.Vsh + j;
         const SiteCoord sc = decode_site(g, i, par);
         uint32_t bits = 0;
-        if (MODE == CT_LOCAL || MODE == CT_DERIV) bits = noise_bits(lex_of_site(g, sc), seed, sid, kind);
+        if (MODE == CT_LOCAL || MODE == CT_DERIV || MODE == CT_MOMENTUM) bits = noise_bits(lex_of_site(g, sc), seed, sid, kind);
         T v[24], sv[24];
         if (MODE == CT_GEN_ONE_END) {
             load_spinor<PREC>(s_same, i, sv);
@@ -80,6 +86,20 @@ __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs
                 su3_mul(ub, sb + 6 * al, b);
 #pragma unroll
                 for (int k = 0; k < 6; k++) v[6 * al + k] = (T)0.5 * (ph_f * a[k] - ph_b * b[k]);
+            }
+        }
+        if (MODE == CT_MOMENTUM) {   // s <- exp(2 pi i n.x/L) s; the fraction is reduced in integers first
+            const int x = 2 * sc.xh + sc.rowpar;
+            const double fr = (double)(((long long)mom.n[mu][0] * x) % g.L[0]) / g.L[0] +
+                              (double)(((long long)mom.n[mu][1] * sc.y) % g.L[1]) / g.L[1] +
+                              (double)(((long long)mom.n[mu][2] * sc.z) % g.L[2]) / g.L[2];
+            double sn, cs;
+            sincospi(2.0 * fr, &sn, &cs);
+#pragma unroll
+            for (int q = 0; q < 12; q++) {
+                const double re = (double)v[2 * q], im = (double)v[2 * q + 1];
+                v[2 * q] = (T)(cs * re - sn * im);
+                v[2 * q + 1] = (T)(cs * im + sn * re);
             }
         }
 #pragma unroll
@@ -119,7 +139,7 @@ __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs
     if (threadIdx.x < 32) {
         double tot = 0;
         for (int ww = 0; ww < CT_BS / 32; ww++) tot += sm[ww][threadIdx.x];
-        const int group = MODE == CT_DERIV ? 1 + mu : (MODE == CT_ONE_END ? 5 : (MODE == CT_GEN_ONE_END ? 6 : 0));
+        const int group = MODE == CT_DERIV ? 1 + mu : (MODE == CT_ONE_END ? 5 : (MODE == CT_GEN_ONE_END ? 6 : (MODE == CT_MOMENTUM ? 7 + mu : 0)));
         const size_t o = ((((size_t)rhs * CT_NGROUP + group) * g.L[3] + t) * 2 + par) * nblk + blk;
         partials[o * 32 + threadIdx.x] = tot;
     }
@@ -147,7 +167,7 @@ __global__ void k_contract_finish(const int Lt, const int nblk, const int n_ops,
             const int be = gt.col[k][al];
             // one-end: (gamma5 Gamma)_{al,be} = +-Gamma_{al,be} (gamma5 = diag(1,1,-1,-1): phase + 2 on rows 2,3)
             // generalised one-end: (gamma5 Gamma gamma5)_{al,be}: one more sign when be is a lower spin
-            const int ph = (gt.ph[k][al] + ((group >= 5 && al >= 2) ? 2 : 0) + ((group == 6 && be >= 2) ? 2 : 0)) & 3;
+            const int ph = (gt.ph[k][al] + (((group == 5 || group == 6) && al >= 2) ? 2 : 0) + ((group == 6 && be >= 2) ? 2 : 0)) & 3;
             const double cr = C[2 * (4 * al + be)], ci = C[2 * (4 * al + be) + 1];
             // multiply by i^ph
             re += (ph == 0) ? cr : (ph == 1) ? -ci : (ph == 2) ? -cr : ci;
@@ -228,7 +248,10 @@ int launch_contract(tsm_ctx* ctx, int slot)
     const uint32_t* ids = ctx->ids_dev + slot * TSM_MAX_NRHS;
     const uint64_t seed = ctx->slot_seed[slot];
     const int kind = ctx->slot_kind[slot];
-    const dim3 grid_l(nblk, g.L[3], nrhs * 2), grid_d(nblk * 4, g.L[3], nrhs * 2);
+    const dim3 grid_l(nblk, g.L[3], nrhs * 2), grid_d(nblk * 4, g.L[3], nrhs * 2), grid_m(nblk * (ctx->n_mom > 0 ? ctx->n_mom : 1), g.L[3], nrhs * 2);
+    Momenta mom;
+    for (int m = 0; m < TSM_MAX_MOMENTA; m++)
+        for (int k = 0; k < 3; k++) mom.n[m][k] = m < ctx->n_mom ? ctx->mom[m][k] : 0;
     const void* sol = ctx->slot[slot];
     // N2: second = D_W s = (1 - kappa D_hop) s on the full lattice, into the (idle) solver vectors
     void* second = ctx->vec[0];
@@ -246,24 +269,30 @@ int launch_contract(tsm_ctx* ctx, int slot)
         const void* p0 = (P == TSM_F64) ? ctx->gauge64[0] : ctx->gauge32[0];                                                 \
         const void* p1 = (P == TSM_F64) ? ctx->gauge64[1] : ctx->gauge32[1];                                                 \
         int pi = prof_begin(ctx, P, 5, nrhs);                                                                                \
-        k_contract<P, R, CT_LOCAL><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials); \
+        k_contract<P, R, CT_LOCAL><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials, mom); \
         prof_end(ctx, pi);                                                                                                   \
         ctx->launches++;                                                                                                     \
         if (ctx->with_deriv) {                                                                                               \
             pi = prof_begin(ctx, P, 6, nrhs);                                                                                \
-            k_contract<P, R, CT_DERIV><<<grid_d, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials); \
+            k_contract<P, R, CT_DERIV><<<grid_d, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials, mom); \
+            prof_end(ctx, pi);                                                                                               \
+            ctx->launches++;                                                                                                 \
+        }                                                                                                                    \
+        if (ctx->with_momenta && ctx->n_mom > 0) {                                                                           \
+            pi = prof_begin(ctx, P, 9, nrhs);                                                                                \
+            k_contract<P, R, CT_MOMENTUM><<<grid_m, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials, mom); \
             prof_end(ctx, pi);                                                                                               \
             ctx->launches++;                                                                                                 \
         }                                                                                                                    \
         if (ctx->with_gen_one_end) {                                                                                         \
             pi = prof_begin(ctx, P, 8, nrhs);                                                                                \
-            k_contract<P, R, CT_GEN_ONE_END><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials); \
+            k_contract<P, R, CT_GEN_ONE_END><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials, mom); \
             prof_end(ctx, pi);                                                                                               \
             ctx->launches++;                                                                                                 \
         }                                                                                                                    \
         if (ctx->with_one_end) {                                                                                             \
             pi = prof_begin(ctx, P, 7, nrhs);                                                                                \
-            k_contract<P, R, CT_ONE_END><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials); \
+            k_contract<P, R, CT_ONE_END><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials, mom); \
             prof_end(ctx, pi);                                                                                               \
             ctx->launches++;                                                                                                 \
         }                                                                                                                    \
@@ -279,6 +308,11 @@ int launch_contract(tsm_ctx* ctx, int slot)
     for (int m = 0; m < 4; m++) ob.v[1 + m] = ctx->with_deriv ? TSM_N_LOCAL_OPS + 16 * m : -1;
     ob.v[5] = ctx->with_one_end ? TSM_N_LOCAL_OPS + (ctx->with_deriv ? TSM_N_DERIV_OPS : 0) : -1;
     ob.v[6] = ctx->with_gen_one_end ? TSM_N_LOCAL_OPS + (ctx->with_deriv ? TSM_N_DERIV_OPS : 0) + (ctx->with_one_end ? TSM_N_ONE_END_OPS : 0) : -1;
+    {
+        const int base = TSM_N_LOCAL_OPS + (ctx->with_deriv ? TSM_N_DERIV_OPS : 0) + (ctx->with_one_end ? TSM_N_ONE_END_OPS : 0) +
+                         (ctx->with_gen_one_end ? TSM_N_GEN_ONE_END_OPS : 0);
+        for (int m = 0; m < TSM_MAX_MOMENTA; m++) ob.v[7 + m] = (ctx->with_momenta && m < ctx->n_mom) ? base + 16 * m : -1;
+    }
     if (ctx->with_one_end && !ctx->have_params) return tsm_fail(ctx, TSM_ESTATE, "one-end loops need kappa/mu (tsm_set_params)");
     const dim3 grid_f(g.L[3], CT_NGROUP, nrhs);
     k_contract_finish<<<grid_f, 32, 0, ctx->stream>>>(g.L[3], nblk, ctx->n_ops, ctx->gam, ob, 2.0 * (2.0 * ctx->kappa * ctx->mu),

@@ -424,7 +424,8 @@ struct tsm_ctx {
     double* host_small;              // pinned scratch (loops, unitarity)
     uint32_t* ids_dev;               // [2][TSM_MAX_NRHS]
     GammaTable gam;
-    int n_ops, with_deriv, with_one_end, with_gen_one_end, n_hp, n_lp;
+    int n_ops, with_deriv, with_one_end, with_gen_one_end, with_momenta, n_hp, n_lp;
+    int n_mom, mom[TSM_MAX_MOMENTA][3];   // momenta of the projected loops (tsm_loops_set_momenta)
     long long launches;
     bool prof_on;
     std::vector<ProfRec> prof;

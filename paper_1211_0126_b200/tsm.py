@@ -20,14 +20,15 @@ F64, F32, BF16 = 0, 1, 2
 Z4, Z2 = 0, 1
 OP_D_EO, OP_D_OE, OP_MHAT, OP_MHAT_DAG, OP_M_FULL = 0, 1, 2, 3, 4
 MAX_NRHS = 16
-OPS_DERIVATIVE, OPS_ONE_END, OPS_GEN_ONE_END = 1, 2, 4
+OPS_DERIVATIVE, OPS_ONE_END, OPS_GEN_ONE_END, OPS_MOMENTA = 1, 2, 4, 8
+MAX_MOMENTA = 16
 PREC = {"f64": F64, "f32": F32, "bf16": BF16}
 
 EXPORTS = [
     "tsm_create", "tsm_destroy", "tsm_last_error", "tsm_field_bytes", "tsm_workspace_bytes",
     "tsm_set_workspace", "tsm_set_stream", "tsm_set_params", "tsm_set_gauge", "tsm_noise",
     "tsm_pack", "tsm_unpack", "tsm_dslash", "tsm_solve", "tsm_get_solution", "tsm_set_solution",
-    "tsm_loops_reset", "tsm_loops_add_correction", "tsm_loops_add_lp", "tsm_loops_source",
+    "tsm_loops_reset", "tsm_loops_set_momenta", "tsm_loops_add_correction", "tsm_loops_add_lp", "tsm_loops_source",
     "tsm_loops_finalize", "tsm_loops_get_state", "tsm_loops_set_state", "tsm_run_loop_set",
     "tsm_launch_count", "tsm_profile", "tsm_profile_read",
 ]
@@ -78,6 +79,7 @@ def load_library():
     lib.tsm_get_solution.argtypes = [vp, i, i, dp]
     lib.tsm_set_solution.argtypes = [vp, i, i, dp]
     lib.tsm_loops_reset.argtypes = [vp, i]
+    lib.tsm_loops_set_momenta.argtypes = [vp, i, ip]
     lib.tsm_loops_add_correction.argtypes = [vp, i, i]
     lib.tsm_loops_add_lp.argtypes = [vp, i]
     lib.tsm_loops_source.argtypes = [vp, i, i, dp]
@@ -240,10 +242,18 @@ class Tsm:
         return ((OPS_DERIVATIVE if with_derivative else 0) | (OPS_ONE_END if one_end else 0)
                 | (OPS_GEN_ONE_END if gen_one_end else 0))
 
-    def loops_reset(self, with_derivative: bool = False, one_end: bool = False, gen_one_end: bool = False):
-        """n_ops = 16 local [+ 64 derivative] [+ 16 one-end (Eq. 2.5)] [+ 16 generalised one-end (Eq. 2.6)]."""
-        self.n_ops = 16 + (64 if with_derivative else 0) + (16 if one_end else 0) + (16 if gen_one_end else 0)
-        self._check(self.lib.tsm_loops_reset(self._h, self._ops(with_derivative, one_end, gen_one_end)))
+    def loops_reset(self, with_derivative: bool = False, one_end: bool = False, gen_one_end: bool = False, momenta=None):
+        """n_ops = 16 local [+ 64 derivative] [+ 16 one-end (Eq. 2.5)] [+ 16 generalised one-end (Eq. 2.6)]
+        [+ 16 per momentum of `momenta` ([nmom][3] integers, p_i = 2 pi n_i / L_i)]."""
+        ops = self._ops(with_derivative, one_end, gen_one_end)
+        nmom = 0
+        if momenta is not None:
+            mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+            nmom = mom.shape[0]
+            self._check(self.lib.tsm_loops_set_momenta(self._h, nmom, mom.ctypes.data_as(ctypes.POINTER(ctypes.c_int))))
+            ops |= OPS_MOMENTA
+        self.n_ops = 16 + (64 if with_derivative else 0) + (16 if one_end else 0) + (16 if gen_one_end else 0) + 16 * nmom
+        self._check(self.lib.tsm_loops_reset(self._h, ops))
 
     def loops_add_correction(self, slot_hp: int, slot_lp: int):
         self._check(self.lib.tsm_loops_add_correction(self._h, slot_hp, slot_lp))
@@ -275,12 +285,20 @@ class Tsm:
 
     def run_loop_set(self, seed: int, n_hp: int, n_lp: int, lp_prec: int, lp_tol: float, lp_iters: int,
                      hp_tol: float = 1e-10, hp_max_iter: int = 5000, nrhs: int = 1,
-                     with_derivative: bool = False, kind: int = Z4, one_end: bool = False, gen_one_end: bool = False):
+                     with_derivative: bool = False, kind: int = Z4, one_end: bool = False, gen_one_end: bool = False,
+                     momenta=None):
         """Eq. 2.4 for one configuration.  Returns (loops [n_ops][Lt], device seconds, rc)."""
-        self.n_ops = 16 + (64 if with_derivative else 0) + (16 if one_end else 0) + (16 if gen_one_end else 0)
+        ops = self._ops(with_derivative, one_end, gen_one_end)
+        nmom = 0
+        if momenta is not None:
+            mom = np.ascontiguousarray(momenta, dtype=np.int32).reshape(-1, 3)
+            nmom = mom.shape[0]
+            self._check(self.lib.tsm_loops_set_momenta(self._h, nmom, mom.ctypes.data_as(ctypes.POINTER(ctypes.c_int))))
+            ops |= OPS_MOMENTA
+        self.n_ops = 16 + (64 if with_derivative else 0) + (16 if one_end else 0) + (16 if gen_one_end else 0) + 16 * nmom
         out = np.empty((self.n_ops, self.Lt), dtype=np.complex128)
         secs = ctypes.c_double(0.0)
         rc = self.lib.tsm_run_loop_set(self._h, seed, kind, n_hp, n_lp, lp_prec, lp_tol, lp_iters, hp_tol,
-                                       hp_max_iter, nrhs, self._ops(with_derivative, one_end, gen_one_end), _dptr(out), ctypes.byref(secs))
+                                       hp_max_iter, nrhs, ops, _dptr(out), ctypes.byref(secs))
         self._check(rc, allow=(EBREAKDOWN, ENOCONV))
         return out, secs.value, rc

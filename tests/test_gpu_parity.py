@@ -504,3 +504,47 @@ def test_gen_one_end_alone_and_fp32(ragged):
     assert got.shape == (32, c.dims[3])
     assert rel(got[16:], want) < 1e-5
     c.t.loops_reset(False)
+
+
+# ---------------------------------------------------------------- N3: momentum-projected loops (reading A25)
+MOMENTA = [(0, 0, 0), (1, 0, 0), (0, -1, 0), (0, 0, 1), (1, 1, -1), (-2, 3, 1)]
+
+
+def test_momentum_loops_parity_on_the_oracle_solution(small, ragged):
+    for c in (small, ragged):
+        seed = 55
+        c.t.loops_reset(True, one_end=True, gen_one_end=True, momenta=MOMENTA)
+        rc, _ = c.t.solve(seed, [3, 4], F64, 0.0, 1, slot=0)
+        for j, sid in enumerate((3, 4)):
+            eta = oracle.noise(c.dims, seed, sid)
+            s, _ = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, 1e-10, 2000)
+            c.t.set_solution(0, j, s)
+            want = oracle.all_loops(c.dims, c.theta, c.U, eta, s, True, one_end=(c.kappa, c.mu), gen_one_end=c.kappa,
+                                    momenta=MOMENTA)
+            got = c.t.loops_source(0, j)
+            assert got.shape == want.shape == (112 + 16 * len(MOMENTA), c.dims[3])
+            assert rel(got[112:], want[112:]) < 1e-12
+            assert np.array_equal(got[112:128], got[:16])          # n = 0 is the local loop, bit for bit
+            assert rel(got[:112], want[:112]) < 1e-12
+        c.t.loops_reset(False)
+
+
+def test_momentum_loops_through_eq_2_4_and_fp32(ragged):
+    c = ragged
+    moms = MOMENTA[1:4]
+    got, secs, rc = c.t.run_loop_set(99, 1, 2, F32, 0.0, 6, hp_tol=1e-10, hp_max_iter=2000, nrhs=2, momenta=moms)
+    assert rc == 0 and got.shape == (16 + 48, c.dims[3])
+    corr = np.zeros_like(got)
+    lp = np.zeros_like(got)
+    c.t.loops_reset(False, momenta=moms)
+    for j in range(3):
+        eta = oracle.noise(c.dims, 99, j)
+        c.t.solve(99, [j], F32, 0.0, 6, slot=1)
+        l_lp = oracle.all_loops(c.dims, c.theta, c.U, eta, c.t.get_solution(1, 0), False, momenta=moms)
+        if j < 1:
+            c.t.solve(99, [j], F64, 1e-10, 2000, slot=0)
+            corr += oracle.all_loops(c.dims, c.theta, c.U, eta, c.t.get_solution(0, 0), False, momenta=moms) - l_lp
+        else:
+            lp += l_lp
+    assert rel(got, corr / 1 + lp / 2) < 1e-5
+    c.t.loops_reset(False)
