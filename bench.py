@@ -347,20 +347,22 @@ def extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U):
 
     # ---- contraction kernels (H8, H9, the one-end loops of Eq. 2.5 (N1) and of Eq. 2.6 (N2; its two D_W stencil
     # launches are counted with the stencils, not here) on the slot the timed steps left
-    t.loops_reset(wl.derivative, one_end=True, gen_one_end=True)
+    bench_momenta = [(1, 0, 0), (0, 1, 0), (0, 0, 1), (-1, 0, 0), (0, -1, 0), (0, 0, -1)]
+    t.loops_reset(wl.derivative, one_end=True, gen_one_end=True, momenta=bench_momenta)
     t.profile(True)
     for _ in range(3):
         t.loops_add_lp(1)
     t.profile(False)
     sp = PRECS["f32" if prec_name == "bf16" else prec_name]
     w_sol = 8 if prec_name == "f64" else 4
-    names = {5: "local_16_gamma", 6: "derivative_4_directions", 7: "one_end_eq_2_5", 8: "gen_one_end_eq_2_6_contraction_only"}
+    names = {5: "local_16_gamma", 6: "derivative_4_directions", 7: "one_end_eq_2_5", 8: "gen_one_end_eq_2_6_contraction_only",
+             9: "momentum_projected_6_momenta"}
     # algorithmic bytes per site of the full lattice and source: s once (eta is regenerated, never read);
     # derivative: s once + the 8 links of the site
     n_g = 18 if prec_name == "f64" else wl.reconstruct
-    by_site = {5: 24 * w_sol, 6: 24 * w_sol + 8 * n_g * (8 if prec_name == "f64" else 4), 7: 24 * w_sol, 8: 48 * w_sol}
+    by_site = {5: 24 * w_sol, 6: 24 * w_sol + 8 * n_g * (8 if prec_name == "f64" else 4), 7: 24 * w_sol, 8: 48 * w_sol, 9: 24 * w_sol}
     ct = {}
-    for k in (5, 6, 7, 8):
+    for k in (5, 6, 7, 8, 9):
         ms_k, n_k = t.profile_read(sp, k, nrhs)
         if n_k:
             us = ms_k * 1e3 / n_k
@@ -378,6 +380,16 @@ def extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U):
         rc, info = t.solve(wl.noise_seed, list(range(min(nrhs, wl.n_hp))), tsm.F64, wl.hp_tol, 5000, slot=0, want_true_resid=True)
         out["hp_solve"] = {"iters": [i["iters"] for i in info], "secs_batch": info[0]["secs"],
                            "true_resid_max": max(i["rel_resid_true"] for i in info)}
+        # N4: the same HP solves as fp64 defect correction around the fp32 CG, and Eq. 2.4 with them
+        rc, info = t.solve(wl.noise_seed, list(range(min(nrhs, wl.n_hp))), tsm.MIXED, wl.hp_tol, 5000, slot=0, want_true_resid=True)
+        out["hp_solve_mixed"] = {"iters_fp32_total": [i["iters"] for i in info], "secs_batch": info[0]["secs"],
+                                 "true_resid_max": max(i["rel_resid_true"] for i in info)}
+        t.set_hp_precision(tsm.MIXED)
+        loops_m, secs_m, rc_m = t.run_loop_set(wl.noise_seed, wl.n_hp, wl.n_lp, prec, wl.lp_tol, wl.lp_iters, hp_tol=wl.hp_tol,
+                                               hp_max_iter=5000, nrhs=nrhs, with_derivative=wl.derivative)
+        t.set_hp_precision(tsm.F64)
+        out["tsm_loop_set_mixed_hp"] = {"seconds": secs_m, "rc": rc_m,
+                                        "max_rel_diff_to_fp64_hp": float(np.abs(loops_m - loops).max() / np.abs(loops).max())}
 
     # ---- the oracle on this box's host cores, bounded sample
     if not args.no_cpu_baseline:

@@ -56,7 +56,8 @@ typedef struct tsm_ctx tsm_ctx; /* opaque; owned by the library */
 
 enum { TSM_OK = 0, TSM_EINVAL = -1, TSM_ESTATE = -2, TSM_ECUDA = -3, TSM_ENOTUNITARY = -4,
        TSM_EBREAKDOWN = -5, TSM_ENOCONV = -6 };
-enum { TSM_F64 = 0, TSM_F32 = 1, TSM_BF16 = 2 };          /* spinor storage precision */
+enum { TSM_F64 = 0, TSM_F32 = 1, TSM_BF16 = 2,           /* spinor storage precision */
+       TSM_MIXED = 3 };  /* tsm_solve only: fp64 defect correction around the fp32 CG (fp64 solution, tol > 0) */
 enum { TSM_Z4 = 0, TSM_Z2 = 1 };                           /* noise kind (A5)          */
 enum { TSM_OP_D_EO = 0,      /* out_e = D_eo in_o                         (H5)           */
        TSM_OP_D_OE = 1,      /* out_o = D_oe in_e                                        */
@@ -125,7 +126,10 @@ int tsm_dslash(tsm_ctx* ctx, int op, int prec, int nrhs, const void* dev_in, voi
  *             that has not got there after max_iter iterations reports TSM_ENOCONV.
  *   tol == 0: exactly max_iter iterations, no residual test (A9).
  * The full-lattice solutions stay in workspace slot `slot` (0 or 1), in precision `prec`
- * (BF16 solves leave fp32 solutions).  info (may be NULL) is a host array [nrhs];
+ * (BF16 solves leave fp32 solutions).  prec = TSM_MIXED (needs tol > 0) reaches the same fp64 solution as
+ * TSM_F64 at low-precision cost: it stops on the TRUE fp64 residual |b' - A x|/|b'| <= tol of the
+ * preconditioned normal system, corrections e come from fp32 CG solves of A e = r to 1e-5; `iters` is the
+ * total of fp32 iterations, rel_resid_rec that true residual.  info (may be NULL) is a host array [nrhs];
  * rel_resid_true (the fp64 |eta - M s|/|eta| of the full system) is filled only when
  * want_true_resid != 0.  Returns TSM_OK if every source ended TSM_OK, else the first
  * non-OK per-source status (solutions are kept either way). */
@@ -169,6 +173,9 @@ int tsm_loops_set_state(tsm_ctx* ctx, const double* host_corr, const double* hos
 int tsm_run_loop_set(tsm_ctx* ctx, uint64_t seed, int kind, int n_hp, int n_lp, int lp_prec,
                      double lp_tol, int lp_iters, double hp_tol, int hp_max_iter, int nrhs,
                      int ops, double* host_out, double* secs_out);
+
+/* Precision of the HP solves of tsm_run_loop_set: TSM_F64 (default) or TSM_MIXED. */
+int tsm_set_hp_precision(tsm_ctx* ctx, int prec);
 
 /* Number of kernels this library has launched on the context since creation. */
 long long tsm_launch_count(const tsm_ctx* ctx);

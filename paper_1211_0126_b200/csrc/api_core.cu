@@ -103,6 +103,7 @@ int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
     ctx->with_one_end = 0;
     ctx->with_gen_one_end = 0;
     ctx->with_momenta = 0;
+    ctx->hp_prec = TSM_F64;
     ctx->n_mom = 0;
     ctx->n_hp = ctx->n_lp = 0;
     ctx->launches = 0;

@@ -89,6 +89,84 @@ int fetch_scalars(tsm_ctx* ctx)
     return TSM_OK;
 }
 
+// `max_iter` CG iterations at most, in chunks of 4; residual mode polls the all-done flag after each chunk.
+int cg_run(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, void* r, void* p, void* w, void* t, double tol, int max_iter)
+{
+    // iterations run in chunks of `poll`; in residual mode the host reads the all-done flag after each chunk
+    // (a finished batch makes every later kernel return at once), in fixed-iteration mode it never does.
+    // The first chunk is launched kernel by kernel (it also sets up the kernels' attributes), full later
+    // chunks as one cached CUDA graph.
+    int rc;
+    const int poll = 4;
+    const bool use_graph = graphs_enabled(ctx);
+    for (int k = 0; k < max_iter;) {
+        const int chunk = max_iter - k < poll ? max_iter - k : poll;
+        if (use_graph && k > 0 && chunk == poll) {
+            if ((rc = cg_iterations_graph(ctx, prec, nrhs, chunk, tw, x, r, p, w, t, tol))) return rc;
+        } else {
+            for (int j = 0; j < chunk; j++)
+                if ((rc = cg_iteration(ctx, prec, nrhs, tw, x, r, p, w, t, tol))) return rc;
+        }
+        k += chunk;
+        if (tol > 0 && k < max_iter) {
+            TSM_CUDA(ctx, cudaMemcpyAsync(&ctx->cg_host->all_done, &ctx->cg->all_done, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+            TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+            if (ctx->cg_host->all_done) break;
+        }
+    }
+    return TSM_OK;
+}
+
+
+// N4 (north_star "mixed-precision CG"): the HP solve as fp64 defect correction around the fp32
+// CG.  On entry vec[0] = b' (fp64) and x64 is the slot's even half.  Loop: r = b' - A x in fp64 (the four
+// stencil launches of an iteration, the last one with the residual epilogue and alpha = 1) -> stop when
+// |r|/|b'| <= tol (A8, now the TRUE residual of the preconditioned normal system) -> e = fp32 CG on A e = r to
+// MIXED_INNER_TOL -> x += e in fp64.  Every source has its own outer state and is frozen once converged (A14).
+constexpr double MIXED_INNER_TOL = 1e-5;
+
+int solve_mixed(tsm_ctx* ctx, int nrhs, const Twists& tw, void* x64, double tol, int max_iter)
+{
+    const int Vh = ctx->g.Vh;
+    const size_t fb64 = field_bytes(TSM_F64, Vh, nrhs), fb32 = field_bytes(TSM_F32, Vh, nrhs);
+    char* v0 = (char*)ctx->vec[0];
+    void *R64 = ctx->vec[1], *b64 = ctx->vec[2], *w64 = ctx->vec[3], *t64 = ctx->vec[4];
+    void *r32 = v0, *p32 = v0 + fb32, *w32 = ctx->vec[3], *t32 = (char*)ctx->vec[3] + fb32, *e32 = ctx->vec[5];
+    int rc;
+    TSM_CUDA(ctx, cudaMemcpyAsync(b64, ctx->vec[0], fb64, cudaMemcpyDeviceToDevice, ctx->stream));
+    if ((rc = launch_cg_init(ctx, TSM_F64, nrhs, ctx->vec[0], R64, x64))) return rc;   // x = 0, R64 = b' = r(x = 0), |b'|^2
+    if ((rc = launch_mixed_ctl(ctx, 0, nrhs, tol))) return rc;
+    int prev[TSM_MAX_NRHS];
+    for (int round = 0;; round++) {
+        if ((rc = fetch_scalars(ctx))) return rc;
+        const CgScalars sc = *ctx->cg_host;
+        if (sc.all_outer_done) break;
+        int most = 0;
+        bool moved = round == 0;
+        for (int j = 0; j < nrhs; j++) {
+            if (!sc.outer_done[j] && sc.iters_outer[j] > most) most = sc.iters_outer[j];
+            if (round > 0 && sc.iters_outer[j] != prev[j]) moved = true;
+            prev[j] = sc.iters_outer[j];
+        }
+        if (most >= max_iter) break;   // TSM_ENOCONV for the live sources
+        if (!moved) break;             // zero or broken-down inner systems: stop rather than spin
+        if ((rc = launch_convert(ctx, TSM_F64, TSM_F32, nrhs, R64, r32))) return rc;
+        if ((rc = launch_cg_init(ctx, TSM_F32, nrhs, r32, p32, e32))) return rc;
+        if ((rc = launch_mixed_ctl(ctx, 1, nrhs, tol))) return rc;
+        if ((rc = cg_run(ctx, TSM_F32, nrhs, tw, e32, r32, p32, w32, t32, MIXED_INNER_TOL, max_iter - most))) return rc;
+        if ((rc = launch_mixed_ctl(ctx, 2, nrhs, tol))) return rc;
+        if ((rc = launch_mixed_axpy(ctx, nrhs, x64, e32))) return rc;
+        TSM_CUDA(ctx, cudaMemcpyAsync(R64, b64, fb64, cudaMemcpyDeviceToDevice, ctx->stream));
+        if ((rc = launch_dslash(ctx, TSM_F64, 1, false, nrhs, x64, nullptr, t64, {tw.zero, tw.Rinv}, 0))) return rc;
+        if ((rc = launch_dslash(ctx, TSM_F64, 0, false, nrhs, t64, x64, w64, {tw.R, tw.mk2}, 0))) return rc;
+        if ((rc = launch_dslash(ctx, TSM_F64, 1, true, nrhs, w64, nullptr, t64, {tw.zero, tw.Rbinv}, 0))) return rc;
+        if ((rc = launch_dslash(ctx, TSM_F64, 0, true, nrhs, t64, w64, R64, {tw.Rb, tw.mk2}, 4))) return rc;   // R64 = b' - A x
+        if ((rc = launch_cg_reduce(ctx, 1, nrhs, 1))) return rc;
+        if ((rc = launch_mixed_ctl(ctx, 3, nrhs, tol))) return rc;
+    }
+    return launch_mixed_ctl(ctx, 4, nrhs, tol);
+}
+
 // fp64 |eta - M s| / |eta| of the full system for every source of a slot (reading A8/A17).
 int true_residuals(tsm_ctx* ctx, int slot, double* out)
 {
@@ -130,12 +208,12 @@ int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs,
 {
     int rc = ctx_enter(ctx, true, true, true);
     if (rc) return rc;
-    if (!source_ids || nrhs < 1 || nrhs > ctx->max_nrhs || (kind != TSM_Z4 && kind != TSM_Z2) || prec < 0 || prec > 2 ||
-        !(tol >= 0) || max_iter < 0 || slot < 0 || slot > 1)
+    if (!source_ids || nrhs < 1 || nrhs > ctx->max_nrhs || (kind != TSM_Z4 && kind != TSM_Z2) || prec < 0 || prec > TSM_MIXED ||
+        !(tol >= 0) || max_iter < 0 || slot < 0 || slot > 1 || (prec == TSM_MIXED && !(tol > 0)))
         return tsm_fail(ctx, TSM_EINVAL, "bad solve arguments");
     // bf16 storage (config 4): source preparation, x, r, q, reconstruction and the stored solution are
     // fp32; only the search direction p and the stencil temporaries t, w are bf16 (fp32 arithmetic).
-    const int sp = prec == TSM_BF16 ? TSM_F32 : prec;   // precision of the stored solution
+    const int sp = prec == TSM_BF16 ? TSM_F32 : (prec == TSM_MIXED ? TSM_F64 : prec);   // precision of the stored solution
     const int Vh = ctx->g.Vh;
     const Twists tw = make_twists(ctx);
     ctx->slot_prec[slot] = sp;
@@ -159,27 +237,11 @@ int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs,
     if ((rc = launch_dslash(ctx, sp, 0, true, nrhs, t, w, r, {tw.Rb, tw.mk2}, 0))) return rc;
     // O5: x0 = 0 (x lives in the slot's even half), r0 = p0 = b'
     void* x = s_e;
-    if ((rc = launch_cg_init(ctx, prec, nrhs, r, p, x))) return rc;
-    // iterations run in chunks of `poll`; in residual mode the host reads the all-done flag after each chunk
-    // (a finished batch makes every later kernel return at once), in fixed-iteration mode it never does.
-    // The first chunk is launched kernel by kernel (it also sets up the kernels' attributes), full later
-    // chunks as one cached CUDA graph.
-    const int poll = 4;
-    const bool use_graph = graphs_enabled(ctx);
-    for (int k = 0; k < max_iter;) {
-        const int chunk = max_iter - k < poll ? max_iter - k : poll;
-        if (use_graph && k > 0 && chunk == poll) {
-            if ((rc = cg_iterations_graph(ctx, prec, nrhs, chunk, tw, x, r, p, w, t, tol))) return rc;
-        } else {
-            for (int j = 0; j < chunk; j++)
-                if ((rc = cg_iteration(ctx, prec, nrhs, tw, x, r, p, w, t, tol))) return rc;
-        }
-        k += chunk;
-        if (tol > 0 && k < max_iter) {
-            TSM_CUDA(ctx, cudaMemcpyAsync(&ctx->cg_host->all_done, &ctx->cg->all_done, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
-            TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-            if (ctx->cg_host->all_done) break;
-        }
+    if (prec == TSM_MIXED) {
+        if ((rc = solve_mixed(ctx, nrhs, tw, s_e, tol, max_iter))) return rc;
+    } else {
+        if ((rc = launch_cg_init(ctx, prec, nrhs, r, p, x))) return rc;
+        if ((rc = cg_run(ctx, prec, nrhs, tw, x, r, p, w, t, tol, max_iter))) return rc;
     }
     // H7: s_e = x, s_o = R^-1 (eta_o + kappa D_oe x)
     if ((rc = launch_dslash(ctx, sp, 1, false, nrhs, x, s_o, aux, {tw.Rinv, tw.kRinv}, 0))) return rc;
@@ -259,6 +321,14 @@ int tsm_loops_reset(tsm_ctx* ctx, int ops)
     const size_t lb = (size_t)ctx->n_ops * ctx->g.L[3] * 2 * sizeof(double);
     TSM_CUDA(ctx, cudaMemsetAsync(ctx->acc_corr, 0, lb, ctx->stream));
     TSM_CUDA(ctx, cudaMemsetAsync(ctx->acc_lp, 0, lb, ctx->stream));
+    return TSM_OK;
+}
+
+int tsm_set_hp_precision(tsm_ctx* ctx, int prec)
+{
+    if (!ctx) return TSM_EINVAL;
+    if (prec != TSM_F64 && prec != TSM_MIXED) return tsm_fail(ctx, TSM_EINVAL, "HP precision must be TSM_F64 or TSM_MIXED");
+    ctx->hp_prec = prec;
     return TSM_OK;
 }
 
@@ -376,7 +446,7 @@ int tsm_run_loop_set(tsm_ctx* ctx, uint64_t seed, int kind, int n_hp, int n_lp, 
         uint32_t ids[TSM_MAX_NRHS];
         for (int k = 0; k < nb; k++) ids[k] = (uint32_t)(j0 + k);
         if (hp) {
-            rc = tsm_solve(ctx, seed, ids, nb, kind, TSM_F64, hp_tol, hp_max_iter, 0, 0, nullptr);
+            rc = tsm_solve(ctx, seed, ids, nb, kind, ctx->hp_prec, hp_tol, hp_max_iter, 0, 0, nullptr);
             if (rc == TSM_ECUDA || rc == TSM_EINVAL || rc == TSM_ESTATE) goto fail;
             if (rc && !worst) worst = rc;
         }

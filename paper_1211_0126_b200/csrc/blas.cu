@@ -68,10 +68,10 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_init(const int Vh, const int nrh
 //   which == 0 (after w = Mhat p, EPI_NORM):  pq = |w|^2 = Re<p,q>;  alpha = rr / pq, or 0 for a frozen
 //              source; 0 / non-finite pq or rr freezes the source and flags TSM_EBREAKDOWN (A13)
 //   which == 1 (after r -= alpha q, EPI_RESID): rr_new = |r|^2
-__global__ void __launch_bounds__(BLAS_BS) k_cg_reduce(const int which, const double* __restrict__ norm_partials, const int ntiles,
-                                                       CgScalars* cg)
+__global__ void __launch_bounds__(BLAS_BS) k_cg_reduce(const int which, const int force, const double* __restrict__ norm_partials,
+                                                       const int ntiles, CgScalars* cg)
 {
-    if (cg->all_done) return;
+    if (cg->all_done && !force) return;
     const int rhs = blockIdx.x;
     __shared__ double smem[32];
     double v = 0;
@@ -177,9 +177,9 @@ int launch_cg_init(tsm_ctx* ctx, int prec, int nrhs, const void* r, void* p, voi
     return TSM_OK;
 }
 
-int launch_cg_reduce(tsm_ctx* ctx, int which, int nrhs)
+int launch_cg_reduce(tsm_ctx* ctx, int which, int nrhs, int force)
 {
-    k_cg_reduce<<<nrhs, BLAS_BS, 0, ctx->stream>>>(which, ctx->norm_partials, ctx->norm_ntiles, ctx->cg);
+    k_cg_reduce<<<nrhs, BLAS_BS, 0, ctx->stream>>>(which, force, ctx->norm_partials, ctx->norm_ntiles, ctx->cg);
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;
@@ -191,6 +191,90 @@ int launch_cg_update_xp(tsm_ctx* ctx, int prec, int nrhs, void* x, void* p, cons
     const int pi = prof_begin(ctx, prec, 4, nrhs);
     BLAS_SWITCH(prec, (k_cg_update_xp<PV, PP><<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, nrhs, x, p, r, tol, ctx->cg)));
     prof_end(ctx, pi);
+    ctx->launches++;
+    TSM_CUDA(ctx, cudaGetLastError());
+    return TSM_OK;
+}
+
+// ------------------------------------------------------------------ N4: mixed-precision HP solver (api_solve.cu: solve_mixed)
+namespace {
+// Scalar bookkeeping of the fp64 defect-correction loop around the fp32 CG; one block, thread j = source j.
+//   mode 0 (after the fp64 cg_init on b'): outer state <- |b'|^2, nothing done, no iterations yet
+//   mode 1 (after the inner fp32 cg_init):  sources whose outer residual has converged stay frozen
+//   mode 2 (after the inner solve):          iteration total += inner iterations; alpha = 1 (live) or 0 (frozen),
+//                                            so that the residual stencil computes r = b' - A x for live sources
+//   mode 3 (after the outer residual):       rr_outer <- |b' - A x|^2; stopping test against tol (A8)
+//   mode 4 (at the end):                     copy the outer state into the fields tsm_solve reports
+__global__ void k_mixed_ctl(const int mode, const int nrhs, const double tol, CgScalars* cg)
+{
+    const int j = threadIdx.x;
+    if (j < nrhs) {
+        if (mode == 0) {
+            cg->bb_outer[j] = cg->bb[j];
+            cg->rr_outer[j] = cg->bb[j];
+            cg->iters_outer[j] = 0;
+            cg->outer_done[j] = cg->done[j];
+        } else if (mode == 1) {
+            if (cg->outer_done[j]) cg->done[j] = 1;
+        } else if (mode == 2) {
+            if (!cg->outer_done[j]) cg->iters_outer[j] += cg->iters[j];
+            if (!cg->outer_done[j] && cg->status[j] == TSM_EBREAKDOWN && cg->iters[j] == 0) cg->outer_done[j] = 2;   // no progress possible
+            cg->alpha[j] = cg->outer_done[j] ? 0.0 : 1.0;
+        } else if (mode == 3) {
+            if (!cg->outer_done[j]) {
+                cg->rr_outer[j] = cg->rr_new[j];
+                if (sqrt(cg->rr_new[j] / cg->bb_outer[j]) <= tol) cg->outer_done[j] = 1;
+            }
+        } else {
+            cg->iters[j] = cg->iters_outer[j];
+            cg->rr[j] = cg->rr_outer[j];
+            cg->bb[j] = cg->bb_outer[j];
+            cg->done[j] = cg->outer_done[j] == 1;
+            cg->status[j] = cg->outer_done[j] == 2 ? TSM_EBREAKDOWN : TSM_OK;
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int all = 1;
+        for (int k = 0; k < nrhs; k++) all &= (mode == 0 || mode == 3 || mode == 2) ? (cg->outer_done[k] != 0) : (cg->done[k] != 0);
+        if (mode == 1) cg->all_done = all;                    // the inner CG's early-exit flag
+        if (mode == 0 || mode == 2 || mode == 3) cg->all_outer_done = all;
+    }
+}
+
+// x64 += e32 for the sources whose outer residual has not converged (fp64 accumulation of the fp32 correction)
+__global__ void __launch_bounds__(BLAS_BS) k_mixed_axpy(const int Vh, void* __restrict__ x_, const void* __restrict__ e_, const CgScalars* cg)
+{
+    const int rhs = blockIdx.y;
+    if (cg->outer_done[rhs]) return;
+    char* x = (char*)x_ + field_bytes(TSM_F64, Vh, 1) * rhs;
+    const char* e = (const char*)e_ + field_bytes(TSM_F32, Vh, 1) * rhs;
+    const int n = 3 * (int)padded_sites(Vh);
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += gridDim.x * blockDim.x) {
+        const int k8 = (idx >> 5) % 3, i = (idx >> 5) / 3 * LB + (idx & 31);
+        if (i >= Vh) continue;
+        double xv[8];
+        float ev[8];
+        load8<TSM_F64>(x, i, k8, xv);
+        load8<TSM_F32>(e, i, k8, ev);
+#pragma unroll
+        for (int k = 0; k < 8; k++) xv[k] += (double)ev[k];
+        store8<TSM_F64>(x, i, k8, xv);
+    }
+}
+}  // namespace
+
+int launch_mixed_ctl(tsm_ctx* ctx, int mode, int nrhs, double tol)
+{
+    k_mixed_ctl<<<1, 32, 0, ctx->stream>>>(mode, nrhs, tol, ctx->cg);
+    ctx->launches++;
+    TSM_CUDA(ctx, cudaGetLastError());
+    return TSM_OK;
+}
+
+int launch_mixed_axpy(tsm_ctx* ctx, int nrhs, void* x64, const void* e32)
+{
+    k_mixed_axpy<<<blas_grid(ctx, nrhs), BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, x64, e32, ctx->cg);
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;

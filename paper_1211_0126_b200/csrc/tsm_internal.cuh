@@ -353,6 +353,11 @@ struct CgScalars {
     double beta[TSM_MAX_NRHS];
     double alpha[TSM_MAX_NRHS];   // rr / Re<p,q> of this iteration; 0 for a frozen source
     double rr_new[TSM_MAX_NRHS];  // |r|^2 after this iteration's residual update
+    // N4 mixed-precision solver: state of the fp64 defect-correction loop around the fp32 CG
+    double bb_outer[TSM_MAX_NRHS], rr_outer[TSM_MAX_NRHS];
+    int iters_outer[TSM_MAX_NRHS];
+    int outer_done[TSM_MAX_NRHS];   // 0 live, 1 converged, 2 broken down
+    int all_outer_done;
     int iters[TSM_MAX_NRHS];
     int done[TSM_MAX_NRHS];       // frozen: converged, broken down, or zero source
     int status[TSM_MAX_NRHS];
@@ -425,6 +430,7 @@ struct tsm_ctx {
     uint32_t* ids_dev;               // [2][TSM_MAX_NRHS]
     GammaTable gam;
     int n_ops, with_deriv, with_one_end, with_gen_one_end, with_momenta, n_hp, n_lp;
+    int hp_prec;                     // TSM_F64 or TSM_MIXED (tsm_set_hp_precision)
     int n_mom, mom[TSM_MAX_MOMENTA][3];   // momenta of the projected loops (tsm_loops_set_momenta)
     long long launches;
     bool prof_on;
@@ -477,7 +483,9 @@ int launch_pack_spinor(tsm_ctx* ctx, int prec, int nrhs, const double* dev_lex, 
 int launch_unpack_spinor(tsm_ctx* ctx, int prec, int nrhs, const void* dev_native, double* dev_lex);
 int launch_noise(tsm_ctx* ctx, int prec, int nrhs, uint64_t seed, const uint32_t* dev_ids, int kind, void* dev_full);
 int launch_cg_init(tsm_ctx* ctx, int prec, int nrhs, const void* r, void* p, void* x);
-int launch_cg_reduce(tsm_ctx* ctx, int which, int nrhs);
+int launch_cg_reduce(tsm_ctx* ctx, int which, int nrhs, int force = 0);
+int launch_mixed_ctl(tsm_ctx* ctx, int mode, int nrhs, double tol);
+int launch_mixed_axpy(tsm_ctx* ctx, int nrhs, void* x64, const void* e32);
 int launch_cg_update_xp(tsm_ctx* ctx, int prec, int nrhs, void* x, void* p, const void* r, double tol);
 int launch_convert(tsm_ctx* ctx, int prec_in, int prec_out, int nrhs_fields, const void* in, void* out);
 int launch_contract(tsm_ctx* ctx, int slot);

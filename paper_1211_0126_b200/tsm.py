@@ -16,13 +16,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtsm.so")
 
 OK, EINVAL, ESTATE, ECUDA, ENOTUNITARY, EBREAKDOWN, ENOCONV = 0, -1, -2, -3, -4, -5, -6
-F64, F32, BF16 = 0, 1, 2
+F64, F32, BF16, MIXED = 0, 1, 2, 3
 Z4, Z2 = 0, 1
 OP_D_EO, OP_D_OE, OP_MHAT, OP_MHAT_DAG, OP_M_FULL = 0, 1, 2, 3, 4
 MAX_NRHS = 16
 OPS_DERIVATIVE, OPS_ONE_END, OPS_GEN_ONE_END, OPS_MOMENTA = 1, 2, 4, 8
 MAX_MOMENTA = 16
-PREC = {"f64": F64, "f32": F32, "bf16": BF16}
+PREC = {"f64": F64, "f32": F32, "bf16": BF16, "mixed": MIXED}
 
 EXPORTS = [
     "tsm_create", "tsm_destroy", "tsm_last_error", "tsm_field_bytes", "tsm_workspace_bytes",
@@ -30,7 +30,7 @@ EXPORTS = [
     "tsm_pack", "tsm_unpack", "tsm_dslash", "tsm_solve", "tsm_get_solution", "tsm_set_solution",
     "tsm_loops_reset", "tsm_loops_set_momenta", "tsm_loops_add_correction", "tsm_loops_add_lp", "tsm_loops_source",
     "tsm_loops_finalize", "tsm_loops_get_state", "tsm_loops_set_state", "tsm_run_loop_set",
-    "tsm_launch_count", "tsm_profile", "tsm_profile_read",
+    "tsm_set_hp_precision", "tsm_launch_count", "tsm_profile", "tsm_profile_read",
 ]
 
 
@@ -87,6 +87,7 @@ def load_library():
     lib.tsm_loops_get_state.argtypes = [vp, dp, dp, ip, ip]
     lib.tsm_loops_set_state.argtypes = [vp, dp, dp, i, i]
     lib.tsm_run_loop_set.argtypes = [vp, u64, i, i, i, i, ctypes.c_double, i, ctypes.c_double, i, i, i, dp, dp]
+    lib.tsm_set_hp_precision.argtypes = [vp, i]
     lib.tsm_launch_count.argtypes = [vp]
     lib.tsm_launch_count.restype = ctypes.c_longlong
     lib.tsm_profile.argtypes = [vp, i]
@@ -178,6 +179,10 @@ class Tsm:
     # ------------------------------------------------------------------ the calls of include/tsm.h
     def set_params(self, kappa: float, mu: float):
         self._check(self.lib.tsm_set_params(self._h, kappa, mu))
+
+    def set_hp_precision(self, prec: int):
+        """F64 (default) or MIXED: how tsm_run_loop_set does its HP solves."""
+        self._check(self.lib.tsm_set_hp_precision(self._h, prec))
 
     def set_gauge(self, links, reconstruct: int = 18) -> float:
         """links: host complex128 [4][V][3][3], or a pinned torch tensor viewing the same bytes."""

@@ -548,3 +548,37 @@ def test_momentum_loops_through_eq_2_4_and_fp32(ragged):
             lp += l_lp
     assert rel(got, corr / 1 + lp / 2) < 1e-5
     c.t.loops_reset(False)
+
+
+# ---------------------------------------------------------------- N4: mixed-precision HP solver
+def test_mixed_precision_hp_solve(small, medium, ragged, tsm_mod):
+    """fp64 defect correction around the fp32 CG: same solution as the fp64 solve to the accuracy two converged
+    solves can agree (A16(iii)): fp64 true residual of the full system <= 1.5e-10, s within 1e-8, loops within
+    1e-8; batch independent (A14); tolerance not reached is flagged with the iterate kept."""
+    MIXED = tsm_mod.MIXED
+    for c, seed in ((small, W.WORKLOADS[1].noise_seed), (medium, W.WORKLOADS[2].noise_seed), (ragged, 17)):
+        ids = [1, 6, 2]
+        rc, info = c.t.solve(seed, ids, MIXED, 1e-10, 2000, slot=0, want_true_resid=True)
+        assert rc == 0, info
+        c.t.loops_reset(True)
+        for j, sid in enumerate(ids):
+            eta = oracle.noise(c.dims, seed, sid)
+            s_ref, info_ref = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, 1e-10, 2000)
+            s = c.t.get_solution(0, j)
+            rho = oracle.true_residual(c.dims, c.theta, c.kappa, c.mu, c.U, eta, s)
+            assert rho <= 1.5e-10, (c.dims, j, rho)
+            assert np.isclose(info[j]["rel_resid_true"], rho, rtol=1e-3)
+            assert info[j]["status"] == 0 and info[j]["rel_resid_rec"] <= 1e-10
+            assert info_ref["iters"] <= info[j]["iters"] <= 3 * info_ref["iters"]
+            assert rel(s, s_ref) < 1e-8
+            want = oracle.all_loops(c.dims, c.theta, c.U, eta, s_ref, True)
+            assert rel(c.t.loops_source(0, j), want) < 1e-8
+        batch = [c.t.get_solution(0, j) for j in range(3)]
+        rc, _ = c.t.solve(seed, [ids[1]], MIXED, 1e-10, 2000, slot=1)
+        assert np.array_equal(c.t.get_solution(1, 0), batch[1])
+        c.t.loops_reset(False)
+    c = small
+    rc, info = c.t.solve(5, [0], MIXED, 1e-10, 6, slot=0)
+    assert rc == tsm_mod.ENOCONV and info[0]["status"] == tsm_mod.ENOCONV and info[0]["rel_resid_rec"] > 1e-10
+    with pytest.raises(tsm_mod.TsmError):
+        c.t.solve(5, [0], MIXED, 0.0, 10, slot=0)            # needs a tolerance
