@@ -582,3 +582,63 @@ def test_mixed_precision_hp_solve(small, medium, ragged, tsm_mod):
     assert rc == tsm_mod.ENOCONV and info[0]["status"] == tsm_mod.ENOCONV and info[0]["rel_resid_rec"] > 1e-10
     with pytest.raises(tsm_mod.TsmError):
         c.t.solve(5, [0], MIXED, 0.0, 10, slot=0)            # needs a tolerance
+
+
+# ---------------------------------------------------------------- edge cases
+@pytest.mark.parametrize("nrhs", [5, 7, 16])
+def test_dslash_odd_and_maximum_batch_sizes(tsm_mod, nrhs):
+    """Batch sizes that leave source rows of the CTA idle (5, 7) and the maximum (TSM_MAX_NRHS = 16)."""
+    c = Case(tsm_mod, (8, 4, 6, 4), 0.6, 91, 0.157, 0.02, -1, max_nrhs=16)
+    psi = W.random_spinor(c.dims, 900 + nrhs, nrhs=nrhs)
+    for prec, tol in ((F64, 1e-12), (F32, 1e-5)):
+        got = _gpu_op(c, 2, prec, psi)
+        for j in (0, nrhs // 2, nrhs - 1):
+            src = psi[j] if prec == F64 else psi[j].astype(np.complex64).astype(np.complex128)
+            assert rel(got[j], _oracle_op(c, 2, src)) < tol, (prec, j)
+    rc, info = c.t.solve(3, list(range(nrhs)), F32, 1e-4, 500, slot=1, want_true_resid=True)
+    assert rc == 0 and all(i["rel_resid_true"] < 2e-4 for i in info)
+    with pytest.raises(tsm_mod.TsmError):
+        tsm_mod.Tsm(c.dims, max_nrhs=17)
+    c.t.close()
+
+
+def test_empty_source_sets_and_z2_noise(small):
+    """Eq. 2.4 with an empty HP set is Eq. 2.2; with an empty LP set only the correction remains; no sources: zeros."""
+    c = small
+    seed = 71
+    got, _, rc = c.t.run_loop_set(seed, 0, 3, F64, 0.0, 5, nrhs=2)
+    assert rc == 0
+    want = np.zeros_like(got)
+    for j in range(3):
+        eta = oracle.noise(c.dims, seed, j)
+        s, _ = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, 0.0, 5)
+        want += oracle.loops(c.dims, eta, s) / 3
+    assert rel(got, want) < 1e-12
+    got, _, rc = c.t.run_loop_set(seed, 2, 0, F64, 0.0, 5, hp_tol=1e-10, hp_max_iter=2000, nrhs=2)
+    corr, lp, n_hp, n_lp = c.t.loops_get_state()
+    assert rc == 0 and (n_hp, n_lp) == (2, 0) and not lp.any() and np.array_equal(got, corr / 2)
+    got, _, rc = c.t.run_loop_set(seed, 0, 0, F64, 0.0, 5, nrhs=2)
+    assert rc == 0 and not got.any()
+    # Z2 sources through the solver and the contraction
+    rc, info = c.t.solve(seed, [4], F64, 1e-10, 2000, slot=0, kind=1)
+    eta = oracle.noise(c.dims, seed, 4, 1)
+    assert set(np.unique(eta.real)) == {-1.0, 1.0} and not eta.imag.any()
+    s_ref, _ = oracle.solve(c.dims, c.theta, c.kappa, c.mu, c.U, eta, 1e-10, 2000)
+    assert rel(c.t.get_solution(0, 0), s_ref) < 1e-11
+    c.t.loops_reset(False)
+    assert rel(c.t.loops_source(0, 0), oracle.loops(c.dims, eta, s_ref)) < 1e-8
+
+
+def test_fixed_iterations_far_past_convergence_stay_finite(small):
+    """A13: 400 fp64 iterations on a system that converges in ~32: the residual reaches zero / rounding level;
+    a source whose <p,Ap> or |r|^2 vanishes is frozen and flagged, never NaN; the solution stays converged."""
+    c = small
+    rc, info = c.t.solve(8, [0, 1], F64, 0.0, 400, slot=0, want_true_resid=True)
+    assert rc in (0, -5)
+    for j, i in enumerate(info):
+        assert i["status"] in (0, -5) and i["iters"] <= 400
+        s = c.t.get_solution(0, j)
+        assert np.isfinite(s.view(np.float64)).all()
+        assert i["rel_resid_true"] < 1e-12
+    rc, info = c.t.solve(8, [0, 1], F32, 0.0, 400, slot=1, want_true_resid=True)
+    assert all(np.isfinite(i["rel_resid_true"]) and i["rel_resid_true"] < 1e-5 for i in info)
