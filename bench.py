@@ -345,6 +345,15 @@ def extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U):
         del a, b
     out["dslash"] = table
 
+    # ---- the same step with bf16-storage spinors (reading A15: fp32 is the headline, bf16 storage is reported beside it)
+    if prec_name == "f32":
+        ids = list(range(900000, 900000 + nrhs))
+        t.solve(wl.noise_seed, ids, tsm.BF16, wl.lp_tol, wl.lp_iters, slot=1)
+        rc_b, info_b = t.solve(wl.noise_seed, ids, tsm.BF16, wl.lp_tol, wl.lp_iters, slot=1, want_true_resid=True)
+        out["lp_bf16_storage"] = {"solves_per_s": nrhs / info_b[0]["secs"], "secs_batch": info_b[0]["secs"], "iters": info_b[0]["iters"],
+                                  "true_resid_max": max(i["rel_resid_true"] for i in info_b),
+                                  "note": "solve only (no contraction); p, t, w in bf16, x, r and all sums fp32/fp64"}
+
     # ---- contraction kernels (H8, H9, the one-end loops of Eq. 2.5 (N1) and of Eq. 2.6 (N2; its two D_W stencil
     # launches are counted with the stencils, not here) on the slot the timed steps left
     bench_momenta = [(1, 0, 0), (0, 1, 0), (0, 0, 1), (-1, 0, 0), (0, -1, 0), (0, 0, -1)]

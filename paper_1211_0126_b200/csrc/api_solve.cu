@@ -54,6 +54,15 @@ bool graphs_enabled(const tsm_ctx* ctx)
     return on != 0 && !ctx->prof_on && ctx->stream != nullptr && ctx->stream != cudaStreamLegacy && ctx->stream != cudaStreamPerThread;
 }
 
+bool cg_graph_cached(const tsm_ctx* ctx, int prec, int nrhs, int iters, const void* x, const void* r, const void* p, const void* w,
+                     const void* t, double tol)
+{
+    for (const CgGraph& g : ctx->graphs)
+        if (g.prec == prec && g.nrhs == nrhs && g.iters == iters && g.x == x && g.r == r && g.p == p && g.w == w && g.t == t && g.tol == tol)
+            return true;
+    return false;
+}
+
 int cg_iterations_graph(tsm_ctx* ctx, int prec, int nrhs, int iters, const Twists& tw, void* x, void* r, void* p, void* w, void* t, double tol)
 {
     for (const CgGraph& g : ctx->graphs)
@@ -94,14 +103,15 @@ int cg_run(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, void* r,
 {
     // iterations run in chunks of `poll`; in residual mode the host reads the all-done flag after each chunk
     // (a finished batch makes every later kernel return at once), in fixed-iteration mode it never does.
-    // The first chunk is launched kernel by kernel (it also sets up the kernels' attributes), full later
-    // chunks as one cached CUDA graph.
+    // Full chunks run as one cached CUDA graph; the very first chunk of an argument set is launched kernel by
+    // kernel (that also sets up the kernels' attributes, which must not happen inside a capture).
     int rc;
     const int poll = 4;
     const bool use_graph = graphs_enabled(ctx);
+    const bool cached = use_graph && cg_graph_cached(ctx, prec, nrhs, poll, x, r, p, w, t, tol);
     for (int k = 0; k < max_iter;) {
         const int chunk = max_iter - k < poll ? max_iter - k : poll;
-        if (use_graph && k > 0 && chunk == poll) {
+        if (use_graph && (k > 0 || cached) && chunk == poll) {
             if ((rc = cg_iterations_graph(ctx, prec, nrhs, chunk, tw, x, r, p, w, t, tol))) return rc;
         } else {
             for (int j = 0; j < chunk; j++)
