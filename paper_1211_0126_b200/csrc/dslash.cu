@@ -122,10 +122,8 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const int 
                 T rv[24];
                 load_spinor<PR>(out, i, rv);
 #pragma unroll
-                for (int k = 0; k < 24; k++) {
-                    rv[k] -= alpha * o[k];
-                    nrm += (double)rv[k] * (double)rv[k];
-                }
+                for (int k = 0; k < 24; k++) rv[k] -= alpha * o[k];
+                nrm += norm2_site(rv);
                 store_spinor<PR>(out, i, rv);
             } else {
                 store_spinor<PREC>(out, i, o);
@@ -135,11 +133,9 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const int 
                     T ob[24];
 #pragma unroll
                     for (int k8 = 0; k8 < 3; k8++) { const uint4 pk = float_to_bf16x8((const float*)(o + 8 * k8)); bf16x8_to_float(pk, (float*)(ob + 8 * k8)); }
-#pragma unroll
-                    for (int k = 0; k < 24; k++) nrm += (double)ob[k] * (double)ob[k];
+                    nrm += norm2_site(ob);
                 } else {
-#pragma unroll
-                    for (int k = 0; k < 24; k++) nrm += (double)o[k] * (double)o[k];
+                    nrm += norm2_site(o);
                 }
             }
         }

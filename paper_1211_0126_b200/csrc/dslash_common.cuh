@@ -53,3 +53,26 @@ template <typename T, int MU, int SGN> __device__ __forceinline__ void accumulat
     }
 }
 
+
+// Sum of the 24 squares of a site's spinor for the fused norm / residual epilogues.  fp64 data: a plain fp64
+// chain.  fp32 data: four fp32 partial sums of six squares each (FFMA chains), converted and added in fp64 --
+// one quarter-rate F2F per partial instead of one per element (24 conversions per site cost ~10 % of the
+// kernel); sums ACROSS sites stay fp64 with fixed trees (A19).  Both stencil kernels use this, so a source's
+// partial sums are the same in any batch (A14).
+template <typename T> __device__ __forceinline__ double norm2_site(const T* v)
+{
+    double s = 0.0;
+    if constexpr (sizeof(T) == 8) {
+#pragma unroll
+        for (int k = 0; k < 24; k++) s += v[k] * v[k];
+    } else {
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            float p = v[6 * j] * v[6 * j];
+#pragma unroll
+            for (int k = 1; k < 6; k++) p = fmaf(v[6 * j + k], v[6 * j + k], p);
+            s += (double)p;
+        }
+    }
+    return s;
+}

@@ -198,10 +198,8 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
                         float rv[24];
                         load_spinor<PR>((const char*)out_ + fbo * (rhs0 + r), i, rv);
 #pragma unroll
-                        for (int k = 0; k < 24; k++) {
-                            rv[k] -= alpha * o[k];
-                            nrm[r] += (double)rv[k] * (double)rv[k];
-                        }
+                        for (int k = 0; k < 24; k++) rv[k] -= alpha * o[k];
+                        nrm[r] += norm2_site(rv);
                         store_spinor<PR>((char*)out_ + fbo * (rhs0 + r), i, rv);
                     } else {
                         store_spinor<PREC>((char*)out_ + fbo * (rhs0 + r), i, o);
@@ -211,11 +209,9 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
                             float ob[24];
 #pragma unroll
                             for (int k8 = 0; k8 < 3; k8++) { const uint4 pk = float_to_bf16x8(o + 8 * k8); bf16x8_to_float(pk, ob + 8 * k8); }
-#pragma unroll
-                            for (int k = 0; k < 24; k++) nrm[r] += (double)ob[k] * (double)ob[k];
+                            nrm[r] += norm2_site(ob);
                         } else {
-#pragma unroll
-                            for (int k = 0; k < 24; k++) nrm[r] += (double)o[k] * (double)o[k];
+                            nrm[r] += norm2_site(o);
                         }
                     }
                 }
