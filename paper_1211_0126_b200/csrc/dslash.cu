@@ -28,7 +28,7 @@ __device__ __forceinline__ void hop_direction(const void* pack, const void* in, 
     load_link_pair<PREC, RECON>(pack, i, MU, uf, ub);
     load_spinor<PREC>(in, nb[2 * MU], psi);
     project<T, MU, SF>(psi, h);
-    if (MU == 3) {
+    if (MU == 3 && ph_f != 1) {   // time-boundary phase (A22); skipping a multiplication by one is exact
 #pragma unroll
         for (int k = 0; k < 12; k++) h[k] *= ph_f;
     }
@@ -37,7 +37,7 @@ __device__ __forceinline__ void hop_direction(const void* pack, const void* in, 
     accumulate<T, MU, SF>(gq, acc);
     load_spinor<PREC>(in, nb[2 * MU + 1], psi);
     project<T, MU, -SF>(psi, h);
-    if (MU == 3) {
+    if (MU == 3 && ph_b != 1) {
 #pragma unroll
         for (int k = 0; k < 12; k++) h[k] *= ph_b;
     }
@@ -73,6 +73,7 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const int 
     const size_t fb = field_bytes(PREC, Vh, 1), fbo = field_bytes(EPI == EPI_RESID ? PR : PREC, Vh, 1);
     const T cxur = (T)cf.x.up_re, cxui = (T)cf.x.up_im, cxlr = (T)cf.x.lo_re, cxli = (T)cf.x.lo_im;
     const T cdur = (T)cf.d.up_re, cdui = (T)cf.d.up_im, cdlr = (T)cf.d.lo_re, cdli = (T)cf.d.lo_im;
+    const bool d_real = cdui == 0 && cdli == 0;
     __shared__ double smem[EPI != EPI_NONE ? 32 * 4 : 1];
 
     for (int w = blockIdx.x; w < ntiles * gy; w += gridDim.x) {
@@ -104,8 +105,13 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const int 
 #pragma unroll
             for (int q = 0; q < 12; q++) {
                 const T cr = (q < 6) ? cdur : cdlr, ci = (q < 6) ? cdui : cdli;
-                o[2 * q] = cr * acc[2 * q] - ci * acc[2 * q + 1];
-                o[2 * q + 1] = cr * acc[2 * q + 1] + ci * acc[2 * q];
+                if (d_real) {   // Td real (-kappa^2): the same values without the zero products
+                    o[2 * q] = cr * acc[2 * q];
+                    o[2 * q + 1] = cr * acc[2 * q + 1];
+                } else {
+                    o[2 * q] = cr * acc[2 * q] - ci * acc[2 * q + 1];
+                    o[2 * q + 1] = cr * acc[2 * q + 1] + ci * acc[2 * q];
+                }
             }
             if (XPAY) {
                 T xv[24];

@@ -67,7 +67,7 @@ __device__ __forceinline__ void hop_direction_r(const char* tile_links, int tx, 
         float psi[24], h[12], gq[12];
         load_spinor<PREC>(in + fb * r, nb[2 * MU], psi);
         project<float, MU, SF>(psi, h);
-        if (MU == 3) {
+        if (MU == 3 && ph_f != 1) {   // time-boundary phase (A22); skipping a multiplication by one is exact
 #pragma unroll
             for (int k = 0; k < 12; k++) h[k] *= ph_f;
         }
@@ -80,7 +80,7 @@ __device__ __forceinline__ void hop_direction_r(const char* tile_links, int tx, 
         float psi[24], h[12], gq[12];
         load_spinor<PREC>(in + fb * r, nb[2 * MU + 1], psi);
         project<float, MU, -SF>(psi, h);
-        if (MU == 3) {
+        if (MU == 3 && ph_b != 1) {
 #pragma unroll
             for (int k = 0; k < 12; k++) h[k] *= ph_b;
         }
@@ -122,6 +122,7 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
     const size_t fb = field_bytes(PREC, Vh, 1), fbo = field_bytes(EPI == EPI_RESID ? PR : PREC, Vh, 1);
     const float cxur = (float)cf.x.up_re, cxui = (float)cf.x.up_im, cxlr = (float)cf.x.lo_re, cxli = (float)cf.x.lo_im;
     const float cdur = (float)cf.d.up_re, cdui = (float)cf.d.up_im, cdlr = (float)cf.d.lo_re, cdli = (float)cf.d.lo_im;
+    const bool d_real = cdui == 0.f && cdli == 0.f;
     const int tx = threadIdx.x, ty = threadIdx.y;
     const bool leader = (tx == 0 && ty == 0);
 
@@ -180,8 +181,13 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
 #pragma unroll
                     for (int q = 0; q < 12; q++) {
                         const float cr = (q < 6) ? cdur : cdlr, ci = (q < 6) ? cdui : cdli;
-                        o[2 * q] = cr * acc[r][2 * q] - ci * acc[r][2 * q + 1];
-                        o[2 * q + 1] = cr * acc[r][2 * q + 1] + ci * acc[r][2 * q];
+                        if (d_real) {   // Td real (-kappa^2): the same values without the zero products
+                            o[2 * q] = cr * acc[r][2 * q];
+                            o[2 * q + 1] = cr * acc[r][2 * q + 1];
+                        } else {
+                            o[2 * q] = cr * acc[r][2 * q] - ci * acc[r][2 * q + 1];
+                            o[2 * q + 1] = cr * acc[r][2 * q + 1] + ci * acc[r][2 * q];
+                        }
                     }
                     if (XPAY) {
                         float xv[24];
