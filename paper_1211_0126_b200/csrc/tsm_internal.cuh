@@ -409,7 +409,7 @@ struct tsm_ctx {
     void* gauge32[2];                // fp32 packs
     void* staging;                   // raw host-layout staging (links or spinors), fp64
     size_t staging_bytes;
-    void* vec[6];                    // CG vectors r, p, q, w, t, aux: single-parity, max_nrhs, fp64-sized
+    void* vec[6];                    // solver vectors r, p, b (mixed solver only), w, t, aux: single-parity, max_nrhs, fp64-sized
     void* slot[2];                   // solutions: [parity][rhs][chunk][cb], fp64-sized
     int slot_prec[2], slot_nrhs[2], slot_kind[2];
     uint64_t slot_seed[2];
