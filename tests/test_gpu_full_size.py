@@ -100,9 +100,9 @@ def test_full_size_lp_solve_and_loops_cfg5(cfg5):
     assert np.isclose(info[j]["rel_resid_true"], rho, rtol=1e-3)
     c.t.loops_reset(True)
     got = c.t.loops_source(1, j)
-    want = oracle.all_loops(wl.dims, wl.t_boundary, c.U, eta, s, True)  # the oracle contracts the GPU's own s
+    want = oracle.all_loops(wl.dims, wl.t_boundary, c.U, eta, s_ref, True)   # the oracle's own iterate
     assert got.shape == (80, wl.dims[3])
-    assert rel(got, want) < 1e-5
+    assert rel(got[:16], want[:16]) < 1e-4 and rel(got[16:], want[16:]) < 1e-4   # s agrees to 2e-5 elementwise
 
 
 def test_full_size_cfg5_100_iterations_reach_the_fp32_floor(cfg5):
