@@ -652,3 +652,28 @@ def test_fixed_iterations_far_past_convergence_stay_finite(small):
         assert i["rel_resid_true"] < 1e-12
     rc, info = c.t.solve(8, [0, 1], F32, 0.0, 400, slot=1, want_true_resid=True)
     assert all(np.isfinite(i["rel_resid_true"]) and i["rel_resid_true"] < 1e-5 for i in info)
+
+
+def test_stencils_write_nothing_outside_their_output(ragged, tsm_mod):
+    """compute-sanitizer is closed on this pool: canaries instead.  Output fields sit between guard bands; the
+    bands, and the layout padding inside the field (V_h = 720 is padded to 736 sites per source), must be
+    untouched by the single-source and the tile kernels (fp64, fp32, bf16; 1, 3 and 12 sources)."""
+    import torch
+    c = ragged
+    Vh = c.t.V // 2
+    guard = 4096
+    for prec, width in ((F64, 192), (F32, 96), (BF16, 48)):
+        for nrhs in (1, 3, 12):
+            fb = c.t.field_bytes(prec, nrhs)
+            assert fb == width * 736 * nrhs
+            src = c.t.pack(prec, W.random_spinor(c.dims, 31, nrhs=nrhs))
+            buf = torch.full((guard + 2 * fb + guard,), 0xA5, dtype=torch.uint8, device="cuda")
+            out = buf[guard:guard + 2 * fb]
+            c.t.dslash(tsm_mod.OP_M_FULL, prec, nrhs, src, out)
+            c.t.dslash(tsm_mod.OP_MHAT, prec, nrhs, src[:fb], out[:fb])
+            torch.cuda.synchronize()
+            assert bool((buf[:guard] == 0xA5).all()) and bool((buf[guard + 2 * fb:] == 0xA5).all()), (prec, nrhs)
+            # padding: the last layout block of every source holds 16 live and 16 padding sites
+            blk = out[fb:].view(nrhs, 736 // 32, width // 16, 32, 16)
+            assert bool((blk[:, -1, :, 16:, :] == 0xA5).all()), (prec, nrhs)
+            assert not bool((blk[:, -1, :, :16, :] == 0xA5).all())
