@@ -29,8 +29,11 @@
  *     vectors, solution slots, reduction scratch) lives in ONE caller-provided workspace
  *     (a torch tensor's data_ptr()), sized by tsm_workspace_bytes().  The context owns
  *     only metadata, a few KB of pinned host memory and a few KB of device scalars.
- *   - Work is enqueued on the stream given to tsm_set_stream() (default: the legacy
- *     default stream).  Calls that return host scalars or arrays synchronise that stream
+ *   - Work is enqueued on the stream given to tsm_set_stream().  By default, and when that call is given
+ *     NULL, the library uses a BLOCKING stream of its own: it is ordered with the caller's legacy default
+ *     stream exactly as default-stream work would be, and unlike the legacy stream it can be captured, which
+ *     lets the solver replay its CG iterations as cached CUDA graphs (chunks of 4 iterations; TSM_GRAPH=0 in
+ *     the environment turns that off).  Calls that return host scalars or arrays synchronise that stream
  *     before returning; calls that only take dev_* pointers are asynchronous.
  *   - "Native layout" of a single-parity spinor field with V_h = V/2 sites, nrhs sources:
  *       [rhs][block of 32 cb sites][chunk][site in block] of 16-byte vectors (V_h is padded up
@@ -91,7 +94,7 @@ size_t tsm_field_bytes(const tsm_ctx* ctx, int prec, int nrhs);
  * must be 256-byte aligned device memory that outlives every later call. */
 size_t tsm_workspace_bytes(const tsm_ctx* ctx, int max_nrhs);
 int tsm_set_workspace(tsm_ctx* ctx, void* dev_ptr, size_t bytes, int max_nrhs);
-int tsm_set_stream(tsm_ctx* ctx, void* cuda_stream);
+int tsm_set_stream(tsm_ctx* ctx, void* cuda_stream);   /* a cudaStream_t; NULL = the library's own stream */
 
 /* kappa, mu of the kappa-normalised twisted-mass operator of O2:
  * M = 1 + 2 i kappa mu gamma5 - kappa D_hop  (= 2 kappa x the paper's M_u). */
