@@ -279,6 +279,16 @@ def run_ours(args, wl):
     l2_note = (f"inputs larger than L2 (links {link_mb:.0f} MB + {nrhs} x {vec_mb / nrhs:.0f} MB per vector)" if link_mb + 5 * vec_mb > 126
                else f"L2-RESIDENT working set (links {link_mb:.1f} MB + 5 vectors x {vec_mb:.1f} MB < 126 MB): the method re-reads the same "
                     "fields every iteration, so no flush is applied; GB/s figures of this workload are not HBM figures")
+    # second kernel class of the step: the CG x/p update (reads x, p, r; writes x, p)
+    w_p = {"f64": 8, "f32": 4, "bf16": 2}[prec_name]
+    w_x = 4 if prec_name == "bf16" else w_p
+    xp_bytes = (48 * w_x + 24 * w_x + 48 * w_p) * Vh * nrhs
+    xp_ms, xp_n = prof[4]
+    roofline_xp = None
+    if xp_n:
+        xp_gbs = xp_bytes * xp_n / (xp_ms * 1e-3) / 1e9
+        roofline_xp = {"bound": "hbm", "achieved": xp_gbs, "peak": peak, "unit": "GB/s", "frac": xp_gbs / peak,
+                       "kernel": "k_cg_update_xp", "avg_launch_us": xp_ms * 1e3 / xp_n, "algorithmic_bytes_per_launch": xp_bytes}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": prec_name, "data": "synthetic",
@@ -287,7 +297,7 @@ def run_ours(args, wl):
                        "derivative_loops": wl.derivative, "parallelism": f"replicas x{world}",
                        "roofline_events": "inside the timed steps" if events_in_timed else "in a repeat of the timed steps (the timed steps run CG as CUDA graphs)",
                        "l2": l2_note},
-            "gpu_launches": int(launches), "clocks": clk.summary(), "roofline": roofline,
+            "gpu_launches": int(launches), "clocks": clk.summary(), "roofline": roofline, "roofline_cg_update": roofline_xp,
             "lp_iters_done": [i["iters"] for i in info]}
 
     if rank == 0 and not args.skip_extras:
