@@ -677,3 +677,25 @@ def test_stencils_write_nothing_outside_their_output(ragged, tsm_mod):
             blk = out[fb:].view(nrhs, 736 // 32, width // 16, 32, 16)
             assert bool((blk[:, -1, :, 16:, :] == 0xA5).all()), (prec, nrhs)
             assert not bool((blk[:, -1, :, :16, :] == 0xA5).all())
+
+
+@pytest.mark.parametrize("dims", [(16, 16, 4, 4), (8, 32, 4, 4), (32, 8, 4, 6), (64, 4, 4, 4)])
+def test_tile_kernel_in_slab_order_on_small_lattices(tsm_mod, dims):
+    """Lattices with Lxh * Ly a multiple of 128 take the z-slab tile order (like 32^3 x 64) in both stencil kernels:
+    parity with the oracle and bit-identity of batches with the single-source kernel, fp32 and bf16, theta = -1."""
+    c = Case(tsm_mod, dims, 0.6, 33, 0.157, 0.02, -1, max_nrhs=12)
+    psi = W.random_spinor(dims, 77, nrhs=12)
+    for nrhs in (3, 5, 12):
+        for op in (0, 1, 3):
+            got = _gpu_op(c, op, F32, psi[:nrhs])
+            for j in (0, nrhs - 1):
+                src = psi[j].astype(np.complex64).astype(np.complex128)
+                assert rel(got[j], _oracle_op(c, op, src)) < 1e-5, (dims, nrhs, op, j)
+                single = _gpu_op(c, op, F32, psi[j:j + 1])[0]
+                assert np.array_equal(single, got[j]), (dims, nrhs, op, j)
+    for prec in (F32, BF16):
+        rc, info = c.t.solve(9, [0, 1, 2, 3, 4], prec, 0.0, 7, slot=0)
+        batch = c.t.get_solution(0, 3)
+        rc, _ = c.t.solve(9, [3], prec, 0.0, 7, slot=1)
+        assert np.array_equal(c.t.get_solution(1, 0), batch), (dims, prec)
+    c.t.close()
