@@ -418,6 +418,16 @@ def extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U):
         t0 = time.perf_counter()
         oracle.loops_one_end(wl.dims, wl.kappa, wl.mu, oracle.noise(wl.dims, wl.noise_seed, 0))
         detail["t_one_end_contract_s"] = time.perf_counter() - t0
+        if wl.V <= 131072:   # configs 1-3: the same sample on ONE host thread as well
+            try:
+                import ctypes
+                gomp = ctypes.CDLL("libgomp.so.1")
+                gomp.omp_set_num_threads(1)
+                t1, d1 = oracle_sample(wl, U)
+                gomp.omp_set_num_threads(oracle.n_threads())
+                detail["one_thread"] = {"solves_per_s": 1.0 / t1, "t_per_cg_iteration_s": d1["t_per_cg_iteration_s"]}
+            except OSError:
+                pass
         t0 = time.perf_counter()
         oracle.loops_gen_one_end(wl.dims, wl.t_boundary, wl.kappa, U, oracle.noise(wl.dims, wl.noise_seed, 0))
         detail["t_gen_one_end_contract_s"] = time.perf_counter() - t0
