@@ -4,7 +4,8 @@ precision, link storage and sources per batch), on outputs the oracle can afford
   config 5 (32^3 x 64, fp32, 18-real links, 12 sources per batch, derivative loops): the stencil on the
       whole lattice for sampled sources of the batch, element by element; one truncated fp32 solve of a
       12-source batch against the oracle's iterate at equal iteration count and by fp64 true residual;
-      the 80 per-timeslice loops of that source;
+      the 80 per-timeslice loops of that source plus its one-end, generalised one-end and momentum-projected loops;
+      a 12-source mixed-precision HP batch by fp64 true residual;
   config 4 (24^3 x 48, bf16 storage, 12-real links, 4 sources per batch): the stencil, and the solve at
       its residual truncation 5e-3 by true residual;
   config 3 (16^3 x 32, fp32, 12-real links, single source): 50 fixed iterations, true residual.
@@ -98,11 +99,27 @@ def test_full_size_lp_solve_and_loops_cfg5(cfg5):
     rho = oracle.true_residual(wl.dims, wl.t_boundary, wl.kappa, wl.mu, c.U, eta, s)
     assert rho <= max(2 * info_ref["rel_resid_true"], 100 * 6e-8)       # A17, fixed-k mode
     assert np.isclose(info[j]["rel_resid_true"], rho, rtol=1e-3)
-    c.t.loops_reset(True)
+    moms = [(1, 0, 0), (0, -1, 1)]
+    c.t.loops_reset(True, one_end=True, gen_one_end=True, momenta=moms)
     got = c.t.loops_source(1, j)
-    want = oracle.all_loops(wl.dims, wl.t_boundary, c.U, eta, s_ref, True)   # the oracle's own iterate
-    assert got.shape == (80, wl.dims[3])
-    assert rel(got[:16], want[:16]) < 1e-4 and rel(got[16:], want[16:]) < 1e-4   # s agrees to 2e-5 elementwise
+    want = oracle.all_loops(wl.dims, wl.t_boundary, c.U, eta, s_ref, True, one_end=(wl.kappa, wl.mu),
+                            gen_one_end=wl.kappa, momenta=moms)             # the oracle's own iterate
+    assert got.shape == want.shape == (80 + 16 + 16 + 32, wl.dims[3])
+    for lo, hi in ((0, 16), (16, 80), (80, 96), (96, 112), (112, 144)):      # s agrees to 2e-5 elementwise
+        assert rel(got[lo:hi], want[lo:hi]) < 1e-4, (lo, hi)
+    c.t.loops_reset(True)
+
+
+def test_full_size_mixed_precision_hp_batch_cfg5(cfg5):
+    """N4 at the headline size: 12 sources, fp64 defect correction around the fp32 CG to 1e-10; the oracle checks
+    the fp64 true residual of the full system for a sampled source."""
+    c, wl = cfg5, cfg5.wl
+    rc, info = c.t.solve(wl.noise_seed, list(range(12)), c.tsm.MIXED, wl.hp_tol, 5000, slot=0, want_true_resid=True)
+    assert rc == 0
+    assert all(i["status"] == 0 and i["rel_resid_rec"] <= wl.hp_tol and i["rel_resid_true"] <= 1.5e-10 for i in info)
+    eta = oracle.noise(wl.dims, wl.noise_seed, 7)
+    rho = oracle.true_residual(wl.dims, wl.t_boundary, wl.kappa, wl.mu, c.U, eta, c.t.get_solution(0, 7))
+    assert rho <= 1.5e-10 and np.isclose(info[7]["rel_resid_true"], rho, rtol=1e-2)
 
 
 def test_full_size_cfg5_100_iterations_reach_the_fp32_floor(cfg5):
