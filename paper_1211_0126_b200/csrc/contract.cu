@@ -16,7 +16,8 @@
 //     sum_{x in t} tr[Gamma (M_u^-1 + M_d^-1)(x,x)].
 // N3  momentum-projected local loops (PAPER.md:72 uses cuFFT for the Fourier transform; reading A25): for a
 //     short list of integer momenta n, L_Gamma(t, p) = sum_{x in t} exp(+2 pi i n.x/L) eta^dag Gamma s, as one
-//     more block group per momentum (a direct phase sum: a handful of momenta, not a full FFT).
+//     a direct phase sum over a handful of momenta (not a full FFT), all momenta in one pass over s
+//     (k_contract_momenta).
 // H10 Eq. 2.4 accumulators (O7).
 #include "reduce.cuh"
 
@@ -27,11 +28,11 @@ constexpr int CT_MAXBLK = 8;   // blocks per (timeslice, parity)
 
 // grid = (nblk * ngroup_in_launch, Lt, nrhs * 2); MODE 0: local; 1: derivative, mu = blockIdx.x / nblk; 2: one-end;
 // 3: generalised one-end (second = D_W s, same [parity][rhs] layout as sol).
-// 4: momentum-projected local, momentum index = blockIdx.x / nblk.
+// (the momentum-projected loops have their own kernel, k_contract_momenta)
 // partials: [rhs][group][t][par][blk][32], group 0 local, 1..4 derivative mu, 5 one-end, 6 generalised one-end,
 // 7 + m momentum m
 constexpr int CT_NGROUP = 7 + TSM_MAX_MOMENTA;
-enum { CT_LOCAL = 0, CT_DERIV = 1, CT_ONE_END = 2, CT_GEN_ONE_END = 3, CT_MOMENTUM = 4 };
+enum { CT_LOCAL = 0, CT_DERIV = 1, CT_ONE_END = 2, CT_GEN_ONE_END = 3 };
 struct Momenta { int n[TSM_MAX_MOMENTA][3]; };
 template <int PREC, int RECON, int MODE>
 __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs, const int nblk, const void* __restrict__ sol,
@@ -58,7 +59,7 @@ __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs
         const int i = t * g.Vsh + j;
         const SiteCoord sc = decode_site(g, i, par);
         uint32_t bits = 0;
-        if (MODE == CT_LOCAL || MODE == CT_DERIV || MODE == CT_MOMENTUM) bits = noise_bits(lex_of_site(g, sc), seed, sid, kind);
+        if (MODE == CT_LOCAL || MODE == CT_DERIV) bits = noise_bits(lex_of_site(g, sc), seed, sid, kind);
         T v[24], sv[24];
         if (MODE == CT_GEN_ONE_END) {
             load_spinor<PREC>(s_same, i, sv);
@@ -86,20 +87,6 @@ __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs
                 su3_mul(ub, sb + 6 * al, b);
 #pragma unroll
                 for (int k = 0; k < 6; k++) v[6 * al + k] = (T)0.5 * (ph_f * a[k] - ph_b * b[k]);
-            }
-        }
-        if (MODE == CT_MOMENTUM) {   // s <- exp(2 pi i n.x/L) s; the fraction is reduced in integers first
-            const int x = 2 * sc.xh + sc.rowpar;
-            const double fr = (double)(((long long)mom.n[mu][0] * x) % g.L[0]) / g.L[0] +
-                              (double)(((long long)mom.n[mu][1] * sc.y) % g.L[1]) / g.L[1] +
-                              (double)(((long long)mom.n[mu][2] * sc.z) % g.L[2]) / g.L[2];
-            double sn, cs;
-            sincospi(2.0 * fr, &sn, &cs);
-#pragma unroll
-            for (int q = 0; q < 12; q++) {
-                const double re = (double)v[2 * q], im = (double)v[2 * q + 1];
-                v[2 * q] = (T)(cs * re - sn * im);
-                v[2 * q + 1] = (T)(cs * im + sn * re);
             }
         }
 #pragma unroll
@@ -139,9 +126,118 @@ __global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs
     if (threadIdx.x < 32) {
         double tot = 0;
         for (int ww = 0; ww < CT_BS / 32; ww++) tot += sm[ww][threadIdx.x];
-        const int group = MODE == CT_DERIV ? 1 + mu : (MODE == CT_ONE_END ? 5 : (MODE == CT_GEN_ONE_END ? 6 : (MODE == CT_MOMENTUM ? 7 + mu : 0)));
+        const int group = MODE == CT_DERIV ? 1 + mu : (MODE == CT_ONE_END ? 5 : (MODE == CT_GEN_ONE_END ? 6 : 0));
         const size_t o = ((((size_t)rhs * CT_NGROUP + group) * g.L[3] + t) * 2 + par) * nblk + blk;
         partials[o * 32 + threadIdx.x] = tot;
+    }
+}
+
+// N3 in ONE pass over s for all momenta.  grid = (nblk, Lt, nrhs * 2), 256 threads, dynamic shared memory.
+// Per batch of 256 sites of the timeslice: (A) thread = site: regenerate eta, read s once, leave the site's 16
+// complex d_{ab} = sum_c conj(eta_ac) s_bc in D[site][(ab + site) & 15] (swizzled: conflict-free both ways) and its
+// nmom phases exp(2 pi i n.x/L) in P[m][site]; (B) thread = (entry ab, site lane sl): for its 16 sites of the
+// batch, acc[m] += P[m][site] * D[site][ab] for every m (one D read serves all momenta).  At the end the 16 site
+// lanes of an entry are summed in a fixed order and written where k_contract_finish expects group 7 + m.
+constexpr int CM_BS = 256;
+template <int PREC, int NM>   // NM: compile-time bound on nmom (8 or 16): the accumulators live in registers
+__global__ void __launch_bounds__(CM_BS, NM <= 8 ? 2 : 1) k_contract_momenta(const Geom g, const int nrhs, const int nblk, const int nmom,
+                                                            const void* __restrict__ sol, const uint64_t seed,
+                                                            const uint32_t* __restrict__ ids, const int kind,
+                                                            double* __restrict__ partials, const Momenta mom)
+{
+    using T = typename PT<PREC>::real;
+    extern __shared__ __align__(16) double2 cm_smem[];
+    double2* D = cm_smem;                       // [256 sites][16 entries]
+    double2* P = cm_smem + CM_BS * 16;          // [nmom][256 sites]
+    const int nl = g.L[0] + g.L[1] + g.L[2];
+    double2* TB = P + nmom * CM_BS;             // [nmom][Lx + Ly + Lz]: exp(2 pi i n_d k / L_d), k = 0..L_d-1
+    for (int o = threadIdx.x; o < nmom * nl; o += CM_BS) {
+        const int m = o / nl, k = o - m * nl;
+        const int d = k < g.L[0] ? 0 : (k < g.L[0] + g.L[1] ? 1 : 2);
+        const int kk = k - (d == 0 ? 0 : (d == 1 ? g.L[0] : g.L[0] + g.L[1])), L = g.L[d];
+        const int n = ((mom.n[m][d] % L) + L) % L;             // the fraction n k / L reduced in integers first
+        double sn, cs;
+        sincospi(2.0 * (double)((n * kk) % L) / (double)L, &sn, &cs);
+        TB[o] = make_double2(cs, sn);
+    }
+    __syncthreads();
+    const int Vh = g.Vh, tid = threadIdx.x;
+    const int blk = blockIdx.x, t = blockIdx.y, rhs = blockIdx.z >> 1, par = blockIdx.z & 1;
+    const char* s_same = (const char*)sol + field_bytes(PREC, Vh, nrhs) * par + field_bytes(PREC, Vh, 1) * rhs;
+    const uint32_t sid = ids[rhs];
+    const int e = tid & 15, sl = tid >> 4;
+    double2 acc[NM];
+#pragma unroll
+    for (int m = 0; m < NM; m++) acc[m] = make_double2(0.0, 0.0);
+
+    for (int base = blk * CM_BS; base < g.Vsh; base += nblk * CM_BS) {
+        {   // (A)
+            const int j = base + tid;
+            double d[32];
+#pragma unroll
+            for (int k = 0; k < 32; k++) d[k] = 0.0;
+            if (j < g.Vsh) {
+                const int i = t * g.Vsh + j;
+                const SiteCoord sc = decode_site(g, i, par);
+                const uint32_t bits = noise_bits(lex_of_site(g, sc), seed, sid, kind);
+                T v[24];
+                load_spinor<PREC>(s_same, i, v);
+#pragma unroll
+                for (int al = 0; al < 4; al++)
+#pragma unroll
+                    for (int c = 0; c < 3; c++) {
+                        float er, ei;
+                        noise_value((bits >> (2 * (3 * al + c))) & 3, kind, er, ei);
+                        const double cr = er, ci = -ei;   // conj(eta)
+#pragma unroll
+                        for (int be = 0; be < 4; be++) {
+                            const double sr = (double)v[2 * (3 * be + c)], si = (double)v[2 * (3 * be + c) + 1];
+                            d[2 * (4 * al + be)] += cr * sr - ci * si;
+                            d[2 * (4 * al + be) + 1] += cr * si + ci * sr;
+                        }
+                    }
+                const int x = 2 * sc.xh + sc.rowpar;
+                for (int m = 0; m < nmom; m++) {   // exp(2 pi i n.x/L) as the product of the three tabulated 1-d phases
+                    const double2 a = TB[m * nl + x], b = TB[m * nl + g.L[0] + sc.y], c = TB[m * nl + g.L[0] + g.L[1] + sc.z];
+                    const double abr = a.x * b.x - a.y * b.y, abi = a.x * b.y + a.y * b.x;
+                    P[m * CM_BS + tid] = make_double2(abr * c.x - abi * c.y, abr * c.y + abi * c.x);
+                }
+            } else {
+                for (int m = 0; m < nmom; m++) P[m * CM_BS + tid] = make_double2(0.0, 0.0);
+            }
+#pragma unroll
+            for (int k = 0; k < 16; k++) D[tid * 16 + ((k + tid) & 15)] = make_double2(d[2 * k], d[2 * k + 1]);
+        }
+        __syncthreads();
+        // (B)
+#pragma unroll 4
+        for (int q = 0; q < 16; q++) {
+            const int site = sl + 16 * q;
+            const double2 dv = D[site * 16 + ((e + site) & 15)];
+#pragma unroll
+            for (int m = 0; m < NM; m++) {
+                if (m < nmom) {
+                    const double2 ph = P[m * CM_BS + site];
+                    acc[m].x += ph.x * dv.x - ph.y * dv.y;
+                    acc[m].y += ph.x * dv.y + ph.y * dv.x;
+                }
+            }
+        }
+        __syncthreads();
+    }
+    // sum over the 16 site lanes of each entry, fixed order (A19); R[m][sl][e] reuses D
+    double2* R = D;
+#pragma unroll
+    for (int m = 0; m < NM; m++)
+        if (m < nmom) R[(m * 16 + sl) * 16 + e] = acc[m];
+    __syncthreads();
+    for (int o = tid; o < nmom * 16; o += CM_BS) {
+        const int m = o >> 4, ee = o & 15;
+        double re = 0, im = 0;
+        for (int l = 0; l < 16; l++) { const double2 v = R[(m * 16 + l) * 16 + ee]; re += v.x; im += v.y; }
+        const size_t ob = ((((size_t)rhs * CT_NGROUP + 7 + m) * g.L[3] + t) * 2 + par) * nblk + blk;
+        partials[ob * 32 + 2 * ee] = re;
+        partials[ob * 32 + 2 * ee + 1] = im;
     }
 }
 
@@ -248,7 +344,16 @@ int launch_contract(tsm_ctx* ctx, int slot)
     const uint32_t* ids = ctx->ids_dev + slot * TSM_MAX_NRHS;
     const uint64_t seed = ctx->slot_seed[slot];
     const int kind = ctx->slot_kind[slot];
-    const dim3 grid_l(nblk, g.L[3], nrhs * 2), grid_d(nblk * 4, g.L[3], nrhs * 2), grid_m(nblk * (ctx->n_mom > 0 ? ctx->n_mom : 1), g.L[3], nrhs * 2);
+    const dim3 grid_l(nblk, g.L[3], nrhs * 2), grid_d(nblk * 4, g.L[3], nrhs * 2);
+    const size_t cm_smem_bytes = (size_t)CM_BS * 16 * sizeof(double2) +
+                                 (size_t)(ctx->n_mom > 0 ? ctx->n_mom : 1) * (CM_BS + g.L[0] + g.L[1] + g.L[2]) * sizeof(double2);
+    if (ctx->with_momenta && ctx->n_mom > 0) {
+        TSM_CUDA(ctx, cudaFuncSetAttribute(k_contract_momenta<TSM_F64, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cm_smem_bytes));
+        TSM_CUDA(ctx, cudaFuncSetAttribute(k_contract_momenta<TSM_F32, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cm_smem_bytes));
+        TSM_CUDA(ctx, cudaFuncSetAttribute(k_contract_momenta<TSM_F64, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cm_smem_bytes));
+        TSM_CUDA(ctx, cudaFuncSetAttribute(k_contract_momenta<TSM_F32, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cm_smem_bytes));
+        if (cm_smem_bytes > 200 * 1024) return tsm_fail(ctx, TSM_EINVAL, "lattice too wide for the momentum phase tables");
+    }
     Momenta mom;
     for (int m = 0; m < TSM_MAX_MOMENTA; m++)
         for (int k = 0; k < 3; k++) mom.n[m][k] = m < ctx->n_mom ? ctx->mom[m][k] : 0;
@@ -280,7 +385,10 @@ int launch_contract(tsm_ctx* ctx, int slot)
         }                                                                                                                    \
         if (ctx->with_momenta && ctx->n_mom > 0) {                                                                           \
             pi = prof_begin(ctx, P, 9, nrhs);                                                                                \
-            k_contract<P, R, CT_MOMENTUM><<<grid_m, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials, mom); \
+            if (ctx->n_mom <= 8)                                                                                             \
+                k_contract_momenta<P, 8><<<grid_l, CM_BS, cm_smem_bytes, ctx->stream>>>(g, nrhs, nblk, ctx->n_mom, sol, seed, ids, kind, ctx->partials, mom); \
+            else                                                                                                             \
+                k_contract_momenta<P, 16><<<grid_l, CM_BS, cm_smem_bytes, ctx->stream>>>(g, nrhs, nblk, ctx->n_mom, sol, seed, ids, kind, ctx->partials, mom); \
             prof_end(ctx, pi);                                                                                               \
             ctx->launches++;                                                                                                 \
         }                                                                                                                    \

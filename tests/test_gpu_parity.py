@@ -535,7 +535,7 @@ def test_momentum_loops_parity_on_the_oracle_solution(small, ragged):
             got = c.t.loops_source(0, j)
             assert got.shape == want.shape == (112 + 16 * len(MOMENTA), c.dims[3])
             assert rel(got[112:], want[112:]) < 1e-12
-            assert np.array_equal(got[112:128], got[:16])          # n = 0 is the local loop, bit for bit
+            assert rel(got[112:128], got[:16]) < 1e-13             # n = 0 is the local loop (other summation order)
             assert rel(got[:112], want[:112]) < 1e-12
         c.t.loops_reset(False)
 
