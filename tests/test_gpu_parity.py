@@ -699,3 +699,26 @@ def test_tile_kernel_in_slab_order_on_small_lattices(tsm_mod, dims):
         rc, _ = c.t.solve(9, [3], prec, 0.0, 7, slot=1)
         assert np.array_equal(c.t.get_solution(1, 0), batch), (dims, prec)
     c.t.close()
+
+
+def test_caller_stream(small, tsm_mod):
+    """tsm_set_stream with a caller-owned (non-blocking) torch stream: same results as on the library's own stream,
+    including the CUDA-graph replay of the CG iterations on that stream."""
+    import torch
+    c = small
+    rc, info = c.t.solve(11, [0, 1], F32, 0.0, 13, slot=0)
+    want = [c.t.get_solution(0, j) for j in range(2)]
+    stream = torch.cuda.Stream()
+    t2 = tsm_mod.Tsm(c.dims, t_boundary=c.theta, max_nrhs=2, stream=stream)
+    t2.set_params(c.kappa, c.mu)
+    t2.set_gauge(c.U, 18)
+    for _ in range(2):   # the second solve replays cached graphs from the first chunk on
+        rc, info2 = t2.solve(11, [0, 1], F32, 0.0, 13, slot=0)
+        assert rc == 0 and [i["iters"] for i in info2] == [13, 13]
+        for j in range(2):
+            assert np.array_equal(t2.get_solution(0, j), want[j])
+    t2.loops_reset(True)
+    c.t.loops_reset(True)
+    assert np.array_equal(t2.loops_source(0, 1), c.t.loops_source(0, 1))
+    c.t.loops_reset(False)
+    t2.close()
