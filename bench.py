@@ -325,6 +325,7 @@ def run_ours(args, wl):
         print(json.dumps(line), flush=True)
     t.close()
     if world > 1:
+        dist.barrier()   # rank 0 runs the single-rank extras; the others wait here instead of tearing NCCL down under it
         dist.destroy_process_group()
 
 
