@@ -722,3 +722,21 @@ def test_caller_stream(small, tsm_mod):
     assert np.array_equal(t2.loops_source(0, 1), c.t.loops_source(0, 1))
     c.t.loops_reset(False)
     t2.close()
+
+
+def test_loop_set_is_bit_reproducible(medium):
+    """A19: no atomics, fixed reduction trees: the same loop set run twice, and run with another batch size, gives
+    bit-identical loops (fp32 LP batches through the tile kernel and CUDA graphs, fp64 and mixed-precision HP)."""
+    c = medium
+    wl = W.WORKLOADS[2]
+    kw = dict(hp_tol=1e-10, hp_max_iter=2000, with_derivative=True, one_end=True)
+    a, _, rc = c.t.run_loop_set(wl.noise_seed, 3, 9, F32, wl.lp_tol, 1000, nrhs=4, **kw)
+    b, _, _ = c.t.run_loop_set(wl.noise_seed, 3, 9, F32, wl.lp_tol, 1000, nrhs=4, **kw)
+    d, _, _ = c.t.run_loop_set(wl.noise_seed, 3, 9, F32, wl.lp_tol, 1000, nrhs=3, **kw)
+    assert rc == 0 and np.array_equal(a, b) and np.array_equal(a, d)
+    c.t.set_hp_precision(3)
+    e, _, _ = c.t.run_loop_set(wl.noise_seed, 3, 9, F32, wl.lp_tol, 1000, nrhs=4, **kw)
+    f, _, _ = c.t.run_loop_set(wl.noise_seed, 3, 9, F32, wl.lp_tol, 1000, nrhs=1, **kw)
+    c.t.set_hp_precision(0)
+    assert np.array_equal(e, f) and rel(e, a) < 1e-8
+    c.t.loops_reset(False)
