@@ -13,14 +13,19 @@ and one-derivative loop contractions, accumulation into the Eq. 2.4 sums.
               reads the loops back to the host
   roofline  = the stencil kernels inside the timed steps: algorithmic bytes / CUDA-event time
   cpu_baseline = the oracle timed on this box's host cores on a bounded sample
+  workloads = the same figures, compact, for BASELINE.json configs 1-4 (north_star: "for each workload")
 
 python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload 1..5]
+
+With --gpus N > 1 and no WORLD_SIZE in the environment the script starts its N ranks itself
+(torch.distributed.run on 127.0.0.1); N replicas, no data-path collective.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -68,13 +73,33 @@ def stencil_bytes_per_site(prec: str, recon: int, nrhs: int, kind: int) -> float
     return (48 + (24 if kind else 0)) * w_s + links
 
 
-# DRAM traffic per stencil launch from ncu (dram__bytes_read.sum + dram__bytes_write.sum, mean of the four
-# stencil launches of one CG iteration), keyed by (workload, precision, sources per batch); the capture and
-# its command are in profiles/r01_dslash_r12_tile.md and profiles/r01_dslash_r1.md.  None when not captured.
-NCU_TRAFFIC_BYTES = {
-    ("cfg5_32x32x32x64", "f32", 12): (4.628e9 + 3.420e9 + 5.987e9 + 3.391e9) / 4,
-    ("cfg5_32x32x32x64", "f32", 1): (0.906e9 + 0.789e9 + 0.905e9 + 0.789e9) / 4,
-}
+def ncu_traffic(workload: str, prec: str, nrhs: int):
+    """DRAM traffic per stencil launch (dram__bytes_read.sum + dram__bytes_write.sum, mean of the four stencil
+    launches of one CG iteration) from the committed ncu summary profiles/r02_traffic.json, written by
+    `python -m paper_1211_0126_b200.ncu_summary` from an `ncu --set full` capture; the entry names the commit
+    of the kernels it was captured at.  None when there is no capture for this case."""
+    path = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    if not os.path.exists(path):
+        return None
+    try:
+        return json.load(open(path)).get(f"{workload}/{prec}/nrhs{nrhs}")
+    except (OSError, ValueError):
+        return None
+
+
+def workload_config(wl, nrhs: int, world: int) -> dict:
+    """The `config` object of the JSON line: a pure function of the workload, so both arms print the same one."""
+    Vh = wl.V // 2
+    w_s = {"f64": 8, "f32": 4, "bf16": 2}[wl.lp_prec]
+    link_mb = 2 * Vh * 8 * (18 * 8 if wl.lp_prec == "f64" else wl.reconstruct * 4) / 1e6
+    vec_mb = Vh * 24 * w_s * nrhs / 1e6
+    l2 = (f"inputs larger than L2 (links {link_mb:.0f} MB + {nrhs} x {vec_mb / nrhs:.0f} MB per vector); no flush needed"
+          if link_mb + 5 * vec_mb > 126 else
+          f"L2-RESIDENT working set (links {link_mb:.1f} MB + 5 vectors x {vec_mb:.1f} MB < 126 MB): the method re-reads the same "
+          "fields every iteration, so no flush is applied; GB/s figures of this workload are not HBM figures")
+    return {"workload": wl.name, "lattice": list(wl.dims), "kappa": wl.kappa, "mu": wl.mu, "links_eps": wl.eps,
+            "nrhs_per_batch": nrhs, "lp_prec": wl.lp_prec, "lp_iters": wl.lp_iters, "lp_tol": wl.lp_tol, "reconstruct": wl.reconstruct,
+            "derivative_loops": wl.derivative, "parallelism": f"replicas x{world}", "l2": l2}
 
 
 class ClockSampler:
@@ -131,59 +156,231 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------- the oracle legs
-def oracle_sample(wl, U, sid: int = 0):
-    """Bounded sample of one step on the host cores, with the oracle as it stands: one source,
-    source preparation + 1 and 3 CG iterations + reconstruction (+ residual check), and one
-    pass of the loop contractions; the full lp_iters-iteration solve is extrapolated linearly
-    in the iteration count.  Returns (seconds per solve incl. contraction, detail dict)."""
+# An LP solve the oracle finishes within about a minute on the box's cores is run IN FULL (configs 1-4);
+# config 5's 100-iteration solve (~275 s) is extrapolated linearly from 1- and 3-iteration solves.
+def oracle_runs_in_full(wl) -> bool:
+    return not (wl.lp_tol == 0 and wl.lp_iters * wl.V > 5e7)
+
+
+def oracle_warm(wl, U):
+    """One untimed call: thread pool start-up, page faults and the library load stay out of the timings."""
+    import oracle
+    oracle.hop(wl.dims, wl.t_boundary, U, oracle.noise(wl.dims, wl.noise_seed, 0), 0)
+
+
+def oracle_lp_step(wl, U, sid: int, k_short: int | None = None):
+    """One bounded sample of a step on the host cores, the oracle as it stands: one source; either the whole LP
+    solve at the workload's truncation (source preparation, CG, reconstruction, fp64 residual), or -- config 5 --
+    the same solve cut at k_short iterations.  Returns (seconds, iterations done, solution)."""
     import oracle
     eta = oracle.noise(wl.dims, wl.noise_seed, sid)
     t0 = time.perf_counter()
-    s1, _ = oracle.solve(wl.dims, wl.t_boundary, wl.kappa, wl.mu, U, eta, 0.0, 1)
-    t1 = time.perf_counter()
-    s3, _ = oracle.solve(wl.dims, wl.t_boundary, wl.kappa, wl.mu, U, eta, 0.0, 3)
-    t3 = time.perf_counter()
-    oracle.all_loops(wl.dims, wl.t_boundary, U, eta, s3, wl.derivative)
-    tl = time.perf_counter()
-    t_iter = ((t3 - t1) - (t1 - t0)) / 2.0
-    iters = wl.lp_iters if wl.lp_tol == 0 else 10
-    t_solve = (t1 - t0) + (iters - 1) * t_iter + (tl - t3)
-    detail = {"t_1iter_solve_s": t1 - t0, "t_per_cg_iteration_s": t_iter, "t_contract_s": tl - t3,
-              "iterations_extrapolated_to": iters}
-    return t_solve, detail
+    if k_short is None:
+        s, info = oracle.solve(wl.dims, wl.t_boundary, wl.kappa, wl.mu, U, eta, wl.lp_tol, wl.lp_iters)
+    else:
+        s, info = oracle.solve(wl.dims, wl.t_boundary, wl.kappa, wl.mu, U, eta, 0.0, k_short)
+    return time.perf_counter() - t0, info["iters"], (eta, s)
+
+
+def oracle_contract_time(wl, U, eta, s) -> float:
+    import oracle
+    t0 = time.perf_counter()
+    oracle.all_loops(wl.dims, wl.t_boundary, U, eta, s, wl.derivative)
+    return time.perf_counter() - t0
+
+
+def oracle_baseline(wl, U, with_one_thread: bool):
+    """cpu_baseline of our arm: the oracle on a bounded sample of the step (one source).  Returns the dict."""
+    import oracle
+    oracle_warm(wl, U)
+    detail = {}
+    if oracle_runs_in_full(wl):
+        t_solve, iters, (eta, s) = oracle_lp_step(wl, U, 0)
+        t_contract = oracle_contract_time(wl, U, eta, s)
+        detail.update(t_lp_solve_s=t_solve, lp_iterations=iters, t_contract_s=t_contract, extrapolated=False)
+        sample = (f"1 source in full: source preparation, the {iters}-iteration LP solve at the workload's truncation, "
+                  "reconstruction, fp64 residual and one contraction pass")
+    else:
+        t1, _, _ = oracle_lp_step(wl, U, 0, 1)
+        t3, _, (eta, s) = oracle_lp_step(wl, U, 0, 3)
+        t_iter = (t3 - t1) / 2.0
+        assert t_iter > 0, "oracle timing sample is inconsistent (3 iterations faster than 1)"
+        t_contract = oracle_contract_time(wl, U, eta, s)
+        t_solve = t1 + (wl.lp_iters - 1) * t_iter
+        detail.update(t_1iter_solve_s=t1, t_3iter_solve_s=t3, t_per_cg_iteration_s=t_iter, t_contract_s=t_contract,
+                      lp_iterations=wl.lp_iters, t_lp_solve_s=t_solve, extrapolated=True)
+        sample = ("1 source: source preparation, 1- and 3-iteration CG solves, reconstruction, fp64 residual and one "
+                  f"contraction pass run in full; the {wl.lp_iters}-iteration solve extrapolated linearly in the iteration count")
+    # one full-lattice application of the hopping term (the oracle's Dslash), median of 5
+    psi = oracle.noise(wl.dims, wl.noise_seed, 1)
+    ts = []
+    for _ in range(5):
+        t0 = time.perf_counter()
+        oracle.hop(wl.dims, wl.t_boundary, U, psi, -1)
+        ts.append(time.perf_counter() - t0)
+    detail["t_full_lattice_dslash_s_median_of_5"] = float(np.median(ts))
+    if with_one_thread and wl.V <= 131072:   # configs 1-3: the same on ONE host thread as well (BASELINE.md section 3)
+        try:
+            import ctypes
+            gomp = ctypes.CDLL("libgomp.so.1")
+            gomp.omp_set_num_threads(1)
+            t1s, it1, _ = oracle_lp_step(wl, U, 0)
+            t0 = time.perf_counter()
+            oracle.hop(wl.dims, wl.t_boundary, U, psi, -1)
+            td = time.perf_counter() - t0
+            gomp.omp_set_num_threads(oracle.n_threads())
+            detail["one_thread"] = {"t_lp_solve_s": t1s, "lp_iterations": it1, "t_full_lattice_dslash_s": td}
+        except OSError:
+            pass
+    return {"value": 1.0 / (detail["t_lp_solve_s"] + detail["t_contract_s"]), "unit": UNIT, "cores": oracle.n_threads(),
+            "kind": "oracle", "sample": sample, "extrapolated": detail["extrapolated"], "detail": detail}
 
 
 def run_reference(args, wl):
-    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only).  A step is a bounded sample
+    of the workload's step: the whole LP solve + contraction where the oracle finishes it within about a minute,
+    else (config 5) alternately a 1- and a 3-iteration solve, from which the full solve is extrapolated.
+    `ms_per_step` is the time actually spent per timed step; `value` the (extrapolated) rate of full steps."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
     import oracle
     oracle.build()
     U = wl.links()
-    times = []
-    detail = {}
+    oracle_warm(wl, U)
+    full = oracle_runs_in_full(wl)
+    spent, by_k, t_contract, iters_seen = [], {1: [], 3: []}, None, None
     for k in range(args.warmup + args.steps):
-        t, detail = oracle_sample(wl, U, sid=k)
-        if k >= args.warmup:
-            times.append(t)
-    t = float(np.mean(times))
-    value = 1.0 / t
+        timed = k >= args.warmup
+        t0 = time.perf_counter()
+        if full:
+            t_s, iters_seen, (eta, s) = oracle_lp_step(wl, U, k)
+            t_c = oracle_contract_time(wl, U, eta, s)
+            if timed:
+                by_k[1].append(t_s + t_c)
+        else:
+            kk = 1 if k % 2 == 0 else 3
+            t_s, _, (eta, s) = oracle_lp_step(wl, U, k, kk)
+            if timed or not by_k[kk]:
+                by_k[kk].append(t_s)
+            if t_contract is None:          # one contraction pass, in the first (warm-up) step
+                t_contract = oracle_contract_time(wl, U, eta, s)
+        if timed:
+            spent.append(time.perf_counter() - t0)
     cores = oracle.n_threads()
-    sample = ("per step: 1 source of the workload; source preparation, 1- and 3-iteration CG solves, "
-              "reconstruction, fp64 residual and one contraction pass run in full, the "
-              f"{detail['iterations_extrapolated_to']}-iteration solve extrapolated linearly")
+    if full:
+        t_step = float(np.mean(by_k[1]))
+        detail = {"lp_iterations": iters_seen, "extrapolated": False}
+        sample = (f"per step: 1 source of the workload in full: source preparation, the LP solve at the workload's truncation "
+                  f"({iters_seen} iterations), reconstruction, fp64 residual, one contraction pass")
+    else:
+        t1, t3 = float(np.mean(by_k[1])), float(np.mean(by_k[3]))
+        t_iter = (t3 - t1) / 2.0
+        assert t_iter > 0, "oracle timing sample is inconsistent"
+        t_step = t1 + (wl.lp_iters - 1) * t_iter + t_contract
+        detail = {"t_1iter_solve_s": t1, "t_3iter_solve_s": t3, "t_per_cg_iteration_s": t_iter, "t_contract_s": t_contract,
+                  "lp_iterations": wl.lp_iters, "extrapolated": True, "s_per_full_step_extrapolated": t_step}
+        sample = ("per step: 1 source of the workload; source preparation, a 1- or a 3-iteration CG solve (alternating), "
+                  f"reconstruction and fp64 residual run in full; one contraction pass in the first warm-up step; the "
+                  f"{wl.lp_iters}-iteration solve is extrapolated linearly in the iteration count, so `value` is an "
+                  "extrapolated rate while `ms_per_step` is the time actually spent per step")
+    value = 1.0 / t_step
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(np.mean(spent)) * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl.name, "lattice": list(wl.dims), "lp_iters": wl.lp_iters, "lp_tol": wl.lp_tol,
-                       "derivative_loops": wl.derivative},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
-                             "detail": detail},
+            "config": workload_config(wl, args.nrhs if args.nrhs > 0 else wl.nrhs, max(1, args.gpus)),
+            "extrapolated": not full,
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "detail": detail},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
 
 
 # ----------------------------------------------------------------------------- our arm
+def finite_max(torch, buf, pname):
+    v = buf.view({"f32": torch.float32, "f64": torch.float64, "bf16": torch.bfloat16}[pname]).float().abs().max().item()
+    return v
+
+
+def stencil_table(t, tsm, torch, wl, cases, peak, reps=50):
+    """Single-launch stencil timings on FIXED inputs: D_eo a -> b and D_oe a -> c, the output never fed back
+    (repeated applications multiply the norm by 4-6.5 and overflow fp32 within ~50 launches)."""
+    table = {}
+    stream = torch.cuda.current_stream()
+    for pname, n in cases:
+        p = PRECS[pname]
+        a, b, c = t.alloc_field(p, n), t.alloc_field(p, n), t.alloc_field(p, n)
+        if pname == "bf16":
+            a.view(torch.bfloat16).copy_(torch.randn(a.numel() // 2, device=a.device, dtype=torch.float32))
+        else:
+            (a.view(torch.float32) if pname == "f32" else a.view(torch.float64)).normal_()
+        for _ in range(5):
+            t.dslash(tsm.OP_D_EO, p, n, a, b)
+            t.dslash(tsm.OP_D_OE, p, n, a, c)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            t.dslash(tsm.OP_D_EO, p, n, a, b)
+            t.dslash(tsm.OP_D_OE, p, n, a, c)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        us = e0.elapsed_time(e1) * 1e3 / (2 * reps)
+        by = stencil_bytes_per_site(pname, wl.reconstruct, n, 0) * (wl.V // 2) * n
+        mx = max(finite_max(torch, b, pname), finite_max(torch, c, pname))
+        table[f"{pname}_nrhs{n}"] = {"us": us, "algorithmic_GBs": by / us / 1e3, "frac_of_measured_peak": by / us / 1e3 / peak,
+                                     "frac_of_8000": by / us / 1e3 / 8000.0, "gflops": 1320.0 * (wl.V // 2) * n / us / 1e3,
+                                     "max_abs_out": mx, "finite": bool(np.isfinite(mx))}
+        del a, b, c
+    return table
+
+
+def workload_summary(cfg: int, tsm, torch, peak, with_oracle: bool):
+    """Compact figures for one of the small workloads (configs 1-4): single-launch stencil, LP solves/s in the
+    workload's own launch configuration, the whole Eq. 2.4 set, iteration counts, and the oracle beside them."""
+    wl = W.WORKLOADS[cfg]
+    U = wl.links()
+    stream = torch.cuda.current_stream()
+    t = tsm.Tsm(wl.dims, t_boundary=wl.t_boundary, device=torch.cuda.current_device(), max_nrhs=wl.nrhs, stream=stream)
+    t.set_params(wl.kappa, wl.mu)
+    t.set_gauge(U, wl.reconstruct)
+    if wl.lp_prec == "f64":
+        t.set_hp_precision(tsm.F64)     # config 1 is "fp64 throughout"
+    prec = PRECS[wl.lp_prec]
+    out = {"lattice": list(wl.dims), "lp": f"{wl.lp_prec}, " + (f"tol {wl.lp_tol:g}" if wl.lp_tol > 0 else f"{wl.lp_iters} iterations"),
+           "nrhs_per_batch": wl.nrhs, "reconstruct": wl.reconstruct}
+    cases = [("f32", 1), ("f64", 1)] + ([(wl.lp_prec, wl.nrhs)] if (wl.lp_prec, wl.nrhs) not in (("f32", 1), ("f64", 1)) else [])
+    out["dslash"] = {k: {"us": v["us"], "algorithmic_GBs": v["algorithmic_GBs"], "frac_of_measured_peak": v["frac_of_measured_peak"],
+                         "gflops": v["gflops"], "finite": v["finite"]}
+                     for k, v in stencil_table(t, tsm, torch, wl, cases, peak, reps=100).items()}
+    out["l2_resident"] = wl.V <= 131072
+    t.loops_reset(wl.derivative)
+    steps, nb = 20, 0
+    for k in range(3):
+        t.solve(wl.noise_seed, list(range(k * wl.nrhs, (k + 1) * wl.nrhs)), prec, wl.lp_tol, wl.lp_iters, slot=1)
+        t.loops_add_lp(1)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for k in range(steps):
+        rc, info = t.solve(wl.noise_seed, list(range(1000 + k * wl.nrhs, 1000 + (k + 1) * wl.nrhs)), prec, wl.lp_tol, wl.lp_iters, slot=1)
+        t.loops_add_lp(1)
+        nb += wl.nrhs
+    e1.record(stream)
+    torch.cuda.synchronize()
+    out["lp_solves_per_s"] = nb / (e0.elapsed_time(e1) * 1e-3)
+    out["lp_iters"] = sorted(set(i["iters"] for i in info))
+    loops, secs, rc = t.run_loop_set(wl.noise_seed, wl.n_hp, wl.n_lp, prec, wl.lp_tol, wl.lp_iters, hp_tol=wl.hp_tol,
+                                     hp_max_iter=5000, nrhs=wl.nrhs, with_derivative=wl.derivative)
+    out["tsm_loop_set"] = {"seconds": secs, "n_hp": wl.n_hp, "n_lp": wl.n_lp, "rc": rc, "hp_solver": t.hp_precision_name(),
+                           "finite": bool(np.isfinite(loops.view(np.float64)).all())}
+    rc, info = t.solve(wl.noise_seed, list(range(min(wl.nrhs, wl.n_hp))), tsm.F64, wl.hp_tol, 5000, slot=0, want_true_resid=True)
+    out["hp_solve"] = {"iters": sorted(set(i["iters"] for i in info)), "secs_batch": info[0]["secs"],
+                       "true_resid_max": max(i["rel_resid_true"] for i in info)}
+    t.close()
+    if with_oracle:
+        ob = oracle_baseline(wl, U, with_one_thread=True)
+        out["oracle"] = {"lp_solves_per_s": ob["value"], "cores": ob["cores"], "extrapolated": ob["extrapolated"], **ob["detail"]}
+    return out
+
+
 def run_ours(args, wl):
     import torch
     import torch.distributed as dist
@@ -194,6 +391,10 @@ def run_ours(args, wl):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device (there is no CPU fallback for the product path)")
+    if world != args.gpus:
+        raise RuntimeError(f"--gpus {args.gpus} but {world} rank(s) were started")
+    if local >= torch.cuda.device_count():
+        raise RuntimeError(f"rank {rank}: local rank {local} has no GPU ({torch.cuda.device_count()} visible)")
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
@@ -203,10 +404,16 @@ def run_ours(args, wl):
     nrhs = args.nrhs if args.nrhs > 0 else wl.nrhs
     tol, iters = wl.lp_tol, wl.lp_iters
 
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
     t0 = time.perf_counter()
-    U = wl.links()
-    log(f"[bench] rank {rank}: links {wl.name} generated in {time.perf_counter() - t0:.1f} s")
-    links_host = torch.from_numpy(U.view(np.float64).reshape(-1)).pin_memory()
+    U = replicas.node_shared_links(wl, local, world, barrier if world > 1 else None)   # generated once per node
+    log(f"[bench] rank {rank}: links {wl.name} ready in {time.perf_counter() - t0:.1f} s")
+    links_host = torch.from_numpy(np.ascontiguousarray(U).view(np.float64).reshape(-1)).pin_memory()
     stream = torch.cuda.current_stream()
     t = tsm.Tsm(wl.dims, t_boundary=wl.t_boundary, device=local, max_nrhs=nrhs, stream=stream)
     t.set_params(wl.kappa, wl.mu)
@@ -222,12 +429,6 @@ def run_ours(args, wl):
         rc, info = t.solve(wl.noise_seed, ids, prec, tol, iters, slot=1)
         t.loops_add_lp(1)
         return info
-
-    def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-            torch.cuda.synchronize()
 
     for _ in range(args.warmup):
         info = step()
@@ -264,21 +465,21 @@ def run_ours(args, wl):
     st_ms = sum(prof[k][0] for k in range(4))
     st_n = sum(prof[k][1] for k in range(4))
     achieved = alg_bytes / (st_ms * 1e-3) / 1e9 if st_ms > 0 else 0.0
+    traffic = ncu_traffic(wl.name, prec_name, nrhs)
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get((wl.name, prec_name, nrhs)), "traffic_unit": "bytes per launch (ncu, profiles/)",
-                "peak_source": peak_src, "kernel": f"{'k_dslash_tile' if nrhs > 1 and prec_name != 'f64' else 'k_dslash'}<{prec_name}, recon {wl.reconstruct}> x {nrhs} sources (the 4 stencil launches of a CG iteration)",
+                "traffic": traffic["bytes_per_launch"] if traffic else None,
+                "traffic_source": ({k: traffic[k] for k in ("commit", "summary", "kernels") if k in traffic} if traffic else None),
+                "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r02_traffic.json)",
+                "peak_source": peak_src, "kernel": f"{t.stencil_kernel_name(prec, nrhs)}<{prec_name}, recon {wl.reconstruct}> x {nrhs} sources (the 4 stencil launches of a CG iteration)",
                 "launches_timed": st_n, "avg_launch_us": st_ms * 1e3 / max(st_n, 1),
                 "algorithmic_bytes_per_launch": alg_bytes / max(st_n, 1),
                 "share_of_step": {"stencil": st_ms / ms, "cg_update_xp": prof[4][0] / ms} if events_in_timed else None,
                 "per_kind_us": {str(k): (prof[k][0] * 1e3 / prof[k][1] if prof[k][1] else None) for k in range(5)},
-                "gflops_at_1320_per_site": 1320.0 * Vh * nrhs * st_n / (st_ms * 1e-3) / 1e9 if st_ms > 0 else 0.0}
+                "per_kind_frac": {str(k): (stencil_bytes_per_site(prec_name, wl.reconstruct, nrhs, k) * Vh * nrhs * prof[k][1] / (prof[k][0] * 1e-3) / 1e9 / peak
+                                           if prof[k][1] else None) for k in range(4)},
+                "gflops_at_1320_per_site": 1320.0 * Vh * nrhs * st_n / (st_ms * 1e-3) / 1e9 if st_ms > 0 else 0.0,
+                "events": "inside the timed steps" if events_in_timed else "in a repeat of the timed steps (the timed steps run CG as CUDA graphs)"}
 
-    w_s = {"f64": 8, "f32": 4, "bf16": 2}[prec_name]
-    link_mb = 2 * Vh * 8 * (18 * 8 if prec_name == "f64" else wl.reconstruct * 4) / 1e6
-    vec_mb = Vh * 24 * w_s * nrhs / 1e6
-    l2_note = (f"inputs larger than L2 (links {link_mb:.0f} MB + {nrhs} x {vec_mb / nrhs:.0f} MB per vector)" if link_mb + 5 * vec_mb > 126
-               else f"L2-RESIDENT working set (links {link_mb:.1f} MB + 5 vectors x {vec_mb:.1f} MB < 126 MB): the method re-reads the same "
-                    "fields every iteration, so no flush is applied; GB/s figures of this workload are not HBM figures")
     # second kernel class of the step: the CG x/p update (reads x, p, r; writes x, p)
     w_p = {"f64": 8, "f32": 4, "bf16": 2}[prec_name]
     w_x = 4 if prec_name == "bf16" else w_p
@@ -291,12 +492,7 @@ def run_ours(args, wl):
                        "kernel": "k_cg_update_xp", "avg_launch_us": xp_ms * 1e3 / xp_n, "algorithmic_bytes_per_launch": xp_bytes}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": prec_name, "data": "synthetic",
-            "config": {"workload": wl.name, "lattice": list(wl.dims), "kappa": wl.kappa, "mu": wl.mu, "links_eps": wl.eps,
-                       "nrhs_per_batch": nrhs, "lp_iters": iters, "lp_tol": tol, "reconstruct": wl.reconstruct,
-                       "derivative_loops": wl.derivative, "parallelism": f"replicas x{world}",
-                       "roofline_events": "inside the timed steps" if events_in_timed else "in a repeat of the timed steps (the timed steps run CG as CUDA graphs)",
-                       "l2": l2_note},
+            "dtype": prec_name, "data": "synthetic", "config": workload_config(wl, nrhs, world),
             "gpu_launches": int(launches), "clocks": clk.summary(), "roofline": roofline, "roofline_cg_update": roofline_xp,
             "lp_iters_done": [i["iters"] for i in info]}
 
@@ -320,45 +516,24 @@ def run_ours(args, wl):
                                "contracted, the loops read back; in production one upload serves N_HP+N_LP solves"}
 
     if rank == 0 and not args.skip_extras:
-        line.update(extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U))
+        line.update(extras(args, wl, t, tsm, torch, prec, prec_name, peak, U, world))
+    t.close()
+    if rank == 0 and not args.skip_extras and not args.no_workloads and world == 1 and args.workload == 5:
+        # north_star: "report, for each workload": configs 1-4, compact, in the same driver-run line
+        line["workloads"] = {W.WORKLOADS[c].name: workload_summary(c, tsm, torch, peak, not args.no_cpu_baseline) for c in (1, 2, 3, 4)}
     if rank == 0:
         print(json.dumps(line), flush=True)
-    t.close()
     if world > 1:
         dist.barrier()   # rank 0 runs the single-rank extras; the others wait here instead of tearing NCCL down under it
         dist.destroy_process_group()
 
 
-def extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U):
-    """e2e through the host-buffer API, single-launch stencil table, full loop set, oracle baseline."""
+def extras(args, wl, t, tsm, torch, prec, prec_name, peak, U, world):
+    """Single-launch stencil table, contraction kernels, full loop set, HP solves, oracle baseline."""
     out = {}
     nrhs = args.nrhs if args.nrhs > 0 else wl.nrhs
-    stream = torch.cuda.current_stream()
     # ---- single-launch stencil table (north_star: >= 70 % of HBM peak on single-RHS fp32 / fp64)
-    table = {}
-    for pname, n in (("f32", 1), ("f64", 1), ("f32", nrhs), ("bf16", 1)):
-        p = PRECS[pname]
-        a = t.alloc_field(p, n)
-        b = t.alloc_field(p, n)
-        a.view(torch.int16)[:] = 0x3C00 if pname == "bf16" else 0
-        if pname != "bf16":
-            (a.view(torch.float32) if pname == "f32" else a.view(torch.float64)).normal_()
-        reps = 50
-        for _ in range(5):
-            t.dslash(tsm.OP_D_EO, p, n, a, b)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        for _ in range(reps):
-            t.dslash(tsm.OP_D_EO, p, n, a, b)
-            t.dslash(tsm.OP_D_OE, p, n, b, a)
-        e1.record(stream)
-        torch.cuda.synchronize()
-        us = e0.elapsed_time(e1) * 1e3 / (2 * reps)
-        by = stencil_bytes_per_site(pname, wl.reconstruct, n, 0) * (wl.V // 2) * n
-        table[f"{pname}_nrhs{n}"] = {"us": us, "algorithmic_GBs": by / us / 1e3, "frac_of_measured_peak": by / us / 1e3 / peak,
-                                     "frac_of_8000": by / us / 1e3 / 8000.0, "gflops": 1320.0 * (wl.V // 2) * n / us / 1e3}
-        del a, b
-    out["dslash"] = table
+    out["dslash"] = stencil_table(t, tsm, torch, wl, (("f32", 1), ("f64", 1), ("f32", nrhs), ("bf16", 1)), peak)
 
     # ---- the same step with bf16-storage spinors (reading A15: fp32 is the headline, bf16 storage is reported beside it)
     if prec_name == "f32":
@@ -368,6 +543,7 @@ def extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U):
         out["lp_bf16_storage"] = {"solves_per_s": nrhs / info_b[0]["secs"], "secs_batch": info_b[0]["secs"], "iters": info_b[0]["iters"],
                                   "true_resid_max": max(i["rel_resid_true"] for i in info_b),
                                   "note": "solve only (no contraction); p, t, w in bf16, x, r and all sums fp32/fp64"}
+        t.solve(wl.noise_seed, ids, prec, wl.lp_tol, wl.lp_iters, slot=1)   # leave an fp32 solution of this batch in the slot
 
     # ---- contraction kernels (H8, H9, the one-end loops of Eq. 2.5 (N1) and of Eq. 2.6 (N2; its two D_W stencil
     # launches are counted with the stencils, not here) on the slot the timed steps left
@@ -381,10 +557,10 @@ def extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U):
     w_sol = 8 if prec_name == "f64" else 4
     names = {5: "local_16_gamma", 6: "derivative_4_directions", 7: "one_end_eq_2_5", 8: "gen_one_end_eq_2_6_contraction_only",
              9: "momentum_projected_6_momenta"}
-    # algorithmic bytes per site of the full lattice and source: s once (eta is regenerated, never read);
-    # derivative: s once + the 8 links of the site
+    # algorithmic bytes per site of the full lattice and source (SURVEY.md 8(d) convention): s once (eta is regenerated,
+    # never read); derivative: s once + the 8 links of the site ONCE PER BATCH
     n_g = 18 if prec_name == "f64" else wl.reconstruct
-    by_site = {5: 24 * w_sol, 6: 24 * w_sol + 8 * n_g * (8 if prec_name == "f64" else 4), 7: 24 * w_sol, 8: 48 * w_sol, 9: 24 * w_sol}
+    by_site = {5: 24 * w_sol, 6: 24 * w_sol + 8 * n_g * (8 if prec_name == "f64" else 4) / nrhs, 7: 24 * w_sol, 8: 48 * w_sol, 9: 24 * w_sol}
     ct = {}
     for k in (5, 6, 7, 8, 9):
         ms_k, n_k = t.profile_read(sp, k, nrhs)
@@ -399,49 +575,46 @@ def extras(args, wl, t, tsm, torch, links_host, prec, prec_name, step, peak, U):
     if not args.no_full_set:
         loops, secs, rc = t.run_loop_set(wl.noise_seed, wl.n_hp, wl.n_lp, prec, wl.lp_tol, wl.lp_iters, hp_tol=wl.hp_tol,
                                          hp_max_iter=5000, nrhs=nrhs, with_derivative=wl.derivative)
-        out["tsm_loop_set"] = {"seconds": secs, "n_hp": wl.n_hp, "n_lp": wl.n_lp, "rc": rc,
+        out["tsm_loop_set"] = {"seconds": secs, "n_hp": wl.n_hp, "n_lp": wl.n_lp, "rc": rc, "hp_solver": t.hp_precision_name(),
                                "finite": bool(np.isfinite(loops.view(np.float64)).all())}
         rc, info = t.solve(wl.noise_seed, list(range(min(nrhs, wl.n_hp))), tsm.F64, wl.hp_tol, 5000, slot=0, want_true_resid=True)
-        out["hp_solve"] = {"iters": [i["iters"] for i in info], "secs_batch": info[0]["secs"],
-                           "true_resid_max": max(i["rel_resid_true"] for i in info)}
-        # N4: the same HP solves as fp64 defect correction around the fp32 CG, and Eq. 2.4 with them
+        out["hp_solve_fp64"] = {"iters": [i["iters"] for i in info], "secs_batch": info[0]["secs"],
+                                "true_resid_max": max(i["rel_resid_true"] for i in info)}
+        # N4: the same HP solves as fp64 defect correction around the fp32 CG
         rc, info = t.solve(wl.noise_seed, list(range(min(nrhs, wl.n_hp))), tsm.MIXED, wl.hp_tol, 5000, slot=0, want_true_resid=True)
         out["hp_solve_mixed"] = {"iters_fp32_total": [i["iters"] for i in info], "secs_batch": info[0]["secs"],
                                  "true_resid_max": max(i["rel_resid_true"] for i in info)}
-        t.set_hp_precision(tsm.MIXED)
-        loops_m, secs_m, rc_m = t.run_loop_set(wl.noise_seed, wl.n_hp, wl.n_lp, prec, wl.lp_tol, wl.lp_iters, hp_tol=wl.hp_tol,
+        other = tsm.F64 if t.hp_precision == tsm.MIXED else tsm.MIXED
+        mine = t.hp_precision
+        t.set_hp_precision(other)
+        loops_o, secs_o, rc_o = t.run_loop_set(wl.noise_seed, wl.n_hp, wl.n_lp, prec, wl.lp_tol, wl.lp_iters, hp_tol=wl.hp_tol,
                                                hp_max_iter=5000, nrhs=nrhs, with_derivative=wl.derivative)
-        t.set_hp_precision(tsm.F64)
-        out["tsm_loop_set_mixed_hp"] = {"seconds": secs_m, "rc": rc_m,
-                                        "max_rel_diff_to_fp64_hp": float(np.abs(loops_m - loops).max() / np.abs(loops).max())}
+        t.set_hp_precision(mine)
+        out["tsm_loop_set_other_hp_solver"] = {"seconds": secs_o, "rc": rc_o, "hp_solver": "fp64" if other == tsm.F64 else "mixed",
+                                               "max_rel_diff_of_the_loops": float(np.abs(loops_o - loops).max() / np.abs(loops).max())}
 
-    # ---- the oracle on this box's host cores, bounded sample
-    if not args.no_cpu_baseline:
+    # ---- the oracle on this box's host cores, bounded sample (rank 0, N = 1 only)
+    if not args.no_cpu_baseline and world == 1:
         import oracle
         oracle.build()
-        tcpu, detail = oracle_sample(wl, U)
-        t0 = time.perf_counter()
-        oracle.loops_one_end(wl.dims, wl.kappa, wl.mu, oracle.noise(wl.dims, wl.noise_seed, 0))
-        detail["t_one_end_contract_s"] = time.perf_counter() - t0
-        if wl.V <= 131072:   # configs 1-3: the same sample on ONE host thread as well
-            try:
-                import ctypes
-                gomp = ctypes.CDLL("libgomp.so.1")
-                gomp.omp_set_num_threads(1)
-                t1, d1 = oracle_sample(wl, U)
-                gomp.omp_set_num_threads(oracle.n_threads())
-                detail["one_thread"] = {"solves_per_s": 1.0 / t1, "t_per_cg_iteration_s": d1["t_per_cg_iteration_s"]}
-            except OSError:
-                pass
-        t0 = time.perf_counter()
-        oracle.loops_gen_one_end(wl.dims, wl.t_boundary, wl.kappa, U, oracle.noise(wl.dims, wl.noise_seed, 0))
-        detail["t_gen_one_end_contract_s"] = time.perf_counter() - t0
-        out["cpu_baseline"] = {"value": 1.0 / tcpu, "unit": UNIT, "cores": oracle.n_threads(), "kind": "oracle",
-                               "sample": ("1 source: source preparation, 1- and 3-iteration CG solves, reconstruction, residual and one "
-                                          f"contraction pass run in full; the {detail['iterations_extrapolated_to']}-iteration solve "
-                                          "extrapolated linearly in the iteration count"),
-                               "detail": detail}
+        out["cpu_baseline"] = oracle_baseline(wl, U, with_one_thread=True)
     return out
+
+
+def spawn_ranks(args) -> int:
+    """`python bench.py --gpus N` without a launcher: start the N ranks ourselves (one process per GPU)."""
+    if args.impl == "ours":
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < args.gpus:
+            log(f"[bench] --gpus {args.gpus} needs {args.gpus} CUDA devices, {have} visible: refusing to run fewer ranks than asked")
+            return 2
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -452,10 +625,15 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", type=int, default=5)
     ap.add_argument("--nrhs", type=int, default=0, help="sources per batch (default: the workload's; other values are profiling aids, not the headline)")
-    ap.add_argument("--skip-extras", action="store_true", help="only the timed steps (no e2e/table/full set/oracle)")
+    ap.add_argument("--skip-extras", action="store_true", help="only the timed steps (no e2e/table/full set/oracle/workloads)")
     ap.add_argument("--no-full-set", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-workloads", action="store_true", help="skip the compact block for configs 1-4")
     args = ap.parse_args()
+    if args.gpus < 1:
+        ap.error("--gpus must be >= 1")
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(spawn_ranks(args))
     wl = W.WORKLOADS[args.workload]
     if args.impl == "reference":
         run_reference(args, wl)

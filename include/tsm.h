@@ -177,8 +177,14 @@ int tsm_run_loop_set(tsm_ctx* ctx, uint64_t seed, int kind, int n_hp, int n_lp, 
                      double lp_tol, int lp_iters, double hp_tol, int hp_max_iter, int nrhs,
                      int ops, double* host_out, double* secs_out);
 
-/* Precision of the HP solves of tsm_run_loop_set: TSM_F64 (default) or TSM_MIXED. */
+/* Solver of the HP solves of tsm_run_loop_set ("high precision" inversions): TSM_MIXED (default:
+ * fp64 defect correction around the fp32 CG, stopped on the fp64 TRUE residual -- the same fp64 solution at
+ * low-precision bandwidth cost) or TSM_F64 (plain fp64 CG; what a workload that is "fp64 throughout" asks for). */
 int tsm_set_hp_precision(tsm_ctx* ctx, int prec);
+
+/* Name of the stencil kernel the library launches for spinor precision `prec` and a batch of `nrhs` sources in this
+ * context (static string; measurement aid: bench.py prints it beside the roofline). */
+const char* tsm_stencil_kernel_name(const tsm_ctx* ctx, int prec, int nrhs);
 
 /* Number of kernels this library has launched on the context since creation. */
 long long tsm_launch_count(const tsm_ctx* ctx);

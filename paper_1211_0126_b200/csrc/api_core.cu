@@ -103,11 +103,12 @@ int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
     ctx->with_one_end = 0;
     ctx->with_gen_one_end = 0;
     ctx->with_momenta = 0;
-    ctx->hp_prec = TSM_F64;
+    ctx->hp_prec = TSM_MIXED;
     ctx->n_mom = 0;
     ctx->n_hp = ctx->n_lp = 0;
     ctx->launches = 0;
     ctx->prof_on = false;
+    ctx->loops_ready = false;
     ctx->cg = nullptr; ctx->cg_host = nullptr; ctx->host_small = nullptr; ctx->ids_dev = nullptr;
     for (int s = 0; s < 2; s++) { ctx->slot_prec[s] = -1; ctx->slot_nrhs[s] = 0; }
     build_gamma_table(ctx->gam);
@@ -208,7 +209,9 @@ int tsm_set_workspace(tsm_ctx* ctx, void* dev_ptr, size_t bytes, int max_nrhs)
     ctx->have_gauge = false;
     ctx_drop_graphs(ctx);
     for (int s = 0; s < 2; s++) { ctx->slot_prec[s] = -1; ctx->slot_nrhs[s] = 0; }
-    return TSM_OK;
+    // the caller's buffer is uninitialised: start from the default operator set (16 local loops) with zeroed sums
+    ctx->loops_ready = false;
+    return tsm_loops_reset(ctx, 0);
 }
 
 int tsm_set_stream(tsm_ctx* ctx, void* cuda_stream)
@@ -248,7 +251,7 @@ int tsm_set_gauge(tsm_ctx* ctx, const double* host_links, int reconstruct, doubl
     TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     const double dev = ctx->host_small[0];
     if (max_unitarity_dev) *max_unitarity_dev = dev;
-    if (!(dev == dev)) return tsm_fail(ctx, TSM_EINVAL, "non-finite gauge links");
+    if (!std::isfinite(dev)) return tsm_fail(ctx, TSM_EINVAL, "non-finite gauge links");
     if (reconstruct == 12 && dev > 1e-10) return tsm_fail(ctx, TSM_ENOTUNITARY, "links are not SU(3) to 1e-10; 12-real reconstruction refused");
     ctx->have_gauge = true;
     return TSM_OK;

@@ -201,6 +201,12 @@ int true_residuals(tsm_ctx* ctx, int slot, double* out)
     return TSM_OK;
 }
 
+int check_loops(tsm_ctx* ctx)
+{
+    if (!ctx->loops_ready) return tsm_fail(ctx, TSM_ESTATE, "loop accumulators not set up: call tsm_loops_reset (also after tsm_loops_set_momenta)");
+    return TSM_OK;
+}
+
 int check_slot(tsm_ctx* ctx, int slot, int rhs)
 {
     if (slot < 0 || slot > 1) return tsm_fail(ctx, TSM_EINVAL, "slot must be 0 or 1");
@@ -288,13 +294,12 @@ int tsm_get_solution(tsm_ctx* ctx, int slot, int rhs, double* host_out)
     if ((rc = check_slot(ctx, slot, rhs))) return rc;
     if (!host_out) return tsm_fail(ctx, TSM_EINVAL, "null output");
     const int sp = ctx->slot_prec[slot], nrhs = ctx->slot_nrhs[slot], Vh = ctx->g.Vh;
-    // gather the two parities of source `rhs` into a one-source full-lattice field, then unpack
-    char* tmp = (char*)ctx->vec[5];
-    const size_t f1 = field_bytes(sp, Vh, 1);
-    for (int par = 0; par < 2; par++)
-        TSM_CUDA(ctx, cudaMemcpyAsync(tmp + par * f1, (char*)ctx->slot[slot] + field_bytes(sp, Vh, nrhs) * par + f1 * rhs, f1,
-                                      cudaMemcpyDeviceToDevice, ctx->stream));
-    return tsm_unpack(ctx, sp, 1, tmp, host_out);
+    // unpack the two parities of source `rhs` straight from the slot (parity stride = the slot's [rhs] extent)
+    const char* src = (const char*)ctx->slot[slot] + field_bytes(sp, Vh, 1) * rhs;
+    if ((rc = launch_unpack_spinor(ctx, sp, 1, src, (double*)ctx->staging, field_bytes(sp, Vh, nrhs)))) return rc;
+    TSM_CUDA(ctx, cudaMemcpyAsync(host_out, ctx->staging, (size_t)ctx->g.V * 24 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return TSM_OK;
 }
 
 int tsm_set_solution(tsm_ctx* ctx, int slot, int rhs, const double* host_in)
@@ -304,12 +309,9 @@ int tsm_set_solution(tsm_ctx* ctx, int slot, int rhs, const double* host_in)
     if ((rc = check_slot(ctx, slot, rhs))) return rc;
     if (!host_in) return tsm_fail(ctx, TSM_EINVAL, "null input");
     const int sp = ctx->slot_prec[slot], nrhs = ctx->slot_nrhs[slot], Vh = ctx->g.Vh;
-    char* tmp = (char*)ctx->vec[5];
-    if ((rc = tsm_pack(ctx, sp, 1, host_in, tmp))) return rc;
-    const size_t f1 = field_bytes(sp, Vh, 1);
-    for (int par = 0; par < 2; par++)
-        TSM_CUDA(ctx, cudaMemcpyAsync((char*)ctx->slot[slot] + field_bytes(sp, Vh, nrhs) * par + f1 * rhs, tmp + par * f1, f1,
-                                      cudaMemcpyDeviceToDevice, ctx->stream));
+    char* dst = (char*)ctx->slot[slot] + field_bytes(sp, Vh, 1) * rhs;
+    TSM_CUDA(ctx, cudaMemcpyAsync(ctx->staging, host_in, (size_t)ctx->g.V * 24 * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    if ((rc = launch_pack_spinor(ctx, sp, 1, (const double*)ctx->staging, dst, field_bytes(sp, Vh, nrhs)))) return rc;
     TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return TSM_OK;
 }
@@ -331,6 +333,7 @@ int tsm_loops_reset(tsm_ctx* ctx, int ops)
     const size_t lb = (size_t)ctx->n_ops * ctx->g.L[3] * 2 * sizeof(double);
     TSM_CUDA(ctx, cudaMemsetAsync(ctx->acc_corr, 0, lb, ctx->stream));
     TSM_CUDA(ctx, cudaMemsetAsync(ctx->acc_lp, 0, lb, ctx->stream));
+    ctx->loops_ready = true;
     return TSM_OK;
 }
 
@@ -347,6 +350,7 @@ int tsm_loops_set_momenta(tsm_ctx* ctx, int nmom, const int* n)
     if (!ctx) return TSM_EINVAL;
     if (nmom < 0 || nmom > TSM_MAX_MOMENTA || (nmom > 0 && !n)) return tsm_fail(ctx, TSM_EINVAL, "bad momentum list");
     ctx->n_mom = nmom;
+    ctx->loops_ready = false;   // n_ops and the accumulators' shape are fixed by the next tsm_loops_reset
     for (int m = 0; m < nmom; m++)
         for (int k = 0; k < 3; k++) ctx->mom[m][k] = n[3 * m + k];
     return TSM_OK;
@@ -356,6 +360,7 @@ int tsm_loops_add_correction(tsm_ctx* ctx, int slot_hp, int slot_lp)
 {
     int rc = ctx_enter(ctx, true, true, false);
     if (rc) return rc;
+    if ((rc = check_loops(ctx))) return rc;
     if ((rc = check_slot(ctx, slot_hp, 0)) || (rc = check_slot(ctx, slot_lp, 0))) return rc;
     if (slot_hp == slot_lp) return tsm_fail(ctx, TSM_EINVAL, "HP and LP slots must differ");
     const int nrhs = ctx->slot_nrhs[slot_hp];
@@ -374,6 +379,7 @@ int tsm_loops_add_lp(tsm_ctx* ctx, int slot_lp)
 {
     int rc = ctx_enter(ctx, true, true, false);
     if (rc) return rc;
+    if ((rc = check_loops(ctx))) return rc;
     if ((rc = check_slot(ctx, slot_lp, 0))) return rc;
     const int nrhs = ctx->slot_nrhs[slot_lp];
     if ((rc = launch_contract(ctx, slot_lp))) return rc;
@@ -386,6 +392,7 @@ int tsm_loops_source(tsm_ctx* ctx, int slot, int rhs, double* host_out)
 {
     int rc = ctx_enter(ctx, true, true, false);
     if (rc) return rc;
+    if ((rc = check_loops(ctx))) return rc;
     if ((rc = check_slot(ctx, slot, rhs))) return rc;
     if (!host_out) return tsm_fail(ctx, TSM_EINVAL, "null output");
     if ((rc = launch_contract(ctx, slot))) return rc;
@@ -401,6 +408,7 @@ int tsm_loops_finalize(tsm_ctx* ctx, double* host_out)
     int rc = ctx_enter(ctx, true, false, false);
     if (rc) return rc;
     if (!host_out) return tsm_fail(ctx, TSM_EINVAL, "null output");
+    if ((rc = check_loops(ctx))) return rc;
     if ((rc = launch_finalize(ctx))) return rc;
     const size_t lb = (size_t)ctx->n_ops * ctx->g.L[3] * 2 * sizeof(double);
     TSM_CUDA(ctx, cudaMemcpyAsync(ctx->host_small, ctx->loops_out, lb, cudaMemcpyDeviceToHost, ctx->stream));
@@ -414,6 +422,7 @@ int tsm_loops_get_state(tsm_ctx* ctx, double* host_corr, double* host_lp, int* n
     int rc = ctx_enter(ctx, true, false, false);
     if (rc) return rc;
     if (!host_corr || !host_lp || !n_hp || !n_lp) return tsm_fail(ctx, TSM_EINVAL, "null output");
+    if ((rc = check_loops(ctx))) return rc;
     const size_t lb = (size_t)ctx->n_ops * ctx->g.L[3] * 2 * sizeof(double);
     TSM_CUDA(ctx, cudaMemcpyAsync(host_corr, ctx->acc_corr, lb, cudaMemcpyDeviceToHost, ctx->stream));
     TSM_CUDA(ctx, cudaMemcpyAsync(host_lp, ctx->acc_lp, lb, cudaMemcpyDeviceToHost, ctx->stream));
@@ -428,6 +437,7 @@ int tsm_loops_set_state(tsm_ctx* ctx, const double* host_corr, const double* hos
     int rc = ctx_enter(ctx, true, false, false);
     if (rc) return rc;
     if (!host_corr || !host_lp || n_hp < 0 || n_lp < 0) return tsm_fail(ctx, TSM_EINVAL, "bad state");
+    if ((rc = check_loops(ctx))) return rc;
     const size_t lb = (size_t)ctx->n_ops * ctx->g.L[3] * 2 * sizeof(double);
     TSM_CUDA(ctx, cudaMemcpyAsync(ctx->acc_corr, host_corr, lb, cudaMemcpyHostToDevice, ctx->stream));
     TSM_CUDA(ctx, cudaMemcpyAsync(ctx->acc_lp, host_lp, lb, cudaMemcpyHostToDevice, ctx->stream));

@@ -63,7 +63,7 @@ constexpr int TILE = 128;   // sites per tile = blockDim.x
 template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI>
 __global__ void __launch_bounds__(DslashCfg<PREC>::MAXT, 1)
 k_dslash(const Geom g, const int par, const int gy, const int ntiles, const int slab, const void* __restrict__ pack,
-         const void* __restrict__ in_, const void* __restrict__ x_, void* __restrict__ out_, const DslashCoef cf,
+         const void* __restrict__ in_, const void* __restrict__ x_, void* out_, const DslashCoef cf,
          double* __restrict__ partials, const CgScalars* __restrict__ cg, const int check_done)
 {
     using T = typename PT<PREC>::real;
@@ -126,7 +126,7 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const int 
             if (EPI == EPI_RESID) {
                 const T alpha = (T)cg->alpha[rhs];
                 T rv[24];
-                load_spinor<PR>(out, i, rv);
+                load_spinor<PR, false>(out, i, rv);   // r is read and rewritten here: coherent load, not ld.global.nc
 #pragma unroll
                 for (int k = 0; k < 24; k++) rv[k] -= alpha * o[k];
                 nrm += norm2_site(rv);
@@ -239,4 +239,11 @@ int launch_dslash(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs,
         return launch_p<TSM_BF16, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
     }
     return tsm_fail(ctx, TSM_EINVAL, "bad precision");
+}
+
+extern "C" const char* tsm_stencil_kernel_name(const tsm_ctx* ctx, int prec, int nrhs)
+{
+    if (!ctx || prec < 0 || prec > TSM_BF16 || nrhs < 1) return "none";
+    if ((prec == TSM_F32 || prec == TSM_BF16) && tile_stencil_enabled(nrhs)) return "k_dslash_tile";
+    return "k_dslash";
 }

@@ -107,7 +107,7 @@ __device__ __forceinline__ int tile_base(const Geom& g, int tile, int slab)
 template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI, int RY, int R>
 __global__ void __launch_bounds__(TT * RY, 1)
 k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, const int slab, const int nbuf, const void* __restrict__ pack,
-              const void* __restrict__ in_, const void* __restrict__ x_, void* __restrict__ out_, const DslashCoef cf,
+              const void* __restrict__ in_, const void* __restrict__ x_, void* out_, const DslashCoef cf,
               double* __restrict__ partials, const CgScalars* __restrict__ cg, const int check_done)
 {
     constexpr int NCH = RECON == 18 ? 36 : 24;
@@ -202,7 +202,7 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
                     if (EPI == EPI_RESID) {   // out_ is r: r -= alpha q, |r|^2 (q itself is never stored)
                         const float alpha = (float)cg->alpha[rhs0 + r];
                         float rv[24];
-                        load_spinor<PR>((const char*)out_ + fbo * (rhs0 + r), i, rv);
+                        load_spinor<PR, false>((const char*)out_ + fbo * (rhs0 + r), i, rv);   // coherent load: r is rewritten below
 #pragma unroll
                         for (int k = 0; k < 24; k++) rv[k] -= alpha * o[k];
                         nrm[r] += norm2_site(rv);

@@ -11,6 +11,9 @@ __device__ __forceinline__ void atomic_max_nonneg(double* addr, double v)
     atomicMax(reinterpret_cast<unsigned long long*>(addr), (unsigned long long)__double_as_longlong(v));
 }
 
+// max that keeps a NaN operand (fmax drops it: a link full of NaN would report deviation 0)
+__device__ __forceinline__ double max_nan(double a, double b) { return (a != a || b != b) ? __longlong_as_double(0x7ff8000000000000LL) : (a > b ? a : b); }
+
 // |U^dag U - 1|_max and |det U - 1| of one row-major complex 3x3 matrix (18 doubles)
 __device__ double unitarity_dev(const double* u)
 {
@@ -24,7 +27,7 @@ __device__ double unitarity_dev(const double* u)
                 re += ar * br + ai * bi;
                 im += ar * bi - ai * br;
             }
-            dev = fmax(dev, fmax(fabs(re), fabs(im)));
+            dev = max_nan(dev, max_nan(fabs(re), fabs(im)));
         }
     double dr = 0, di = 0;
     for (int c = 0; c < 3; c++) {
@@ -37,7 +40,7 @@ __device__ double unitarity_dev(const double* u)
         dr += u[2 * c] * cr - u[2 * c + 1] * ci;
         di += u[2 * c] * ci + u[2 * c + 1] * cr;
     }
-    return fmax(dev, fmax(fabs(dr - 1.0), fabs(di)));
+    return max_nan(dev, max_nan(fabs(dr - 1.0), fabs(di)));
 }
 
 // raw: [4][V][3][3][2] fp64 in lex order.  One thread per (parity, cb site): writes its 8 links
@@ -67,7 +70,7 @@ __global__ void k_gauge_pack(const Geom g, const int recon, const double* __rest
                     b[2 * (3 * r + c)] = um[2 * (3 * c + r)];
                     b[2 * (3 * r + c) + 1] = -um[2 * (3 * c + r) + 1];
                 }
-            dev = fmax(dev, unitarity_dev(f));
+            dev = max_nan(dev, unitarity_dev(f));
             for (int j = 0; j < 9; j++) {
                 *reinterpret_cast<double2*>(p64 + (18 * mu + j) * LB_ROW) = make_double2(f[2 * j], f[2 * j + 1]);
                 *reinterpret_cast<double2*>(p64 + (18 * mu + 9 + j) * LB_ROW) = make_double2(b[2 * j], b[2 * j + 1]);
@@ -89,7 +92,7 @@ __global__ void k_gauge_pack(const Geom g, const int recon, const double* __rest
 }
 
 template <int PREC>
-__global__ void k_pack_spinor(const Geom g, const int nrhs, const double* __restrict__ lexf, void* native)
+__global__ void k_pack_spinor(const Geom g, const int nrhs, const size_t par_stride, const double* __restrict__ lexf, void* native)
 {
     using T = typename PT<PREC>::real;
     const int Vh = g.Vh;
@@ -103,13 +106,13 @@ __global__ void k_pack_spinor(const Geom g, const int nrhs, const double* __rest
         T v[24];
 #pragma unroll
         for (int k = 0; k < 24; k++) v[k] = (T)src[k];
-        char* dst = (char*)native + field_bytes(PREC, Vh, nrhs) * par + field_bytes(PREC, Vh, 1) * rhs;
+        char* dst = (char*)native + par_stride * par + field_bytes(PREC, Vh, 1) * rhs;
         store_spinor<PREC>(dst, i, v);
     }
 }
 
 template <int PREC>
-__global__ void k_unpack_spinor(const Geom g, const int nrhs, const void* __restrict__ native, double* lexf)
+__global__ void k_unpack_spinor(const Geom g, const int nrhs, const size_t par_stride, const void* __restrict__ native, double* lexf)
 {
     using T = typename PT<PREC>::real;
     const int Vh = g.Vh;
@@ -119,7 +122,7 @@ __global__ void k_unpack_spinor(const Geom g, const int nrhs, const void* __rest
         const int rhs = (int)((tid / Vh) % nrhs);
         const int par = (int)(tid / ((long long)Vh * nrhs));
         const SiteCoord s = decode_site(g, i, par);
-        const char* src = (const char*)native + field_bytes(PREC, Vh, nrhs) * par + field_bytes(PREC, Vh, 1) * rhs;
+        const char* src = (const char*)native + par_stride * par + field_bytes(PREC, Vh, 1) * rhs;
         T v[24];
         load_spinor<PREC>(src, i, v);
         double* dst = lexf + ((size_t)rhs * g.V + lex_of_site(g, s)) * 24;
@@ -222,19 +225,22 @@ int launch_gauge_pack(tsm_ctx* ctx, double* max_dev_out)
         default: return tsm_fail(ctx, TSM_EINVAL, "bad precision");      \
     }
 
-int launch_pack_spinor(tsm_ctx* ctx, int prec, int nrhs, const double* dev_lex, void* dev_native)
+// par_stride: bytes between the parity-0 and the parity-1 part of the native field (0: the dense [parity][rhs] field)
+int launch_pack_spinor(tsm_ctx* ctx, int prec, int nrhs, const double* dev_lex, void* dev_native, size_t par_stride)
 {
     const int gx = grid_for(ctx, 2LL * ctx->g.Vh * nrhs, 256);
-    PREC_SWITCH(prec, (k_pack_spinor<P><<<gx, 256, 0, ctx->stream>>>(ctx->g, nrhs, dev_lex, dev_native)));
+    if (par_stride == 0) par_stride = field_bytes(prec, ctx->g.Vh, nrhs);
+    PREC_SWITCH(prec, (k_pack_spinor<P><<<gx, 256, 0, ctx->stream>>>(ctx->g, nrhs, par_stride, dev_lex, dev_native)));
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;
 }
 
-int launch_unpack_spinor(tsm_ctx* ctx, int prec, int nrhs, const void* dev_native, double* dev_lex)
+int launch_unpack_spinor(tsm_ctx* ctx, int prec, int nrhs, const void* dev_native, double* dev_lex, size_t par_stride)
 {
     const int gx = grid_for(ctx, 2LL * ctx->g.Vh * nrhs, 256);
-    PREC_SWITCH(prec, (k_unpack_spinor<P><<<gx, 256, 0, ctx->stream>>>(ctx->g, nrhs, dev_native, dev_lex)));
+    if (par_stride == 0) par_stride = field_bytes(prec, ctx->g.Vh, nrhs);
+    PREC_SWITCH(prec, (k_unpack_spinor<P><<<gx, 256, 0, ctx->stream>>>(ctx->g, nrhs, par_stride, dev_native, dev_lex)));
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;

@@ -168,18 +168,25 @@ __device__ __forceinline__ uint4 float_to_bf16x8(const float* o)
     return make_uint4(w[0], w[1], w[2], w[3]);
 }
 
-// Load / store 8 consecutive reals (reals 8*k8 .. 8*k8+7 of site i) of a field.
-template <int PREC> __device__ __forceinline__ void load8(const void* f, int i, int k8, typename PT<PREC>::real* o)
+// Load / store 8 consecutive reals (reals 8*k8 .. 8*k8+7 of site i) of a field.  NC: through the read-only
+// path (ld.global.nc), valid only for data no thread writes during the kernel; NC = false is a plain coherent
+// load (the CG residual that the RESID epilogue reads and then overwrites).
+template <bool NC, typename V> __device__ __forceinline__ V ld16(const char* p)
+{
+    if constexpr (NC) return __ldg(reinterpret_cast<const V*>(p));
+    else return *reinterpret_cast<const V*>(p);
+}
+template <int PREC, bool NC = true> __device__ __forceinline__ void load8(const void* f, int i, int k8, typename PT<PREC>::real* o)
 {
     const char* p = site_ptr<PT<PREC>::NCHUNK>(f, i);
     if constexpr (PREC == TSM_F64) {
 #pragma unroll
-        for (int j = 0; j < 4; j++) { const double2 v = __ldg(reinterpret_cast<const double2*>(p + (4 * k8 + j) * LB_ROW)); o[2 * j] = v.x; o[2 * j + 1] = v.y; }
+        for (int j = 0; j < 4; j++) { const double2 v = ld16<NC, double2>(p + (4 * k8 + j) * LB_ROW); o[2 * j] = v.x; o[2 * j + 1] = v.y; }
     } else if constexpr (PREC == TSM_F32) {
 #pragma unroll
-        for (int j = 0; j < 2; j++) { const float4 v = __ldg(reinterpret_cast<const float4*>(p + (2 * k8 + j) * LB_ROW)); o[4 * j] = v.x; o[4 * j + 1] = v.y; o[4 * j + 2] = v.z; o[4 * j + 3] = v.w; }
+        for (int j = 0; j < 2; j++) { const float4 v = ld16<NC, float4>(p + (2 * k8 + j) * LB_ROW); o[4 * j] = v.x; o[4 * j + 1] = v.y; o[4 * j + 2] = v.z; o[4 * j + 3] = v.w; }
     } else {
-        const uint4 v = __ldg(reinterpret_cast<const uint4*>(p + k8 * LB_ROW));
+        const uint4 v = ld16<NC, uint4>(p + k8 * LB_ROW);
         bf16x8_to_float(v, o);
     }
 }
@@ -196,10 +203,10 @@ template <int PREC> __device__ __forceinline__ void store8(void* f, int i, int k
         *reinterpret_cast<uint4*>(p + k8 * LB_ROW) = float_to_bf16x8(o);
     }
 }
-template <int PREC> __device__ __forceinline__ void load_spinor(const void* f, int i, typename PT<PREC>::real* s)
+template <int PREC, bool NC = true> __device__ __forceinline__ void load_spinor(const void* f, int i, typename PT<PREC>::real* s)
 {
 #pragma unroll
-    for (int k = 0; k < 3; k++) load8<PREC>(f, i, k, s + 8 * k);
+    for (int k = 0; k < 3; k++) load8<PREC, NC>(f, i, k, s + 8 * k);
 }
 template <int PREC> __device__ __forceinline__ void store_spinor(void* f, int i, const typename PT<PREC>::real* s)
 {
@@ -430,6 +437,7 @@ struct tsm_ctx {
     uint32_t* ids_dev;               // [2][TSM_MAX_NRHS]
     GammaTable gam;
     int n_ops, with_deriv, with_one_end, with_gen_one_end, with_momenta, n_hp, n_lp;
+    bool loops_ready;                // the Eq. 2.4 accumulators are zeroed / consistent with n_ops (tsm_loops_reset)
     int hp_prec;                     // TSM_F64 or TSM_MIXED (tsm_set_hp_precision)
     int n_mom, mom[TSM_MAX_MOMENTA][3];   // momenta of the projected loops (tsm_loops_set_momenta)
     long long launches;
@@ -479,8 +487,8 @@ int launch_dslash_tile(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int 
                        void* out, const DslashCoef& c, int mode);
 int launch_twist(tsm_ctx* ctx, int prec, int nrhs, const void* in, void* out, const TwistCoef& c);
 int launch_gauge_pack(tsm_ctx* ctx, double* max_dev_out);
-int launch_pack_spinor(tsm_ctx* ctx, int prec, int nrhs, const double* dev_lex, void* dev_native);
-int launch_unpack_spinor(tsm_ctx* ctx, int prec, int nrhs, const void* dev_native, double* dev_lex);
+int launch_pack_spinor(tsm_ctx* ctx, int prec, int nrhs, const double* dev_lex, void* dev_native, size_t par_stride = 0);
+int launch_unpack_spinor(tsm_ctx* ctx, int prec, int nrhs, const void* dev_native, double* dev_lex, size_t par_stride = 0);
 int launch_noise(tsm_ctx* ctx, int prec, int nrhs, uint64_t seed, const uint32_t* dev_ids, int kind, void* dev_full);
 int launch_cg_init(tsm_ctx* ctx, int prec, int nrhs, const void* r, void* p, void* x);
 int launch_cg_reduce(tsm_ctx* ctx, int which, int nrhs, int force = 0);

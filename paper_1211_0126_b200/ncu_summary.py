@@ -1,0 +1,142 @@
+"""Summarise an ncu raw-page CSV as a markdown table, and record the DRAM traffic per launch.
+
+    ncu -i capture.ncu-rep --page raw --csv > capture.csv
+    python -m paper_1211_0126_b200.ncu_summary capture.csv --out profiles/r02_dslash_r12.md \
+        --title "..." --command "ncu --set full ..." \
+        [--traffic profiles/r02_traffic.json --key cfg5_32x32x32x64/f32/nrhs12 --commit <hash>]
+
+The markdown lists, per captured launch, the counters DESIGN.md section 6 argues with (duration, DRAM bytes and
+throughput, L2 sectors and L2 throughput, L1 hit rate, LSU wavefronts, issue slots, stalls, occupancy).  With
+--traffic, the mean over the captured launches of dram__bytes_read.sum + dram__bytes_write.sum is stored under
+--key together with the commit of the kernels; bench.py reports that number as `roofline.traffic`.
+No arithmetic of the method lives here; this is a measurement aid for users of the library.
+"""
+from __future__ import annotations
+
+import argparse
+import csv
+import json
+import os
+
+WANT = [
+    ("Kernel Name", "kernel"), ("gpu__time_duration.sum", "duration"), ("launch__grid_size", "grid"), ("launch__block_size", "block"),
+    ("launch__registers_per_thread", "regs/thread"), ("launch__shared_mem_per_block_dynamic", "dyn smem/block"),
+    ("dram__bytes_read.sum", "DRAM read"), ("dram__bytes_write.sum", "DRAM write"),
+    ("gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed", "DRAM throughput % of peak"),
+    ("lts__t_sectors_srcunit_tex.sum", "L2 sectors from SMs"),
+    ("lts__t_sectors.sum", "L2 sectors, all sources"),
+    ("lts__throughput.avg.pct_of_peak_sustained_elapsed", "L2 (lts) throughput % of peak"),
+    ("lts__t_sectors.avg.pct_of_peak_sustained_elapsed", "L2 sector throughput % of peak"),
+    ("lts__t_sector_hit_rate.pct", "L2 hit rate %"),
+    ("l1tex__t_sector_hit_rate.pct", "L1 hit rate %"),
+    ("l1tex__throughput.avg.pct_of_peak_sustained_active", "L1/TEX throughput % of peak"),
+    ("l1tex__data_pipe_lsu_wavefronts.sum.pct_of_peak_sustained_elapsed", "LSU data-pipe wavefronts % of peak"),
+    ("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum", "shared-memory wavefronts"),
+    ("smsp__inst_executed.sum", "warp instructions"), ("smsp__issue_active.avg.pct_of_peak_sustained_active", "issue slots busy %"),
+    ("sm__warps_active.avg.pct_of_peak_sustained_active", "achieved occupancy %"),
+    ("smsp__warps_eligible.avg.per_cycle_active", "eligible warps per scheduler cycle"),
+    ("sm__inst_executed_pipe_fma.sum.pct_of_peak_sustained_active", "FMA pipe %"),
+    ("sm__inst_executed_pipe_fp64.sum.pct_of_peak_sustained_active", "FP64 pipe %"),
+    ("sm__inst_executed_pipe_tensor.sum.pct_of_peak_sustained_active", "tensor pipe %"),
+    ("smsp__average_warps_issue_stalled_long_scoreboard_per_issue_active.ratio", "stall long_scoreboard (warps/issue)"),
+    ("smsp__average_warps_issue_stalled_barrier_per_issue_active.ratio", "stall barrier"),
+    ("smsp__average_warps_issue_stalled_short_scoreboard_per_issue_active.ratio", "stall short_scoreboard"),
+    ("smsp__average_warps_issue_stalled_lg_throttle_per_issue_active.ratio", "stall lg_throttle"),
+    ("smsp__average_warps_issue_stalled_mio_throttle_per_issue_active.ratio", "stall mio_throttle"),
+    ("smsp__average_warps_issue_stalled_math_pipe_throttle_per_issue_active.ratio", "stall math_pipe_throttle"),
+    ("smsp__average_warps_issue_stalled_wait_per_issue_active.ratio", "stall wait"),
+    ("smsp__average_warps_issue_stalled_not_selected_per_issue_active.ratio", "stall not_selected"),
+    ("sm__cycles_elapsed.avg.per_second", "SM clock"),
+]
+
+
+def read_rows(path):
+    rows = list(csv.reader(open(path)))
+    while rows and (not rows[0] or rows[0][0] != "ID"):      # ncu prints "==PROF==" lines before the table
+        rows.pop(0)
+    if len(rows) < 3:
+        raise SystemExit(f"{path}: no ncu raw table found")
+    return rows[0], rows[1], rows[2:]
+
+
+def to_float(v):
+    try:
+        return float(v.replace(",", ""))
+    except ValueError:
+        return None
+
+
+def table(hdr, units, rows):
+    idx = {h: i for i, h in enumerate(hdr)}
+    n = len(rows)
+    out = ["| metric | " + " | ".join(f"launch {k + 1}" for k in range(n)) + " |", "|---|" + "---|" * n]
+    for key, name in WANT:
+        if key not in idx:
+            continue
+        vals = []
+        for r in rows:
+            v = r[idx[key]]
+            if key == "Kernel Name":
+                v = v.replace("void <unnamed>::", "").split("(")[0]
+            else:
+                f = to_float(v)
+                v = f"{f:.4g}" if f is not None else v
+            vals.append(v)
+        u = units[idx[key]]
+        out.append(f"| {name}{' [' + u + ']' if u else ''} | " + " | ".join(vals) + " |")
+    return "\n".join(out)
+
+
+def dram_bytes(hdr, units, rows):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch, in bytes (ncu prints them in scaled units)."""
+    idx = {h: i for i, h in enumerate(hdr)}
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    tot = []
+    for r in rows:
+        b = 0.0
+        for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            b += to_float(r[idx[key]]) * scale[units[idx[key]]]
+        tot.append(b)
+    return tot
+
+
+def main():
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("csv")
+    ap.add_argument("--out", help="markdown file to write (default: stdout)")
+    ap.add_argument("--title", default="ncu summary")
+    ap.add_argument("--command", default="", help="the full command that made the capture (named in the file)")
+    ap.add_argument("--note", default="")
+    ap.add_argument("--traffic", help="JSON file to update with the mean DRAM bytes per launch")
+    ap.add_argument("--key", help="entry of the JSON file: workload/prec/nrhsN")
+    ap.add_argument("--commit", default="", help="commit of the kernels the capture was taken at")
+    a = ap.parse_args()
+    hdr, units, rows = read_rows(a.csv)
+    per = dram_bytes(hdr, units, rows)
+    text = f"# {a.title}\n\n"
+    if a.command:
+        text += f"Command (B200 box; the same command had just exited 0 without ncu):\n\n    {a.command}\n\n"
+    text += f"read with `ncu -i <report>.ncu-rep --page raw --csv`, summarised by `python -m paper_1211_0126_b200.ncu_summary`.\n\n"
+    text += table(hdr, units, rows) + "\n\n"
+    text += "DRAM bytes per launch (read + write): " + ", ".join(f"{b / 1e9:.3f} GB" for b in per) + f"; mean {sum(per) / len(per) / 1e9:.3f} GB.\n"
+    if a.note:
+        text += "\n" + a.note + "\n"
+    if a.out:
+        with open(a.out, "w") as f:
+            f.write(text)
+    else:
+        print(text)
+    if a.traffic:
+        if not a.key:
+            raise SystemExit("--traffic needs --key")
+        d = json.load(open(a.traffic)) if os.path.exists(a.traffic) else {}
+        idx = {h: i for i, h in enumerate(hdr)}
+        d[a.key] = {"bytes_per_launch": sum(per) / len(per), "per_launch": per, "commit": a.commit,
+                    "summary": a.out or "", "kernels": sorted({r[idx["Kernel Name"]].replace("void <unnamed>::", "").split("(")[0] for r in rows})}
+        with open(a.traffic, "w") as f:
+            json.dump(d, f, indent=1, sort_keys=True)
+            f.write("\n")
+
+
+if __name__ == "__main__":
+    main()

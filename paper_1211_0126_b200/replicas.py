@@ -9,6 +9,10 @@ GPUs, gloo in the CPU tests).  No arithmetic of the method lives here.
 """
 from __future__ import annotations
 
+import os
+
+import numpy as np
+
 REPLICA_STRIDE = 1 << 20   # source ids per rank: rank r owns [r * 2^20, (r + 1) * 2^20)
 
 
@@ -34,3 +38,25 @@ def max_over_ranks(value: float, device=None) -> float:
 def whole_job_throughput(units_per_rank_per_step: int, steps: int, ms_max: float, world: int) -> float:
     """Units all ranks processed / the slowest rank's time (weak scaling: per-rank work is fixed)."""
     return world * units_per_rank_per_step * steps / (ms_max * 1e-3)
+
+
+def node_shared_links(wl, local_rank: int, world: int, barrier=None, shm_dir: str = "/dev/shm") -> np.ndarray:
+    """The workload's gauge configuration, generated ONCE per node: local rank 0 generates it and writes it to a
+    file in shared memory, the other ranks map that file (config 5: 1.2 GB and ~20 s of host work that N ranks
+    would otherwise repeat on the same cores).  `barrier` is the job's barrier (None for a single process).
+    The file is removed again once every rank holds its mapping; the mapping stays valid."""
+    if world == 1 or barrier is None:
+        return wl.links()
+    job = os.environ.get("TORCHELASTIC_RUN_ID") or os.environ.get("MASTER_PORT", "0")
+    path = os.path.join(shm_dir, f"tsm_links_{wl.name}_{wl.gauge_seed}_{job}.npy")
+    if local_rank == 0:
+        tmp = path + ".tmp"
+        with open(tmp, "wb") as f:
+            np.save(f, wl.links())
+        os.replace(tmp, path)
+    barrier()
+    U = np.load(path, mmap_mode="r")
+    barrier()
+    if local_rank == 0:
+        os.unlink(path)
+    return U

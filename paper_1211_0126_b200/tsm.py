@@ -30,7 +30,7 @@ EXPORTS = [
     "tsm_pack", "tsm_unpack", "tsm_dslash", "tsm_solve", "tsm_get_solution", "tsm_set_solution",
     "tsm_loops_reset", "tsm_loops_set_momenta", "tsm_loops_add_correction", "tsm_loops_add_lp", "tsm_loops_source",
     "tsm_loops_finalize", "tsm_loops_get_state", "tsm_loops_set_state", "tsm_run_loop_set",
-    "tsm_set_hp_precision", "tsm_launch_count", "tsm_profile", "tsm_profile_read",
+    "tsm_set_hp_precision", "tsm_launch_count", "tsm_profile", "tsm_profile_read", "tsm_stencil_kernel_name",
 ]
 
 
@@ -90,6 +90,8 @@ def load_library():
     lib.tsm_set_hp_precision.argtypes = [vp, i]
     lib.tsm_launch_count.argtypes = [vp]
     lib.tsm_launch_count.restype = ctypes.c_longlong
+    lib.tsm_stencil_kernel_name.argtypes = [vp, i, i]
+    lib.tsm_stencil_kernel_name.restype = ctypes.c_char_p
     lib.tsm_profile.argtypes = [vp, i]
     lib.tsm_profile_read.argtypes = [vp, i, i, i, dp, ctypes.POINTER(ctypes.c_longlong)]
     _lib = lib
@@ -122,6 +124,7 @@ class Tsm:
         self.device = device
         self.max_nrhs = max_nrhs
         self.n_ops = 16
+        self.hp_precision = MIXED          # the library's default for the HP solves of run_loop_set
         self._h = ctypes.c_void_p()
         rc = self.lib.tsm_create(ctypes.byref(self._h), (ctypes.c_int * 4)(*self.dims), t_boundary, device)
         if rc != OK:
@@ -181,8 +184,16 @@ class Tsm:
         self._check(self.lib.tsm_set_params(self._h, kappa, mu))
 
     def set_hp_precision(self, prec: int):
-        """F64 (default) or MIXED: how tsm_run_loop_set does its HP solves."""
+        """MIXED (default) or F64: how tsm_run_loop_set does its HP solves."""
         self._check(self.lib.tsm_set_hp_precision(self._h, prec))
+        self.hp_precision = prec
+
+    def hp_precision_name(self) -> str:
+        return "mixed" if self.hp_precision == MIXED else "fp64"
+
+    def stencil_kernel_name(self, prec: int, nrhs: int) -> str:
+        """Name of the stencil kernel the library launches for this precision and batch size."""
+        return self.lib.tsm_stencil_kernel_name(self._h, prec, nrhs).decode()
 
     def set_gauge(self, links, reconstruct: int = 18) -> float:
         """links: host complex128 [4][V][3][3], or a pinned torch tensor viewing the same bytes."""

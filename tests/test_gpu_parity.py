@@ -155,6 +155,9 @@ def test_dslash_bf16_storage_parity(ragged, op):
     got = _gpu_op(c, op, BF16, psi)[0]
     want = _oracle_op(c, op, rounded[0])
     assert rel_l2(got, want) < 1e-2
+    # element by element: every stored value is one bf16 rounding (2^-9 relative) of an
+    # fp32 result whose intermediates (the t field of Mhat) were bf16 as well
+    assert rel(got, want) < 1.5e-2
 
 
 @pytest.mark.parametrize("nrhs", [2, 3, 4, 12])
@@ -294,6 +297,7 @@ def test_tsm_loop_set_config1(small):
     """Config 1 in full: fp64 throughout, N_HP=2, N_LP=4, LP at 1e-2 (A11: 6 sources)."""
     c = small
     wl = W.WORKLOADS[1]
+    c.t.set_hp_precision(F64)      # "fp64 throughout"; the library's default HP solver is the mixed-precision one
     per = {}
     want = oracle.tsm_loops(c.dims, c.theta, c.kappa, c.mu, c.U, wl.noise_seed, wl.n_hp, wl.n_lp,
                             wl.hp_tol, 2000, wl.lp_tol, wl.lp_iters, with_derivative=True, per_source=per)
@@ -311,6 +315,11 @@ def test_tsm_loop_set_config1(small):
     corr, lp, n_hp, n_lp = c.t.loops_get_state()
     assert n_hp == 2 and n_lp == 3 and not corr.any()
     assert np.array_equal(got3, lp / 3)
+    # the default HP solver (fp64 defect correction around the fp32 CG) gives the same estimate to the HP tolerance
+    c.t.set_hp_precision(3)
+    got4, _, rc = c.t.run_loop_set(wl.noise_seed, wl.n_hp, wl.n_lp, F64, wl.lp_tol, wl.lp_iters,
+                                   hp_tol=wl.hp_tol, hp_max_iter=2000, nrhs=1, with_derivative=True)
+    assert rc == 0 and rel(got4, want) < 1e-8
 
 
 def test_tsm_manual_accumulation_and_state(small):
@@ -361,6 +370,70 @@ def test_state_and_argument_errors(tsm_mod):
     assert rc == 0
     with pytest.raises(tsm_mod.TsmError):
         tsm_mod.Tsm((4, 4, 5, 4))
+    t.close()
+
+
+def test_single_source_context_solution_round_trip(tsm_mod):
+    """max_nrhs = 1 (the default of Tsm(), and what configs 1-3 use): get_solution / set_solution of an fp64 slot
+    must not touch the other slot or the other parity (the gather buffer used to overlap slot 0)."""
+    wl = W.WORKLOADS[1]
+    U = wl.links()
+    t = tsm_mod.Tsm(wl.dims, t_boundary=-1, max_nrhs=1)
+    t.set_params(wl.kappa, wl.mu)
+    t.set_gauge(U, 18)
+    eta = oracle.noise(wl.dims, wl.noise_seed, 3)
+    s_ref, info_ref = oracle.solve(wl.dims, -1, wl.kappa, wl.mu, U, eta, wl.hp_tol, 2000)
+    rc, info = t.solve(wl.noise_seed, [3], F64, wl.hp_tol, 2000, slot=0)
+    assert rc == 0 and info[0]["iters"] == info_ref["iters"]
+    rc, _ = t.solve(wl.noise_seed, [3], F64, 0.0, 3, slot=1)
+    s1 = t.get_solution(1, 0)
+    s0 = t.get_solution(0, 0)
+    assert rel(s0, s_ref) < 1e-11
+    assert np.array_equal(t.get_solution(0, 0), s0) and np.array_equal(t.get_solution(1, 0), s1)   # reads change nothing
+    assert rel(t.loops_source(0, 0), oracle.loops(wl.dims, eta, s_ref)) < 1e-8                       # slot 0 still whole
+    assert rel(t.loops_source(0, 0), oracle.loops(wl.dims, eta, s0)) < 1e-12
+    t.set_solution(0, 0, s_ref)
+    assert np.array_equal(t.get_solution(0, 0), s_ref)                                                # both parities
+    assert np.array_equal(t.get_solution(1, 0), s1)
+    assert rel(t.loops_source(0, 0), oracle.loops(wl.dims, eta, s_ref)) < 1e-12
+    t.close()
+
+
+def test_non_finite_links_are_refused(tsm_mod):
+    dims = (4, 4, 4, 4)
+    t = tsm_mod.Tsm(dims, max_nrhs=1)
+    for bad_value in (np.nan, np.inf):
+        U = W.unit_links(dims)
+        U[1, 5, 2, 2] = bad_value
+        for recon in (18, 12):
+            with pytest.raises(tsm_mod.TsmError) as e:
+                t.set_gauge(U, recon)
+            assert e.value.code == tsm_mod.EINVAL
+    with pytest.raises(tsm_mod.TsmError) as e:
+        t.set_params(0.1, 0.1)
+        t.solve(1, [0], F64, 1e-6, 10)                   # the refused field is not usable
+    assert e.value.code == tsm_mod.ESTATE
+    t.close()
+
+
+def test_loop_calls_need_a_reset_after_set_momenta(small, tsm_mod):
+    import ctypes
+    t = tsm_mod.Tsm(small.dims, max_nrhs=1)
+    t.set_params(small.kappa, small.mu)
+    t.set_gauge(small.U, 18)
+    t.solve(7, [0], F64, 0.0, 2, slot=1)
+    z = t.loops_finalize()                               # before any reset: the default 16 loops, zeroed sums
+    assert z.shape == (16, small.dims[3]) and not z.any()
+    mom = (ctypes.c_int * 3)(1, 0, 0)
+    assert t.lib.tsm_loops_set_momenta(t._h, 1, mom) == 0
+    out = np.empty((32, small.dims[3]), dtype=np.complex128)
+    dp = out.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+    assert t.lib.tsm_loops_add_lp(t._h, 1) == tsm_mod.ESTATE
+    assert t.lib.tsm_loops_finalize(t._h, dp) == tsm_mod.ESTATE
+    assert t.lib.tsm_loops_source(t._h, 1, 0, dp) == tsm_mod.ESTATE
+    t.loops_reset(momenta=[(1, 0, 0)])
+    t.loops_add_lp(1)
+    assert np.isfinite(t.loops_finalize().view(np.float64)).all()
     t.close()
 
 
@@ -730,6 +803,7 @@ def test_loop_set_is_bit_reproducible(medium):
     c = medium
     wl = W.WORKLOADS[2]
     kw = dict(hp_tol=1e-10, hp_max_iter=2000, with_derivative=True, one_end=True)
+    c.t.set_hp_precision(0)
     a, _, rc = c.t.run_loop_set(wl.noise_seed, 3, 9, F32, wl.lp_tol, 1000, nrhs=4, **kw)
     b, _, _ = c.t.run_loop_set(wl.noise_seed, 3, 9, F32, wl.lp_tol, 1000, nrhs=4, **kw)
     d, _, _ = c.t.run_loop_set(wl.noise_seed, 3, 9, F32, wl.lp_tol, 1000, nrhs=3, **kw)
@@ -737,6 +811,5 @@ def test_loop_set_is_bit_reproducible(medium):
     c.t.set_hp_precision(3)
     e, _, _ = c.t.run_loop_set(wl.noise_seed, 3, 9, F32, wl.lp_tol, 1000, nrhs=4, **kw)
     f, _, _ = c.t.run_loop_set(wl.noise_seed, 3, 9, F32, wl.lp_tol, 1000, nrhs=1, **kw)
-    c.t.set_hp_precision(0)
     assert np.array_equal(e, f) and rel(e, a) < 1e-8
     c.t.loops_reset(False)

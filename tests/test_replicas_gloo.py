@@ -21,7 +21,7 @@ def _free_port():
         return s.getsockname()[1]
 
 
-def _worker(rank, world, port, out):
+def _worker(rank, world, port, out, shm_dir):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
@@ -37,17 +37,24 @@ def _worker(rank, world, port, out):
         assert ms == 100.0 * world
         value = replicas.whole_job_throughput(nrhs, steps, ms, world)
         assert abs(value - world * nrhs * steps / (ms * 1e-3)) < 1e-9
+        # the gauge configuration is generated once per node and mapped by the other ranks
+        from paper_1211_0126_b200 import workloads as W
+        wl = W.WORKLOADS[1]
+        U = replicas.node_shared_links(wl, rank, world, dist.barrier, shm_dir=shm_dir)
+        assert U.shape == (4, wl.V, 3, 3) and bool((U == wl.links()).all())
+        dist.barrier()
+        assert not [f for f in os.listdir(shm_dir) if f.startswith("tsm_links_")]       # removed again
         if rank == 0:
             out.put((flat[:3], ms, value))
     finally:
         dist.destroy_process_group()
 
 
-def test_two_replicas_over_gloo():
+def test_two_replicas_over_gloo(tmp_path):
     ctx = mp.get_context("spawn")
     out = ctx.Queue()
     port = _free_port()
-    procs = [ctx.Process(target=_worker, args=(r, 2, port, out)) for r in range(2)]
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, out, str(tmp_path))) for r in range(2)]
     for p in procs:
         p.start()
     for p in procs:
@@ -69,3 +76,41 @@ def test_reference_arm_runs_on_rank_0_only():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--workload", "1"],
                        capture_output=True, text=True, env=env, timeout=120)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_gpus_n_without_a_launcher_starts_n_ranks_or_fails_loudly():
+    """`python bench.py --gpus 2` with no WORLD_SIZE: the script starts the ranks itself; on a box with fewer than
+    2 GPUs it must refuse (non-zero exit, no JSON line) instead of silently timing one replica."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "1"],
+                       capture_output=True, text=True, env=env, timeout=300)
+    if torch.cuda.is_available() and torch.cuda.device_count() >= 2:
+        assert r.returncode == 0 and '"n_gpus": 2' in r.stdout
+    else:
+        assert r.returncode != 0 and r.stdout.strip() == "" and "refusing" in r.stderr
+
+
+def test_reference_arm_lines(monkeypatch, capsys):
+    """Both forms of the reference arm's step on a small workload: the LP solve run in full, and the 1-/3-iteration
+    sample with the linear extrapolation that config 5 uses; ms_per_step is the time actually spent."""
+    import argparse
+    import json
+    import time
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_1211_0126_b200 import workloads as W
+    args = argparse.Namespace(gpus=1, steps=6, warmup=2, nrhs=0)
+    wl = W.WORKLOADS[2]        # 8^3 x 16: a CG iteration is milliseconds, well above timer noise
+    for forced in (True, False):
+        monkeypatch.setattr(bench, "oracle_runs_in_full", lambda wl, f=forced: f)
+        t0 = time.perf_counter()
+        bench.run_reference(args, wl)
+        wall = time.perf_counter() - t0
+        line = json.loads(capsys.readouterr().out.strip().splitlines()[-1])
+        assert line["impl"] == "reference" and line["extrapolated"] == (not forced)
+        assert line["value"] > 0 and line["cpu_baseline"]["value"] == line["value"] and line["cpu_baseline"]["kind"] == "oracle"
+        assert line["ms_per_step"] * 1e-3 * line["steps"] <= wall                      # fits the wall clock
+        assert line["config"] == bench.workload_config(wl, 1, 1)           # the same object as our arm's
+        if not forced:
+            d = line["cpu_baseline"]["detail"]
+            assert d["t_per_cg_iteration_s"] > 0 and d["s_per_full_step_extrapolated"] > d["t_3iter_solve_s"]
