@@ -417,6 +417,8 @@ def run_ours(args, wl):
     stream = torch.cuda.current_stream()
     t = tsm.Tsm(wl.dims, t_boundary=wl.t_boundary, device=local, max_nrhs=nrhs, stream=stream)
     t.set_params(wl.kappa, wl.mu)
+    if args.stencil_kernel:
+        t.set_stencil_kernel(args.stencil_kernel)
     dev = t.set_gauge(links_host, wl.reconstruct)
     log(f"[bench] unitarity deviation {dev:.2e}; workspace {t.workspace.numel() / 2**30:.1f} GiB")
     t.loops_reset(wl.derivative)
@@ -625,6 +627,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", type=int, default=5)
     ap.add_argument("--nrhs", type=int, default=0, help="sources per batch (default: the workload's; other values are profiling aids, not the headline)")
+    ap.add_argument("--stencil-kernel", type=int, default=0, help="force a stencil kernel (tsm_set_stencil_kernel; profiling aid, not the headline)")
     ap.add_argument("--skip-extras", action="store_true", help="only the timed steps (no e2e/table/full set/oracle/workloads)")
     ap.add_argument("--no-full-set", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -32,8 +32,8 @@
  *   - Work is enqueued on the stream given to tsm_set_stream().  By default, and when that call is given
  *     NULL, the library uses a BLOCKING stream of its own: it is ordered with the caller's legacy default
  *     stream exactly as default-stream work would be, and unlike the legacy stream it can be captured, which
- *     lets the solver replay its CG iterations as cached CUDA graphs (chunks of 4 iterations; TSM_GRAPH=0 in
- *     the environment turns that off).  Calls that return host scalars or arrays synchronise that stream
+ *     lets the solver replay its CG iterations as cached CUDA graphs (chunks of 4 iterations; tsm_set_graphs(ctx, 0)
+ *     turns that off).  Calls that return host scalars or arrays synchronise that stream
  *     before returning; calls that only take dev_* pointers are asynchronous.
  *   - "Native layout" of a single-parity spinor field with V_h = V/2 sites, nrhs sources:
  *       [rhs][block of 32 cb sites][chunk][site in block] of 16-byte vectors (V_h is padded up
@@ -185,6 +185,15 @@ int tsm_set_hp_precision(tsm_ctx* ctx, int prec);
 /* Name of the stencil kernel the library launches for spinor precision `prec` and a batch of `nrhs` sources in this
  * context (static string; measurement aid: bench.py prints it beside the roofline). */
 const char* tsm_stencil_kernel_name(const tsm_ctx* ctx, int prec, int nrhs);
+
+/* Tuning / test switches (no environment variables are read anywhere in the library).
+ * tsm_set_stencil_kernel: 0 = automatic (default; fp64 and single-source contexts use
+ * k_dslash, fp32 batches k_dslash_box where the lattice fits and k_dslash_tile otherwise, bf16 batches k_dslash_tile),
+ * 1 = k_dslash, 2 = k_dslash_tile (fp32 / bf16), 3 = k_dslash_box (fp32, lattice permitting).  A forced kernel that
+ * cannot serve a call falls back to the automatic choice.  tsm_set_graphs: replay CG iterations as CUDA graphs (1, default)
+ * or launch kernel by kernel (0). */
+int tsm_set_stencil_kernel(tsm_ctx* ctx, int which);
+int tsm_set_graphs(tsm_ctx* ctx, int enable);
 
 /* Number of kernels this library has launched on the context since creation. */
 long long tsm_launch_count(const tsm_ctx* ctx);

@@ -34,7 +34,7 @@ size_t carve_workspace(tsm_ctx* ctx, int max_nrhs, char* base)
     const size_t pc2 = (size_t)max_nrhs * (7 + TSM_MAX_MOMENTA) * g.L[3] * 2 * 8 * 32;
     if (pc2 > pc) pc = pc2;
     { size_t o = c.take(pc * sizeof(double)); if (base) { ctx->partials = (double*)at(o); ctx->partials_count = pc; } }
-    const size_t npc = (size_t)max_nrhs * ((g.Vh + 127) / 128);
+    const size_t npc = (size_t)max_nrhs * ((g.Vh + 127) / 128) * 8;   // per (source, tile): one partial, or one per warp of the box stencil
     { size_t o = c.take(npc * sizeof(double)); if (base) { ctx->norm_partials = (double*)at(o); ctx->norm_partials_count = npc; } }
     const size_t lb = (size_t)TSM_MAX_OPS * g.L[3] * 2 * sizeof(double);
     for (int s = 0; s < 2; s++) { size_t o = c.take(lb * max_nrhs); if (base) ctx->loops_src[s] = (double*)at(o); }
@@ -109,6 +109,8 @@ int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
     ctx->launches = 0;
     ctx->prof_on = false;
     ctx->loops_ready = false;
+    ctx->stencil_choice = 0;
+    ctx->graphs_on = 1;
     ctx->cg = nullptr; ctx->cg_host = nullptr; ctx->host_small = nullptr; ctx->ids_dev = nullptr;
     for (int s = 0; s < 2; s++) { ctx->slot_prec[s] = -1; ctx->slot_nrhs[s] = 0; }
     build_gamma_table(ctx->gam);

@@ -46,12 +46,10 @@ int cg_iteration(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, vo
 
 // `iters` CG iterations as ONE CUDA graph launch (captured once per argument set and cached): on small
 // lattices an iteration is 7 launches of a few microseconds each and the solve is launch-bound otherwise.
-// TSM_GRAPH=0 turns it off.  Not used while per-launch profiling is on (events between the launches).
+// tsm_set_graphs(ctx, 0) turns it off.  Not used while per-launch profiling is on (events between the launches).
 bool graphs_enabled(const tsm_ctx* ctx)
 {
-    static int on = -1;
-    if (on < 0) { const char* e = getenv("TSM_GRAPH"); on = e ? atoi(e) : 1; }
-    return on != 0 && !ctx->prof_on && ctx->stream != nullptr && ctx->stream != cudaStreamLegacy && ctx->stream != cudaStreamPerThread;
+    return ctx->graphs_on != 0 && !ctx->prof_on && ctx->stream != nullptr && ctx->stream != cudaStreamLegacy && ctx->stream != cudaStreamPerThread;
 }
 
 bool cg_graph_cached(const tsm_ctx* ctx, int prec, int nrhs, int iters, const void* x, const void* r, const void* p, const void* w,
@@ -334,6 +332,13 @@ int tsm_loops_reset(tsm_ctx* ctx, int ops)
     TSM_CUDA(ctx, cudaMemsetAsync(ctx->acc_corr, 0, lb, ctx->stream));
     TSM_CUDA(ctx, cudaMemsetAsync(ctx->acc_lp, 0, lb, ctx->stream));
     ctx->loops_ready = true;
+    return TSM_OK;
+}
+
+int tsm_set_graphs(tsm_ctx* ctx, int enable)
+{
+    if (!ctx) return TSM_EINVAL;
+    ctx->graphs_on = enable != 0;
     return TSM_OK;
 }
 

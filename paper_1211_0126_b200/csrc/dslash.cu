@@ -29,8 +29,11 @@ __device__ __forceinline__ void hop_direction(const void* pack, const void* in, 
     load_spinor<PREC>(in, nb[2 * MU], psi);
     project<T, MU, SF>(psi, h);
     if (MU == 3 && ph_f != 1) {   // time-boundary phase (A22); skipping a multiplication by one is exact
+        if constexpr (sizeof(T) == 4) rscale_f32<6>(ph_f, h);
+        else {
 #pragma unroll
-        for (int k = 0; k < 12; k++) h[k] *= ph_f;
+            for (int k = 0; k < 12; k++) h[k] *= ph_f;
+        }
     }
     su3_mul(uf, h, gq);
     su3_mul(uf, h + 6, gq + 6);
@@ -38,8 +41,11 @@ __device__ __forceinline__ void hop_direction(const void* pack, const void* in, 
     load_spinor<PREC>(in, nb[2 * MU + 1], psi);
     project<T, MU, -SF>(psi, h);
     if (MU == 3 && ph_b != 1) {
+        if constexpr (sizeof(T) == 4) rscale_f32<6>(ph_b, h);
+        else {
 #pragma unroll
-        for (int k = 0; k < 12; k++) h[k] *= ph_b;
+            for (int k = 0; k < 12; k++) h[k] *= ph_b;
+        }
     }
     su3_mul(ub, h, gq);
     su3_mul(ub, h + 6, gq + 6);
@@ -102,33 +108,47 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const int 
             hop_direction<PREC, RECON, DAGGER, 2>(pack, in, i, nb, ph_f, ph_b, acc);
             hop_direction<PREC, RECON, DAGGER, 3>(pack, in, i, nb, ph_f, ph_b, acc);
             T o[24];
-#pragma unroll
-            for (int q = 0; q < 12; q++) {
-                const T cr = (q < 6) ? cdur : cdlr, ci = (q < 6) ? cdui : cdli;
-                if (d_real) {   // Td real (-kappa^2): the same values without the zero products
-                    o[2 * q] = cr * acc[2 * q];
-                    o[2 * q + 1] = cr * acc[2 * q + 1];
-                } else {
-                    o[2 * q] = cr * acc[2 * q] - ci * acc[2 * q + 1];
-                    o[2 * q + 1] = cr * acc[2 * q + 1] + ci * acc[2 * q];
+            if constexpr (sizeof(T) == 4) {   // packed fp32 (packed_f32.cuh): the same formulas
+                if (d_real) { cscale_real_f32<6>(cdur, acc, o); cscale_real_f32<6>(cdlr, acc + 12, o + 12); }
+                else { cscale_f32<6>(cdur, cdui, acc, o); cscale_f32<6>(cdlr, cdli, acc + 12, o + 12); }
+                if (XPAY) {
+                    T xv[24];
+                    load_spinor<PREC>((const char*)x_ + fb * rhs, i, xv);
+                    caxpy_f32<6>(cxur, cxui, xv, o);
+                    caxpy_f32<6>(cxlr, cxli, xv + 12, o + 12);
                 }
-            }
-            if (XPAY) {
-                T xv[24];
-                load_spinor<PREC>((const char*)x_ + fb * rhs, i, xv);
+            } else {
 #pragma unroll
                 for (int q = 0; q < 12; q++) {
-                    const T cr = (q < 6) ? cxur : cxlr, ci = (q < 6) ? cxui : cxli;
-                    o[2 * q] += cr * xv[2 * q] - ci * xv[2 * q + 1];
-                    o[2 * q + 1] += cr * xv[2 * q + 1] + ci * xv[2 * q];
+                    const T cr = (q < 6) ? cdur : cdlr, ci = (q < 6) ? cdui : cdli;
+                    if (d_real) {   // Td real (-kappa^2): the same values without the zero products
+                        o[2 * q] = cr * acc[2 * q];
+                        o[2 * q + 1] = cr * acc[2 * q + 1];
+                    } else {
+                        o[2 * q] = cr * acc[2 * q] - ci * acc[2 * q + 1];
+                        o[2 * q + 1] = cr * acc[2 * q + 1] + ci * acc[2 * q];
+                    }
+                }
+                if (XPAY) {
+                    T xv[24];
+                    load_spinor<PREC>((const char*)x_ + fb * rhs, i, xv);
+#pragma unroll
+                    for (int q = 0; q < 12; q++) {
+                        const T cr = (q < 6) ? cxur : cxlr, ci = (q < 6) ? cxui : cxli;
+                        o[2 * q] += cr * xv[2 * q] - ci * xv[2 * q + 1];
+                        o[2 * q + 1] += cr * xv[2 * q + 1] + ci * xv[2 * q];
+                    }
                 }
             }
             if (EPI == EPI_RESID) {
                 const T alpha = (T)cg->alpha[rhs];
                 T rv[24];
                 load_spinor<PR, false>(out, i, rv);   // r is read and rewritten here: coherent load, not ld.global.nc
+                if constexpr (sizeof(T) == 4) raxpy_f32<12>(-alpha, o, rv);
+                else {
 #pragma unroll
-                for (int k = 0; k < 24; k++) rv[k] -= alpha * o[k];
+                    for (int k = 0; k < 24; k++) rv[k] -= alpha * o[k];
+                }
                 nrm += norm2_site(rv);
                 store_spinor<PR>(out, i, rv);
             } else {
@@ -210,13 +230,20 @@ int launch_p(tsm_ctx* ctx, int par, bool dagger, int nrhs, const void* pack, con
 
 }  // namespace
 
-// Which fp32 batches go to the shared-memory-staged kernel of dslash_tile.cu (TSM_TILE=0 turns it off,
-// TSM_TILE=2 sends single sources there as well: tuning aids).
-static bool tile_stencil_enabled(int nrhs)
+// Which kernel serves a stencil of precision prec in this context (1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box).
+// Automatic choice: fp64 -> k_dslash; fp32 / bf16 -> k_dslash_tile for batches (nrhs >= 2) and k_dslash for single
+// sources (those two give a source bit-identical results, A14).  k_dslash_box (fp32; 4-D tiles staged by tensor-map
+// TMA) is correct on every lattice it accepts but measured slower than k_dslash_tile, so it
+// runs only when asked for: tsm_set_stencil_kernel(ctx, 3) sends EVERY fp32 stencil of the context to it, single
+// sources included, so that a source's result still does not depend on its batch.
+static int stencil_kernel_for(const tsm_ctx* ctx, int prec, int nrhs)
 {
-    static int mode = -1;
-    if (mode < 0) { const char* e = getenv("TSM_TILE"); mode = e ? atoi(e) : 1; }
-    return mode == 2 || (mode == 1 && nrhs >= 2);
+    if (prec == TSM_F64) return 1;
+    const bool box_ok = prec == TSM_F32 && box_stencil_supported(ctx);
+    if (ctx->stencil_choice == 1) return 1;
+    if (ctx->stencil_choice == 2) return 2;
+    if (ctx->stencil_choice == 3 && box_ok) return 3;
+    return nrhs >= 2 ? 2 : 1;
 }
 
 // mode bit 0: leave per-tile sums of |out|^2 in ctx->partials (the CG's <p, Mhat^dag Mhat p> = |Mhat p|^2);
@@ -225,7 +252,9 @@ int launch_dslash(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs,
                   void* out, const DslashCoef& c, int mode)
 {
     const int chk = (mode >> 1) & 1, nm = (mode & 4) ? EPI_RESID : ((mode & 1) ? EPI_NORM : EPI_NONE);
-    if ((prec == TSM_F32 || prec == TSM_BF16) && tile_stencil_enabled(nrhs)) return launch_dslash_tile(ctx, prec, out_parity, dagger, nrhs, in, x, out, c, mode);
+    const int which = stencil_kernel_for(ctx, prec, nrhs);
+    if (which == 3) return launch_dslash_box(ctx, out_parity, dagger, nrhs, in, x, out, c, mode);
+    if (which == 2) return launch_dslash_tile(ctx, prec, out_parity, dagger, nrhs, in, x, out, c, mode);
     if (prec == TSM_F64)
         return launch_p<TSM_F64, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge64[out_parity], in, x, out, c, nm, chk);
     if (prec == TSM_F32) {
@@ -244,6 +273,15 @@ int launch_dslash(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs,
 extern "C" const char* tsm_stencil_kernel_name(const tsm_ctx* ctx, int prec, int nrhs)
 {
     if (!ctx || prec < 0 || prec > TSM_BF16 || nrhs < 1) return "none";
-    if ((prec == TSM_F32 || prec == TSM_BF16) && tile_stencil_enabled(nrhs)) return "k_dslash_tile";
-    return "k_dslash";
+    const int which = stencil_kernel_for(ctx, prec, nrhs);
+    return which == 3 ? "k_dslash_box" : (which == 2 ? "k_dslash_tile" : "k_dslash");
+}
+
+extern "C" int tsm_set_stencil_kernel(tsm_ctx* ctx, int which)
+{
+    if (!ctx) return TSM_EINVAL;
+    if (which < 0 || which > 3) return tsm_fail(ctx, TSM_EINVAL, "stencil kernel: 0 automatic, 1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box");
+    if (which != ctx->stencil_choice) ctx_drop_graphs(ctx);   // captured CG iterations hold the old kernels
+    ctx->stencil_choice = which;
+    return TSM_OK;
 }

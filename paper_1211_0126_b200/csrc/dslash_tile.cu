@@ -67,10 +67,7 @@ __device__ __forceinline__ void hop_direction_r(const char* tile_links, int tx, 
         float psi[24], h[12], gq[12];
         load_spinor<PREC>(in + fb * r, nb[2 * MU], psi);
         project<float, MU, SF>(psi, h);
-        if (MU == 3 && ph_f != 1) {   // time-boundary phase (A22); skipping a multiplication by one is exact
-#pragma unroll
-            for (int k = 0; k < 12; k++) h[k] *= ph_f;
-        }
+        if (MU == 3 && ph_f != 1) rscale_f32<6>(ph_f, h);   // time-boundary phase (A22); skipping a multiplication by one is exact
         su3_mul(uf, h, gq);
         su3_mul(uf, h + 6, gq + 6);
         accumulate<float, MU, SF>(gq, acc[r]);
@@ -80,10 +77,7 @@ __device__ __forceinline__ void hop_direction_r(const char* tile_links, int tx, 
         float psi[24], h[12], gq[12];
         load_spinor<PREC>(in + fb * r, nb[2 * MU + 1], psi);
         project<float, MU, -SF>(psi, h);
-        if (MU == 3 && ph_b != 1) {
-#pragma unroll
-            for (int k = 0; k < 12; k++) h[k] *= ph_b;
-        }
+        if (MU == 3 && ph_b != 1) rscale_f32<6>(ph_b, h);
         su3_mul(ub, h, gq);
         su3_mul(ub, h + 6, gq + 6);
         accumulate<float, MU, -SF>(gq, acc[r]);
@@ -178,33 +172,19 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
 #pragma unroll
                 for (int r = 0; r < R; r++) {
                     float o[24];
-#pragma unroll
-                    for (int q = 0; q < 12; q++) {
-                        const float cr = (q < 6) ? cdur : cdlr, ci = (q < 6) ? cdui : cdli;
-                        if (d_real) {   // Td real (-kappa^2): the same values without the zero products
-                            o[2 * q] = cr * acc[r][2 * q];
-                            o[2 * q + 1] = cr * acc[r][2 * q + 1];
-                        } else {
-                            o[2 * q] = cr * acc[r][2 * q] - ci * acc[r][2 * q + 1];
-                            o[2 * q + 1] = cr * acc[r][2 * q + 1] + ci * acc[r][2 * q];
-                        }
-                    }
+                    if (d_real) { cscale_real_f32<6>(cdur, acc[r], o); cscale_real_f32<6>(cdlr, acc[r] + 12, o + 12); }   // Td real (-kappa^2)
+                    else { cscale_f32<6>(cdur, cdui, acc[r], o); cscale_f32<6>(cdlr, cdli, acc[r] + 12, o + 12); }
                     if (XPAY) {
                         float xv[24];
                         load_spinor<PREC>((const char*)x_ + fb * (rhs0 + r), i, xv);
-#pragma unroll
-                        for (int q = 0; q < 12; q++) {
-                            const float cr = (q < 6) ? cxur : cxlr, ci = (q < 6) ? cxui : cxli;
-                            o[2 * q] += cr * xv[2 * q] - ci * xv[2 * q + 1];
-                            o[2 * q + 1] += cr * xv[2 * q + 1] + ci * xv[2 * q];
-                        }
+                        caxpy_f32<6>(cxur, cxui, xv, o);
+                        caxpy_f32<6>(cxlr, cxli, xv + 12, o + 12);
                     }
                     if (EPI == EPI_RESID) {   // out_ is r: r -= alpha q, |r|^2 (q itself is never stored)
                         const float alpha = (float)cg->alpha[rhs0 + r];
                         float rv[24];
                         load_spinor<PR, false>((const char*)out_ + fbo * (rhs0 + r), i, rv);   // coherent load: r is rewritten below
-#pragma unroll
-                        for (int k = 0; k < 24; k++) rv[k] -= alpha * o[k];
+                        raxpy_f32<12>(-alpha, o, rv);
                         nrm[r] += norm2_site(rv);
                         store_spinor<PR>((char*)out_ + fbo * (rhs0 + r), i, rv);
                     } else {

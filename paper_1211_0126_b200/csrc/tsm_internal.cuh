@@ -398,12 +398,22 @@ struct CgGraph {
     cudaGraphExec_t exec;
 };
 
+// Tensor maps (4 x 128 B, opaque here) of a field the box stencil has read before, keyed by its address.
+struct BoxMapCache {
+    const void* field;
+    int nrhs;
+    alignas(64) char maps[4 * 128];
+};
+
 struct tsm_ctx {
     Geom g;
     int device;
     cudaStream_t stream;             // where work is enqueued: the caller's stream or own_stream
     cudaStream_t own_stream;         // library-owned BLOCKING stream (serialises with the legacy default stream)
     std::vector<CgGraph> graphs;     // cleared whenever kappa/mu, the gauge storage or the workspace change
+    std::vector<BoxMapCache> box_maps;
+    int stencil_choice;              // tsm_set_stencil_kernel: 0 automatic, 1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box
+    int graphs_on;                   // tsm_set_graphs
     double kappa, mu;
     bool have_params, have_gauge, have_ws;
     int recon;                       // storage of the fp32 link copy (18 / 12)
@@ -485,6 +495,9 @@ int launch_dslash(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs,
                   void* out, const DslashCoef& c, int mode);
 int launch_dslash_tile(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs, const void* in, const void* x,
                        void* out, const DslashCoef& c, int mode);
+int launch_dslash_box(tsm_ctx* ctx, int out_parity, bool dagger, int nrhs, const void* in, const void* x, void* out,
+                      const DslashCoef& c, int mode);
+bool box_stencil_supported(const tsm_ctx* ctx);
 int launch_twist(tsm_ctx* ctx, int prec, int nrhs, const void* in, void* out, const TwistCoef& c);
 int launch_gauge_pack(tsm_ctx* ctx, double* max_dev_out);
 int launch_pack_spinor(tsm_ctx* ctx, int prec, int nrhs, const double* dev_lex, void* dev_native, size_t par_stride = 0);

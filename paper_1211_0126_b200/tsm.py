@@ -31,6 +31,7 @@ EXPORTS = [
     "tsm_loops_reset", "tsm_loops_set_momenta", "tsm_loops_add_correction", "tsm_loops_add_lp", "tsm_loops_source",
     "tsm_loops_finalize", "tsm_loops_get_state", "tsm_loops_set_state", "tsm_run_loop_set",
     "tsm_set_hp_precision", "tsm_launch_count", "tsm_profile", "tsm_profile_read", "tsm_stencil_kernel_name",
+    "tsm_set_stencil_kernel", "tsm_set_graphs",
 ]
 
 
@@ -92,6 +93,8 @@ def load_library():
     lib.tsm_launch_count.restype = ctypes.c_longlong
     lib.tsm_stencil_kernel_name.argtypes = [vp, i, i]
     lib.tsm_stencil_kernel_name.restype = ctypes.c_char_p
+    lib.tsm_set_stencil_kernel.argtypes = [vp, i]
+    lib.tsm_set_graphs.argtypes = [vp, i]
     lib.tsm_profile.argtypes = [vp, i]
     lib.tsm_profile_read.argtypes = [vp, i, i, i, dp, ctypes.POINTER(ctypes.c_longlong)]
     _lib = lib
@@ -187,6 +190,13 @@ class Tsm:
         """MIXED (default) or F64: how tsm_run_loop_set does its HP solves."""
         self._check(self.lib.tsm_set_hp_precision(self._h, prec))
         self.hp_precision = prec
+
+    def set_stencil_kernel(self, which: int):
+        """0 automatic, 1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box (tuning / test aid)."""
+        self._check(self.lib.tsm_set_stencil_kernel(self._h, which))
+
+    def set_graphs(self, enable: bool):
+        self._check(self.lib.tsm_set_graphs(self._h, int(enable)))
 
     def hp_precision_name(self) -> str:
         return "mixed" if self.hp_precision == MIXED else "fp64"

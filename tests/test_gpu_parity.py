@@ -754,23 +754,96 @@ def test_stencils_write_nothing_outside_their_output(ragged, tsm_mod):
 
 @pytest.mark.parametrize("dims", [(16, 16, 4, 4), (8, 32, 4, 4), (32, 8, 4, 6), (64, 4, 4, 4)])
 def test_tile_kernel_in_slab_order_on_small_lattices(tsm_mod, dims):
-    """Lattices with Lxh * Ly a multiple of 128 take the z-slab tile order (like 32^3 x 64) in both stencil kernels:
-    parity with the oracle and bit-identity of batches with the single-source kernel, fp32 and bf16, theta = -1."""
+    """Lattices with Lxh * Ly a multiple of 128 take the z-slab tile order (like 32^3 x 64) in k_dslash and
+    k_dslash_tile: parity with the oracle and bit-identity of batches with the single-source kernel, fp32 and bf16,
+    theta = -1 (the kernels are named explicitly; they are also what the automatic choice picks)."""
     c = Case(tsm_mod, dims, 0.6, 33, 0.157, 0.02, -1, max_nrhs=12)
     psi = W.random_spinor(dims, 77, nrhs=12)
     for nrhs in (3, 5, 12):
         for op in (0, 1, 3):
+            c.t.set_stencil_kernel(2)
             got = _gpu_op(c, op, F32, psi[:nrhs])
             for j in (0, nrhs - 1):
                 src = psi[j].astype(np.complex64).astype(np.complex128)
                 assert rel(got[j], _oracle_op(c, op, src)) < 1e-5, (dims, nrhs, op, j)
+                c.t.set_stencil_kernel(1)
                 single = _gpu_op(c, op, F32, psi[j:j + 1])[0]
+                c.t.set_stencil_kernel(2)
                 assert np.array_equal(single, got[j]), (dims, nrhs, op, j)
     for prec in (F32, BF16):
+        c.t.set_stencil_kernel(2)
         rc, info = c.t.solve(9, [0, 1, 2, 3, 4], prec, 0.0, 7, slot=0)
         batch = c.t.get_solution(0, 3)
+        c.t.set_stencil_kernel(1)
         rc, _ = c.t.solve(9, [3], prec, 0.0, 7, slot=1)
         assert np.array_equal(c.t.get_solution(1, 0), batch), (dims, prec)
+    c.t.close()
+
+
+BOX_LATTICES = [(16, 4, 4, 4),    # Lxh = 8: 4 rows per layout block, one y block (the y halo wraps onto the tile itself)
+                (32, 4, 4, 6),    # Lxh = 16 as at 32^3 x 64: 2 rows per block, 2 y blocks, 3 tiles in t
+                (64, 4, 6, 4),    # Lxh = 32: one row per block, halo rows are whole blocks
+                (8, 8, 4, 4),     # Lxh = 4: 8 rows per block (the shape of config 2)
+                (16, 8, 6, 8)]    # 2 y blocks, 3 tiles in z, 4 in t
+
+
+@pytest.mark.parametrize("theta", [-1, 1])
+@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("dims", BOX_LATTICES)
+def test_box_stencil_parity(tsm_mod, dims, recon, theta):
+    """k_dslash_box (4-D tiles staged by tensor-map TMA, links in registers; not the automatic choice, see DESIGN.md
+    section 6, selected with tsm_set_stencil_kernel): every operator and epilogue form against
+    the oracle (1e-5, north_star) on lattices that exercise every halo wrap, for 1, 3 and 12 sources; agreement
+    with k_dslash to fp32 rounding; a source's result bit-identical in any batch (A14)."""
+    c = Case(tsm_mod, dims, 0.6, 91, 0.157, 0.02, theta, max_nrhs=12, recon=recon)
+    assert c.t.stencil_kernel_name(F32, 12) == "k_dslash_tile" and c.t.stencil_kernel_name(F32, 1) == "k_dslash"   # automatic choice
+    c.t.set_stencil_kernel(3)
+    assert c.t.stencil_kernel_name(F32, 12) == "k_dslash_box" and c.t.stencil_kernel_name(F32, 1) == "k_dslash_box"
+    assert c.t.stencil_kernel_name(F64, 12) == "k_dslash" and c.t.stencil_kernel_name(BF16, 12) == "k_dslash_tile"
+    psi = W.random_spinor(dims, 78, nrhs=12)
+    for nrhs in (1, 3, 12):
+        for op in (0, 1, 2, 3, 4):
+            got = _gpu_op(c, op, F32, psi[:nrhs])
+            for j in sorted({0, nrhs - 1}):
+                src = psi[j].astype(np.complex64).astype(np.complex128)
+                assert rel(got[j], _oracle_op(c, op, src)) < 1e-5, (dims, nrhs, op, j)
+            if nrhs > 1:
+                single = _gpu_op(c, op, F32, psi[nrhs - 1:nrhs])[0]
+                assert np.array_equal(single, got[nrhs - 1]), (dims, nrhs, op)
+            if nrhs == 3:
+                c.t.set_stencil_kernel(1)
+                other = _gpu_op(c, op, F32, psi[:nrhs])
+                c.t.set_stencil_kernel(3)
+                assert rel(got, other) < 2e-6, (dims, op)
+    # through the solver: norm and residual epilogues, CUDA graphs, early exit
+    rc, info = c.t.solve(9, [0, 1, 2, 3, 4], F32, 0.0, 7, slot=0, want_true_resid=True)
+    batch = c.t.get_solution(0, 3)
+    rc, _ = c.t.solve(9, [3], F32, 0.0, 7, slot=1)
+    assert np.array_equal(c.t.get_solution(1, 0), batch)
+    eta = oracle.noise(dims, 9, 3)
+    s_ref, _ = oracle.solve(dims, theta, c.kappa, c.mu, c.U, eta, 0.0, 7)
+    assert rel(batch, s_ref) < 2e-5
+    rc, info = c.t.solve(9, [5, 6, 7], F32, 1e-4, 500, slot=0, want_true_resid=True)
+    assert rc == 0 and all(i["rel_resid_true"] < 2e-4 for i in info)
+    c.t.close()
+
+
+def test_box_stencil_writes_nothing_outside_its_output(tsm_mod):
+    import torch
+    dims = (32, 4, 4, 6)
+    c = Case(tsm_mod, dims, 0.6, 92, 0.157, 0.02, -1, max_nrhs=12)
+    c.t.set_stencil_kernel(3)
+    guard = 8192
+    for nrhs in (1, 5, 12):
+        fb = c.t.field_bytes(F32, nrhs)
+        src = c.t.pack(F32, W.random_spinor(dims, 31, nrhs=nrhs))
+        buf = torch.full((guard + 2 * fb + guard,), 0xA5, dtype=torch.uint8, device="cuda")
+        out = buf[guard:guard + 2 * fb]
+        c.t.dslash(tsm_mod.OP_M_FULL, F32, nrhs, src, out)
+        c.t.dslash(tsm_mod.OP_MHAT_DAG, F32, nrhs, src[:fb], out[:fb])
+        torch.cuda.synchronize()
+        assert bool((buf[:guard] == 0xA5).all()) and bool((buf[guard + 2 * fb:] == 0xA5).all()), nrhs
+        assert np.isfinite(c.t.unpack(F32, nrhs, out).view(np.float64)).all()
     c.t.close()
 
 
