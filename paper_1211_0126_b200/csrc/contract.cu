@@ -19,226 +19,267 @@
 //     a direct phase sum over a handful of momenta (not a full FFT), all momenta in one pass over s
 //     (k_contract_momenta).
 // H10 Eq. 2.4 accumulators (O7).
+#include "dslash_common.cuh"
 #include "reduce.cuh"
 
 namespace {
 
-constexpr int CT_BS = 128;
 constexpr int CT_MAXBLK = 8;   // blocks per (timeslice, parity)
+constexpr int CT_SPB = 8;      // sources (= warps) per block at most
 
-// grid = (nblk * ngroup_in_launch, Lt, nrhs * 2); MODE 0: local; 1: derivative, mu = blockIdx.x / nblk; 2: one-end;
-// 3: generalised one-end (second = D_W s, same [parity][rhs] layout as sol).
-// (the momentum-projected loops have their own kernel, k_contract_momenta)
 // partials: [rhs][group][t][par][blk][32], group 0 local, 1..4 derivative mu, 5 one-end, 6 generalised one-end,
 // 7 + m momentum m
 constexpr int CT_NGROUP = 7 + TSM_MAX_MOMENTA;
 enum { CT_LOCAL = 0, CT_DERIV = 1, CT_ONE_END = 2, CT_GEN_ONE_END = 3 };
 struct Momenta { int n[TSM_MAX_MOMENTA][3]; };
+
+// Transposed butterfly: every lane brings 32 values v[0..31]; lane L returns sum over the warp's lanes of THEIR
+// v[L].  31 shuffles per lane instead of 32 x 5 for 32 separate tree sums, and a fixed tree (A19).  v is destroyed.
+template <typename T> __device__ __forceinline__ T warp_transpose_sum(T* v)
+{
+    const int lane = threadIdx.x & 31;
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) {
+        const bool up = (lane & o) != 0;
+#pragma unroll
+        for (int i = 0; i < o; i++) {
+            const T keep = up ? v[i + o] : v[i];
+            const T send = up ? v[i] : v[i + o];
+            v[i] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+        }
+    }
+    return v[0];
+}
+
+// d[2 (4 al + be) + ri] += conj(l_{al c}) r_{be c} summed over c: the 4 x 4 spin matrix of one site is ADDED to d, in
+// the precision of the field (fp32: packed, two FFMA2 per term; the sums over many sites are taken in fp64 by the caller)
+template <typename T> __device__ __forceinline__ void spin_matrix(const T* l, const T* r, T* d)
+{
+    if constexpr (sizeof(T) == 4) {
+        f2 a[16];
+#pragma unroll
+        for (int k = 0; k < 16; k++) a[k] = pk(d[2 * k], d[2 * k + 1]);
+#pragma unroll
+        for (int al = 0; al < 4; al++)
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+                const float lr = l[2 * (3 * al + c)], li = l[2 * (3 * al + c) + 1];
+#pragma unroll
+                for (int be = 0; be < 4; be++) {
+                    const float rr = r[2 * (3 * be + c)], ri = r[2 * (3 * be + c) + 1];
+                    a[4 * al + be] = fma2(pk(rr, ri), bc(lr), a[4 * al + be]);       // + lr * r
+                    a[4 * al + be] = fma2(c_mi(rr, ri), bc(li), a[4 * al + be]);     // + li * (-i r)
+                }
+            }
+#pragma unroll
+        for (int k = 0; k < 16; k++) upk(a[k], d[2 * k], d[2 * k + 1]);
+    } else {
+#pragma unroll
+        for (int al = 0; al < 4; al++)
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+                const T lr = l[2 * (3 * al + c)], li = l[2 * (3 * al + c) + 1];
+#pragma unroll
+                for (int be = 0; be < 4; be++) {
+                    const T rr = r[2 * (3 * be + c)], ri = r[2 * (3 * be + c) + 1];
+                    d[2 * (4 * al + be)] += lr * rr + li * ri;
+                    d[2 * (4 * al + be) + 1] += lr * ri - li * rr;
+                }
+            }
+    }
+}
+
+// eta_q = i^k (Z4) or 1 - 2 (k & 1) (Z2), k = bits 2q, 2q+1 (O3), straight into IEEE bit patterns: the value is
+// +-1 in the real (k even) or the imaginary (k odd) part, the sign is bit 1 of k (Z4) or bit 0 (Z2)
+template <typename T> __device__ __forceinline__ void noise_spinor(uint32_t bits, int kind, T* eta)
+{
+    const int sign_bit = kind == TSM_Z4 ? 1 : 0;
+    const uint32_t odd_mask = kind == TSM_Z4 ? 1u : 0u;
+#pragma unroll
+    for (int q = 0; q < 12; q++) {
+        const uint32_t k = bits >> (2 * q);
+        const uint32_t one = 0x3f800000u | (((k >> sign_bit) & 1u) << 31);   // +-1.0f
+        const bool odd = (k & odd_mask) != 0;
+        eta[2 * q] = (T)__uint_as_float(odd ? 0u : one);
+        eta[2 * q + 1] = (T)__uint_as_float(odd ? one : 0u);
+    }
+}
+
+// One warp = one source on 32 consecutive cb sites of one (timeslice, parity) at a time; the warps of a block are
+// the sources of the batch on the SAME sites (their link loads meet in L1).  grid = (nblk, 2 Lt, ceil(nrhs /
+// blockDim.y)).  Per site the 4 x 4 spin matrix is formed in the field's precision; a lane adds up the matrices of SPL
+// sites (in that precision: at most 4 x 3 colour terms per entry), the 32 lanes' sums are combined by the transposed
+// butterfly (lane L ends with entry L), and each lane adds its entry to an fp64 accumulator.
+// MODE 0: local; 1: derivative, all four directions in one pass (eta, the site decoding and the neighbour table are
+// made once; one fp64 accumulator per direction); 2: one-end; 3: generalised one-end (second = D_W s, same
+// [parity][rhs] layout as sol).
 template <int PREC, int RECON, int MODE>
-__global__ void __launch_bounds__(CT_BS) k_contract(const Geom g, const int nrhs, const int nblk, const void* __restrict__ sol,
-                                                    const void* __restrict__ second, const void* __restrict__ pack0, const void* __restrict__ pack1,
-                                                    const uint64_t seed, const uint32_t* __restrict__ ids, const int kind,
-                                                    double* __restrict__ partials, const Momenta mom)
+__global__ void __launch_bounds__(32 * CT_SPB, PREC == TSM_F64 ? 1 : 2) k_contract(const Geom g, const int nrhs, const int nblk, const void* __restrict__ sol,
+                                                          const void* __restrict__ second, const void* __restrict__ pack0,
+                                                          const void* __restrict__ pack1, const uint64_t seed, const uint32_t* __restrict__ ids,
+                                                          const int kind, double* __restrict__ partials)
 {
     using T = typename PT<PREC>::real;
+    constexpr int SPL = MODE == CT_DERIV ? 1 : 4;   // sites per lane between two butterflies
+    constexpr int NACC = MODE == CT_DERIV ? 4 : 1;
+    const int lane = threadIdx.x, rhs = blockIdx.z * blockDim.y + threadIdx.y;
+    if (rhs >= nrhs) return;
     const int Vh = g.Vh;
-    const int blk = blockIdx.x % nblk, mu = blockIdx.x / nblk;
-    const int t = blockIdx.y;
-    const int rhs = blockIdx.z >> 1, par = blockIdx.z & 1;
+    const int blk = blockIdx.x;
+    const int t = blockIdx.y >> 1, par = blockIdx.y & 1;
     const size_t fpar = field_bytes(PREC, Vh, nrhs), frhs = field_bytes(PREC, Vh, 1);
     const char* s_same = (const char*)sol + fpar * par + frhs * rhs;
     const char* s_other = (const char*)sol + fpar * (1 - par) + frhs * rhs;
     const void* pack = par ? pack1 : pack0;
     const uint32_t sid = ids[rhs];
-
-    double C[32];
+    const int ngroup = (g.Vsh + 32 * SPL - 1) / (32 * SPL);
+    double acc[NACC];
 #pragma unroll
-    for (int k = 0; k < 32; k++) C[k] = 0;
+    for (int m = 0; m < NACC; m++) acc[m] = 0.0;
 
-    for (int j = blk * CT_BS + threadIdx.x; j < g.Vsh; j += nblk * CT_BS) {
-        const int i = t * g.Vsh + j;
-        const SiteCoord sc = decode_site(g, i, par);
-        uint32_t bits = 0;
-        if (MODE == CT_LOCAL || MODE == CT_DERIV) bits = noise_bits(lex_of_site(g, sc), seed, sid, kind);
-        T v[24], sv[24];
-        if (MODE == CT_GEN_ONE_END) {
-            load_spinor<PREC>(s_same, i, sv);
-            load_spinor<PREC>((const char*)second + fpar * par + frhs * rhs, i, v);
-        } else if (MODE != CT_DERIV) {
-            load_spinor<PREC>(s_same, i, v);
-        } else {
+    if constexpr (MODE == CT_DERIV) {
+        for (int gi = blk; gi < ngroup; gi += nblk) {
+            const int jj = gi * 32 + lane;
+            const bool live = jj < g.Vsh;
+            const int i = t * g.Vsh + (live ? jj : 0);
+            const SiteCoord sc = decode_site(g, i, par);
+            T l[24];
             int nb[8];
+            noise_spinor(noise_bits(lex_of_site(g, sc), seed, sid, kind), kind, l);
             neighbours(g, i, sc, nb);
-            T uf[18], ub[18], sf[24], sb[24], a[6], b[6];
-            // runtime mu: the four directions are four block groups of the same launch
-            switch (mu) {
-                case 0: load_link_pair<PREC, RECON>(pack, i, 0, uf, ub); break;
-                case 1: load_link_pair<PREC, RECON>(pack, i, 1, uf, ub); break;
-                case 2: load_link_pair<PREC, RECON>(pack, i, 2, uf, ub); break;
-                default: load_link_pair<PREC, RECON>(pack, i, 3, uf, ub); break;
-            }
-            load_spinor<PREC>(s_other, nb[2 * mu], sf);
-            load_spinor<PREC>(s_other, nb[2 * mu + 1], sb);
-            const T ph_f = (mu == 3 && sc.t == g.L[3] - 1) ? (T)g.theta : (T)1;
-            const T ph_b = (mu == 3 && sc.t == 0) ? (T)g.theta : (T)1;
 #pragma unroll
-            for (int al = 0; al < 4; al++) {
-                su3_mul(uf, sf + 6 * al, a);
-                su3_mul(ub, sb + 6 * al, b);
+            for (int mu = 0; mu < 4; mu++) {
+                T d[32];
 #pragma unroll
-                for (int k = 0; k < 6; k++) v[6 * al + k] = (T)0.5 * (ph_f * a[k] - ph_b * b[k]);
+                for (int k = 0; k < 32; k++) d[k] = 0;
+                if (live) {
+                    T uf[18], ub[18], sf[24], sb[24], a[6], b[6], r[24];
+                    load_link_pair<PREC, RECON>(pack, i, mu, uf, ub);
+                    load_spinor<PREC>(s_other, nb[2 * mu], sf);
+                    load_spinor<PREC>(s_other, nb[2 * mu + 1], sb);
+                    const T hf = (mu == 3 && sc.t == g.L[3] - 1) ? (T)0.5 * (T)g.theta : (T)0.5;
+                    const T hb = (mu == 3 && sc.t == 0) ? (T)-0.5 * (T)g.theta : (T)-0.5;
+#pragma unroll
+                    for (int al = 0; al < 4; al++) {
+                        su3_mul(uf, sf + 6 * al, a);
+                        su3_mul(ub, sb + 6 * al, b);
+#pragma unroll
+                        for (int k = 0; k < 6; k++) r[6 * al + k] = hf * a[k] + hb * b[k];   // (D_mu s)(x), O6b
+                    }
+                    spin_matrix(l, r, d);
+                }
+                acc[mu] += (double)warp_transpose_sum(d);
             }
         }
+    } else {
+        for (int gi = blk; gi < ngroup; gi += nblk) {
+            T dsum[32];
 #pragma unroll
-        for (int al = 0; al < 4; al++)
+            for (int k = 0; k < 32; k++) dsum[k] = 0;
 #pragma unroll
-            for (int c = 0; c < 3; c++) {
-                double cr, ci;
-                if (MODE == CT_ONE_END) {   // conj(s) in place of conj(eta)
-                    cr = (double)v[2 * (3 * al + c)];
-                    ci = -(double)v[2 * (3 * al + c) + 1];
-                } else if (MODE == CT_GEN_ONE_END) {
-                    cr = (double)sv[2 * (3 * al + c)];
-                    ci = -(double)sv[2 * (3 * al + c) + 1];
-                } else {
-                    float er, ei;
-                    noise_value((bits >> (2 * (3 * al + c))) & 3, kind, er, ei);
-                    cr = er;
-                    ci = -ei;   // conj(eta)
-                }
+            for (int u = 0; u < SPL; u++) {
+                const int jj = (gi * SPL + u) * 32 + lane;
+                if (jj < g.Vsh) {
+                    const int i = t * g.Vsh + jj;
+                    T l[24], r[24];
+                    if (MODE == CT_LOCAL) noise_spinor(noise_bits(lex_of_site(g, decode_site(g, i, par)), seed, sid, kind), kind, l);
+                    if (MODE == CT_GEN_ONE_END) {
+                        load_spinor<PREC>(s_same, i, l);
+                        load_spinor<PREC>((const char*)second + fpar * par + frhs * rhs, i, r);
+                    } else {
+                        load_spinor<PREC>(s_same, i, r);
+                        if (MODE == CT_ONE_END) {
 #pragma unroll
-                for (int be = 0; be < 4; be++) {
-                    const double sr = (double)v[2 * (3 * be + c)], si = (double)v[2 * (3 * be + c) + 1];
-                    C[2 * (4 * al + be)] += cr * sr - ci * si;
-                    C[2 * (4 * al + be) + 1] += cr * si + ci * sr;
+                            for (int k = 0; k < 24; k++) l[k] = r[k];
+                        }
+                    }
+                    spin_matrix(l, r, dsum);
                 }
             }
+            acc[0] += (double)warp_transpose_sum(dsum);
+        }
     }
-    // block reduction of the 32 sums: shuffle tree per warp, fixed serial sum over warps
-    __shared__ double sm[CT_BS / 32][32];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
 #pragma unroll
-    for (int k = 0; k < 32; k++) {
-        const double r = warp_sum(C[k]);
-        if (lane == 0) sm[w][k] = r;
-    }
-    __syncthreads();
-    if (threadIdx.x < 32) {
-        double tot = 0;
-        for (int ww = 0; ww < CT_BS / 32; ww++) tot += sm[ww][threadIdx.x];
-        const int group = MODE == CT_DERIV ? 1 + mu : (MODE == CT_ONE_END ? 5 : (MODE == CT_GEN_ONE_END ? 6 : 0));
+    for (int m = 0; m < NACC; m++) {
+        const int group = MODE == CT_DERIV ? 1 + m : (MODE == CT_ONE_END ? 5 : (MODE == CT_GEN_ONE_END ? 6 : 0));
         const size_t o = ((((size_t)rhs * CT_NGROUP + group) * g.L[3] + t) * 2 + par) * nblk + blk;
-        partials[o * 32 + threadIdx.x] = tot;
+        partials[o * 32 + lane] = acc[m];
     }
 }
 
-// N3 in ONE pass over s for all momenta.  grid = (nblk, Lt, nrhs * 2), 256 threads, dynamic shared memory.
-// Per batch of 256 sites of the timeslice: (A) thread = site: regenerate eta, read s once, leave the site's 16
-// complex d_{ab} = sum_c conj(eta_ac) s_bc in D[site][(ab + site) & 15] (swizzled: conflict-free both ways) and its
-// nmom phases exp(2 pi i n.x/L) in P[m][site]; (B) thread = (entry ab, site lane sl): for its 16 sites of the
-// batch, acc[m] += P[m][site] * D[site][ab] for every m (one D read serves all momenta).  At the end the 16 site
-// lanes of an entry are summed in a fixed order and written where k_contract_finish expects group 7 + m.
-constexpr int CM_BS = 256;
-template <int PREC, int NM>   // NM: compile-time bound on nmom (8 or 16): the accumulators live in registers
-__global__ void __launch_bounds__(CM_BS, NM <= 8 ? 2 : 1) k_contract_momenta(const Geom g, const int nrhs, const int nblk, const int nmom,
-                                                            const void* __restrict__ sol, const uint64_t seed,
-                                                            const uint32_t* __restrict__ ids, const int kind,
-                                                            double* __restrict__ partials, const Momenta mom)
+// N3: the same for the momentum-projected local loops, all momenta in ONE pass over s: the site's spin matrix is
+// multiplied by each momentum's phase exp(2 pi i n.x/L) (product of three tabulated 1-d phases) before the butterfly;
+// lane L keeps entry L of every momentum's sum in fp64.  Dynamic shared memory: the phase tables [nmom][Lx+Ly+Lz].
+template <int PREC, int NM>   // NM: compile-time bound on nmom (8 or 16)
+__global__ void __launch_bounds__(32 * CT_SPB) k_contract_momenta(const Geom g, const int nrhs, const int nblk, const int nmom,
+                                                                  const void* __restrict__ sol, const uint64_t seed,
+                                                                  const uint32_t* __restrict__ ids, const int kind,
+                                                                  double* __restrict__ partials, const Momenta mom)
 {
     using T = typename PT<PREC>::real;
     extern __shared__ __align__(16) double2 cm_smem[];
-    double2* D = cm_smem;                       // [256 sites][16 entries]
-    double2* P = cm_smem + CM_BS * 16;          // [nmom][256 sites]
+    double2* TB = cm_smem;   // [nmom][Lx + Ly + Lz]: exp(2 pi i n_d k / L_d), k = 0..L_d-1
     const int nl = g.L[0] + g.L[1] + g.L[2];
-    double2* TB = P + nmom * CM_BS;             // [nmom][Lx + Ly + Lz]: exp(2 pi i n_d k / L_d), k = 0..L_d-1
-    for (int o = threadIdx.x; o < nmom * nl; o += CM_BS) {
+    for (int o = threadIdx.y * 32 + threadIdx.x; o < nmom * nl; o += 32 * blockDim.y) {
         const int m = o / nl, k = o - m * nl;
-        const int d = k < g.L[0] ? 0 : (k < g.L[0] + g.L[1] ? 1 : 2);
-        const int kk = k - (d == 0 ? 0 : (d == 1 ? g.L[0] : g.L[0] + g.L[1])), L = g.L[d];
-        const int n = ((mom.n[m][d] % L) + L) % L;             // the fraction n k / L reduced in integers first
+        const int dd = k < g.L[0] ? 0 : (k < g.L[0] + g.L[1] ? 1 : 2);
+        const int kk = k - (dd == 0 ? 0 : (dd == 1 ? g.L[0] : g.L[0] + g.L[1])), L = g.L[dd];
+        const int n = ((mom.n[m][dd] % L) + L) % L;             // the fraction n k / L reduced in integers first
         double sn, cs;
         sincospi(2.0 * (double)((n * kk) % L) / (double)L, &sn, &cs);
         TB[o] = make_double2(cs, sn);
     }
     __syncthreads();
-    const int Vh = g.Vh, tid = threadIdx.x;
-    const int blk = blockIdx.x, t = blockIdx.y, rhs = blockIdx.z >> 1, par = blockIdx.z & 1;
+    const int lane = threadIdx.x, rhs = blockIdx.z * blockDim.y + threadIdx.y;
+    if (rhs >= nrhs) return;
+    const int Vh = g.Vh, blk = blockIdx.x, t = blockIdx.y >> 1, par = blockIdx.y & 1;
     const char* s_same = (const char*)sol + field_bytes(PREC, Vh, nrhs) * par + field_bytes(PREC, Vh, 1) * rhs;
     const uint32_t sid = ids[rhs];
-    const int e = tid & 15, sl = tid >> 4;
-    double2 acc[NM];
+    const int nchunk = (g.Vsh + 31) >> 5;
+    double acc[NM];
 #pragma unroll
-    for (int m = 0; m < NM; m++) acc[m] = make_double2(0.0, 0.0);
+    for (int m = 0; m < NM; m++) acc[m] = 0.0;
 
-    for (int base = blk * CM_BS; base < g.Vsh; base += nblk * CM_BS) {
-        {   // (A)
-            const int j = base + tid;
-            double d[32];
+    for (int ch = blk; ch < nchunk; ch += nblk) {
+        const int jj = ch * 32 + lane;
+        const bool live = jj < g.Vsh;
+        const int i = t * g.Vsh + (live ? jj : 0);
+        T d[32];
 #pragma unroll
-            for (int k = 0; k < 32; k++) d[k] = 0.0;
-            if (j < g.Vsh) {
-                const int i = t * g.Vsh + j;
-                const SiteCoord sc = decode_site(g, i, par);
-                const uint32_t bits = noise_bits(lex_of_site(g, sc), seed, sid, kind);
-                T v[24];
-                load_spinor<PREC>(s_same, i, v);
+        for (int k = 0; k < 32; k++) d[k] = 0;
+        SiteCoord sc = decode_site(g, i, par);
+        if (live) {
+            T l[24], r[24];
+            noise_spinor(noise_bits(lex_of_site(g, sc), seed, sid, kind), kind, l);
+            load_spinor<PREC>(s_same, i, r);
+            spin_matrix(l, r, d);
+        }
+        const int x = 2 * sc.xh + sc.rowpar;
 #pragma unroll
-                for (int al = 0; al < 4; al++)
+        for (int m = 0; m < NM; m++) {
+            if (m < nmom) {   // warp-uniform
+                const double2 a = TB[m * nl + x], b = TB[m * nl + g.L[0] + sc.y], c = TB[m * nl + g.L[0] + g.L[1] + sc.z];
+                const double abr = a.x * b.x - a.y * b.y, abi = a.x * b.y + a.y * b.x;
+                const T pr = (T)(abr * c.x - abi * c.y), pi = (T)(abr * c.y + abi * c.x);
+                T wv[32];
+                if constexpr (sizeof(T) == 4) cscale_f32<16>(pr, pi, d, wv);
+                else {
 #pragma unroll
-                    for (int c = 0; c < 3; c++) {
-                        float er, ei;
-                        noise_value((bits >> (2 * (3 * al + c))) & 3, kind, er, ei);
-                        const double cr = er, ci = -ei;   // conj(eta)
-#pragma unroll
-                        for (int be = 0; be < 4; be++) {
-                            const double sr = (double)v[2 * (3 * be + c)], si = (double)v[2 * (3 * be + c) + 1];
-                            d[2 * (4 * al + be)] += cr * sr - ci * si;
-                            d[2 * (4 * al + be) + 1] += cr * si + ci * sr;
-                        }
+                    for (int k = 0; k < 16; k++) {
+                        wv[2 * k] = pr * d[2 * k] - pi * d[2 * k + 1];
+                        wv[2 * k + 1] = pr * d[2 * k + 1] + pi * d[2 * k];
                     }
-                const int x = 2 * sc.xh + sc.rowpar;
-                for (int m = 0; m < nmom; m++) {   // exp(2 pi i n.x/L) as the product of the three tabulated 1-d phases
-                    const double2 a = TB[m * nl + x], b = TB[m * nl + g.L[0] + sc.y], c = TB[m * nl + g.L[0] + g.L[1] + sc.z];
-                    const double abr = a.x * b.x - a.y * b.y, abi = a.x * b.y + a.y * b.x;
-                    P[m * CM_BS + tid] = make_double2(abr * c.x - abi * c.y, abr * c.y + abi * c.x);
                 }
-            } else {
-                for (int m = 0; m < nmom; m++) P[m * CM_BS + tid] = make_double2(0.0, 0.0);
-            }
-#pragma unroll
-            for (int k = 0; k < 16; k++) D[tid * 16 + ((k + tid) & 15)] = make_double2(d[2 * k], d[2 * k + 1]);
-        }
-        __syncthreads();
-        // (B)
-#pragma unroll 4
-        for (int q = 0; q < 16; q++) {
-            const int site = sl + 16 * q;
-            const double2 dv = D[site * 16 + ((e + site) & 15)];
-#pragma unroll
-            for (int m = 0; m < NM; m++) {
-                if (m < nmom) {
-                    const double2 ph = P[m * CM_BS + site];
-                    acc[m].x += ph.x * dv.x - ph.y * dv.y;
-                    acc[m].y += ph.x * dv.y + ph.y * dv.x;
-                }
+                acc[m] += (double)warp_transpose_sum(wv);
             }
         }
-        __syncthreads();
     }
-    // sum over the 16 site lanes of each entry, fixed order (A19); R[m][sl][e] reuses D
-    double2* R = D;
 #pragma unroll
     for (int m = 0; m < NM; m++)
-        if (m < nmom) R[(m * 16 + sl) * 16 + e] = acc[m];
-    __syncthreads();
-    for (int o = tid; o < nmom * 16; o += CM_BS) {
-        const int m = o >> 4, ee = o & 15;
-        double re = 0, im = 0;
-        for (int l = 0; l < 16; l++) { const double2 v = R[(m * 16 + l) * 16 + ee]; re += v.x; im += v.y; }
-        const size_t ob = ((((size_t)rhs * CT_NGROUP + 7 + m) * g.L[3] + t) * 2 + par) * nblk + blk;
-        partials[ob * 32 + 2 * ee] = re;
-        partials[ob * 32 + 2 * ee + 1] = im;
-    }
+        if (m < nmom) {
+            const size_t ob = ((((size_t)rhs * CT_NGROUP + 7 + m) * g.L[3] + t) * 2 + par) * nblk + blk;
+            partials[ob * 32 + lane] = acc[m];
+        }
 }
 
 // grid = (Lt, 6, nrhs), 32 threads: finish the sums and apply the 16 Gamma.  op_base[group] is the first op
@@ -337,16 +378,19 @@ int launch_contract(tsm_ctx* ctx, int slot)
 {
     const Geom& g = ctx->g;
     const int nrhs = ctx->slot_nrhs[slot], prec = ctx->slot_prec[slot];
-    int nblk = (g.Vsh + CT_BS - 1) / CT_BS;
+    int nblk = (g.Vsh + 32 * 32 - 1) / (32 * 32);   // 32 chunks of 32 sites per warp where the timeslice allows
+    if (nblk < 1) nblk = 1;
     if (nblk > CT_MAXBLK) nblk = CT_MAXBLK;
+    const int spb = nrhs < CT_SPB ? nrhs : CT_SPB;        // sources (warps) per block
+    const int gz = (nrhs + spb - 1) / spb;
+    const dim3 cblock(32, spb);
     const size_t need = (size_t)nrhs * CT_NGROUP * g.L[3] * 2 * nblk * 32;
     if (need > ctx->partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
     const uint32_t* ids = ctx->ids_dev + slot * TSM_MAX_NRHS;
     const uint64_t seed = ctx->slot_seed[slot];
     const int kind = ctx->slot_kind[slot];
-    const dim3 grid_l(nblk, g.L[3], nrhs * 2), grid_d(nblk * 4, g.L[3], nrhs * 2);
-    const size_t cm_smem_bytes = (size_t)CM_BS * 16 * sizeof(double2) +
-                                 (size_t)(ctx->n_mom > 0 ? ctx->n_mom : 1) * (CM_BS + g.L[0] + g.L[1] + g.L[2]) * sizeof(double2);
+    const dim3 grid_l(nblk, 2 * g.L[3], gz), grid_d = grid_l;
+    const size_t cm_smem_bytes = (size_t)(ctx->n_mom > 0 ? ctx->n_mom : 1) * (g.L[0] + g.L[1] + g.L[2]) * sizeof(double2);
     if (ctx->with_momenta && ctx->n_mom > 0) {
         TSM_CUDA(ctx, cudaFuncSetAttribute(k_contract_momenta<TSM_F64, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cm_smem_bytes));
         TSM_CUDA(ctx, cudaFuncSetAttribute(k_contract_momenta<TSM_F32, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cm_smem_bytes));
@@ -374,33 +418,33 @@ int launch_contract(tsm_ctx* ctx, int slot)
         const void* p0 = (P == TSM_F64) ? ctx->gauge64[0] : ctx->gauge32[0];                                                 \
         const void* p1 = (P == TSM_F64) ? ctx->gauge64[1] : ctx->gauge32[1];                                                 \
         int pi = prof_begin(ctx, P, 5, nrhs);                                                                                \
-        k_contract<P, R, CT_LOCAL><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials, mom); \
+        k_contract<P, R, CT_LOCAL><<<grid_l, cblock, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials); \
         prof_end(ctx, pi);                                                                                                   \
         ctx->launches++;                                                                                                     \
         if (ctx->with_deriv) {                                                                                               \
             pi = prof_begin(ctx, P, 6, nrhs);                                                                                \
-            k_contract<P, R, CT_DERIV><<<grid_d, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials, mom); \
+            k_contract<P, R, CT_DERIV><<<grid_d, cblock, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials); \
             prof_end(ctx, pi);                                                                                               \
             ctx->launches++;                                                                                                 \
         }                                                                                                                    \
         if (ctx->with_momenta && ctx->n_mom > 0) {                                                                           \
             pi = prof_begin(ctx, P, 9, nrhs);                                                                                \
             if (ctx->n_mom <= 8)                                                                                             \
-                k_contract_momenta<P, 8><<<grid_l, CM_BS, cm_smem_bytes, ctx->stream>>>(g, nrhs, nblk, ctx->n_mom, sol, seed, ids, kind, ctx->partials, mom); \
+                k_contract_momenta<P, 8><<<grid_l, cblock, cm_smem_bytes, ctx->stream>>>(g, nrhs, nblk, ctx->n_mom, sol, seed, ids, kind, ctx->partials, mom); \
             else                                                                                                             \
-                k_contract_momenta<P, 16><<<grid_l, CM_BS, cm_smem_bytes, ctx->stream>>>(g, nrhs, nblk, ctx->n_mom, sol, seed, ids, kind, ctx->partials, mom); \
+                k_contract_momenta<P, 16><<<grid_l, cblock, cm_smem_bytes, ctx->stream>>>(g, nrhs, nblk, ctx->n_mom, sol, seed, ids, kind, ctx->partials, mom); \
             prof_end(ctx, pi);                                                                                               \
             ctx->launches++;                                                                                                 \
         }                                                                                                                    \
         if (ctx->with_gen_one_end) {                                                                                         \
             pi = prof_begin(ctx, P, 8, nrhs);                                                                                \
-            k_contract<P, R, CT_GEN_ONE_END><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials, mom); \
+            k_contract<P, R, CT_GEN_ONE_END><<<grid_l, cblock, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials); \
             prof_end(ctx, pi);                                                                                               \
             ctx->launches++;                                                                                                 \
         }                                                                                                                    \
         if (ctx->with_one_end) {                                                                                             \
             pi = prof_begin(ctx, P, 7, nrhs);                                                                                \
-            k_contract<P, R, CT_ONE_END><<<grid_l, CT_BS, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials, mom); \
+            k_contract<P, R, CT_ONE_END><<<grid_l, cblock, 0, ctx->stream>>>(g, nrhs, nblk, sol, second, p0, p1, seed, ids, kind, ctx->partials); \
             prof_end(ctx, pi);                                                                                               \
             ctx->launches++;                                                                                                 \
         }                                                                                                                    \

@@ -288,7 +288,9 @@ def test_contraction_fp32_slot(ragged):
     (eta, s32), = _oracle_solution_in_fp32_slot(c, 5, [1], 30)
     want = oracle.all_loops(c.dims, c.theta, c.U, eta, s32, True)
     got = c.t.loops_source(1, 0)
-    assert rel(got[:16], want[:16]) < 1e-12          # fp32 values, fp64 sums
+    # fp32 values; per lane the 4 x 4 spin matrices of up to 4 sites and the warp's 32 lanes are added in fp32 (the
+    # transposed butterfly), everything beyond that in fp64: 1e-6 of the largest loop
+    assert rel(got[:16], want[:16]) < 1e-6
     assert rel(got[16:], want[16:]) < 1e-5           # covariant difference in fp32 arithmetic
 
 
@@ -552,7 +554,7 @@ def test_one_end_fp32_slot(ragged):
     c.t.loops_reset(False, one_end=True)
     sols = _oracle_solution_in_fp32_slot(c, 6, [2, 3], 25)
     want = oracle.loops_one_end(c.dims, c.kappa, c.mu, sols[1][1])
-    assert rel(c.t.loops_source(1, 1)[16:], want) < 1e-12
+    assert rel(c.t.loops_source(1, 1)[16:], want) < 1e-6     # fp32 slot: per-warp sums in fp32, then fp64
     c.t.loops_reset(False)
 
 
