@@ -419,6 +419,8 @@ def run_ours(args, wl):
     t.set_params(wl.kappa, wl.mu)
     if args.stencil_kernel:
         t.set_stencil_kernel(args.stencil_kernel)
+    if args.graphs >= 0:
+        t.set_graphs(args.graphs)
     dev = t.set_gauge(links_host, wl.reconstruct)
     log(f"[bench] unitarity deviation {dev:.2e}; workspace {t.workspace.numel() / 2**30:.1f} GiB")
     t.loops_reset(wl.derivative)
@@ -603,6 +605,31 @@ def extras(args, wl, t, tsm, torch, prec, prec_name, peak, U, world):
     return out
 
 
+def run_probe_mma(args):
+    """--probe-mma: the tensor-core clause of north_star measured once (csrc/mma_probe.cu):
+    the per-(site, hop) SU(3) x (3 x 24) product, L2-resident operands, in five formulations.  One JSON line."""
+    import torch
+    from paper_1211_0126_b200 import tsm
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (there is no CPU fallback for the product path)")
+    t = tsm.Tsm((4, 4, 4, 8), max_nrhs=1, stream=torch.cuda.current_stream())
+    nsites, inner, reps = 1 << 16, 64, args.probe_reps
+    names = {0: "fp32 packed FMA (FFMA2), thread per (site, source)", 1: "mma.sync m16n8k8 TF32", 2: "mma.sync m16n8k8 3xTF32 (split operands)",
+             3: "fp64 FMA (DFMA), thread per (site, source)", 4: "mma.sync m8n8k4 fp64 (DMMA)"}
+    out = {}
+    for v in range(5):
+        us, err = t.probe_su3_tensor(v, nsites, inner, reps)
+        flops = nsites * inner * 24 * 3 * 8 * 3      # 3 complex rows x 3 complex MACs (8 real flops) per column
+        out[names[v]] = {"us_per_launch": us, "site_hops_per_us": nsites * inner / us, "useful_gflops": flops / us / 1e3, "max_rel_err": err}
+    # what one batched stencil launch of config 5 needs: V_h x 8 hops products of this shape
+    wl = W.WORKLOADS[5]
+    need = (wl.V // 2) * 8
+    line = {"probe": "su3_x_3x24_per_site_hop", "nsites": nsites, "inner": inner, "reps": reps, "site_hops_per_stencil_launch_cfg5_nrhs12": need,
+            "us_for_one_stencil_launch_worth": {k: need / v["site_hops_per_us"] for k, v in out.items()}, "variants": out}
+    t.close()
+    print(json.dumps(line), flush=True)
+
+
 def spawn_ranks(args) -> int:
     """`python bench.py --gpus N` without a launcher: start the N ranks ourselves (one process per GPU)."""
     if args.impl == "ours":
@@ -628,13 +655,19 @@ def main():
     ap.add_argument("--workload", type=int, default=5)
     ap.add_argument("--nrhs", type=int, default=0, help="sources per batch (default: the workload's; other values are profiling aids, not the headline)")
     ap.add_argument("--stencil-kernel", type=int, default=0, help="force a stencil kernel (tsm_set_stencil_kernel; profiling aid, not the headline)")
+    ap.add_argument("--graphs", type=int, default=-1, help="tsm_set_graphs mode (profiling aid; default: the library's)")
     ap.add_argument("--skip-extras", action="store_true", help="only the timed steps (no e2e/table/full set/oracle/workloads)")
     ap.add_argument("--no-full-set", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-workloads", action="store_true", help="skip the compact block for configs 1-4")
+    ap.add_argument("--probe-mma", action="store_true", help="only the tensor-core probe of csrc/mma_probe.cu (DESIGN.md section 6)")
+    ap.add_argument("--probe-reps", type=int, default=200, help="timed launches per variant of --probe-mma (1 under ncu)")
     args = ap.parse_args()
     if args.gpus < 1:
         ap.error("--gpus must be >= 1")
+    if args.probe_mma:
+        run_probe_mma(args)
+        return
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         sys.exit(spawn_ranks(args))
     wl = W.WORKLOADS[args.workload]

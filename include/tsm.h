@@ -32,8 +32,7 @@
  *   - Work is enqueued on the stream given to tsm_set_stream().  By default, and when that call is given
  *     NULL, the library uses a BLOCKING stream of its own: it is ordered with the caller's legacy default
  *     stream exactly as default-stream work would be, and unlike the legacy stream it can be captured, which
- *     lets the solver replay its CG iterations as cached CUDA graphs (chunks of 4 iterations; tsm_set_graphs(ctx, 0)
- *     turns that off).  Calls that return host scalars or arrays synchronise that stream
+ *     lets the solver run its CG iterations as a cached CUDA graph (tsm_set_graphs).  Calls that return host scalars or arrays synchronise that stream
  *     before returning; calls that only take dev_* pointers are asynchronous.
  *   - "Native layout" of a single-parity spinor field with V_h = V/2 sites, nrhs sources:
  *       [rhs][block of 32 cb sites][chunk][site in block] of 16-byte vectors (V_h is padded up
@@ -89,11 +88,14 @@ const char* tsm_last_error(const tsm_ctx* ctx);
 /* Bytes of one single-parity native field of `nrhs` sources in precision `prec`. */
 size_t tsm_field_bytes(const tsm_ctx* ctx, int prec, int nrhs);
 
-/* Workspace: bytes needed for up to max_nrhs simultaneous sources (all precisions, both
- * link copies, two solution slots, staging for host<->device conversion).  The pointer
- * must be 256-byte aligned device memory that outlives every later call. */
-size_t tsm_workspace_bytes(const tsm_ctx* ctx, int max_nrhs);
-int tsm_set_workspace(tsm_ctx* ctx, void* dev_ptr, size_t bytes, int max_nrhs);
+/* Workspace: bytes needed for up to max_nrhs simultaneous sources in a context whose widest spinor precision is
+ * `prec`: TSM_F64 = everything (fp64 and fp32 link copies, fp64-sized solver vectors and solution
+ * slots, staging for host<->device conversion); TSM_F32 = a low-precision-only workspace for fp32 / bf16-storage
+ * solves (no fp64 link copy, vectors and slots sized for fp32: about half the bytes) -- on it fp64 / mixed solves,
+ * fp64 stencils and the fp64 true residual return TSM_ESTATE.  Any other `prec` is an error (0 bytes / TSM_EINVAL).
+ * The pointer must be 256-byte aligned device memory that outlives every later call. */
+size_t tsm_workspace_bytes(const tsm_ctx* ctx, int max_nrhs, int prec);
+int tsm_set_workspace(tsm_ctx* ctx, void* dev_ptr, size_t bytes, int max_nrhs, int prec);
 int tsm_set_stream(tsm_ctx* ctx, void* cuda_stream);   /* a cudaStream_t; NULL = the library's own stream */
 
 /* kappa, mu of the kappa-normalised twisted-mass operator of O2:
@@ -187,13 +189,28 @@ int tsm_set_hp_precision(tsm_ctx* ctx, int prec);
 const char* tsm_stencil_kernel_name(const tsm_ctx* ctx, int prec, int nrhs);
 
 /* Tuning / test switches (no environment variables are read anywhere in the library).
- * tsm_set_stencil_kernel: 0 = automatic (default; fp64 and single-source contexts use
- * k_dslash, fp32 batches k_dslash_box where the lattice fits and k_dslash_tile otherwise, bf16 batches k_dslash_tile),
- * 1 = k_dslash, 2 = k_dslash_tile (fp32 / bf16), 3 = k_dslash_box (fp32, lattice permitting).  A forced kernel that
- * cannot serve a call falls back to the automatic choice.  tsm_set_graphs: replay CG iterations as CUDA graphs (1, default)
- * or launch kernel by kernel (0). */
+ * tsm_set_stencil_kernel: 0 = automatic (default; on lattices of at most 16 384 sites per
+ * parity every fp64 / fp32 stencil runs in k_dslash_small; otherwise fp64 and single sources use k_dslash and
+ * fp32 / bf16 batches k_dslash_tile), 1 = k_dslash, 2 = k_dslash_tile (fp32 / bf16), 3 = k_dslash_box (fp32, lattice
+ * permitting), 5 = k_dslash_small (fp64 / fp32).  A forced kernel that cannot serve a call falls back to the
+ * automatic choice.  k_dslash and k_dslash_tile give a source bit-identical results; k_dslash_box and k_dslash_small
+ * each differ from them in rounding, so a context should stay with one choice while results are being compared.  tsm_set_graphs: how the CG iterations are launched: 1 (default) = cached CUDA graphs
+ * of 4 iterations, the host reads the all-done flag between them in residual mode; 2 = the whole iteration loop as
+ * ONE graph launch, a WHILE node whose body is one captured iteration and whose condition (a source is still live
+ * and the iteration budget is not used up) is set on the device by the last kernel of the body: no host round trip,
+ * but measured 4.5 us per pass slower than mode 1 on this driver; 0 = kernel by kernel.
+ * All three give bit-identical iterates. */
 int tsm_set_stencil_kernel(tsm_ctx* ctx, int which);
-int tsm_set_graphs(tsm_ctx* ctx, int enable);
+int tsm_set_graphs(tsm_ctx* ctx, int mode);
+
+/* Measurement aid for the tensor-core clause of north_star (csrc/mma_probe.cu): times the only dense
+ * contraction of the stencil -- per site and hop, G = U H with U one SU(3) link and H the 3 x 24 block of 12 sources'
+ * projected half spinors -- on `nsites` (site, hop) pairs held in registers, repeated `inner` times per launch on
+ * H + it * eps with G accumulated (so the arithmetic, not operand traffic, is timed), `reps` launches, in one formulation:
+ * variant 0 packed fp32 FMAs (the stencil's own), 1 mma.sync TF32, 2 mma.sync 3xTF32, 3 fp64 FMAs, 4 fp64 mma.sync.
+ * Outputs (host): microseconds per launch and the largest error relative to the largest fp64 reference value.
+ * Allocates and frees its own small device buffers; blocks until done.  Not part of the hot path. */
+int tsm_probe_su3_tensor(tsm_ctx* ctx, int variant, int nsites, int inner, int reps, double* us_per_launch, double* max_rel_err);
 
 /* Number of kernels this library has launched on the context since creation. */
 long long tsm_launch_count(const tsm_ctx* ctx);

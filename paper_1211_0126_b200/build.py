@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libtsm.so")
-SOURCES = ["dslash.cu", "dslash_tile.cu", "dslash_box.cu", "fields.cu", "blas.cu", "contract.cu", "api_core.cu", "api_solve.cu"]
+SOURCES = ["dslash.cu", "dslash_tile.cu", "dslash_box.cu", "dslash_small.cu", "fields.cu", "blas.cu", "contract.cu", "mma_probe.cu", "api_core.cu", "api_solve.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC"]

@@ -16,18 +16,23 @@ struct Carve {
 };
 
 // One place that defines the workspace layout; used both to size it and to carve it.
-size_t carve_workspace(tsm_ctx* ctx, int max_nrhs, char* base)
+// prec: TSM_F64 = everything (fp64 link packs, fp64-sized vectors and slots); TSM_F32 = a low-precision-only
+// workspace (fp32 / bf16 solves: no fp64 link packs, vectors and slots sized for fp32 fields).
+size_t carve_workspace(tsm_ctx* ctx, int max_nrhs, int prec, char* base)
 {
     const Geom& g = ctx->g;
     Carve c;
     auto at = [&](size_t o) -> void* { return base ? base + o : nullptr; };
-    for (int p = 0; p < 2; p++) { size_t o = c.take(gauge_pack_bytes(1, 18, g.Vh)); if (base) ctx->gauge64[p] = at(o); }
+    const bool wide = prec == TSM_F64;
+    if (base) ctx->gauge64[0] = ctx->gauge64[1] = nullptr;
+    if (wide)
+        for (int p = 0; p < 2; p++) { size_t o = c.take(gauge_pack_bytes(1, 18, g.Vh)); if (base) ctx->gauge64[p] = at(o); }
     for (int p = 0; p < 2; p++) { size_t o = c.take(gauge_pack_bytes(0, 18, g.Vh)); if (base) ctx->gauge32[p] = at(o); }
     size_t stg = (size_t)4 * g.V * 18 * sizeof(double);
     const size_t stg2 = (size_t)max_nrhs * g.V * 24 * sizeof(double);
     if (stg2 > stg) stg = stg2;
     { size_t o = c.take(stg); if (base) { ctx->staging = at(o); ctx->staging_bytes = stg; } }
-    const size_t fb = align256(field_bytes(TSM_F64, g.Vh, max_nrhs));
+    const size_t fb = align256(field_bytes(wide ? TSM_F64 : TSM_F32, g.Vh, max_nrhs));
     { size_t o = c.take(6 * fb); if (base) for (int k = 0; k < 6; k++) ctx->vec[k] = at(o + k * fb); }
     for (int s = 0; s < 2; s++) { size_t o = c.take(2 * fb); if (base) ctx->slot[s] = at(o); }
     size_t pc = (size_t)ctx->nsm * 16 * max_nrhs;
@@ -98,6 +103,8 @@ int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
     ctx->have_params = ctx->have_gauge = ctx->have_ws = false;
     ctx->recon = 18;
     ctx->max_nrhs = 0;
+    ctx->norm_reduced = false;
+    ctx->ws_prec = TSM_F64;
     ctx->n_ops = TSM_N_LOCAL_OPS;
     ctx->with_deriv = 0;
     ctx->with_one_end = 0;
@@ -111,6 +118,7 @@ int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
     ctx->loops_ready = false;
     ctx->stencil_choice = 0;
     ctx->graphs_on = 1;
+    ctx->loop_per_pass = 0;
     ctx->cg = nullptr; ctx->cg_host = nullptr; ctx->host_small = nullptr; ctx->ids_dev = nullptr;
     for (int s = 0; s < 2; s++) { ctx->slot_prec[s] = -1; ctx->slot_nrhs[s] = 0; }
     build_gamma_table(ctx->gam);
@@ -191,22 +199,23 @@ size_t tsm_field_bytes(const tsm_ctx* ctx, int prec, int nrhs)
     return field_bytes(prec, ctx->g.Vh, nrhs);
 }
 
-size_t tsm_workspace_bytes(const tsm_ctx* ctx, int max_nrhs)
+size_t tsm_workspace_bytes(const tsm_ctx* ctx, int max_nrhs, int prec)
 {
-    if (!ctx || max_nrhs < 1 || max_nrhs > TSM_MAX_NRHS) return 0;
-    return carve_workspace(const_cast<tsm_ctx*>(ctx), max_nrhs, nullptr);
+    if (!ctx || max_nrhs < 1 || max_nrhs > TSM_MAX_NRHS || (prec != TSM_F64 && prec != TSM_F32)) return 0;
+    return carve_workspace(const_cast<tsm_ctx*>(ctx), max_nrhs, prec, nullptr);
 }
 
-int tsm_set_workspace(tsm_ctx* ctx, void* dev_ptr, size_t bytes, int max_nrhs)
+int tsm_set_workspace(tsm_ctx* ctx, void* dev_ptr, size_t bytes, int max_nrhs, int prec)
 {
     if (!ctx) return TSM_EINVAL;
-    if (!dev_ptr || max_nrhs < 1 || max_nrhs > TSM_MAX_NRHS) return tsm_fail(ctx, TSM_EINVAL, "bad workspace arguments");
+    if (!dev_ptr || max_nrhs < 1 || max_nrhs > TSM_MAX_NRHS || (prec != TSM_F64 && prec != TSM_F32)) return tsm_fail(ctx, TSM_EINVAL, "bad workspace arguments");
     if (((uintptr_t)dev_ptr & 255) != 0) return tsm_fail(ctx, TSM_EINVAL, "workspace must be 256-byte aligned");
-    if (bytes < carve_workspace(ctx, max_nrhs, nullptr)) return tsm_fail(ctx, TSM_EINVAL, "workspace too small");
+    if (bytes < carve_workspace(ctx, max_nrhs, prec, nullptr)) return tsm_fail(ctx, TSM_EINVAL, "workspace too small");
     ctx->ws = (char*)dev_ptr;
     ctx->ws_bytes = bytes;
     ctx->max_nrhs = max_nrhs;
-    carve_workspace(ctx, max_nrhs, ctx->ws);
+    ctx->ws_prec = prec;
+    carve_workspace(ctx, max_nrhs, prec, ctx->ws);
     ctx->have_ws = true;
     ctx->have_gauge = false;
     ctx_drop_graphs(ctx);
@@ -291,9 +300,10 @@ int tsm_noise(tsm_ctx* ctx, uint64_t seed, uint32_t source_id, int kind, double*
     if (rc) return rc;
     if (!host_out || (kind != TSM_Z4 && kind != TSM_Z2)) return tsm_fail(ctx, TSM_EINVAL, "bad noise arguments");
     TSM_CUDA(ctx, cudaMemcpyAsync(ctx->ids_dev, &source_id, sizeof(uint32_t), cudaMemcpyHostToDevice, ctx->stream));
-    rc = launch_noise(ctx, TSM_F64, 1, seed, ctx->ids_dev, kind, ctx->vec[0]);
+    const int np = ctx->ws_prec;   // the noise values (+-1, +-i) are exact in every precision
+    rc = launch_noise(ctx, np, 1, seed, ctx->ids_dev, kind, ctx->vec[0]);
     if (rc) return rc;
-    return tsm_unpack(ctx, TSM_F64, 1, ctx->vec[0], host_out);
+    return tsm_unpack(ctx, np, 1, ctx->vec[0], host_out);
 }
 
 int tsm_dslash(tsm_ctx* ctx, int op, int prec, int nrhs, const void* dev_in, void* dev_out)
@@ -302,6 +312,7 @@ int tsm_dslash(tsm_ctx* ctx, int op, int prec, int nrhs, const void* dev_in, voi
     if (rc) return rc;
     if (!dev_in || !dev_out || dev_in == dev_out || nrhs < 1 || nrhs > ctx->max_nrhs || prec < 0 || prec > 2)
         return tsm_fail(ctx, TSM_EINVAL, "bad dslash arguments");
+    if (prec == TSM_F64 && ctx->ws_prec != TSM_F64) return tsm_fail(ctx, TSM_ESTATE, "fp64 stencil on a low-precision-only workspace (tsm_set_workspace prec)");
     const double k = ctx->kappa, a = 2.0 * ctx->kappa * ctx->mu, n = 1.0 / (1.0 + a * a);
     const TwistCoef zero = {0, 0, 0, 0}, one = {1, 0, 1, 0};
     const TwistCoef R = {1, a, 1, -a}, Rinv = {n, -a * n, n, a * n}, Rb = {1, -a, 1, a}, Rbinv = {n, a * n, n, -a * n};

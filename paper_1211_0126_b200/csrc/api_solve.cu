@@ -32,7 +32,8 @@ Twists make_twists(const tsm_ctx* ctx)
 // one fused BLAS launch.  Re<p,q> = <p, Mhat^dag Mhat p> is taken as |Mhat p|^2 = |w|^2 from the epilogue of
 // the second stencil launch (same number up to rounding; saves re-reading p and q).  q = Mhat^dag w is never
 // stored: the fourth stencil launch applies r -= alpha q in its epilogue and leaves |r|^2 per tile.
-int cg_iteration(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, void* r, void* p, void* w, void* t, double tol)
+int cg_iteration(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, void* r, void* p, void* w, void* t, double tol,
+                 unsigned long long loop = 0, int in_loop = 0)
 {
     int rc;
     if ((rc = launch_dslash(ctx, prec, 1, false, nrhs, p, nullptr, t, {tw.zero, tw.Rinv}, 2))) return rc;   // t = R^-1 D_oe p
@@ -41,7 +42,7 @@ int cg_iteration(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, vo
     if ((rc = launch_dslash(ctx, prec, 1, true, nrhs, w, nullptr, t, {tw.zero, tw.Rbinv}, 2))) return rc;   // t = Rb^-1 D_oe^dag w
     if ((rc = launch_dslash(ctx, prec, 0, true, nrhs, t, w, r, {tw.Rb, tw.mk2}, 6))) return rc;             // r -= alpha Mhat^dag w; |r|^2 per tile
     if ((rc = launch_cg_reduce(ctx, 1, nrhs))) return rc;                                                   // rr'
-    return launch_cg_update_xp(ctx, prec, nrhs, x, p, r, tol);                                              // x += alpha p; p = r + beta p
+    return launch_cg_update_xp(ctx, prec, nrhs, x, p, r, tol, loop, in_loop);                               // x += alpha p; p = r + beta p
 }
 
 // `iters` CG iterations as ONE CUDA graph launch (captured once per argument set and cached): on small
@@ -66,7 +67,7 @@ int cg_iterations_graph(tsm_ctx* ctx, int prec, int nrhs, int iters, const Twist
     for (const CgGraph& g : ctx->graphs)
         if (g.prec == prec && g.nrhs == nrhs && g.iters == iters && g.x == x && g.r == r && g.p == p && g.w == w && g.t == t && g.tol == tol) {
             TSM_CUDA(ctx, cudaGraphLaunch(g.exec, ctx->stream));
-            ctx->launches += 7LL * iters;
+            ctx->launches += g.launches;
             return TSM_OK;
         }
     const long long l0 = ctx->launches;
@@ -75,17 +76,71 @@ int cg_iterations_graph(tsm_ctx* ctx, int prec, int nrhs, int iters, const Twist
     for (int k = 0; k < iters && rc == TSM_OK; k++) rc = cg_iteration(ctx, prec, nrhs, tw, x, r, p, w, t, tol);
     cudaGraph_t graph = nullptr;
     const cudaError_t e = cudaStreamEndCapture(ctx->stream, &graph);
+    const long long in_graph = ctx->launches - l0;
     ctx->launches = l0;
     if (rc != TSM_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
     TSM_CUDA(ctx, e);
-    CgGraph g{prec, nrhs, iters, x, r, p, w, t, tol, nullptr};
+    CgGraph g{prec, nrhs, iters, x, r, p, w, t, tol, in_graph, nullptr};
     const cudaError_t ei = cudaGraphInstantiate(&g.exec, graph, 0);
     cudaGraphDestroy(graph);
     TSM_CUDA(ctx, ei);
     if (ctx->graphs.size() >= 16) { cudaGraphExecDestroy(ctx->graphs.front().exec); ctx->graphs.erase(ctx->graphs.begin()); }
     ctx->graphs.push_back(g);
     TSM_CUDA(ctx, cudaGraphLaunch(g.exec, ctx->stream));
-    ctx->launches += 7LL * iters;
+    ctx->launches += in_graph;
+    return TSM_OK;
+}
+
+// The whole iteration loop as ONE graph launch: a WHILE node whose body is one captured CG iteration; the last
+// block of k_cg_update_xp decides on the device whether another pass follows (sources left, cg->loop_left > 0).
+// Residual mode then needs no host polling, and a solve on a small lattice is a handful of launches.
+int cg_loop_graph(tsm_ctx* ctx, int prec, int nrhs, int n_iter, int eager, const Twists& tw, void* x, void* r, void* p, void* w, void* t,
+                  double tol)
+{
+    int rc;
+    if ((rc = launch_cg_loop_begin(ctx, n_iter))) return rc;
+    ctx->loop_eager = eager;
+    ctx->loop_nrhs = nrhs;
+    for (const CgGraph& g : ctx->graphs)
+        if (g.prec == prec && g.nrhs == nrhs && g.iters == 0 && g.x == x && g.r == r && g.p == p && g.w == w && g.t == t && g.tol == tol) {
+            TSM_CUDA(ctx, cudaGraphLaunch(g.exec, ctx->stream));
+            // one pass of the loop is counted here; the other passes (their number is known to the device only) are
+            // added by fetch_scalars from the iteration counts
+            ctx->launches += g.launches;
+            ctx->loop_per_pass = g.launches;
+            return TSM_OK;
+        }
+    cudaGraph_t graph = nullptr;
+    TSM_CUDA(ctx, cudaGraphCreate(&graph, 0));
+    cudaGraphConditionalHandle handle;
+    cudaError_t e = cudaGraphConditionalHandleCreate(&handle, graph, 1, cudaGraphCondAssignDefault);
+    cudaGraphNodeParams np = {};
+    np.type = cudaGraphNodeTypeConditional;
+    np.conditional.handle = handle;
+    np.conditional.type = cudaGraphCondTypeWhile;
+    np.conditional.size = 1;
+    cudaGraphNode_t node;
+    if (e == cudaSuccess) e = cudaGraphAddNode(&node, graph, nullptr, 0, &np);
+    if (e != cudaSuccess) { cudaGraphDestroy(graph); TSM_CUDA(ctx, e); }
+    cudaGraph_t body = np.conditional.phGraph_out[0];
+    const long long l0 = ctx->launches;
+    e = cudaStreamBeginCaptureToGraph(ctx->stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+    if (e != cudaSuccess) { cudaGraphDestroy(graph); TSM_CUDA(ctx, e); }
+    rc = cg_iteration(ctx, prec, nrhs, tw, x, r, p, w, t, tol, (unsigned long long)handle, 1);
+    e = cudaStreamEndCapture(ctx->stream, nullptr);
+    const long long in_graph = ctx->launches - l0;
+    ctx->launches = l0;
+    if (rc != TSM_OK) { cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) { cudaGraphDestroy(graph); TSM_CUDA(ctx, e); }
+    CgGraph g{prec, nrhs, 0, x, r, p, w, t, tol, in_graph, nullptr};
+    e = cudaGraphInstantiate(&g.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    TSM_CUDA(ctx, e);
+    if (ctx->graphs.size() >= 16) { cudaGraphExecDestroy(ctx->graphs.front().exec); ctx->graphs.erase(ctx->graphs.begin()); }
+    ctx->graphs.push_back(g);
+    TSM_CUDA(ctx, cudaGraphLaunch(g.exec, ctx->stream));
+    ctx->launches += in_graph;
+    ctx->loop_per_pass = in_graph;
     return TSM_OK;
 }
 
@@ -93,6 +148,13 @@ int fetch_scalars(tsm_ctx* ctx)
 {
     TSM_CUDA(ctx, cudaMemcpyAsync(ctx->cg_host, ctx->cg, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx->stream));
     TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (ctx->loop_per_pass > 0) {   // settle the launch count of the device-side loop that has just finished
+        int most = 0;
+        for (int j = 0; j < ctx->loop_nrhs; j++) most = ctx->cg_host->iters[j] > most ? ctx->cg_host->iters[j] : most;
+        const int passes = most - ctx->loop_eager;
+        if (passes > 1) ctx->launches += (long long)(passes - 1) * ctx->loop_per_pass;
+        ctx->loop_per_pass = 0;
+    }
     return TSM_OK;
 }
 
@@ -106,6 +168,17 @@ int cg_run(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, void* r,
     int rc;
     const int poll = 4;
     const bool use_graph = graphs_enabled(ctx);
+    if (use_graph && ctx->graphs_on == 2) {
+        // device-side loop: the first iteration of an argument set runs kernel by kernel (kernel attributes
+        // cannot be set inside a capture), everything after it is one graph launch
+        int k = 0;
+        if (!cg_graph_cached(ctx, prec, nrhs, 0, x, r, p, w, t, tol) && max_iter > 0) {
+            if ((rc = cg_iteration(ctx, prec, nrhs, tw, x, r, p, w, t, tol))) return rc;
+            k = 1;
+        }
+        if (k < max_iter) return cg_loop_graph(ctx, prec, nrhs, max_iter - k, k, tw, x, r, p, w, t, tol);
+        return TSM_OK;
+    }
     const bool cached = use_graph && cg_graph_cached(ctx, prec, nrhs, poll, x, r, p, w, t, tol);
     for (int k = 0; k < max_iter;) {
         const int chunk = max_iter - k < poll ? max_iter - k : poll;
@@ -225,6 +298,8 @@ int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs,
     if (!source_ids || nrhs < 1 || nrhs > ctx->max_nrhs || (kind != TSM_Z4 && kind != TSM_Z2) || prec < 0 || prec > TSM_MIXED ||
         !(tol >= 0) || max_iter < 0 || slot < 0 || slot > 1 || (prec == TSM_MIXED && !(tol > 0)))
         return tsm_fail(ctx, TSM_EINVAL, "bad solve arguments");
+    if (ctx->ws_prec != TSM_F64 && (prec == TSM_F64 || prec == TSM_MIXED || want_true_resid))
+        return tsm_fail(ctx, TSM_ESTATE, "fp64 solve or fp64 true residual on a low-precision-only workspace (tsm_set_workspace prec)");
     // bf16 storage (config 4): source preparation, x, r, q, reconstruction and the stored solution are
     // fp32; only the search direction p and the stencil temporaries t, w are bf16 (fp32 arithmetic).
     const int sp = prec == TSM_BF16 ? TSM_F32 : (prec == TSM_MIXED ? TSM_F64 : prec);   // precision of the stored solution
@@ -335,10 +410,11 @@ int tsm_loops_reset(tsm_ctx* ctx, int ops)
     return TSM_OK;
 }
 
-int tsm_set_graphs(tsm_ctx* ctx, int enable)
+int tsm_set_graphs(tsm_ctx* ctx, int mode)
 {
     if (!ctx) return TSM_EINVAL;
-    ctx->graphs_on = enable != 0;
+    if (mode < 0 || mode > 2) return tsm_fail(ctx, TSM_EINVAL, "graphs: 0 off, 1 chunks of 4 iterations, 2 device-side loop");
+    ctx->graphs_on = mode;
     return TSM_OK;
 }
 

@@ -77,20 +77,7 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_reduce(const int which, const in
     double v = 0;
     for (int k = threadIdx.x; k < ntiles; k += BLAS_BS) v += __ldcg(norm_partials + (size_t)rhs * ntiles + k);
     v = block_sum_all(v, smem);
-    if (threadIdx.x != 0) return;
-    if (which == 1) { cg->rr_new[rhs] = v; return; }
-    cg->pq[rhs] = v;
-    double alpha = 0.0;
-    if (!cg->done[rhs]) {
-        const double rr = cg->rr[rhs];
-        if (!(v > 0) || !isfinite(v) || !(rr > 0) || !isfinite(rr)) {
-            cg->done[rhs] = 1;
-            cg->status[rhs] = TSM_EBREAKDOWN;
-        } else {
-            alpha = rr / v;
-        }
-    }
-    cg->alpha[rhs] = alpha;
+    if (threadIdx.x == 0) cg_after_reduction(which, rhs, v, cg);
 }
 
 // x += alpha p; p = r + beta p with beta = rr_new / rr (one pass: reads x, p, r; writes x, p).  r was already
@@ -98,11 +85,15 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_reduce(const int which, const in
 // bookkeeping of O5: iteration count, rr <- rr_new, the stopping test |r|/|b'| <= tol (A8), freeze flags.
 template <int PV, int PP>
 __global__ void __launch_bounds__(BLAS_BS) k_cg_update_xp(const int Vh, const int nrhs, void* __restrict__ x_, void* __restrict__ p_,
-                                                          const void* __restrict__ r_, const double tol, CgScalars* cg)
+                                                          const void* __restrict__ r_, const double tol, CgScalars* cg,
+                                                          const cudaGraphConditionalHandle loop, const int in_loop)
 {
     using TV = typename PT<PV>::real;
     using TP = typename PT<PP>::real;
-    if (cg->all_done) return;
+    if (cg->all_done) {   // every source frozen: leave the device-side iteration loop, if this launch is inside one
+        if (in_loop && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) cudaGraphSetConditional(loop, 0u);
+        return;
+    }
     const int rhs = blockIdx.y;
     if (!cg->done[rhs]) {
         const TV alpha = (TV)cg->alpha[rhs];
@@ -142,9 +133,17 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_update_xp(const int Vh, const in
                 all &= cg->done[j];
             }
             cg->all_done = all;
+            // inside the WHILE node of a CUDA graph (api_solve.cu: cg_run): one more iteration?
+            if (in_loop) {
+                const int left = cg->loop_left - 1;
+                cg->loop_left = left;
+                cudaGraphSetConditional(loop, (!all && left > 0) ? 1u : 0u);
+            }
         }
     }
 }
+
+__global__ void k_cg_loop_begin(CgScalars* cg, const int n) { cg->loop_left = n; }
 
 inline dim3 blas_grid(const tsm_ctx* ctx, int nrhs)
 {
@@ -179,17 +178,30 @@ int launch_cg_init(tsm_ctx* ctx, int prec, int nrhs, const void* r, void* p, voi
 
 int launch_cg_reduce(tsm_ctx* ctx, int which, int nrhs, int force)
 {
+    if (ctx->norm_reduced) {   // k_dslash_small's last block has already summed its partials and done this step
+        ctx->norm_reduced = false;
+        return TSM_OK;
+    }
     k_cg_reduce<<<nrhs, BLAS_BS, 0, ctx->stream>>>(which, force, ctx->norm_partials, ctx->norm_ntiles, ctx->cg);
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;
 }
 
-int launch_cg_update_xp(tsm_ctx* ctx, int prec, int nrhs, void* x, void* p, const void* r, double tol)
+int launch_cg_loop_begin(tsm_ctx* ctx, int n)
+{
+    k_cg_loop_begin<<<1, 1, 0, ctx->stream>>>(ctx->cg, n);
+    ctx->launches++;
+    TSM_CUDA(ctx, cudaGetLastError());
+    return TSM_OK;
+}
+
+int launch_cg_update_xp(tsm_ctx* ctx, int prec, int nrhs, void* x, void* p, const void* r, double tol, unsigned long long loop, int in_loop)
 {
     const dim3 grid = blas_grid(ctx, nrhs);
     const int pi = prof_begin(ctx, prec, 4, nrhs);
-    BLAS_SWITCH(prec, (k_cg_update_xp<PV, PP><<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, nrhs, x, p, r, tol, ctx->cg)));
+    BLAS_SWITCH(prec, (k_cg_update_xp<PV, PP><<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, nrhs, x, p, r, tol, ctx->cg,
+                                                                                (cudaGraphConditionalHandle)loop, in_loop)));
     prof_end(ctx, pi);
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());

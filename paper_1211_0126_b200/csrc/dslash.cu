@@ -14,6 +14,7 @@
 #include <cstdlib>
 
 #include "dslash_common.cuh"
+#include "reduce.cuh"
 
 namespace {
 
@@ -70,7 +71,7 @@ template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI>
 __global__ void __launch_bounds__(DslashCfg<PREC>::MAXT, 1)
 k_dslash(const Geom g, const int par, const int gy, const int ntiles, const int slab, const void* __restrict__ pack,
          const void* __restrict__ in_, const void* __restrict__ x_, void* out_, const DslashCoef cf,
-         double* __restrict__ partials, const CgScalars* __restrict__ cg, const int check_done)
+         double* __restrict__ partials, CgScalars* __restrict__ cg, const int check_done, const int fuse_reduce)
 {
     using T = typename PT<PREC>::real;
     if (check_done && cg->all_done) return;
@@ -170,6 +171,18 @@ k_dslash(const Geom g, const int par, const int gy, const int ntiles, const int 
             if (threadIdx.x == 0) partials[(size_t)rhs * ntiles + tile] = tot;
         }
     }
+    // Lattices of at most FUSE_NTILES tiles: the last block of the grid to finish sums every source's partials (one
+    // warp per source, an order that depends on ntiles only) and does what k_cg_reduce would -- there a separate
+    // reduction launch costs half as much as the stencil itself.
+    if (EPI != EPI_NONE && fuse_reduce) {
+        if (last_block_arrive(&cg->ticket)) {
+            const int wid = (threadIdx.y * blockDim.x + threadIdx.x) >> 5, nw = (blockDim.x * blockDim.y) >> 5;
+            for (int j = wid; j < gy * (int)blockDim.y; j += nw) {
+                const double v = sum_partials_warp(partials, j, ntiles);
+                if ((threadIdx.x & 31) == 0) cg_after_reduction(EPI == EPI_RESID ? 1 : 0, j, v, cg);
+            }
+        }
+    }
 }
 
 // resident blocks per SM of each instantiation, queried once
@@ -203,11 +216,13 @@ int launch_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void* in, 
     if (grid > (long long)ntiles * gy) grid = (long long)ntiles * gy;
     if (EPI != EPI_NONE && (size_t)ntiles * nrhs > ctx->norm_partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
     const int pi = prof_begin(ctx, PREC, EPI == EPI_RESID ? 3 : (EPI == EPI_NORM ? 2 : (XPAY ? 1 : 0)), nrhs);
+    const int fuse = (EPI != EPI_NONE && ntiles <= FUSE_NTILES) ? 1 : 0;
     k_dslash<PREC, RECON, DAGGER, XPAY, EPI><<<(unsigned)grid, block, 0, ctx->stream>>>(ctx->g, par, gy, ntiles, (ctx->g.S % TILE == 0) ? 1 : 0, pack, in, x, out, c,
-                                                                                         ctx->norm_partials, ctx->cg, check_done);
+                                                                                         ctx->norm_partials, ctx->cg, check_done, fuse);
     prof_end(ctx, pi);
     ctx->launches++;
     ctx->norm_ntiles = ntiles;
+    ctx->norm_reduced = fuse != 0;
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;
 }
@@ -230,14 +245,19 @@ int launch_p(tsm_ctx* ctx, int par, bool dagger, int nrhs, const void* pack, con
 
 }  // namespace
 
-// Which kernel serves a stencil of precision prec in this context (1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box).
-// Automatic choice: fp64 -> k_dslash; fp32 / bf16 -> k_dslash_tile for batches (nrhs >= 2) and k_dslash for single
-// sources (those two give a source bit-identical results, A14).  k_dslash_box (fp32; 4-D tiles staged by tensor-map
+// Which kernel serves a stencil of precision prec in this context (1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box,
+// 5 k_dslash_small).  Automatic choice: on the smallest lattices (V_h <= SMALL_VH: configs 1, 2) every fp64 / fp32
+// stencil, single sources and batches alike, goes to k_dslash_small (directions spread over warps: a latency, not a
+// bandwidth, problem there); otherwise fp64 -> k_dslash; fp32 / bf16 -> k_dslash_tile for batches (nrhs >= 2) and
+// k_dslash for single sources (those two give a source bit-identical results, A14).  k_dslash_box (fp32; 4-D tiles staged by tensor-map
 // TMA) is correct on every lattice it accepts but measured slower than k_dslash_tile, so it
 // runs only when asked for: tsm_set_stencil_kernel(ctx, 3) sends EVERY fp32 stencil of the context to it, single
 // sources included, so that a source's result still does not depend on its batch.
+constexpr int SMALL_VH = 16384;   // measured: +19 % LP solves/s at 4^3 x 8, +9 % at 8^3 x 16, -15 % at 16^3 x 32 (V_h = 65 536)
 static int stencil_kernel_for(const tsm_ctx* ctx, int prec, int nrhs)
 {
+    if (ctx->stencil_choice == 0 && prec != TSM_BF16 && ctx->g.Vh <= SMALL_VH) return 5;
+    if (ctx->stencil_choice == 5 && prec != TSM_BF16) return 5;
     if (prec == TSM_F64) return 1;
     const bool box_ok = prec == TSM_F32 && box_stencil_supported(ctx);
     if (ctx->stencil_choice == 1) return 1;
@@ -253,6 +273,7 @@ int launch_dslash(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs,
 {
     const int chk = (mode >> 1) & 1, nm = (mode & 4) ? EPI_RESID : ((mode & 1) ? EPI_NORM : EPI_NONE);
     const int which = stencil_kernel_for(ctx, prec, nrhs);
+    if (which == 5) return launch_dslash_small(ctx, prec, out_parity, dagger, nrhs, in, x, out, c, mode);
     if (which == 3) return launch_dslash_box(ctx, out_parity, dagger, nrhs, in, x, out, c, mode);
     if (which == 2) return launch_dslash_tile(ctx, prec, out_parity, dagger, nrhs, in, x, out, c, mode);
     if (prec == TSM_F64)
@@ -274,13 +295,14 @@ extern "C" const char* tsm_stencil_kernel_name(const tsm_ctx* ctx, int prec, int
 {
     if (!ctx || prec < 0 || prec > TSM_BF16 || nrhs < 1) return "none";
     const int which = stencil_kernel_for(ctx, prec, nrhs);
-    return which == 3 ? "k_dslash_box" : (which == 2 ? "k_dslash_tile" : "k_dslash");
+    return which == 5 ? "k_dslash_small" : (which == 3 ? "k_dslash_box" : (which == 2 ? "k_dslash_tile" : "k_dslash"));
 }
 
 extern "C" int tsm_set_stencil_kernel(tsm_ctx* ctx, int which)
 {
     if (!ctx) return TSM_EINVAL;
-    if (which < 0 || which > 3) return tsm_fail(ctx, TSM_EINVAL, "stencil kernel: 0 automatic, 1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box");
+    if (which < 0 || which > 5 || which == 4)
+        return tsm_fail(ctx, TSM_EINVAL, "stencil kernel: 0 automatic, 1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box, 5 k_dslash_small");
     if (which != ctx->stencil_choice) ctx_drop_graphs(ctx);   // captured CG iterations hold the old kernels
     ctx->stencil_choice = which;
     return TSM_OK;

@@ -561,6 +561,7 @@ int launch_dslash_box(tsm_ctx* ctx, int out_parity, bool dagger, int nrhs, const
     a.partials = ctx->norm_partials;
     a.cg = ctx->cg;
     ctx->norm_ntiles = bg.ntiles * 8;
+    ctx->norm_reduced = false;
     if (ctx->recon == 18) return launch_box_v<18>(ctx, bg, maps, a, dagger, x != nullptr, epi);
     return launch_box_v<12>(ctx, bg, maps, a, dagger, x != nullptr, epi);
 }

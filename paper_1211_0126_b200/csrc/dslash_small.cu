@@ -1,0 +1,222 @@
+// dslash_small.cu -- H5 for lattices that fit in L2 (hard part 4: configs 1-3): the stencil
+// with the four directions of a site spread over four warps.
+//
+// On a 16^3 x 32 lattice a stencil launch has 65 536 output sites and takes ~10 us in k_dslash, on 4^3 x 8 (256
+// sites) still ~6 us: not bandwidth (the fields sit in L2) but the CHAIN of eight dependent hop latencies per thread,
+// with too few threads on the chip to hide it.  Here a CTA is 32 sites x 4 directions: warp mu loads the link pair
+// and the two neighbour spinors of direction mu for its 32 sites (all loads independent: one memory latency instead
+// of eight in sequence, four times as many threads in flight), forms the two hops, and leaves its 24 partial sums in
+// shared memory; after one barrier warp a (= spin component a) adds the four directions' partials of its spin in a
+// fixed order, applies the twist / x term / residual-update epilogue to those 3 complex numbers and stores them.
+//
+// The sum over directions is associated as (d0 + d1) + (d2 + d3), not sequentially as in k_dslash: a source's result
+// differs from the other kernels' in rounding, so the library sends EVERY fp64 / fp32 stencil of a small-lattice
+// context here (single sources and batches alike: grid = (blocks of 32 sites, sources)), and a source's result is
+// still independent of its batch (A14).  Norm partials: one per (source, 32-site block), fixed trees (A19).
+#include "dslash_common.cuh"
+#include "reduce.cuh"
+
+namespace {
+
+// reals 6a .. 6a+5 (spin component a: three complex numbers) of site i
+template <int PREC, bool NC> __device__ __forceinline__ void load_spin(const void* f, int i, int a, typename PT<PREC>::real* v)
+{
+    if constexpr (PREC == TSM_F64) {
+        const char* p = site_ptr<12>(f, i) + (3 * a) * LB_ROW;
+#pragma unroll
+        for (int c = 0; c < 3; c++) { const double2 w = ld16<NC, double2>(p + c * LB_ROW); v[2 * c] = w.x; v[2 * c + 1] = w.y; }
+    } else {
+        const char* p = site_ptr<6>(f, i);
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            const int r = 6 * a + 2 * c;   // even: an 8-byte piece of chunk r / 4
+            const char* q = p + (r >> 2) * LB_ROW + (r & 3) * 4;
+            float2 w;
+            if constexpr (NC) w = __ldg(reinterpret_cast<const float2*>(q));
+            else w = *reinterpret_cast<const float2*>(q);
+            v[2 * c] = w.x; v[2 * c + 1] = w.y;
+        }
+    }
+}
+template <int PREC> __device__ __forceinline__ void store_spin(void* f, int i, int a, const typename PT<PREC>::real* v)
+{
+    if constexpr (PREC == TSM_F64) {
+        char* p = site_ptr<12>(f, i) + (3 * a) * LB_ROW;
+#pragma unroll
+        for (int c = 0; c < 3; c++) *reinterpret_cast<double2*>(p + c * LB_ROW) = make_double2(v[2 * c], v[2 * c + 1]);
+    } else {
+        char* p = site_ptr<6>(f, i);
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            const int r = 6 * a + 2 * c;
+            *reinterpret_cast<float2*>(p + (r >> 2) * LB_ROW + (r & 3) * 4) = make_float2(v[2 * c], v[2 * c + 1]);
+        }
+    }
+}
+
+// both hops of direction MU of site i into part[24] (zero on entry)
+template <int PREC, int RECON, bool DAGGER, int MU>
+__device__ __forceinline__ void two_hops(const void* pack, const char* in, int i, int nf, int nbk, typename PT<PREC>::real ph_f,
+                                         typename PT<PREC>::real ph_b, typename PT<PREC>::real* part)
+{
+    using T = typename PT<PREC>::real;
+    constexpr int SF = DAGGER ? +1 : -1;   // forward hop carries (1 - g_mu), dagger swaps
+    T uf[18], ub[18], pf[24], pb[24], h[12], gq[12];
+    load_link_pair<PREC, RECON>(pack, i, MU, uf, ub);
+    load_spinor<PREC>(in, nf, pf);
+    load_spinor<PREC>(in, nbk, pb);
+    project<T, MU, SF>(pf, h);
+    if (MU == 3 && ph_f != 1) {   // time-boundary phase (A22)
+#pragma unroll
+        for (int k = 0; k < 12; k++) h[k] *= ph_f;
+    }
+    su3_mul(uf, h, gq);
+    su3_mul(uf, h + 6, gq + 6);
+    accumulate<T, MU, SF>(gq, part);
+    project<T, MU, -SF>(pb, h);
+    if (MU == 3 && ph_b != 1) {
+#pragma unroll
+        for (int k = 0; k < 12; k++) h[k] *= ph_b;
+    }
+    su3_mul(ub, h, gq);
+    su3_mul(ub, h + 6, gq + 6);
+    accumulate<T, MU, -SF>(gq, part);
+}
+
+template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI>
+__global__ void __launch_bounds__(128) k_dslash_small(const Geom g, const int par, const void* __restrict__ pack, const void* __restrict__ in_,
+                                                      const void* __restrict__ x_, void* out_, const DslashCoef cf,
+                                                      double* __restrict__ partials, CgScalars* __restrict__ cg, const int check_done)
+{
+    using T = typename PT<PREC>::real;
+    __shared__ T sm[4][24][32];
+    __shared__ double red[4];
+    if (check_done && cg->all_done) return;
+    const int Vh = g.Vh;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;   // w: direction in the first half, spin component in the second
+    const int rhs = blockIdx.y, i = blockIdx.x * LB + lane;
+    const bool live = i < Vh;
+    const size_t fb = field_bytes(PREC, Vh, 1);
+    {
+        T part[24];
+#pragma unroll
+        for (int k = 0; k < 24; k++) part[k] = 0;
+        if (live) {
+            const SiteCoord s = decode_site(g, i, par);
+            int nb[8];
+            neighbours(g, i, s, nb);
+            const T ph_f = (s.t == g.L[3] - 1) ? (T)g.theta : (T)1, ph_b = (s.t == 0) ? (T)g.theta : (T)1;
+            const char* in = (const char*)in_ + fb * rhs;
+            switch (w) {   // warp-uniform
+                case 0: two_hops<PREC, RECON, DAGGER, 0>(pack, in, i, nb[0], nb[1], ph_f, ph_b, part); break;
+                case 1: two_hops<PREC, RECON, DAGGER, 1>(pack, in, i, nb[2], nb[3], ph_f, ph_b, part); break;
+                case 2: two_hops<PREC, RECON, DAGGER, 2>(pack, in, i, nb[4], nb[5], ph_f, ph_b, part); break;
+                default: two_hops<PREC, RECON, DAGGER, 3>(pack, in, i, nb[6], nb[7], ph_f, ph_b, part); break;
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 24; k++) sm[w][k][lane] = part[k];
+    }
+    __syncthreads();
+    // second half: warp w finishes spin component w of the 32 sites
+    const int a = w;
+    double nrm = 0.0;
+    if (live) {
+        T v[6], o[6];
+#pragma unroll
+        for (int c = 0; c < 6; c++) v[c] = (sm[0][6 * a + c][lane] + sm[1][6 * a + c][lane]) + (sm[2][6 * a + c][lane] + sm[3][6 * a + c][lane]);
+        const T cdr = (T)(a < 2 ? cf.d.up_re : cf.d.lo_re), cdi = (T)(a < 2 ? cf.d.up_im : cf.d.lo_im);
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            o[2 * c] = cdr * v[2 * c] - cdi * v[2 * c + 1];
+            o[2 * c + 1] = cdr * v[2 * c + 1] + cdi * v[2 * c];
+        }
+        if (XPAY) {
+            const T cxr = (T)(a < 2 ? cf.x.up_re : cf.x.lo_re), cxi = (T)(a < 2 ? cf.x.up_im : cf.x.lo_im);
+            T xv[6];
+            load_spin<PREC, true>((const char*)x_ + fb * rhs, i, a, xv);
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+                o[2 * c] += cxr * xv[2 * c] - cxi * xv[2 * c + 1];
+                o[2 * c + 1] += cxr * xv[2 * c + 1] + cxi * xv[2 * c];
+            }
+        }
+        if (EPI == EPI_RESID) {   // out_ is the CG residual r (same precision as the spinors here): r -= alpha q
+            const T alpha = (T)cg->alpha[rhs];
+            T rv[6];
+            load_spin<PREC, false>((const char*)out_ + fb * rhs, i, a, rv);
+#pragma unroll
+            for (int c = 0; c < 6; c++) { rv[c] -= alpha * o[c]; nrm += (double)rv[c] * (double)rv[c]; }
+            store_spin<PREC>((char*)out_ + fb * rhs, i, a, rv);
+        } else {
+            store_spin<PREC>((char*)out_ + fb * rhs, i, a, o);
+            if (EPI == EPI_NORM) {
+#pragma unroll
+                for (int c = 0; c < 6; c++) nrm += (double)o[c] * (double)o[c];
+            }
+        }
+    }
+    if (EPI != EPI_NONE) {
+        const double tot = warp_sum(nrm);
+        if (lane == 0) red[w] = tot;
+        __syncthreads();
+        if (threadIdx.x == 0) partials[(size_t)rhs * gridDim.x + blockIdx.x] = (red[0] + red[1]) + (red[2] + red[3]);
+        // The last block of the grid to finish sums every source's partials (one warp per source, an order that
+        // depends on the number of blocks only) and does what k_cg_reduce would: on these lattices a separate
+        // reduction launch costs as much as the stencil itself.
+        if (last_block_arrive(&cg->ticket)) {
+            for (int j = w; j < (int)gridDim.y; j += 4) {
+                const double v = sum_partials_warp(partials, j, gridDim.x);
+                if (lane == 0) cg_after_reduction(EPI == EPI_RESID ? 1 : 0, j, v, cg);
+            }
+        }
+    }
+}
+
+template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI>
+int launch_small_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void* in, const void* x, void* out, const DslashCoef& c,
+                   int check_done)
+{
+    const int nblocks = (int)(padded_sites(ctx->g.Vh) / LB);
+    if (EPI != EPI_NONE && (size_t)nblocks * nrhs > ctx->norm_partials_count) return tsm_fail(ctx, TSM_ESTATE, "reduction scratch too small");
+    const int pi = prof_begin(ctx, PREC, EPI == EPI_RESID ? 3 : (EPI == EPI_NORM ? 2 : (XPAY ? 1 : 0)), nrhs);
+    k_dslash_small<PREC, RECON, DAGGER, XPAY, EPI><<<dim3(nblocks, nrhs), 128, 0, ctx->stream>>>(ctx->g, par, pack, in, x, out, c, ctx->norm_partials,
+                                                                                                   ctx->cg, check_done);
+    prof_end(ctx, pi);
+    ctx->launches++;
+    ctx->norm_ntiles = nblocks;
+    ctx->norm_reduced = EPI != EPI_NONE;
+    TSM_CUDA(ctx, cudaGetLastError());
+    return TSM_OK;
+}
+
+template <int PREC, int RECON>
+int launch_small_p(tsm_ctx* ctx, int par, bool dagger, int nrhs, const void* pack, const void* in, const void* x, void* out,
+                   const DslashCoef& c, int epi, int check_done)
+{
+    const bool xpay = x != nullptr;
+#define GO(DG, XP, EP) return launch_small_t<PREC, RECON, DG, XP, EP>(ctx, par, nrhs, pack, in, x, out, c, check_done)
+    if (!dagger && !xpay && epi == EPI_NONE) GO(false, false, EPI_NONE);
+    if (!dagger && xpay && epi == EPI_NONE) GO(false, true, EPI_NONE);
+    if (dagger && !xpay && epi == EPI_NONE) GO(true, false, EPI_NONE);
+    if (dagger && xpay && epi == EPI_NONE) GO(true, true, EPI_NONE);
+    if (!dagger && xpay && epi == EPI_NORM) GO(false, true, EPI_NORM);
+    if (dagger && xpay && epi == EPI_RESID) GO(true, true, EPI_RESID);
+#undef GO
+    return tsm_fail(ctx, TSM_EINVAL, "unsupported dslash variant");
+}
+
+}  // namespace
+
+// fp64 / fp32, any nrhs >= 1.  mode bits as in launch_dslash.
+int launch_dslash_small(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs, const void* in, const void* x, void* out,
+                        const DslashCoef& c, int mode)
+{
+    const int chk = (mode >> 1) & 1, nm = (mode & 4) ? EPI_RESID : ((mode & 1) ? EPI_NORM : EPI_NONE);
+    if (prec == TSM_F64) return launch_small_p<TSM_F64, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge64[out_parity], in, x, out, c, nm, chk);
+    if (prec == TSM_F32) {
+        if (ctx->recon == 18) return launch_small_p<TSM_F32, 18>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
+        return launch_small_p<TSM_F32, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
+    }
+    return tsm_fail(ctx, TSM_EINVAL, "small-lattice stencil: unsupported precision");
+}

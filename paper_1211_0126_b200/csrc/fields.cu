@@ -55,7 +55,7 @@ __global__ void k_gauge_pack(const Geom g, const int recon, const double* __rest
         const SiteCoord s = decode_site(g, i, par);
         const long long lex = lex_of_site(g, s);
         const int x[4] = {2 * s.xh + s.rowpar, s.y, s.z, s.t};
-        char* p64 = site_ptr<72>(par ? pack64_1 : pack64_0, i);
+        char* p64 = pack64_0 ? site_ptr<72>(par ? pack64_1 : pack64_0, i) : nullptr;   // no fp64 pack in a low-precision-only workspace
         char* p32 = recon == 18 ? site_ptr<36>(par ? pack32_1 : pack32_0, i) : site_ptr<24>(par ? pack32_1 : pack32_0, i);
         for (int mu = 0; mu < 4; mu++) {
             int xm[4] = {x[0], x[1], x[2], x[3]};
@@ -71,10 +71,11 @@ __global__ void k_gauge_pack(const Geom g, const int recon, const double* __rest
                     b[2 * (3 * r + c) + 1] = -um[2 * (3 * c + r) + 1];
                 }
             dev = max_nan(dev, unitarity_dev(f));
-            for (int j = 0; j < 9; j++) {
-                *reinterpret_cast<double2*>(p64 + (18 * mu + j) * LB_ROW) = make_double2(f[2 * j], f[2 * j + 1]);
-                *reinterpret_cast<double2*>(p64 + (18 * mu + 9 + j) * LB_ROW) = make_double2(b[2 * j], b[2 * j + 1]);
-            }
+            if (p64)
+                for (int j = 0; j < 9; j++) {
+                    *reinterpret_cast<double2*>(p64 + (18 * mu + j) * LB_ROW) = make_double2(f[2 * j], f[2 * j + 1]);
+                    *reinterpret_cast<double2*>(p64 + (18 * mu + 9 + j) * LB_ROW) = make_double2(b[2 * j], b[2 * j + 1]);
+                }
             if (recon == 18) {
                 float l[36];
                 for (int k = 0; k < 18; k++) { l[k] = (float)f[k]; l[18 + k] = (float)b[k]; }

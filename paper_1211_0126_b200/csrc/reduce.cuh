@@ -38,6 +38,27 @@ __device__ __forceinline__ bool last_block_arrive(unsigned* ticket)
     return is_last != 0;
 }
 
+// What follows the sum v of a stencil epilogue's partials for source rhs (O5; one thread):
+//   which == 0 (after w = Mhat p, EPI_NORM):  pq = |w|^2 = Re<p,q>;  alpha = rr / pq, or 0 for a frozen
+//              source; 0 / non-finite pq or rr freezes the source and flags TSM_EBREAKDOWN (A13)
+//   which == 1 (after r -= alpha q, EPI_RESID): rr_new = |r|^2
+__device__ __forceinline__ void cg_after_reduction(int which, int rhs, double v, CgScalars* cg)
+{
+    if (which == 1) { cg->rr_new[rhs] = v; return; }
+    cg->pq[rhs] = v;
+    double alpha = 0.0;
+    if (!cg->done[rhs]) {
+        const double rr = cg->rr[rhs];
+        if (!(v > 0) || !isfinite(v) || !(rr > 0) || !isfinite(rr)) {
+            cg->done[rhs] = 1;
+            cg->status[rhs] = TSM_EBREAKDOWN;
+        } else {
+            alpha = rr / v;
+        }
+    }
+    cg->alpha[rhs] = alpha;
+}
+
 // In the last block: total of partials[rhs * nblk + 0 .. nblk), summed by ONE warp (lane-strided,
 // then the fixed shuffle tree), so the order depends on nblk only -- not on the block shape or on
 // how many sources are in the batch (A14: a source's iterate is bit-identical in any batch).

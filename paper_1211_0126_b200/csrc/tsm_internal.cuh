@@ -129,6 +129,7 @@ template <> struct PT<TSM_BF16> {
 // chunks sit at COMPILE-TIME offsets (k * 512 B) from one base address (one address computation per
 // site instead of one per vector), and a block is one contiguous piece of memory.  Fields are
 // padded to a whole number of blocks; kernels never touch the padding.
+constexpr int FUSE_NTILES = 1024; // stencils on at most this many 128-site tiles finish their own norm reductions (section 6b)
 constexpr int LB = 32;            // sites per layout block
 constexpr int LB_ROW = LB * 16;   // bytes of one chunk row of a block
 __host__ __device__ inline long long padded_sites(long long Vh) { return (Vh + LB - 1) / LB * LB; }
@@ -369,6 +370,7 @@ struct CgScalars {
     int done[TSM_MAX_NRHS];       // frozen: converged, broken down, or zero source
     int status[TSM_MAX_NRHS];
     int all_done;
+    int loop_left;                // iterations the device-side loop (WHILE node of the CG graph) may still run
     unsigned ticket;              // last-block counter, always left at 0
 };
 
@@ -390,11 +392,14 @@ struct GammaTable {          // Gamma_{alpha, col[alpha]} = i^ph[alpha], all oth
 // stencil / BLAS launch.  kind: 0 stencil, 1 stencil+xpay, 2 stencil+xpay+norm, 3 stencil+xpay+residual update, 4 update_xp.
 struct ProfRec { int prec, kind, nrhs; cudaEvent_t a, b; };
 
-// A captured run of CG iterations (CUDA graph), keyed by everything the captured launches depend on.
+// A captured run of CG iterations (CUDA graph), keyed by everything the captured launches depend on.  iters > 0: that
+// many iterations in a row; iters == 0: ONE iteration as the body of a WHILE node, repeated on the device until
+// every source is frozen or cg->loop_left runs out (no host round trip for the stopping test).
 struct CgGraph {
     int prec, nrhs, iters;
     void *x, *r, *p, *w, *t;
     double tol;
+    long long launches;              // kernels inside the graph
     cudaGraphExec_t exec;
 };
 
@@ -412,12 +417,15 @@ struct tsm_ctx {
     cudaStream_t own_stream;         // library-owned BLOCKING stream (serialises with the legacy default stream)
     std::vector<CgGraph> graphs;     // cleared whenever kappa/mu, the gauge storage or the workspace change
     std::vector<BoxMapCache> box_maps;
-    int stencil_choice;              // tsm_set_stencil_kernel: 0 automatic, 1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box
-    int graphs_on;                   // tsm_set_graphs
+    int stencil_choice;              // tsm_set_stencil_kernel: 0 automatic, 1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box, 5 k_dslash_small
+    int graphs_on;                   // tsm_set_graphs: 0 off, 1 chunks of 4 iterations, 2 device-side loop
+    long long loop_per_pass;         // launch accounting of the last device-side loop: kernels per pass (0: none pending),
+    int loop_eager, loop_nrhs;       // iterations run before the loop, sources of that solve (settled in fetch_scalars)
     double kappa, mu;
     bool have_params, have_gauge, have_ws;
     int recon;                       // storage of the fp32 link copy (18 / 12)
     int max_nrhs;
+    int ws_prec;                     // TSM_F64: full workspace; TSM_F32: low-precision-only (no fp64 packs, fp32-sized vectors)
     int nsm;
     // workspace carving (device pointers into the caller's buffer)
     char* ws;
@@ -436,6 +444,7 @@ struct tsm_ctx {
     double* norm_partials;           // [rhs][tile] sums of |out|^2 left by the stencil's NORM epilogue
     size_t norm_partials_count;
     int norm_ntiles;
+    bool norm_reduced;               // the last stencil launch finished its own reduction (k_dslash_small): skip k_cg_reduce
     double* loops_src[2];            // per-source loops of a slot [rhs][n_ops][T][2]
     double* acc_corr;                // [n_ops][T][2]
     double* acc_lp;
@@ -495,6 +504,8 @@ int launch_dslash(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs,
                   void* out, const DslashCoef& c, int mode);
 int launch_dslash_tile(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs, const void* in, const void* x,
                        void* out, const DslashCoef& c, int mode);
+int launch_dslash_small(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs, const void* in, const void* x,
+                        void* out, const DslashCoef& c, int mode);
 int launch_dslash_box(tsm_ctx* ctx, int out_parity, bool dagger, int nrhs, const void* in, const void* x, void* out,
                       const DslashCoef& c, int mode);
 bool box_stencil_supported(const tsm_ctx* ctx);
@@ -507,7 +518,9 @@ int launch_cg_init(tsm_ctx* ctx, int prec, int nrhs, const void* r, void* p, voi
 int launch_cg_reduce(tsm_ctx* ctx, int which, int nrhs, int force = 0);
 int launch_mixed_ctl(tsm_ctx* ctx, int mode, int nrhs, double tol);
 int launch_mixed_axpy(tsm_ctx* ctx, int nrhs, void* x64, const void* e32);
-int launch_cg_update_xp(tsm_ctx* ctx, int prec, int nrhs, void* x, void* p, const void* r, double tol);
+int launch_cg_update_xp(tsm_ctx* ctx, int prec, int nrhs, void* x, void* p, const void* r, double tol, unsigned long long loop = 0,
+                        int in_loop = 0);
+int launch_cg_loop_begin(tsm_ctx* ctx, int n);
 int launch_convert(tsm_ctx* ctx, int prec_in, int prec_out, int nrhs_fields, const void* in, void* out);
 int launch_contract(tsm_ctx* ctx, int slot);
 int launch_accumulate(tsm_ctx* ctx, double* acc, const double* a, const double* b, int nrhs);

@@ -32,6 +32,9 @@ WANT = [
     ("l1tex__throughput.avg.pct_of_peak_sustained_active", "L1/TEX throughput % of peak"),
     ("l1tex__data_pipe_lsu_wavefronts.sum.pct_of_peak_sustained_elapsed", "LSU data-pipe wavefronts % of peak"),
     ("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum", "shared-memory wavefronts"),
+    ("l1tex__data_pipe_lsu_wavefronts.sum", "LSU data-pipe wavefronts"),
+    ("l1tex__m_xbar2l1tex_read_bytes.sum", "L2 -> SM bytes over the crossbar (reads)"),
+    ("l1tex__m_l1tex2xbar_write_bytes.sum", "SM -> L2 bytes over the crossbar (writes)"),
     ("smsp__inst_executed.sum", "warp instructions"), ("smsp__issue_active.avg.pct_of_peak_sustained_active", "issue slots busy %"),
     ("sm__warps_active.avg.pct_of_peak_sustained_active", "achieved occupancy %"),
     ("smsp__warps_eligible.avg.per_cycle_active", "eligible warps per scheduler cycle"),

@@ -31,7 +31,7 @@ EXPORTS = [
     "tsm_loops_reset", "tsm_loops_set_momenta", "tsm_loops_add_correction", "tsm_loops_add_lp", "tsm_loops_source",
     "tsm_loops_finalize", "tsm_loops_get_state", "tsm_loops_set_state", "tsm_run_loop_set",
     "tsm_set_hp_precision", "tsm_launch_count", "tsm_profile", "tsm_profile_read", "tsm_stencil_kernel_name",
-    "tsm_set_stencil_kernel", "tsm_set_graphs",
+    "tsm_set_stencil_kernel", "tsm_set_graphs", "tsm_probe_su3_tensor",
 ]
 
 
@@ -66,9 +66,9 @@ def load_library():
     lib.tsm_last_error.restype = ctypes.c_char_p
     lib.tsm_field_bytes.argtypes = [vp, i, i]
     lib.tsm_field_bytes.restype = sz
-    lib.tsm_workspace_bytes.argtypes = [vp, i]
+    lib.tsm_workspace_bytes.argtypes = [vp, i, i]
     lib.tsm_workspace_bytes.restype = sz
-    lib.tsm_set_workspace.argtypes = [vp, vp, sz, i]
+    lib.tsm_set_workspace.argtypes = [vp, vp, sz, i, i]
     lib.tsm_set_stream.argtypes = [vp, vp]
     lib.tsm_set_params.argtypes = [vp, ctypes.c_double, ctypes.c_double]
     lib.tsm_set_gauge.argtypes = [vp, vp, i, dp]
@@ -94,6 +94,7 @@ def load_library():
     lib.tsm_stencil_kernel_name.argtypes = [vp, i, i]
     lib.tsm_stencil_kernel_name.restype = ctypes.c_char_p
     lib.tsm_set_stencil_kernel.argtypes = [vp, i]
+    lib.tsm_probe_su3_tensor.argtypes = [vp, i, i, i, i, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     lib.tsm_set_graphs.argtypes = [vp, i]
     lib.tsm_profile.argtypes = [vp, i]
     lib.tsm_profile_read.argtypes = [vp, i, i, i, dp, ctypes.POINTER(ctypes.c_longlong)]
@@ -115,7 +116,7 @@ def _host_c128(a, shape) -> np.ndarray:
 class Tsm:
     """One lattice geometry on one GPU; owns the context and the torch workspace tensor."""
 
-    def __init__(self, dims, t_boundary: int = -1, device: int = 0, max_nrhs: int = 1, stream=None):
+    def __init__(self, dims, t_boundary: int = -1, device: int = 0, max_nrhs: int = 1, stream=None, workspace_prec: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1211_0126_b200 needs a CUDA device; there is no CPU fallback")
@@ -132,11 +133,12 @@ class Tsm:
         rc = self.lib.tsm_create(ctypes.byref(self._h), (ctypes.c_int * 4)(*self.dims), t_boundary, device)
         if rc != OK:
             raise TsmError(rc, "tsm_create failed (extents must be even and >= 4; device must exist)")
-        nbytes = self.lib.tsm_workspace_bytes(self._h, max_nrhs)
+        nbytes = self.lib.tsm_workspace_bytes(self._h, max_nrhs, workspace_prec)
         if nbytes == 0:
-            raise TsmError(EINVAL, "bad max_nrhs")
+            raise TsmError(EINVAL, "bad max_nrhs or workspace precision (F64 = everything, F32 = low-precision solves only)")
+        self.workspace_prec = workspace_prec
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=f"cuda:{device}")
-        self._check(self.lib.tsm_set_workspace(self._h, self.workspace.data_ptr(), nbytes, max_nrhs))
+        self._check(self.lib.tsm_set_workspace(self._h, self.workspace.data_ptr(), nbytes, max_nrhs, workspace_prec))
         if stream is not None:
             self.set_stream(stream)
 
@@ -192,11 +194,20 @@ class Tsm:
         self.hp_precision = prec
 
     def set_stencil_kernel(self, which: int):
-        """0 automatic, 1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box (tuning / test aid)."""
+        """0 automatic, 1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box, 5 k_dslash_small (tuning / test aid)."""
         self._check(self.lib.tsm_set_stencil_kernel(self._h, which))
 
-    def set_graphs(self, enable: bool):
-        self._check(self.lib.tsm_set_graphs(self._h, int(enable)))
+    def probe_su3_tensor(self, variant: int, nsites: int, inner: int, reps: int):
+        """(microseconds per launch, max error relative to the largest fp64 reference value) of the per-site
+        SU(3) x (3 x 24) product in formulation `variant` (include/tsm.h: tsm_probe_su3_tensor)."""
+        us, err = ctypes.c_double(), ctypes.c_double()
+        self._check(self.lib.tsm_probe_su3_tensor(self._h, variant, nsites, inner, reps, ctypes.byref(us), ctypes.byref(err)))
+        return us.value, err.value
+
+    def set_graphs(self, mode):
+        """1 / True (default): cached graphs of 4 CG iterations; 2: the CG loop as one graph launch with a device-side
+        WHILE node; 0 / False: kernel by kernel."""
+        self._check(self.lib.tsm_set_graphs(self._h, int(mode)))
 
     def hp_precision_name(self) -> str:
         return "mixed" if self.hp_precision == MIXED else "fp64"

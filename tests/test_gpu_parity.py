@@ -501,9 +501,27 @@ def test_cuda_graph_chunks_equal_kernel_by_kernel_launches(medium):
         assert [i["iters"] for i in info_g] == [i["iters"] for i in info_d]
         for j in range(2):
             assert np.array_equal(a[j], c.t.get_solution(1, j)), (prec, j)
-    n0 = c.t.launch_count()
-    c.t.solve(seed, [3], F32, 0.0, 12, slot=0)
-    assert c.t.launch_count() - n0 == 6 + 7 * 12 + 1      # noise, twist, 3 stencils, init; 7 per iteration; reconstruction
+    # the three launch modes (kernel by kernel, graphs of 4 iterations, device-side WHILE loop) give the same iterates
+    # and the same launch count: noise, twist, 3 stencils, init; per iteration 4 stencils + update (k_dslash_small
+    # finishes its own reductions on this lattice); the loop's begin kernel; reconstruction
+    ref = None
+    for mode in (0, 1, 1, 2, 2):
+        c.t.set_graphs(mode)
+        for tol, k in ((0.0, 12), (1e-4, 500)):
+            n0 = c.t.launch_count()
+            rc, info = c.t.solve(seed, [3, 5], F32, tol, k, slot=0)
+            n_l = c.t.launch_count() - n0
+            got = (info[0]["iters"], info[1]["iters"], c.t.get_solution(0, 0), c.t.get_solution(0, 1))
+            if tol == 0.0:
+                assert n_l == 6 + 5 * 12 + 1 + (1 if mode == 2 else 0), (mode, n_l)
+                if ref is None:
+                    ref = got
+                assert got[0] == 12 and np.array_equal(got[2], ref[2]) and np.array_equal(got[3], ref[3]), mode
+            else:
+                if mode == 0:
+                    ref_t = got
+                assert got[:2] == ref_t[:2] and np.array_equal(got[2], ref_t[2]) and np.array_equal(got[3], ref_t[3]), mode
+    c.t.set_graphs(1)
 
 
 # ---------------------------------------------------------------- N1: one-end trick loops (Eq. 2.5)
@@ -798,7 +816,7 @@ def test_box_stencil_parity(tsm_mod, dims, recon, theta):
     the oracle (1e-5, north_star) on lattices that exercise every halo wrap, for 1, 3 and 12 sources; agreement
     with k_dslash to fp32 rounding; a source's result bit-identical in any batch (A14)."""
     c = Case(tsm_mod, dims, 0.6, 91, 0.157, 0.02, theta, max_nrhs=12, recon=recon)
-    assert c.t.stencil_kernel_name(F32, 12) == "k_dslash_tile" and c.t.stencil_kernel_name(F32, 1) == "k_dslash"   # automatic choice
+    assert c.t.stencil_kernel_name(F32, 12) == "k_dslash_small" and c.t.stencil_kernel_name(F32, 1) == "k_dslash_small"   # automatic choice on an L2-resident lattice
     c.t.set_stencil_kernel(3)
     assert c.t.stencil_kernel_name(F32, 12) == "k_dslash_box" and c.t.stencil_kernel_name(F32, 1) == "k_dslash_box"
     assert c.t.stencil_kernel_name(F64, 12) == "k_dslash" and c.t.stencil_kernel_name(BF16, 12) == "k_dslash_tile"
@@ -888,3 +906,79 @@ def test_loop_set_is_bit_reproducible(medium):
     f, _, _ = c.t.run_loop_set(wl.noise_seed, 3, 9, F32, wl.lp_tol, 1000, nrhs=1, **kw)
     assert np.array_equal(e, f) and rel(e, a) < 1e-8
     c.t.loops_reset(False)
+
+
+def test_tensor_core_probe_is_correct(small):
+    """csrc/mma_probe.cu (the measurement behind DESIGN.md section 6's tensor-core paragraph): every formulation of
+    the per-site SU(3) x (3 x 24) product agrees with the fp64 reference it carries -- fp32 FMAs and 3xTF32 to fp32
+    rounding, plain TF32 only to ~1e-3 (which is why it cannot serve the 1e-5 stencil), both fp64 forms to 1e-14."""
+    for variant, lo, hi in ((0, 0.0, 2e-6), (1, 2e-5, 5e-3), (2, 0.0, 2e-6), (3, 0.0, 1e-14), (4, 0.0, 1e-14)):
+        us, err = small.t.probe_su3_tensor(variant, 4096, 8, 2)
+        assert us > 0 and lo <= err < hi, (variant, err)
+
+
+def test_low_precision_only_workspace(small, tsm_mod):
+    """tsm_workspace_bytes / tsm_set_workspace with prec = TSM_F32: no fp64 link copy, fp32-sized
+    vectors -- fp32 and bf16 solves and their loops are bit-identical to those on the full workspace, noise is still
+    bit-exact, fp64 / mixed solves and the fp64 true residual are refused with TSM_ESTATE."""
+    c = small
+    t2 = tsm_mod.Tsm(c.dims, t_boundary=c.theta, max_nrhs=4, workspace_prec=F32)
+    assert t2.workspace.numel() < 0.8 * c.t.workspace.numel()   # 0.59 at 32^3 x 64 with 12 sources; staging weighs more on 4^3 x 8
+    t2.set_params(c.kappa, c.mu)
+    assert t2.set_gauge(c.U, 18) < 1e-13
+    assert np.array_equal(t2.noise(77, 3), oracle.noise(c.dims, 77, 3))
+    for prec in (F32, BF16):
+        rc, _ = c.t.solve(5, [0, 1, 2], prec, 0.0, 9, slot=1)
+        rc2, _ = t2.solve(5, [0, 1, 2], prec, 0.0, 9, slot=1)
+        assert rc == 0 and rc2 == 0
+        for j in range(3):
+            assert np.array_equal(t2.get_solution(1, j), c.t.get_solution(1, j)), (prec, j)
+    c.t.loops_reset(True)
+    t2.loops_reset(True)
+    assert np.array_equal(t2.loops_source(1, 2), c.t.loops_source(1, 2))
+    c.t.loops_reset(False)
+    for bad in (dict(prec=F64, tol=1e-8), dict(prec=3, tol=1e-8), dict(prec=F32, tol=1e-3, want_true_resid=True)):
+        with pytest.raises(tsm_mod.TsmError) as e:
+            t2.solve(5, [0], bad["prec"], bad["tol"], 50, slot=0, want_true_resid=bad.get("want_true_resid", False))
+        assert e.value.code == tsm_mod.ESTATE, bad
+    t2.close()
+
+
+@pytest.mark.parametrize("recon", [18, 12])
+def test_small_lattice_stencil(tsm_mod, recon):
+    """k_dslash_small (the automatic choice on lattices of at most 16 384 sites per parity: four warps = four
+    directions per 32 sites): every operator and epilogue form against the oracle, fp64 1e-12 and fp32 1e-5, on the
+    ragged lattice (last 32-site block half empty) for 1, 3 and 12 sources; agreement with k_dslash to rounding
+    (the sum over directions is associated differently); a source's result bit-identical in any batch (A14); and
+    through the solver (norm and residual epilogues, graphs), fp64 iterates at equal iteration count to 1e-12."""
+    dims, theta = (6, 10, 4, 6), +1
+    c = Case(tsm_mod, dims, 0.6, 77, 0.157, 0.02, theta, max_nrhs=12, recon=recon)
+    assert c.t.stencil_kernel_name(F64, 1) == "k_dslash_small" and c.t.stencil_kernel_name(BF16, 4) == "k_dslash_tile"
+    psi = W.random_spinor(dims, 80, nrhs=12)
+    for prec, tol, close in ((F64, 1e-12, 1e-14), (F32, 1e-5, 2e-6)):
+        for nrhs in (1, 3, 12):
+            for op in (0, 1, 2, 3, 4):
+                got = _gpu_op(c, op, prec, psi[:nrhs])
+                for j in sorted({0, nrhs - 1}):
+                    src = psi[j] if prec == F64 else psi[j].astype(np.complex64).astype(np.complex128)
+                    assert rel(got[j], _oracle_op(c, op, src)) < tol, (prec, nrhs, op, j)
+                if nrhs == 12:
+                    single = _gpu_op(c, op, prec, psi[5:6])[0]
+                    assert np.array_equal(single, got[5]), (prec, op)
+                if nrhs == 3:
+                    c.t.set_stencil_kernel(1)
+                    other = _gpu_op(c, op, prec, psi[:nrhs])
+                    c.t.set_stencil_kernel(0)
+                    assert rel(got, other) < close, (prec, op)
+    eta = oracle.noise(dims, 9, 3)
+    for k in (1, 4, 9):
+        s_ref, _ = oracle.solve(dims, theta, c.kappa, c.mu, c.U, eta, 0.0, k)
+        rc, info = c.t.solve(9, [1, 2, 3, 4], F64, 0.0, k, slot=0)
+        assert rc == 0 and rel(c.t.get_solution(0, 2), s_ref) < 1e-12, k
+    rc, info = c.t.solve(9, [0, 1, 2, 3, 4], F32, 0.0, 7, slot=0)
+    batch = c.t.get_solution(0, 3)
+    rc, _ = c.t.solve(9, [3], F32, 0.0, 7, slot=1)
+    assert np.array_equal(c.t.get_solution(1, 0), batch)
+    rc, info = c.t.solve(9, [5, 6, 7], F32, 1e-4, 500, slot=0, want_true_resid=True)
+    assert rc == 0 and all(i["rel_resid_true"] < 2e-4 for i in info)
+    c.t.close()
