@@ -4,9 +4,17 @@
 #include <cstdlib>
 #include <cstring>
 
+#include <nvtx3/nvToolsExt.h>   // header-only: ranges for an nsys / ncu timeline, no-ops without a profiler attached
+
 #include "tsm_internal.cuh"
 
 namespace {
+
+// NVTX range for one phase of the path (noise / prepare / CG / reconstruct / contract): closes when it goes out of scope
+struct Phase {
+    explicit Phase(const char* name) { nvtxRangePushA(name); }
+    ~Phase() { nvtxRangePop(); }
+};
 
 struct Twists {
     TwistCoef zero, one, R, Rinv, Rb, Rbinv, mk2, k, kRinv;
@@ -317,24 +325,32 @@ int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs,
     char* s_e = (char*)ctx->slot[slot];
     char* s_o = s_e + field_bytes(sp, Vh, nrhs);
     void *r = ctx->vec[0], *p = ctx->vec[1], *w = ctx->vec[3], *t = ctx->vec[4], *aux = ctx->vec[5];
-    // H3: eta straight into the slot (eta_e where s_e will be, eta_o where s_o will be)
-    if ((rc = launch_noise(ctx, sp, nrhs, seed, ids_dev, kind, s_e))) return rc;
-    // H4: bhat = eta_e + kappa D_eo R^-1 eta_o (into w);  b' = Mhat^dag bhat (into r)
-    if ((rc = launch_twist(ctx, sp, nrhs, s_o, aux, tw.Rinv))) return rc;
-    if ((rc = launch_dslash(ctx, sp, 0, false, nrhs, aux, s_e, w, {tw.one, tw.k}, 0))) return rc;
-    if ((rc = launch_dslash(ctx, sp, 1, true, nrhs, w, nullptr, t, {tw.zero, tw.Rbinv}, 0))) return rc;
-    if ((rc = launch_dslash(ctx, sp, 0, true, nrhs, t, w, r, {tw.Rb, tw.mk2}, 0))) return rc;
-    // O5: x0 = 0 (x lives in the slot's even half), r0 = p0 = b'
     void* x = s_e;
-    if (prec == TSM_MIXED) {
-        if ((rc = solve_mixed(ctx, nrhs, tw, s_e, tol, max_iter))) return rc;
-    } else {
-        if ((rc = launch_cg_init(ctx, prec, nrhs, r, p, x))) return rc;
-        if ((rc = cg_run(ctx, prec, nrhs, tw, x, r, p, w, t, tol, max_iter))) return rc;
+    {   // H3: eta straight into the slot (eta_e where s_e will be, eta_o where s_o will be)
+        Phase ph("tsm: noise");
+        if ((rc = launch_noise(ctx, sp, nrhs, seed, ids_dev, kind, s_e))) return rc;
     }
-    // H7: s_e = x, s_o = R^-1 (eta_o + kappa D_oe x)
-    if ((rc = launch_dslash(ctx, sp, 1, false, nrhs, x, s_o, aux, {tw.Rinv, tw.kRinv}, 0))) return rc;
-    TSM_CUDA(ctx, cudaMemcpyAsync(s_o, aux, field_bytes(sp, Vh, nrhs), cudaMemcpyDeviceToDevice, ctx->stream));
+    {   // H4: bhat = eta_e + kappa D_eo R^-1 eta_o (into w);  b' = Mhat^dag bhat (into r)
+        Phase ph("tsm: prepare");
+        if ((rc = launch_twist(ctx, sp, nrhs, s_o, aux, tw.Rinv))) return rc;
+        if ((rc = launch_dslash(ctx, sp, 0, false, nrhs, aux, s_e, w, {tw.one, tw.k}, 0))) return rc;
+        if ((rc = launch_dslash(ctx, sp, 1, true, nrhs, w, nullptr, t, {tw.zero, tw.Rbinv}, 0))) return rc;
+        if ((rc = launch_dslash(ctx, sp, 0, true, nrhs, t, w, r, {tw.Rb, tw.mk2}, 0))) return rc;
+    }
+    {   // O5: x0 = 0 (x lives in the slot's even half), r0 = p0 = b'
+        Phase ph(prec == TSM_MIXED ? "tsm: CG (mixed precision)" : "tsm: CG");
+        if (prec == TSM_MIXED) {
+            if ((rc = solve_mixed(ctx, nrhs, tw, s_e, tol, max_iter))) return rc;
+        } else {
+            if ((rc = launch_cg_init(ctx, prec, nrhs, r, p, x))) return rc;
+            if ((rc = cg_run(ctx, prec, nrhs, tw, x, r, p, w, t, tol, max_iter))) return rc;
+        }
+    }
+    {   // H7: s_e = x, s_o = R^-1 (eta_o + kappa D_oe x)
+        Phase ph("tsm: reconstruct");
+        if ((rc = launch_dslash(ctx, sp, 1, false, nrhs, x, s_o, aux, {tw.Rinv, tw.kRinv}, 0))) return rc;
+        TSM_CUDA(ctx, cudaMemcpyAsync(s_o, aux, field_bytes(sp, Vh, nrhs), cudaMemcpyDeviceToDevice, ctx->stream));
+    }
     TSM_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
     if ((rc = fetch_scalars(ctx))) return rc;
     float ms = 0;
@@ -449,6 +465,7 @@ int tsm_loops_add_correction(tsm_ctx* ctx, int slot_hp, int slot_lp)
         ctx->slot_kind[slot_hp] != ctx->slot_kind[slot_lp] ||
         memcmp(ctx->slot_ids[slot_hp], ctx->slot_ids[slot_lp], nrhs * sizeof(uint32_t)) != 0)
         return tsm_fail(ctx, TSM_ESTATE, "HP and LP slots hold different sources (Eq. 2.4 needs the same eta_j)");
+    Phase ph("tsm: contract (HP - LP)");
     if ((rc = launch_contract(ctx, slot_hp))) return rc;
     if ((rc = launch_contract(ctx, slot_lp))) return rc;
     if ((rc = launch_accumulate(ctx, ctx->acc_corr, ctx->loops_src[slot_hp], ctx->loops_src[slot_lp], nrhs))) return rc;
@@ -463,6 +480,7 @@ int tsm_loops_add_lp(tsm_ctx* ctx, int slot_lp)
     if ((rc = check_loops(ctx))) return rc;
     if ((rc = check_slot(ctx, slot_lp, 0))) return rc;
     const int nrhs = ctx->slot_nrhs[slot_lp];
+    Phase ph("tsm: contract (LP)");
     if ((rc = launch_contract(ctx, slot_lp))) return rc;
     if ((rc = launch_accumulate(ctx, ctx->acc_lp, ctx->loops_src[slot_lp], nullptr, nrhs))) return rc;
     ctx->n_lp += nrhs;

@@ -83,15 +83,19 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_reduce(const int which, const in
 // x += alpha p; p = r + beta p with beta = rr_new / rr (one pass: reads x, p, r; writes x, p).  r was already
 // updated by the stencil that produced q (EPI_RESID).  The last block to finish does the per-source
 // bookkeeping of O5: iteration count, rr <- rr_new, the stopping test |r|/|b'| <= tol (A8), freeze flags.
-template <int PV, int PP>
+// LOOP: the launch is the last kernel of the body of a WHILE graph node and decides whether another pass follows.  A
+// separate instantiation, because ncu cannot profile graph kernel nodes that are able to set a conditional handle.
+template <int PV, int PP, bool LOOP>
 __global__ void __launch_bounds__(BLAS_BS) k_cg_update_xp(const int Vh, const int nrhs, void* __restrict__ x_, void* __restrict__ p_,
                                                           const void* __restrict__ r_, const double tol, CgScalars* cg,
-                                                          const cudaGraphConditionalHandle loop, const int in_loop)
+                                                          const cudaGraphConditionalHandle loop)
 {
     using TV = typename PT<PV>::real;
     using TP = typename PT<PP>::real;
     if (cg->all_done) {   // every source frozen: leave the device-side iteration loop, if this launch is inside one
-        if (in_loop && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) cudaGraphSetConditional(loop, 0u);
+        if constexpr (LOOP) {
+            if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) cudaGraphSetConditional(loop, 0u);
+        }
         return;
     }
     const int rhs = blockIdx.y;
@@ -134,7 +138,7 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_update_xp(const int Vh, const in
             }
             cg->all_done = all;
             // inside the WHILE node of a CUDA graph (api_solve.cu: cg_run): one more iteration?
-            if (in_loop) {
+            if constexpr (LOOP) {
                 const int left = cg->loop_left - 1;
                 cg->loop_left = left;
                 cudaGraphSetConditional(loop, (!all && left > 0) ? 1u : 0u);
@@ -200,8 +204,12 @@ int launch_cg_update_xp(tsm_ctx* ctx, int prec, int nrhs, void* x, void* p, cons
 {
     const dim3 grid = blas_grid(ctx, nrhs);
     const int pi = prof_begin(ctx, prec, 4, nrhs);
-    BLAS_SWITCH(prec, (k_cg_update_xp<PV, PP><<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, nrhs, x, p, r, tol, ctx->cg,
-                                                                                (cudaGraphConditionalHandle)loop, in_loop)));
+    if (in_loop) {
+        BLAS_SWITCH(prec, (k_cg_update_xp<PV, PP, true><<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, nrhs, x, p, r, tol, ctx->cg,
+                                                                                          (cudaGraphConditionalHandle)loop)));
+    } else {
+        BLAS_SWITCH(prec, (k_cg_update_xp<PV, PP, false><<<grid, BLAS_BS, 0, ctx->stream>>>(ctx->g.Vh, nrhs, x, p, r, tol, ctx->cg, 0)));
+    }
     prof_end(ctx, pi);
     ctx->launches++;
     TSM_CUDA(ctx, cudaGetLastError());

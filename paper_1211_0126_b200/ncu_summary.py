@@ -5,7 +5,8 @@
         --title "..." --command "ncu --set full ..." \
         [--traffic profiles/r02_traffic.json --key cfg5_32x32x32x64/f32/nrhs12 --commit <hash>]
 
-The markdown lists, per captured launch, the counters DESIGN.md section 6 argues with (duration, DRAM bytes and
+With --launch-list the input is the log of `ncu --metrics gpu__time_duration.sum --csv --log-file ...` and the output a
+per-kernel table of launches / time / share.  Otherwise the markdown lists, per captured launch, the counters DESIGN.md section 6 argues with (duration, DRAM bytes and
 throughput, L2 sectors and L2 throughput, L1 hit rate, LSU wavefronts, issue slots, stalls, occupancy).  With
 --traffic, the mean over the captured launches of dram__bytes_read.sum + dram__bytes_write.sum is stored under
 --key together with the commit of the kernels; bench.py reports that number as `roofline.traffic`.
@@ -103,9 +104,51 @@ def dram_bytes(hdr, units, rows):
     return tot
 
 
+def launch_list(path, out_md, out_csv, title, command, note):
+    """`ncu --metrics gpu__time_duration.sum --csv --log-file x.csv ...` -> a table of launches, total time and share per
+    kernel (markdown) and the log reduced to (id, kernel, duration_us) (csv)."""
+    rows = list(csv.reader(open(path)))
+    while rows and (not rows[0] or rows[0][0] != "ID"):
+        rows.pop(0)
+    if len(rows) < 2:
+        raise SystemExit(f"{path}: no ncu table found")
+    hdr = rows[0]
+    ki, vi, ui, mi = hdr.index("Kernel Name"), hdr.index("Metric Value"), hdr.index("Metric Unit"), hdr.index("Metric Name")
+    scale = {"ns": 1e-3, "us": 1.0, "ms": 1e3, "s": 1e6}
+    recs = []
+    for r in rows[1:]:
+        if len(r) <= vi or r[mi] != "gpu__time_duration.sum":
+            continue
+        name = r[ki].replace("void <unnamed>::", "").replace("<unnamed>::", "").split("(")[0]
+        recs.append((name, to_float(r[vi]) * scale[r[ui]]))
+    tot, cnt = {}, {}
+    for name, us in recs:
+        tot[name] = tot.get(name, 0.0) + us
+        cnt[name] = cnt.get(name, 0) + 1
+    T = sum(tot.values())
+    text = f"# {title}\n\n"
+    if command:
+        text += f"Command (B200 box; the same command had just exited 0 without ncu):\n\n    {command}\n\n"
+    text += (f"`{os.path.basename(out_csv)}` beside this file is that log reduced to (id, kernel, duration). {len(recs)} launches, "
+             f"{T / 1e3:.2f} ms of kernel time; per-launch times under ncu are cold-cache and serialised, so compare SHARES with "
+             "bench.py's `roofline.share_of_step`, not absolutes.\n\n")
+    text += "| launches | total ms | share | avg us | kernel |\n|---|---|---|---|---|\n"
+    for name in sorted(tot, key=lambda k: -tot[k]):
+        text += f"| {cnt[name]} | {tot[name] / 1e3:.2f} | {100 * tot[name] / T:.1f} % | {tot[name] / cnt[name]:.1f} | `{name}` |\n"
+    if note:
+        text += "\n" + note + "\n"
+    with open(out_md, "w") as f:
+        f.write(text)
+    with open(out_csv, "w") as f:
+        f.write("id,kernel,duration_us\n")
+        for k, (name, us) in enumerate(recs):
+            f.write(f'{k},"{name}",{us:.2f}\n')
+
+
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("csv")
+    ap.add_argument("--launch-list", help="treat `csv` as an ncu gpu__time_duration log; write the reduced csv here (markdown to --out)")
     ap.add_argument("--out", help="markdown file to write (default: stdout)")
     ap.add_argument("--title", default="ncu summary")
     ap.add_argument("--command", default="", help="the full command that made the capture (named in the file)")
@@ -114,6 +157,11 @@ def main():
     ap.add_argument("--key", help="entry of the JSON file: workload/prec/nrhsN")
     ap.add_argument("--commit", default="", help="commit of the kernels the capture was taken at")
     a = ap.parse_args()
+    if a.launch_list:
+        if not a.out:
+            raise SystemExit("--launch-list needs --out")
+        launch_list(a.csv, a.out, a.launch_list, a.title, a.command, a.note)
+        return
     hdr, units, rows = read_rows(a.csv)
     per = dram_bytes(hdr, units, rows)
     text = f"# {a.title}\n\n"
