@@ -7,11 +7,14 @@
 // 12): a single cp.async.bulk brings it into shared memory, completion is signalled on an
 // mbarrier, and the copy for the CTA's NEXT tile is issued before the current tile is computed
 // (two buffers), so the only loads that come straight from DRAM are never waited for by the
-// arithmetic.  Every link is then read from HBM/L2 once per tile whatever the batch size.
-// blockDim = (128 sites, RY source rows); a CTA loops over G = ceil(nrhs / RY) groups of sources.
-// Neighbour spinors come through L1/L2 (ld.global.nc).  (Several sources per thread with the link pair held in
-// registers, a single link buffer, a 4-D tile shape and a warp of 8 sites x 4 sources were all measured slower:
-// DESIGN.md section 6.)
+// arithmetic.  Every link is then read from HBM/L2 once per tile whatever the batch size, and
+// R sources are handled per thread with the link pair held in registers (R x fewer shared-memory
+// reads, R independent dependency chains).  blockDim = (128 sites, RY source rows); a CTA loops over
+// G = ceil(nrhs / (RY * R)) groups of sources.  Neighbour spinors come through L1/L2 (ld.global.nc).
+// Shapes in use (measured at 32^3 x 64, 12 sources, inside the CG): the plain launches
+// (no x term, no epilogue) run 3 rows x 2 sources per thread (168 registers, 12 warps: 821 us against 882 us
+// for 4 x 1), every launch with an x term or an epilogue 4 rows x 1 source (128 registers, 16 warps: the second
+// source's x / r vectors do not fit beside the accumulators, 1113-1243 us against 1008-1121 us).
 //
 // Arithmetic per source is the same sequence of operations as in dslash.cu (same projection,
 // same FMA chains, same accumulation order over mu), so a source's result does not depend on the
@@ -56,31 +59,33 @@ template <int RECON, int MU> __device__ __forceinline__ void lds_link_pair(const
     }
 }
 
-// one direction: the link pair from the staged tile, then the forward and the backward hop
-template <int PREC, int RECON, bool DAGGER, int MU>
-__device__ __forceinline__ void hop_direction_s(const char* tile_links, int tx, const char* in, const int* nb, float ph_f, float ph_b,
-                                                float* acc)
+// one direction, R sources: links once, then the forward and the backward hop of every source
+template <int PREC, int RECON, bool DAGGER, int MU, int R>
+__device__ __forceinline__ void hop_direction_r(const char* tile_links, int tx, const char* in, size_t fb, const int* nb, float ph_f,
+                                                float ph_b, float (*acc)[24])
 {
     constexpr int SF = DAGGER ? +1 : -1;   // forward hop carries (1 - g_mu), dagger swaps
     float uf[18], ub[18];
     lds_link_pair<RECON, MU>(tile_links, tx, uf, ub);
-    {
+#pragma unroll
+    for (int r = 0; r < R; r++) {
         float psi[24], h[12], gq[12];
-        load_spinor<PREC>(in, nb[2 * MU], psi);
+        load_spinor<PREC>(in + fb * r, nb[2 * MU], psi);
         project<float, MU, SF>(psi, h);
         if (MU == 3 && ph_f != 1) rscale_f32<6>(ph_f, h);   // time-boundary phase (A22); skipping a multiplication by one is exact
         su3_mul(uf, h, gq);
         su3_mul(uf, h + 6, gq + 6);
-        accumulate<float, MU, SF>(gq, acc);
+        accumulate<float, MU, SF>(gq, acc[r]);
     }
-    {
+#pragma unroll
+    for (int r = 0; r < R; r++) {
         float psi[24], h[12], gq[12];
-        load_spinor<PREC>(in, nb[2 * MU + 1], psi);
+        load_spinor<PREC>(in + fb * r, nb[2 * MU + 1], psi);
         project<float, MU, -SF>(psi, h);
         if (MU == 3 && ph_b != 1) rscale_f32<6>(ph_b, h);
         su3_mul(ub, h, gq);
         su3_mul(ub, h + 6, gq + 6);
-        accumulate<float, MU, -SF>(gq, acc);
+        accumulate<float, MU, -SF>(gq, acc[r]);
     }
 }
 
@@ -98,7 +103,7 @@ __device__ __forceinline__ int tile_base(const Geom& g, int tile, int slab)
     return (int)(t * g.Vsh + (zb * g.bz + zi) * g.S + rest);
 }
 
-template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI, int RY>
+template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI, int RY, int R>
 __global__ void __launch_bounds__(TT * RY, 1)
 k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, const int slab, const void* __restrict__ pack,
               const void* __restrict__ in_, const void* __restrict__ x_, void* out_, const DslashCoef cf,
@@ -109,7 +114,7 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
     extern __shared__ __align__(128) char smem[];
     __shared__ __align__(8) uint64_t bar[2];
     constexpr int PR = PREC == TSM_BF16 ? TSM_F32 : PREC;   // storage of the CG residual (EPI_RESID)
-    __shared__ double red[EPI != EPI_NONE ? RY * 2 * 4 : 1];
+    __shared__ double red[EPI != EPI_NONE ? RY * 2 * 4 * R : 1];
     if (check_done && cg->all_done) return;
     const int Vh = g.Vh;
     const int nblocks = (int)(padded_sites(Vh) / LB);
@@ -152,58 +157,68 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
         mbar_wait(&bar[b], (unsigned)((it >> 1) & 1));
         const char* links = smem + (size_t)b * TILE_BYTES;
 
-        for (int grp = 0; grp * RY < nrhs; grp++) {
-            const int rhs = grp * RY + ty;
-            const bool act = live && rhs < nrhs;
-            double nrm = 0.0;
+        for (int grp = 0; grp * RY * R < nrhs; grp++) {
+            const int rhs0 = (grp * RY + ty) * R;
+            const bool act = live && rhs0 < nrhs;      // R divides nrhs: a row is wholly inside or outside
+            double nrm[R];
+#pragma unroll
+            for (int r = 0; r < R; r++) nrm[r] = 0.0;
             if (act) {
-                const char* in = (const char*)in_ + fb * rhs;
-                float acc[24];
+                const char* in = (const char*)in_ + fb * rhs0;
+                float acc[R][24];
 #pragma unroll
-                for (int k = 0; k < 24; k++) acc[k] = 0.f;
-                hop_direction_s<PREC, RECON, DAGGER, 0>(links, tx, in, nb, ph_f, ph_b, acc);
-                hop_direction_s<PREC, RECON, DAGGER, 1>(links, tx, in, nb, ph_f, ph_b, acc);
-                hop_direction_s<PREC, RECON, DAGGER, 2>(links, tx, in, nb, ph_f, ph_b, acc);
-                hop_direction_s<PREC, RECON, DAGGER, 3>(links, tx, in, nb, ph_f, ph_b, acc);
-                float o[24];
-                if (d_real) { cscale_real_f32<6>(cdur, acc, o); cscale_real_f32<6>(cdlr, acc + 12, o + 12); }   // Td real (-kappa^2)
-                else { cscale_f32<6>(cdur, cdui, acc, o); cscale_f32<6>(cdlr, cdli, acc + 12, o + 12); }
-                if (XPAY) {
-                    float xv[24];
-                    load_spinor<PREC>((const char*)x_ + fb * rhs, i, xv);
-                    caxpy_f32<6>(cxur, cxui, xv, o);
-                    caxpy_f32<6>(cxlr, cxli, xv + 12, o + 12);
-                }
-                if (EPI == EPI_RESID) {   // out_ is r: r -= alpha q, |r|^2 (q itself is never stored)
-                    const float alpha = (float)cg->alpha[rhs];
-                    float rv[24];
-                    load_spinor<PR, false>((const char*)out_ + fbo * rhs, i, rv);   // coherent load: r is rewritten below
-                    raxpy_f32<12>(-alpha, o, rv);
-                    nrm += norm2_site(rv);
-                    store_spinor<PR>((char*)out_ + fbo * rhs, i, rv);
-                } else {
-                    store_spinor<PREC>((char*)out_ + fbo * rhs, i, o);
-                }
-                if (EPI == EPI_NORM) {
-                    if (PREC == TSM_BF16) {   // the norm of what was stored, i.e. of the vector the solver uses
-                        float ob[24];
+                for (int r = 0; r < R; r++)
 #pragma unroll
-                        for (int k8 = 0; k8 < 3; k8++) { const uint4 pk = float_to_bf16x8(o + 8 * k8); bf16x8_to_float(pk, ob + 8 * k8); }
-                        nrm += norm2_site(ob);
+                    for (int k = 0; k < 24; k++) acc[r][k] = 0.f;
+                hop_direction_r<PREC, RECON, DAGGER, 0, R>(links, tx, in, fb, nb, ph_f, ph_b, acc);
+                hop_direction_r<PREC, RECON, DAGGER, 1, R>(links, tx, in, fb, nb, ph_f, ph_b, acc);
+                hop_direction_r<PREC, RECON, DAGGER, 2, R>(links, tx, in, fb, nb, ph_f, ph_b, acc);
+                hop_direction_r<PREC, RECON, DAGGER, 3, R>(links, tx, in, fb, nb, ph_f, ph_b, acc);
+#pragma unroll
+                for (int r = 0; r < R; r++) {
+                    float o[24];
+                    if (d_real) { cscale_real_f32<6>(cdur, acc[r], o); cscale_real_f32<6>(cdlr, acc[r] + 12, o + 12); }   // Td real (-kappa^2)
+                    else { cscale_f32<6>(cdur, cdui, acc[r], o); cscale_f32<6>(cdlr, cdli, acc[r] + 12, o + 12); }
+                    if (XPAY) {
+                        float xv[24];
+                        load_spinor<PREC>((const char*)x_ + fb * (rhs0 + r), i, xv);
+                        caxpy_f32<6>(cxur, cxui, xv, o);
+                        caxpy_f32<6>(cxlr, cxli, xv + 12, o + 12);
+                    }
+                    if (EPI == EPI_RESID) {   // out_ is r: r -= alpha q, |r|^2 (q itself is never stored)
+                        const float alpha = (float)cg->alpha[rhs0 + r];
+                        float rv[24];
+                        load_spinor<PR, false>((const char*)out_ + fbo * (rhs0 + r), i, rv);   // coherent load: r is rewritten below
+                        raxpy_f32<12>(-alpha, o, rv);
+                        nrm[r] += norm2_site(rv);
+                        store_spinor<PR>((char*)out_ + fbo * (rhs0 + r), i, rv);
                     } else {
-                        nrm += norm2_site(o);
+                        store_spinor<PREC>((char*)out_ + fbo * (rhs0 + r), i, o);
+                    }
+                    if (EPI == EPI_NORM) {
+                        if (PREC == TSM_BF16) {   // the norm of what was stored, i.e. of the vector the solver uses
+                            float ob[24];
+#pragma unroll
+                            for (int k8 = 0; k8 < 3; k8++) { const uint4 pk = float_to_bf16x8(o + 8 * k8); bf16x8_to_float(pk, ob + 8 * k8); }
+                            nrm[r] += norm2_site(ob);
+                        } else {
+                            nrm[r] += norm2_site(o);
+                        }
                     }
                 }
             }
-            if (EPI != EPI_NONE && rhs < nrhs) {
+            if (EPI != EPI_NONE && rhs0 < nrhs) {
                 // sum over the row's 128 sites in a fixed order (A19): shuffle tree per warp, then the 4 warps;
                 // only this row's 4 warps synchronise (named barrier), the other rows run on.  `red` is
                 // double-buffered by group parity; a tile ends with __syncthreads().
-                double* w = red + (ty * 2 + (grp & 1)) * 4;
-                const double v = warp_sum(nrm);
-                if ((tx & 31) == 0) w[tx >> 5] = v;
+                double* w = red + (ty * 2 + (grp & 1)) * 4 * R;
+#pragma unroll
+                for (int r = 0; r < R; r++) {
+                    const double v = warp_sum(nrm[r]);
+                    if ((tx & 31) == 0) w[(tx >> 5) * R + r] = v;
+                }
                 row_barrier(1 + ty, TT);
-                if (tx == 0) partials[(size_t)rhs * ntiles + tile] = ((w[0] + w[1]) + w[2]) + w[3];
+                if (tx < R) partials[(size_t)(rhs0 + tx) * ntiles + tile] = ((w[tx] + w[R + tx]) + w[2 * R + tx]) + w[3 * R + tx];
             }
         }
         __syncthreads();
@@ -219,13 +234,13 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
     }
 }
 
-template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI, int RY>
+template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI, int RY, int R>
 int launch_tile_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void* in, const void* x, void* out, const DslashCoef& c,
                   int check_done)
 {
     constexpr int NCH = RECON == 18 ? 36 : 24;
     const size_t SMEM = (size_t)2 * 4 * NCH * LB_ROW;   // two link buffers: the next tile's copy overlaps this tile's arithmetic (1 buffer: 799 vs 725 us)
-    auto kern = k_dslash_tile<PREC, RECON, DAGGER, XPAY, EPI, RY>;
+    auto kern = k_dslash_tile<PREC, RECON, DAGGER, XPAY, EPI, RY, R>;
     static unsigned long long attr_done = 0;   // per device
     if (!((attr_done >> (ctx->device & 63)) & 1ull)) {
         TSM_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
@@ -248,53 +263,64 @@ int launch_tile_t(tsm_ctx* ctx, int par, int nrhs, const void* pack, const void*
     return TSM_OK;
 }
 
-template <int PREC, int RECON, int RY>
+template <int PREC, int RECON, int RY, int R>
 int launch_tile_v(tsm_ctx* ctx, int par, bool dagger, int nrhs, const void* pack, const void* in, const void* x, void* out,
                   const DslashCoef& c, int epi, int check_done)
 {
     const bool xpay = x != nullptr;
-#define GO(DG, XP, EP) return launch_tile_t<PREC, RECON, DG, XP, EP, RY>(ctx, par, nrhs, pack, in, x, out, c, check_done)
+#define GO(DG, XP, EP) return launch_tile_t<PREC, RECON, DG, XP, EP, RY, R>(ctx, par, nrhs, pack, in, x, out, c, check_done)
     if (!dagger && !xpay && epi == EPI_NONE) GO(false, false, EPI_NONE);
-    if (!dagger && xpay && epi == EPI_NONE) GO(false, true, EPI_NONE);
     if (dagger && !xpay && epi == EPI_NONE) GO(true, false, EPI_NONE);
-    if (dagger && xpay && epi == EPI_NONE) GO(true, true, EPI_NONE);
-    if (!dagger && xpay && epi == EPI_NORM) GO(false, true, EPI_NORM);
-    if (dagger && xpay && epi == EPI_RESID) GO(true, true, EPI_RESID);
+    if constexpr (R == 1) {   // two sources per thread only serve the plain launches
+        if (!dagger && xpay && epi == EPI_NONE) GO(false, true, EPI_NONE);
+        if (dagger && xpay && epi == EPI_NONE) GO(true, true, EPI_NONE);
+        if (!dagger && xpay && epi == EPI_NORM) GO(false, true, EPI_NORM);
+        if (dagger && xpay && epi == EPI_RESID) GO(true, true, EPI_RESID);
+    }
 #undef GO
     return tsm_fail(ctx, TSM_EINVAL, "unsupported dslash variant");
 }
 
 template <int PREC, int RECON>
-int launch_tile_s(tsm_ctx* ctx, int ry, int par, bool dagger, int nrhs, const void* pack, const void* in, const void* x,
+int launch_tile_s(tsm_ctx* ctx, int ry, int r, int par, bool dagger, int nrhs, const void* pack, const void* in, const void* x,
                   void* out, const DslashCoef& c, int epi, int check_done)
 {
-#define SHAPE(RY_) if (ry == RY_) return launch_tile_v<PREC, RECON, RY_>(ctx, par, dagger, nrhs, pack, in, x, out, c, epi, check_done)
-    SHAPE(4);
-    SHAPE(2);
-    SHAPE(1);
+#define SHAPE(RY_, R_) if (ry == RY_ && r == R_) return launch_tile_v<PREC, RECON, RY_, R_>(ctx, par, dagger, nrhs, pack, in, x, out, c, epi, check_done)
+    SHAPE(4, 1);
+    SHAPE(3, 2);
+    SHAPE(2, 1);
+    SHAPE(1, 1);
 #undef SHAPE
     return tsm_fail(ctx, TSM_EINVAL, "unsupported tile shape");
 }
 
 }  // namespace
 
-// Source rows of the CTA for a batch of nrhs sources
-static int tile_rows(int nrhs) { return nrhs == 1 ? 1 : (nrhs == 2 ? 2 : 4); }
+// Shape of the CTA for a batch of nrhs sources: RY source rows x R sources per thread; R divides nrhs.  A source's
+// result is the same in every shape (the same operations in the same order per source).
+static void tile_shape(int nrhs, bool plain, int& ry, int& r)
+{
+    if (nrhs == 1) { ry = 1; r = 1; return; }
+    if (nrhs == 2) { ry = 2; r = 1; return; }
+    if (plain && nrhs % 6 == 0) { ry = 3; r = 2; return; }
+    ry = 4; r = 1;
+}
 
 // fp32 / bf16 storage, any nrhs >= 1.  mode bits as in launch_dslash.
 int launch_dslash_tile(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int nrhs, const void* in, const void* x, void* out,
                        const DslashCoef& c, int mode)
 {
     const int chk = (mode >> 1) & 1, nm = (mode & 4) ? EPI_RESID : ((mode & 1) ? EPI_NORM : EPI_NONE);
-    const int ry = tile_rows(nrhs);
+    int ry, r;
+    tile_shape(nrhs, x == nullptr && nm == EPI_NONE, ry, r);
     const void* pack = ctx->gauge32[out_parity];
     if (prec == TSM_F32) {
-        if (ctx->recon == 18) return launch_tile_s<TSM_F32, 18>(ctx, ry, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk);
-        return launch_tile_s<TSM_F32, 12>(ctx, ry, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk);
+        if (ctx->recon == 18) return launch_tile_s<TSM_F32, 18>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk);
+        return launch_tile_s<TSM_F32, 12>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk);
     }
     if (prec == TSM_BF16) {
-        if (ctx->recon == 18) return launch_tile_s<TSM_BF16, 18>(ctx, ry, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk);
-        return launch_tile_s<TSM_BF16, 12>(ctx, ry, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk);
+        if (ctx->recon == 18) return launch_tile_s<TSM_BF16, 18>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk);
+        return launch_tile_s<TSM_BF16, 12>(ctx, ry, r, out_parity, dagger, nrhs, pack, in, x, out, c, nm, chk);
     }
     return tsm_fail(ctx, TSM_EINVAL, "tile stencil: unsupported precision");
 }

@@ -145,9 +145,55 @@ def launch_list(path, out_md, out_csv, title, command, note):
             f.write(f'{k},"{name}",{us:.2f}\n')
 
 
+def sass_histogram(path, out_md, title, command, note, units, inst_executed=0.0):
+    """`ncu -i x.ncu-rep --page source --csv [--kernel-name ... --launch-skip k --launch-count 1]` -> executed warp
+    instructions per opcode and per `units` / 32 warp-units, the share of stall samples per opcode, and for the memory
+    opcodes the L1 tag requests (global) or wavefronts (shared) per executed instruction."""
+    import re
+    rows = list(csv.reader(open(path)))
+    kernel = rows[0][1] if rows and len(rows[0]) > 1 else ""
+    hdr = next(r for r in rows if r and r[0] == "Address")
+    ix = {n: i for i, n in enumerate(hdr)}
+    data = [r for r in rows[rows.index(hdr) + 1:] if len(r) >= len(hdr) and to_float(r[ix["Instructions Executed"]]) is not None]
+    ex, samp, tags, wav = {}, {}, {}, {}
+    for r in data:
+        m = re.match(r"\s*(@!?U?P\d+\s+)?([A-Z0-9_.]+)", r[ix["Source"]])
+        op = (m.group(2) if m else "?").split(".")[0]
+        n = to_float(r[ix["Instructions Executed"]])
+        ex[op] = ex.get(op, 0.0) + n
+        samp[op] = samp.get(op, 0.0) + (to_float(r[ix["# Samples"]]) or 0.0)
+        tags[op] = tags.get(op, 0.0) + (to_float(r[ix["L1 Tag Requests Global"]]) or 0.0)
+        wav[op] = wav.get(op, 0.0) + (to_float(r[ix["L1 Wavefronts Shared"]]) or 0.0)
+    tot, ns, wu = sum(ex.values()), sum(samp.values()) or 1.0, units / 32.0
+    # the source page can count a launch's instructions more than once (it did, twice, for the persistent tile kernel):
+    # normalise to smsp__inst_executed.sum of the same launch when given
+    if inst_executed > 0:
+        f = inst_executed / tot
+        ex = {k: v * f for k, v in ex.items()}
+        tags = {k: v * f for k, v in tags.items()}
+        wav = {k: v * f for k, v in wav.items()}
+        tot = inst_executed
+    text = f"# {title}\n\n"
+    if command:
+        text += f"Command:\n\n    {command}\n\n"
+    text += f"Kernel: `{kernel.replace('void <unnamed>::', '').split('(Geom')[0]}`; {tot:.4g} warp instructions = {tot / wu:.1f} per 32 units ({units} units).\n\n"
+    text += "| opcode | per 32 units | share of instructions | share of stall samples | L1 tag requests / shared wavefronts per instruction |\n|---|---|---|---|---|\n"
+    for op in sorted(ex, key=lambda k: -ex[k]):
+        if ex[op] / tot < 0.002:
+            continue
+        mem = f"{tags[op] / ex[op]:.2f} tags" if tags[op] else (f"{wav[op] / ex[op]:.2f} wavefronts" if wav[op] else "")
+        text += f"| {op} | {ex[op] / wu:.1f} | {100 * ex[op] / tot:.1f} % | {100 * samp[op] / ns:.1f} % | {mem} |\n"
+    if note:
+        text += "\n" + note + "\n"
+    with open(out_md, "w") as f:
+        f.write(text)
+
+
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("csv")
+    ap.add_argument("--sass-histogram", type=int, metavar="UNITS", help="treat `csv` as an ncu source-page csv of ONE launch that processed UNITS (site, source) units; markdown to --out")
+    ap.add_argument("--inst-executed", type=float, default=0.0, help="smsp__inst_executed.sum of that launch (raw page): the histogram is normalised to it")
     ap.add_argument("--launch-list", help="treat `csv` as an ncu gpu__time_duration log; write the reduced csv here (markdown to --out)")
     ap.add_argument("--out", help="markdown file to write (default: stdout)")
     ap.add_argument("--title", default="ncu summary")
@@ -157,6 +203,11 @@ def main():
     ap.add_argument("--key", help="entry of the JSON file: workload/prec/nrhsN")
     ap.add_argument("--commit", default="", help="commit of the kernels the capture was taken at")
     a = ap.parse_args()
+    if a.sass_histogram:
+        if not a.out:
+            raise SystemExit("--sass-histogram needs --out")
+        sass_histogram(a.csv, a.out, a.title, a.command, a.note, a.sass_histogram, a.inst_executed)
+        return
     if a.launch_list:
         if not a.out:
             raise SystemExit("--launch-list needs --out")
