@@ -13,8 +13,11 @@
 // G = ceil(nrhs / (RY * R)) groups of sources.  Neighbour spinors come through L1/L2 (ld.global.nc).
 // Shapes in use (measured at 32^3 x 64, 12 sources, inside the CG): the plain launches
 // (no x term, no epilogue) run 3 rows x 2 sources per thread (168 registers, 12 warps: 821 us against 882 us
-// for 4 x 1), every launch with an x term or an epilogue 4 rows x 1 source (128 registers, 16 warps: the second
-// source's x / r vectors do not fit beside the accumulators, 1113-1243 us against 1008-1121 us).
+// for 4 x 1); the launches with an x term or an epilogue run 3 rows x 1 source (168 registers, 12 warps) and request
+// the own-site x / r vectors BEFORE the hops, so that those first-touch DRAM streams are in flight during the
+// gathers (S2 1039 -> 978 us, S4 1112 -> 1047 us against 4 rows x 1 source with the loads in the epilogue; with two
+// sources per thread they were 1113-1243 us: the second source's x / r vectors do not fit beside the accumulators).
+// Batches whose size is not a multiple of 3 keep 4 rows x 1 source.
 //
 // Arithmetic per source is the same sequence of operations as in dslash.cu (same projection,
 // same FMA chains, same accumulation order over mu), so a source's result does not depend on the
@@ -170,6 +173,12 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
                 for (int r = 0; r < R; r++)
 #pragma unroll
                     for (int k = 0; k < 24; k++) acc[r][k] = 0.f;
+                // 3 rows x 1 source: the registers that 12 warps leave free hold the epilogue's own-site inputs, requested
+                // now (EARLY); otherwise they are loaded where they are used
+                constexpr bool EARLY = RY == 3 && R == 1 && (XPAY || EPI == EPI_RESID);
+                float xe[EARLY && XPAY ? 24 : 1], rve[EARLY && EPI == EPI_RESID ? 24 : 1];
+                if constexpr (EARLY && XPAY) load_spinor<PREC>((const char*)x_ + fb * rhs0, i, xe);
+                if constexpr (EARLY && EPI == EPI_RESID) load_spinor<PR, false>((const char*)out_ + fbo * rhs0, i, rve);   // coherent: r is rewritten below
                 hop_direction_r<PREC, RECON, DAGGER, 0, R>(links, tx, in, fb, nb, ph_f, ph_b, acc);
                 hop_direction_r<PREC, RECON, DAGGER, 1, R>(links, tx, in, fb, nb, ph_f, ph_b, acc);
                 hop_direction_r<PREC, RECON, DAGGER, 2, R>(links, tx, in, fb, nb, ph_f, ph_b, acc);
@@ -181,14 +190,24 @@ k_dslash_tile(const Geom g, const int par, const int nrhs, const int ntiles, con
                     else { cscale_f32<6>(cdur, cdui, acc[r], o); cscale_f32<6>(cdlr, cdli, acc[r] + 12, o + 12); }
                     if (XPAY) {
                         float xv[24];
-                        load_spinor<PREC>((const char*)x_ + fb * (rhs0 + r), i, xv);
+                        if constexpr (EARLY) {
+#pragma unroll
+                            for (int k = 0; k < 24; k++) xv[k] = xe[k];
+                        } else {
+                            load_spinor<PREC>((const char*)x_ + fb * (rhs0 + r), i, xv);
+                        }
                         caxpy_f32<6>(cxur, cxui, xv, o);
                         caxpy_f32<6>(cxlr, cxli, xv + 12, o + 12);
                     }
                     if (EPI == EPI_RESID) {   // out_ is r: r -= alpha q, |r|^2 (q itself is never stored)
                         const float alpha = (float)cg->alpha[rhs0 + r];
                         float rv[24];
-                        load_spinor<PR, false>((const char*)out_ + fbo * (rhs0 + r), i, rv);   // coherent load: r is rewritten below
+                        if constexpr (EARLY) {
+#pragma unroll
+                            for (int k = 0; k < 24; k++) rv[k] = rve[k];
+                        } else {
+                            load_spinor<PR, false>((const char*)out_ + fbo * (rhs0 + r), i, rv);   // coherent load: r is rewritten below
+                        }
                         raxpy_f32<12>(-alpha, o, rv);
                         nrm[r] += norm2_site(rv);
                         store_spinor<PR>((char*)out_ + fbo * (rhs0 + r), i, rv);
@@ -269,9 +288,11 @@ int launch_tile_v(tsm_ctx* ctx, int par, bool dagger, int nrhs, const void* pack
 {
     const bool xpay = x != nullptr;
 #define GO(DG, XP, EP) return launch_tile_t<PREC, RECON, DG, XP, EP, RY, R>(ctx, par, nrhs, pack, in, x, out, c, check_done)
-    if (!dagger && !xpay && epi == EPI_NONE) GO(false, false, EPI_NONE);
-    if (dagger && !xpay && epi == EPI_NONE) GO(true, false, EPI_NONE);
-    if constexpr (R == 1) {   // two sources per thread only serve the plain launches
+    if constexpr (!(RY == 3 && R == 1)) {   // plain launches: every shape but 3 x 1 (tile_shape)
+        if (!dagger && !xpay && epi == EPI_NONE) GO(false, false, EPI_NONE);
+        if (dagger && !xpay && epi == EPI_NONE) GO(true, false, EPI_NONE);
+    }
+    if constexpr (R == 1) {   // x term / epilogues: one source per thread
         if (!dagger && xpay && epi == EPI_NONE) GO(false, true, EPI_NONE);
         if (dagger && xpay && epi == EPI_NONE) GO(true, true, EPI_NONE);
         if (!dagger && xpay && epi == EPI_NORM) GO(false, true, EPI_NORM);
@@ -288,6 +309,7 @@ int launch_tile_s(tsm_ctx* ctx, int ry, int r, int par, bool dagger, int nrhs, c
 #define SHAPE(RY_, R_) if (ry == RY_ && r == R_) return launch_tile_v<PREC, RECON, RY_, R_>(ctx, par, dagger, nrhs, pack, in, x, out, c, epi, check_done)
     SHAPE(4, 1);
     SHAPE(3, 2);
+    SHAPE(3, 1);
     SHAPE(2, 1);
     SHAPE(1, 1);
 #undef SHAPE
@@ -303,6 +325,7 @@ static void tile_shape(int nrhs, bool plain, int& ry, int& r)
     if (nrhs == 1) { ry = 1; r = 1; return; }
     if (nrhs == 2) { ry = 2; r = 1; return; }
     if (plain && nrhs % 6 == 0) { ry = 3; r = 2; return; }
+    if (!plain && nrhs % 3 == 0) { ry = 3; r = 1; return; }
     ry = 4; r = 1;
 }
 
