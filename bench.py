@@ -367,6 +367,16 @@ def workload_summary(cfg: int, tsm, torch, peak, with_oracle: bool):
     torch.cuda.synchronize()
     out["lp_solves_per_s"] = nb / (e0.elapsed_time(e1) * 1e-3)
     out["lp_iters"] = sorted(set(i["iters"] for i in info))
+    # the same steps only ENQUEUED (tsm_solve_async; what tsm_run_loop_set does for its LP-only batches): the host runs
+    # ahead of the device, one wait at the end
+    e0.record(stream)
+    for k in range(steps):
+        t.solve_async(wl.noise_seed, list(range(2000 + k * wl.nrhs, 2000 + (k + 1) * wl.nrhs)), prec, wl.lp_tol, wl.lp_iters, slot=1)
+        t.loops_add_lp(1)
+    e1.record(stream)
+    rc, info = t.solve_wait(1)
+    torch.cuda.synchronize()
+    out["lp_solves_per_s_enqueued"] = nb / (e0.elapsed_time(e1) * 1e-3)
     loops, secs, rc = t.run_loop_set(wl.noise_seed, wl.n_hp, wl.n_lp, prec, wl.lp_tol, wl.lp_iters, hp_tol=wl.hp_tol,
                                      hp_max_iter=5000, nrhs=wl.nrhs, with_derivative=wl.derivative)
     out["tsm_loop_set"] = {"seconds": secs, "n_hp": wl.n_hp, "n_lp": wl.n_lp, "rc": rc, "hp_solver": t.hp_precision_name(),

@@ -148,6 +148,16 @@ typedef struct {
 int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs, int kind,
               int prec, double tol, int max_iter, int slot, int want_true_resid,
               tsm_solve_info* info);
+/* tsm_solve without the wait: tsm_solve_async only ENQUEUES the solve on the context's stream (no host synchronisation:
+ * in residual mode the stopping test runs on the device, tsm_set_graphs mode 2; TSM_MIXED still reads its outer-loop
+ * state on the host) and returns TSM_OK or an argument / state error; the slot may be used by later calls on the same
+ * stream (tsm_loops_add_lp, ...) at once.  tsm_solve_wait synchronises and reports on the solve LAST enqueued into
+ * `slot` exactly as tsm_solve would have (TSM_ESTATE if none is pending).  tsm_solve == tsm_solve_async with host
+ * polling allowed + tsm_solve_wait; the iterates are bit-identical. */
+int tsm_solve_async(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs, int kind, int prec, double tol,
+                    int max_iter, int slot);
+int tsm_solve_wait(tsm_ctx* ctx, int slot, int want_true_resid, tsm_solve_info* info);
+
 int tsm_get_solution(tsm_ctx* ctx, int slot, int rhs, double* host_out /* [V][4][3][2] */);
 /* Overwrite the solution held in a slot (contraction parity with the oracle's s, A16(i));
  * the slot keeps the seed/source ids/kind/nrhs of the last tsm_solve into it. */

@@ -129,6 +129,11 @@ int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
     ok = ok && cudaMalloc(&ctx->cg, sizeof(CgScalars)) == cudaSuccess;
     ok = ok && cudaMemset(ctx->cg, 0, sizeof(CgScalars)) == cudaSuccess;
     ok = ok && cudaMallocHost(&ctx->cg_host, sizeof(CgScalars)) == cudaSuccess;
+    for (int s = 0; s < 2; s++) {
+        ctx->cg_snap[s] = nullptr; ctx->slot_ev0[s] = ctx->slot_ev1[s] = nullptr; ctx->slot_pending[s] = false; ctx->slot_loop_per_pass[s] = 0;
+        ok = ok && cudaMallocHost(&ctx->cg_snap[s], sizeof(CgScalars)) == cudaSuccess;
+        ok = ok && cudaEventCreate(&ctx->slot_ev0[s]) == cudaSuccess && cudaEventCreate(&ctx->slot_ev1[s]) == cudaSuccess;
+    }
     const size_t hs = (size_t)TSM_MAX_OPS * dims[3] * 2 * sizeof(double) * 2 + 256;
     ok = ok && cudaMallocHost(&ctx->host_small, hs) == cudaSuccess;
     ok = ok && cudaMalloc(&ctx->ids_dev, 2 * TSM_MAX_NRHS * sizeof(uint32_t)) == cudaSuccess;
@@ -148,6 +153,11 @@ int tsm_destroy(tsm_ctx* ctx)
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->cg) cudaFree(ctx->cg);
     if (ctx->cg_host) cudaFreeHost(ctx->cg_host);
+    for (int s = 0; s < 2; s++) {
+        if (ctx->cg_snap[s]) cudaFreeHost(ctx->cg_snap[s]);
+        if (ctx->slot_ev0[s]) cudaEventDestroy(ctx->slot_ev0[s]);
+        if (ctx->slot_ev1[s]) cudaEventDestroy(ctx->slot_ev1[s]);
+    }
     if (ctx->host_small) cudaFreeHost(ctx->host_small);
     if (ctx->ids_dev) cudaFree(ctx->ids_dev);
     for (ProfRec& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }

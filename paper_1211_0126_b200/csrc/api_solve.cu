@@ -167,7 +167,8 @@ int fetch_scalars(tsm_ctx* ctx)
 }
 
 // `max_iter` CG iterations at most, in chunks of 4; residual mode polls the all-done flag after each chunk.
-int cg_run(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, void* r, void* p, void* w, void* t, double tol, int max_iter)
+int cg_run(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, void* r, void* p, void* w, void* t, double tol, int max_iter,
+           bool no_poll = false)
 {
     // iterations run in chunks of `poll`; in residual mode the host reads the all-done flag after each chunk
     // (a finished batch makes every later kernel return at once), in fixed-iteration mode it never does.
@@ -176,7 +177,7 @@ int cg_run(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, void* r,
     int rc;
     const int poll = 4;
     const bool use_graph = graphs_enabled(ctx);
-    if (use_graph && ctx->graphs_on == 2) {
+    if (use_graph && (ctx->graphs_on == 2 || (no_poll && tol > 0))) {   // an enqueue-only solve in residual mode must not poll
         // device-side loop: the first iteration of an argument set runs kernel by kernel (kernel attributes
         // cannot be set inside a capture), everything after it is one graph launch
         int k = 0;
@@ -294,20 +295,19 @@ int check_slot(tsm_ctx* ctx, int slot, int rhs)
     return TSM_OK;
 }
 
-}  // namespace
-
-extern "C" {
-
-int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs, int kind, int prec, double tol,
-              int max_iter, int slot, int want_true_resid, tsm_solve_info* info)
+// Everything a solve puts on the stream: noise, source preparation, CG, reconstruction, and a pinned snapshot of the
+// CG scalars for solve_collect.  no_poll: never synchronise with the host (residual mode then runs the device-side
+// iteration loop; the mixed-precision solver still reads its outer-loop state on the host).
+int solve_enqueue(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs, int kind, int prec, double tol, int max_iter, int slot,
+                  bool no_poll)
 {
     int rc = ctx_enter(ctx, true, true, true);
     if (rc) return rc;
     if (!source_ids || nrhs < 1 || nrhs > ctx->max_nrhs || (kind != TSM_Z4 && kind != TSM_Z2) || prec < 0 || prec > TSM_MIXED ||
         !(tol >= 0) || max_iter < 0 || slot < 0 || slot > 1 || (prec == TSM_MIXED && !(tol > 0)))
         return tsm_fail(ctx, TSM_EINVAL, "bad solve arguments");
-    if (ctx->ws_prec != TSM_F64 && (prec == TSM_F64 || prec == TSM_MIXED || want_true_resid))
-        return tsm_fail(ctx, TSM_ESTATE, "fp64 solve or fp64 true residual on a low-precision-only workspace (tsm_set_workspace prec)");
+    if (ctx->ws_prec != TSM_F64 && (prec == TSM_F64 || prec == TSM_MIXED))
+        return tsm_fail(ctx, TSM_ESTATE, "fp64 solve on a low-precision-only workspace (tsm_set_workspace prec)");
     // bf16 storage (config 4): source preparation, x, r, q, reconstruction and the stored solution are
     // fp32; only the search direction p and the stencil temporaries t, w are bf16 (fp32 arithmetic).
     const int sp = prec == TSM_BF16 ? TSM_F32 : (prec == TSM_MIXED ? TSM_F64 : prec);   // precision of the stored solution
@@ -320,7 +320,8 @@ int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs,
     memcpy(ctx->slot_ids[slot], source_ids, nrhs * sizeof(uint32_t));
     uint32_t* ids_dev = ctx->ids_dev + slot * TSM_MAX_NRHS;
     TSM_CUDA(ctx, cudaMemcpyAsync(ids_dev, ctx->slot_ids[slot], nrhs * sizeof(uint32_t), cudaMemcpyHostToDevice, ctx->stream));
-    TSM_CUDA(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
+    TSM_CUDA(ctx, cudaEventRecord(ctx->slot_ev0[slot], ctx->stream));
+    ctx->loop_per_pass = 0;
 
     char* s_e = (char*)ctx->slot[slot];
     char* s_o = s_e + field_bytes(sp, Vh, nrhs);
@@ -343,7 +344,7 @@ int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs,
             if ((rc = solve_mixed(ctx, nrhs, tw, s_e, tol, max_iter))) return rc;
         } else {
             if ((rc = launch_cg_init(ctx, prec, nrhs, r, p, x))) return rc;
-            if ((rc = cg_run(ctx, prec, nrhs, tw, x, r, p, w, t, tol, max_iter))) return rc;
+            if ((rc = cg_run(ctx, prec, nrhs, tw, x, r, p, w, t, tol, max_iter, no_poll))) return rc;
         }
     }
     {   // H7: s_e = x, s_o = R^-1 (eta_o + kappa D_oe x)
@@ -351,11 +352,37 @@ int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs,
         if ((rc = launch_dslash(ctx, sp, 1, false, nrhs, x, s_o, aux, {tw.Rinv, tw.kRinv}, 0))) return rc;
         TSM_CUDA(ctx, cudaMemcpyAsync(s_o, aux, field_bytes(sp, Vh, nrhs), cudaMemcpyDeviceToDevice, ctx->stream));
     }
-    TSM_CUDA(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
-    if ((rc = fetch_scalars(ctx))) return rc;
+    TSM_CUDA(ctx, cudaEventRecord(ctx->slot_ev1[slot], ctx->stream));
+    TSM_CUDA(ctx, cudaMemcpyAsync(ctx->cg_snap[slot], ctx->cg, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx->stream));
+    ctx->slot_tol[slot] = tol;
+    ctx->slot_pending[slot] = true;
+    ctx->slot_loop_per_pass[slot] = ctx->loop_per_pass;   // a device-side loop of this solve whose passes are not yet counted
+    ctx->slot_loop_eager[slot] = ctx->loop_eager;
+    ctx->loop_per_pass = 0;
+    return TSM_OK;
+}
+
+// Waits for the solve last enqueued into `slot` and reports on it (iteration counts, status, residuals, time).
+int solve_collect(tsm_ctx* ctx, int slot, int want_true_resid, tsm_solve_info* info)
+{
+    int rc;
+    if (slot < 0 || slot > 1 || !ctx->slot_pending[slot]) return tsm_fail(ctx, TSM_ESTATE, "no solve is pending on this slot");
+    if (want_true_resid && ctx->ws_prec != TSM_F64)
+        return tsm_fail(ctx, TSM_ESTATE, "fp64 true residual on a low-precision-only workspace (tsm_set_workspace prec)");
+    TSM_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->slot_pending[slot] = false;
+    const CgScalars sc = *ctx->cg_snap[slot];
+    const int nrhs = ctx->slot_nrhs[slot];
+    const double tol = ctx->slot_tol[slot];
+    if (ctx->slot_loop_per_pass[slot] > 0) {   // settle the launch count of the solve's device-side loop
+        int most = 0;
+        for (int j = 0; j < nrhs; j++) most = sc.iters[j] > most ? sc.iters[j] : most;
+        const int passes = most - ctx->slot_loop_eager[slot];
+        if (passes > 1) ctx->launches += (long long)(passes - 1) * ctx->slot_loop_per_pass[slot];
+        ctx->slot_loop_per_pass[slot] = 0;
+    }
     float ms = 0;
-    TSM_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
-    const CgScalars sc = *ctx->cg_host;   // true_residuals() reuses the pinned copy
+    TSM_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->slot_ev0[slot], ctx->slot_ev1[slot]));
     double tr[TSM_MAX_NRHS];
     for (int j = 0; j < nrhs; j++) tr[j] = -1.0;
     if (want_true_resid && (rc = true_residuals(ctx, slot, tr))) return rc;
@@ -374,6 +401,33 @@ int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs,
     }
     if (first != TSM_OK) ctx->err = first == TSM_ENOCONV ? "tolerance not reached in max_iter" : "CG breakdown";
     return first;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tsm_solve(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs, int kind, int prec, double tol,
+              int max_iter, int slot, int want_true_resid, tsm_solve_info* info)
+{
+    if (ctx && want_true_resid && ctx->ws_prec != TSM_F64)
+        return tsm_fail(ctx, TSM_ESTATE, "fp64 true residual on a low-precision-only workspace (tsm_set_workspace prec)");
+    const int rc = solve_enqueue(ctx, seed, source_ids, nrhs, kind, prec, tol, max_iter, slot, false);
+    if (rc) return rc;
+    return solve_collect(ctx, slot, want_true_resid, info);
+}
+
+int tsm_solve_async(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int nrhs, int kind, int prec, double tol,
+                    int max_iter, int slot)
+{
+    return solve_enqueue(ctx, seed, source_ids, nrhs, kind, prec, tol, max_iter, slot, true);
+}
+
+int tsm_solve_wait(tsm_ctx* ctx, int slot, int want_true_resid, tsm_solve_info* info)
+{
+    const int rc = ctx_enter(ctx, true, true, true);
+    if (rc) return rc;
+    return solve_collect(ctx, slot, want_true_resid, info);
 }
 
 int tsm_get_solution(tsm_ctx* ctx, int slot, int rhs, double* host_out)
@@ -557,6 +611,7 @@ int tsm_run_loop_set(tsm_ctx* ctx, uint64_t seed, int kind, int n_hp, int n_lp, 
     TSM_CUDA(ctx, cudaEventCreate(&e1));
     TSM_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
     int worst = TSM_OK;
+    if (cudaMemsetAsync(&ctx->cg->sticky_breakdown, 0, sizeof(int), ctx->stream) != cudaSuccess) { rc = TSM_ECUDA; goto fail; }
     if ((rc = tsm_loops_reset(ctx, ops))) goto fail;
     for (int j0 = 0; j0 < n_hp + n_lp;) {
         const bool hp = j0 < n_hp;
@@ -569,16 +624,26 @@ int tsm_run_loop_set(tsm_ctx* ctx, uint64_t seed, int kind, int n_hp, int n_lp, 
             if (rc == TSM_ECUDA || rc == TSM_EINVAL || rc == TSM_ESTATE) goto fail;
             if (rc && !worst) worst = rc;
         }
-        rc = tsm_solve(ctx, seed, ids, nb, kind, lp_prec, lp_tol, lp_iters, 1, 0, nullptr);
-        // an LP solve that hits its iteration cap is still a valid truncated estimate
-        if (rc == TSM_ECUDA || rc == TSM_EINVAL || rc == TSM_ESTATE) goto fail;
-        if (rc == TSM_EBREAKDOWN && !worst) worst = rc;
+        if (hp) {
+            rc = tsm_solve(ctx, seed, ids, nb, kind, lp_prec, lp_tol, lp_iters, 1, 0, nullptr);
+            // an LP solve that hits its iteration cap is still a valid truncated estimate
+            if (rc == TSM_ECUDA || rc == TSM_EINVAL || rc == TSM_ESTATE) goto fail;
+            if (rc == TSM_EBREAKDOWN && !worst) worst = rc;
+        } else {
+            // LP-only batches are only enqueued: the host runs ahead of the device (on small lattices a solve is a few
+            // dozen launches of a few microseconds); a breakdown in any of them is read from a sticky flag at the end
+            rc = tsm_solve_async(ctx, seed, ids, nb, kind, lp_prec, lp_tol, lp_iters, 1);
+            if (rc) goto fail;
+        }
         rc = hp ? tsm_loops_add_correction(ctx, 0, 1) : tsm_loops_add_lp(ctx, 1);
         if (rc) goto fail;
         j0 += nb;
     }
     if ((rc = launch_finalize(ctx))) goto fail;
     TSM_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
+    if ((rc = fetch_scalars(ctx))) goto fail;
+    ctx->slot_pending[1] = false;
+    if (ctx->cg_host->sticky_breakdown && !worst) worst = TSM_EBREAKDOWN;
     if ((rc = tsm_loops_finalize(ctx, host_out))) goto fail;
     if (secs_out) {
         float ms = 0;

@@ -52,6 +52,7 @@ __device__ __forceinline__ void cg_after_reduction(int which, int rhs, double v,
         if (!(v > 0) || !isfinite(v) || !(rr > 0) || !isfinite(rr)) {
             cg->done[rhs] = 1;
             cg->status[rhs] = TSM_EBREAKDOWN;
+            cg->sticky_breakdown = 1;
         } else {
             alpha = rr / v;
         }

@@ -370,6 +370,7 @@ struct CgScalars {
     int done[TSM_MAX_NRHS];       // frozen: converged, broken down, or zero source
     int status[TSM_MAX_NRHS];
     int all_done;
+    int sticky_breakdown;         // set by any breakdown, cleared only by tsm_run_loop_set (its LP batches are not waited for one by one)
     int loop_left;                // iterations the device-side loop (WHILE node of the CG graph) may still run
     unsigned ticket;              // last-block counter, always left at 0
 };
@@ -420,7 +421,14 @@ struct tsm_ctx {
     int stencil_choice;              // tsm_set_stencil_kernel: 0 automatic, 1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box, 5 k_dslash_small
     int graphs_on;                   // tsm_set_graphs: 0 off, 1 chunks of 4 iterations, 2 device-side loop
     long long loop_per_pass;         // launch accounting of the last device-side loop: kernels per pass (0: none pending),
-    int loop_eager, loop_nrhs;       // iterations run before the loop, sources of that solve (settled in fetch_scalars)
+    int loop_eager, loop_nrhs;       // iterations run before the loop, sources of that solve (settled when the scalars are read)
+    // per solution slot: what tsm_solve_wait needs to report on a solve that was only enqueued (tsm_solve_async)
+    CgScalars* cg_snap[2];           // pinned copies of the CG scalars, made on the stream right after the solve
+    cudaEvent_t slot_ev0[2], slot_ev1[2];
+    double slot_tol[2];
+    bool slot_pending[2];
+    long long slot_loop_per_pass[2];
+    int slot_loop_eager[2];
     double kappa, mu;
     bool have_params, have_gauge, have_ws;
     int recon;                       // storage of the fp32 link copy (18 / 12)

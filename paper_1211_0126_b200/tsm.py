@@ -27,7 +27,7 @@ PREC = {"f64": F64, "f32": F32, "bf16": BF16, "mixed": MIXED}
 EXPORTS = [
     "tsm_create", "tsm_destroy", "tsm_last_error", "tsm_field_bytes", "tsm_workspace_bytes",
     "tsm_set_workspace", "tsm_set_stream", "tsm_set_params", "tsm_set_gauge", "tsm_noise",
-    "tsm_pack", "tsm_unpack", "tsm_dslash", "tsm_solve", "tsm_get_solution", "tsm_set_solution",
+    "tsm_pack", "tsm_unpack", "tsm_dslash", "tsm_solve", "tsm_solve_async", "tsm_solve_wait", "tsm_get_solution", "tsm_set_solution",
     "tsm_loops_reset", "tsm_loops_set_momenta", "tsm_loops_add_correction", "tsm_loops_add_lp", "tsm_loops_source",
     "tsm_loops_finalize", "tsm_loops_get_state", "tsm_loops_set_state", "tsm_run_loop_set",
     "tsm_set_hp_precision", "tsm_launch_count", "tsm_profile", "tsm_profile_read", "tsm_stencil_kernel_name",
@@ -77,6 +77,8 @@ def load_library():
     lib.tsm_unpack.argtypes = [vp, i, i, vp, dp]
     lib.tsm_dslash.argtypes = [vp, i, i, i, vp, vp]
     lib.tsm_solve.argtypes = [vp, u64, u32p, i, i, i, ctypes.c_double, i, i, i, ctypes.POINTER(SolveInfo)]
+    lib.tsm_solve_async.argtypes = [vp, u64, u32p, i, i, i, ctypes.c_double, i, i]
+    lib.tsm_solve_wait.argtypes = [vp, i, i, ctypes.POINTER(SolveInfo)]
     lib.tsm_get_solution.argtypes = [vp, i, i, dp]
     lib.tsm_set_solution.argtypes = [vp, i, i, dp]
     lib.tsm_loops_reset.argtypes = [vp, i]
@@ -261,6 +263,23 @@ class Tsm:
         arr = (ctypes.c_uint32 * n)(*ids)
         info = (SolveInfo * n)()
         rc = self.lib.tsm_solve(self._h, seed, arr, n, kind, prec, tol, max_iter, slot, int(want_true_resid), info)
+        self._check(rc, allow=(EBREAKDOWN, ENOCONV))
+        return rc, [dict(iters=x.iters, status=x.status, rel_resid_rec=x.rel_resid_rec,
+                         rel_resid_true=x.rel_resid_true, secs=x.secs) for x in info]
+
+    def solve_async(self, seed: int, source_ids, prec: int, tol: float, max_iter: int, slot: int = 0, kind: int = Z4):
+        """Enqueue a solve without waiting for it (tsm_solve_async); solve_wait(slot) reports on it later."""
+        ids = [int(s) for s in source_ids]
+        arr = (ctypes.c_uint32 * len(ids))(*ids)
+        self._pending_n = getattr(self, "_pending_n", {})
+        self._pending_n[slot] = len(ids)
+        self._check(self.lib.tsm_solve_async(self._h, seed, arr, len(ids), kind, prec, tol, max_iter, slot))
+
+    def solve_wait(self, slot: int = 0, want_true_resid: bool = False):
+        """(rc, [dict per source]) of the solve last enqueued into `slot`, as solve() would have returned it."""
+        n = getattr(self, "_pending_n", {}).get(slot, self.max_nrhs)
+        info = (SolveInfo * n)()
+        rc = self.lib.tsm_solve_wait(self._h, slot, int(want_true_resid), info)
         self._check(rc, allow=(EBREAKDOWN, ENOCONV))
         return rc, [dict(iters=x.iters, status=x.status, rel_resid_rec=x.rel_resid_rec,
                          rel_resid_true=x.rel_resid_true, secs=x.secs) for x in info]

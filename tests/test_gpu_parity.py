@@ -982,3 +982,29 @@ def test_small_lattice_stencil(tsm_mod, recon):
     rc, info = c.t.solve(9, [5, 6, 7], F32, 1e-4, 500, slot=0, want_true_resid=True)
     assert rc == 0 and all(i["rel_resid_true"] < 2e-4 for i in info)
     c.t.close()
+
+
+def test_async_solves_match_synchronous_ones(medium, tsm_mod):
+    """tsm_solve_async + tsm_solve_wait: the same iterates, iteration counts and statuses as tsm_solve, bit for bit, in
+    fixed-iteration and residual mode (there the stopping test runs on the device), with the next solve enqueued
+    before the first is waited for; the Eq. 2.4 set (whose LP-only batches are enqueued the same way) is unchanged;
+    waiting on a slot with nothing pending is an error."""
+    c = medium
+    for prec, tol, k in ((F32, 0.0, 11), (F32, 1e-4, 500), (F64, 1e-9, 2000), (BF16, 5e-3, 200)):
+        rc, info = c.t.solve(21, [0, 1, 2], prec, tol, k, slot=0)
+        want = [c.t.get_solution(0, j) for j in range(3)]
+        c.t.solve_async(21, [0, 1, 2], prec, tol, k, slot=1)
+        c.t.loops_reset(False)
+        c.t.loops_add_lp(1)                                  # uses the slot on the stream, no wait in between
+        c.t.solve_async(21, [7, 8, 9], prec, tol, k, slot=0)   # and the next solve is already enqueued
+        rc2, info2 = c.t.solve_wait(1)
+        assert rc2 == rc and [i["iters"] for i in info2] == [i["iters"] for i in info], (prec, tol)
+        assert [i["status"] for i in info2] == [i["status"] for i in info]
+        for j in range(3):
+            assert np.array_equal(c.t.get_solution(1, j), want[j]), (prec, tol, j)
+        rc3, info3 = c.t.solve_wait(0)
+        assert rc3 == 0 and len(info3) == 3
+    with pytest.raises(tsm_mod.TsmError) as e:
+        c.t.solve_wait(0)
+    assert e.value.code == tsm_mod.ESTATE
+    c.t.loops_reset(False)
