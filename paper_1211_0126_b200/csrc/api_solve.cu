@@ -611,10 +611,12 @@ int tsm_run_loop_set(tsm_ctx* ctx, uint64_t seed, int kind, int n_hp, int n_lp, 
     TSM_CUDA(ctx, cudaEventCreate(&e1));
     TSM_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
     int worst = TSM_OK;
-    if (cudaMemsetAsync(&ctx->cg->sticky_breakdown, 0, sizeof(int), ctx->stream) != cudaSuccess) { rc = TSM_ECUDA; goto fail; }
     if ((rc = tsm_loops_reset(ctx, ops))) goto fail;
     for (int j0 = 0; j0 < n_hp + n_lp;) {
         const bool hp = j0 < n_hp;
+        // the HP batches are waited for one by one (their status is known); the sticky flag only has to cover the
+        // LP-only batches that follow (an inner fp32 CG of the mixed-precision HP solver may set it harmlessly)
+        if (j0 == n_hp && cudaMemsetAsync(&ctx->cg->sticky_breakdown, 0, sizeof(int), ctx->stream) != cudaSuccess) { rc = TSM_ECUDA; goto fail; }
         const int end = hp ? n_hp : n_hp + n_lp;
         const int nb = (end - j0 < nrhs) ? end - j0 : nrhs;
         uint32_t ids[TSM_MAX_NRHS];
@@ -643,7 +645,7 @@ int tsm_run_loop_set(tsm_ctx* ctx, uint64_t seed, int kind, int n_hp, int n_lp, 
     TSM_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
     if ((rc = fetch_scalars(ctx))) goto fail;
     ctx->slot_pending[1] = false;
-    if (ctx->cg_host->sticky_breakdown && !worst) worst = TSM_EBREAKDOWN;
+    if (n_lp > 0 && ctx->cg_host->sticky_breakdown && !worst) worst = TSM_EBREAKDOWN;
     if ((rc = tsm_loops_finalize(ctx, host_out))) goto fail;
     if (secs_out) {
         float ms = 0;
