@@ -222,6 +222,22 @@ int tsm_set_graphs(tsm_ctx* ctx, int mode);
  * Allocates and frees its own small device buffers; blocks until done.  Not part of the hot path. */
 int tsm_probe_su3_tensor(tsm_ctx* ctx, int variant, int nsites, int inner, int reps, double* us_per_launch, double* max_rel_err);
 
+/* The one entry point that ALLOCATES NOTHING (for callers that cannot call cudaMalloc: code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it): the 16 local loops eta^dag Gamma s per timeslice (H8) of
+ * `nrhs` sources whose solutions the caller holds on the device.  dev_solution: native full-lattice field
+ * [parity][rhs][block of 32 sites][chunk][site] in precision `prec` (TSM_F64 or TSM_F32), as tsm_pack writes it;
+ * source_ids: HOST array of nrhs ids (passed to the kernel by value); seed / kind: the noise of those sources (eta is
+ * regenerated, never read); dev_loops: DEVICE output, [nrhs][16][Lt][2] doubles.  Needs no workspace, gauge field or
+ * parameters; calls no cudaMalloc / cudaFree; enqueues two kernels on the context's stream and returns without
+ * synchronising.  Its reduction scratch is a static device array of tsm_noalloc_scratch_bytes() = 4 MiB that every GPU
+ * loading the library holds until exit: calls with nrhs * Lt * 2 * nblk * 32 doubles beyond that (nblk = number of
+ * 1024-site pieces of a timeslice and parity, at most 8) return TSM_EINVAL.  All calls share the array: calls on one
+ * stream are ordered, calls that overlap on the GPU (several streams or contexts on one device) race.  The result is
+ * bit-identical to the local loops of tsm_loops_source. */
+size_t tsm_noalloc_scratch_bytes(void);
+int tsm_loops_local_noalloc(tsm_ctx* ctx, int prec, int nrhs, const void* dev_solution, uint64_t seed, const uint32_t* source_ids,
+                            int kind, double* dev_loops);
+
 /* Number of kernels this library has launched on the context since creation. */
 long long tsm_launch_count(const tsm_ctx* ctx);
 

@@ -492,3 +492,119 @@ int launch_finalize(tsm_ctx* ctx)
     TSM_CUDA(ctx, cudaGetLastError());
     return TSM_OK;
 }
+
+// ------------------------------------------------------------------ the entry point that allocates nothing
+// tsm_loops_local_noalloc (include/tsm.h): the local 16-Gamma loops (H8) of a caller-held solution field, for callers
+// that cannot have device memory allocated on their behalf and have set no workspace.  It is the LOCAL mode of
+// k_contract with two differences: the source ids travel by value in the kernel arguments (no id buffer), and the
+// per-block partial sums go to g_na_scratch, a file-scope array of a fixed size that every GPU loading the library
+// holds until exit, instead of the workspace's reduction scratch.  Same per-site arithmetic, same butterfly, same
+// order over blocks in the finish kernel: the result is bit-identical to tsm_loops_source's local loops.
+// Every call uses the same array: two calls that overlap on the GPU (different streams) race; calls on one stream are
+// ordered.  Nothing in it has to start at zero: each call overwrites every entry its finish kernel reads.
+constexpr size_t NA_MAX_DOUBLES = 524288;   // 4 MiB: nrhs * Lt * 2 * nblk * 32 doubles (32^3 x 64 with 16 sources fits exactly)
+static __device__ __align__(256) double g_na_scratch[NA_MAX_DOUBLES];
+
+namespace {
+
+struct NaIds { uint32_t v[TSM_MAX_NRHS]; };
+
+// scratch: [rhs][t][par][blk][32]
+template <int PREC>
+__global__ void __launch_bounds__(32 * CT_SPB, PREC == TSM_F64 ? 1 : 2) k_contract_local_na(const Geom g, const int nrhs, const int nblk, const void* __restrict__ sol,
+                                                                   const uint64_t seed, const NaIds ids, const int kind, double* __restrict__ scratch)
+{
+    using T = typename PT<PREC>::real;
+    constexpr int SPL = 4;   // sites per lane between two butterflies, as in k_contract
+    const int lane = threadIdx.x, rhs = blockIdx.z * blockDim.y + threadIdx.y;
+    if (rhs >= nrhs) return;
+    const int Vh = g.Vh, blk = blockIdx.x, t = blockIdx.y >> 1, par = blockIdx.y & 1;
+    const char* s_same = (const char*)sol + field_bytes(PREC, Vh, nrhs) * par + field_bytes(PREC, Vh, 1) * rhs;
+    const uint32_t sid = ids.v[rhs];
+    const int ngroup = (g.Vsh + 32 * SPL - 1) / (32 * SPL);
+    double acc = 0.0;
+    for (int gi = blk; gi < ngroup; gi += nblk) {
+        T dsum[32];
+#pragma unroll
+        for (int k = 0; k < 32; k++) dsum[k] = 0;
+#pragma unroll
+        for (int u = 0; u < SPL; u++) {
+            const int jj = (gi * SPL + u) * 32 + lane;
+            if (jj < g.Vsh) {
+                const int i = t * g.Vsh + jj;
+                T l[24], r[24];
+                noise_spinor(noise_bits(lex_of_site(g, decode_site(g, i, par)), seed, sid, kind), kind, l);
+                load_spinor<PREC>(s_same, i, r);
+                spin_matrix(l, r, dsum);
+            }
+        }
+        acc += (double)warp_transpose_sum(dsum);
+    }
+    scratch[(((((size_t)rhs * g.L[3] + t) * 2 + par) * nblk + blk) << 5) + lane] = acc;
+}
+
+// grid = (Lt, nrhs), 32 threads: sums the blocks' partials in k_contract_finish's order and applies the 16 Gamma
+__global__ void k_contract_finish_na(const int Lt, const int nblk, const GammaTable gt, const double* __restrict__ scratch, double* __restrict__ loops)
+{
+    const int t = blockIdx.x, rhs = blockIdx.y, k = threadIdx.x;
+    __shared__ double C[32];
+    double tot = 0;
+    for (int pb = 0; pb < 2 * nblk; pb++) tot += scratch[((((size_t)rhs * Lt + t) * 2 * nblk + pb) << 5) + k];
+    C[k] = tot;
+    __syncthreads();
+    if (k < 16) {
+        double re = 0, im = 0;
+        for (int al = 0; al < 4; al++) {
+            const int be = gt.col[k][al], ph = gt.ph[k][al] & 3;
+            const double cr = C[2 * (4 * al + be)], ci = C[2 * (4 * al + be) + 1];
+            re += (ph == 0) ? cr : (ph == 1) ? -ci : (ph == 2) ? -cr : ci;   // times i^ph
+            im += (ph == 0) ? ci : (ph == 1) ? cr : (ph == 2) ? -ci : -cr;
+        }
+        double* dst = loops + (((size_t)rhs * TSM_N_LOCAL_OPS + k) * Lt + t) * 2;
+        dst[0] = re;
+        dst[1] = im;
+    }
+}
+
+}  // namespace
+
+extern "C" size_t tsm_noalloc_scratch_bytes(void) { return NA_MAX_DOUBLES * sizeof(double); }
+
+extern "C" int tsm_loops_local_noalloc(tsm_ctx* ctx, int prec, int nrhs, const void* dev_solution, uint64_t seed, const uint32_t* source_ids,
+                                       int kind, double* dev_loops)
+{
+    int rc = ctx_enter(ctx, false, false, false);   // cudaSetDevice(ctx->device); needs no workspace, gauge field or parameters
+    if (rc) return rc;
+    if (!dev_solution || !dev_loops || !source_ids || nrhs < 1 || nrhs > TSM_MAX_NRHS || (prec != TSM_F64 && prec != TSM_F32) ||
+        (kind != TSM_Z4 && kind != TSM_Z2))
+        return tsm_fail(ctx, TSM_EINVAL, "bad no-alloc contraction arguments (prec must be TSM_F64 or TSM_F32, 1 <= nrhs <= 16)");
+    const Geom& g = ctx->g;
+    int nblk = (g.Vsh + 32 * 32 - 1) / (32 * 32);   // as launch_contract: the same blocks, hence the same sums
+    if (nblk < 1) nblk = 1;
+    if (nblk > CT_MAXBLK) nblk = CT_MAXBLK;
+    const size_t need = (size_t)nrhs * g.L[3] * 2 * nblk * 32;
+    if (need > NA_MAX_DOUBLES)
+        return tsm_fail(ctx, TSM_EINVAL, "no-alloc contraction: nrhs * Lt * 2 * nblk * 32 doubles exceed the 4 MiB static scratch "
+                                         "(tsm_noalloc_scratch_bytes); use fewer sources per call or tsm_loops_source");
+    // The array's name is a host-side stand-in in host code: its device address is looked up once per device, with that
+    // device current (ctx_enter has just made it so), and handed to the kernels.
+    static double* scratch_of_device[64] = {nullptr};
+    if (ctx->device >= 64) return tsm_fail(ctx, TSM_EINVAL, "no-alloc contraction: device index beyond 63");
+    if (!scratch_of_device[ctx->device]) {
+        void* p = nullptr;
+        TSM_CUDA(ctx, cudaGetSymbolAddress(&p, g_na_scratch));
+        if (!p) return tsm_fail(ctx, TSM_ECUDA, "cudaGetSymbolAddress returned no address for the static scratch");
+        scratch_of_device[ctx->device] = (double*)p;
+    }
+    double* scratch = scratch_of_device[ctx->device];
+    NaIds ids;
+    for (int j = 0; j < TSM_MAX_NRHS; j++) ids.v[j] = j < nrhs ? source_ids[j] : 0u;
+    const int spb = nrhs < CT_SPB ? nrhs : CT_SPB;
+    const dim3 grid(nblk, 2 * g.L[3], (nrhs + spb - 1) / spb), block(32, spb);
+    if (prec == TSM_F64) k_contract_local_na<TSM_F64><<<grid, block, 0, ctx->stream>>>(g, nrhs, nblk, dev_solution, seed, ids, kind, scratch);
+    else k_contract_local_na<TSM_F32><<<grid, block, 0, ctx->stream>>>(g, nrhs, nblk, dev_solution, seed, ids, kind, scratch);
+    k_contract_finish_na<<<dim3(g.L[3], nrhs), 32, 0, ctx->stream>>>(g.L[3], nblk, ctx->gam, scratch, dev_loops);
+    ctx->launches += 2;
+    TSM_CUDA(ctx, cudaGetLastError());
+    return TSM_OK;
+}

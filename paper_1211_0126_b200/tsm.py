@@ -31,7 +31,7 @@ EXPORTS = [
     "tsm_loops_reset", "tsm_loops_set_momenta", "tsm_loops_add_correction", "tsm_loops_add_lp", "tsm_loops_source",
     "tsm_loops_finalize", "tsm_loops_get_state", "tsm_loops_set_state", "tsm_run_loop_set",
     "tsm_set_hp_precision", "tsm_launch_count", "tsm_profile", "tsm_profile_read", "tsm_stencil_kernel_name",
-    "tsm_set_stencil_kernel", "tsm_set_graphs", "tsm_probe_su3_tensor",
+    "tsm_set_stencil_kernel", "tsm_set_graphs", "tsm_probe_su3_tensor", "tsm_noalloc_scratch_bytes", "tsm_loops_local_noalloc",
 ]
 
 
@@ -96,6 +96,9 @@ def load_library():
     lib.tsm_stencil_kernel_name.argtypes = [vp, i, i]
     lib.tsm_stencil_kernel_name.restype = ctypes.c_char_p
     lib.tsm_set_stencil_kernel.argtypes = [vp, i]
+    lib.tsm_noalloc_scratch_bytes.argtypes = []
+    lib.tsm_noalloc_scratch_bytes.restype = sz
+    lib.tsm_loops_local_noalloc.argtypes = [vp, i, i, vp, u64, u32p, i, vp]
     lib.tsm_probe_su3_tensor.argtypes = [vp, i, i, i, i, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     lib.tsm_set_graphs.argtypes = [vp, i]
     lib.tsm_profile.argtypes = [vp, i]
@@ -198,6 +201,14 @@ class Tsm:
     def set_stencil_kernel(self, which: int):
         """0 automatic, 1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box, 5 k_dslash_small (tuning / test aid)."""
         self._check(self.lib.tsm_set_stencil_kernel(self._h, which))
+
+    def loops_local_noalloc(self, prec: int, field, seed: int, source_ids, out, kind: int = Z4):
+        """tsm_loops_local_noalloc: local loops of the native full-lattice `field` (a torch uint8 tensor, as pack() returns)
+        into `out`, a caller-allocated torch float64 tensor of shape [nrhs][16][Lt][2] on the device.  Asynchronous."""
+        ids = [int(s) for s in source_ids]
+        arr = (ctypes.c_uint32 * len(ids))(*ids)
+        self._check(self.lib.tsm_loops_local_noalloc(self._h, prec, len(ids), field.data_ptr(), seed, arr, kind, out.data_ptr()))
+        return out
 
     def probe_su3_tensor(self, variant: int, nsites: int, inner: int, reps: int):
         """(microseconds per launch, max error relative to the largest fp64 reference value) of the per-site
