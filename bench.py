@@ -665,7 +665,7 @@ def main():
     ap.add_argument("--workload", type=int, default=5)
     ap.add_argument("--nrhs", type=int, default=0, help="sources per batch (default: the workload's; other values are profiling aids, not the headline)")
     ap.add_argument("--stencil-kernel", type=int, default=0, help="force a stencil kernel (tsm_set_stencil_kernel; profiling aid, not the headline)")
-    ap.add_argument("--graphs", type=int, default=-1, help="tsm_set_graphs mode (profiling aid; default: the library's)")
+    ap.add_argument("--graphs", type=int, default=-1, help="tsm_set_graphs mode 0..3 (profiling aid; default: the library's)")
     ap.add_argument("--skip-extras", action="store_true", help="only the timed steps (no e2e/table/full set/oracle/workloads)")
     ap.add_argument("--no-full-set", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

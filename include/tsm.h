@@ -208,8 +208,11 @@ const char* tsm_stencil_kernel_name(const tsm_ctx* ctx, int prec, int nrhs);
  * of 4 iterations, the host reads the all-done flag between them in residual mode; 2 = the whole iteration loop as
  * ONE graph launch, a WHILE node whose body is one captured iteration and whose condition (a source is still live
  * and the iteration budget is not used up) is set on the device by the last kernel of the body: no host round trip,
- * but measured 4.5 us per pass slower than mode 1 on this driver; 0 = kernel by kernel.
- * All three give bit-identical iterates. */
+ * but measured 4.5 us per pass slower than mode 1 on this driver; 3 = the whole loop in ONE
+ * cooperative launch of a persistent kernel (grid-wide barriers between the phases of an iteration, stopping test on
+ * the device; fp64 / fp32, lattices of at most 131 072 sites per parity, other cases fall back to mode 1) whose
+ * stencil arithmetic is k_dslash's; 0 = kernel by kernel.  Modes 0, 1, 2 give bit-identical iterates; so does mode 3
+ * whenever the other modes run k_dslash / k_dslash_tile (i.e. not on the lattices served by k_dslash_small). */
 int tsm_set_stencil_kernel(tsm_ctx* ctx, int which);
 int tsm_set_graphs(tsm_ctx* ctx, int mode);
 

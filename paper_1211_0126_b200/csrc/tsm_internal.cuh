@@ -529,6 +529,9 @@ int launch_mixed_axpy(tsm_ctx* ctx, int nrhs, void* x64, const void* e32);
 int launch_cg_update_xp(tsm_ctx* ctx, int prec, int nrhs, void* x, void* p, const void* r, double tol, unsigned long long loop = 0,
                         int in_loop = 0);
 int launch_cg_loop_begin(tsm_ctx* ctx, int n);
+bool cg_persistent_supported(const tsm_ctx* ctx, int prec, int nrhs);
+int launch_cg_persistent(tsm_ctx* ctx, int prec, int nrhs, void* x, void* r, void* p, void* w, void* t, const DslashCoef& c1,
+                         const DslashCoef& c2, const DslashCoef& c3, const DslashCoef& c4, double tol, int max_iter);
 int launch_convert(tsm_ctx* ctx, int prec_in, int prec_out, int nrhs_fields, const void* in, void* out);
 int launch_contract(tsm_ctx* ctx, int slot);
 int launch_accumulate(tsm_ctx* ctx, double* acc, const double* a, const double* b, int nrhs);

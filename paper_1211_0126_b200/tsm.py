@@ -219,7 +219,7 @@ class Tsm:
 
     def set_graphs(self, mode):
         """1 / True (default): cached graphs of 4 CG iterations; 2: the CG loop as one graph launch with a device-side
-        WHILE node; 0 / False: kernel by kernel."""
+        WHILE node; 3: one cooperative launch of the persistent CG kernel (small lattices); 0 / False: kernel by kernel."""
         self._check(self.lib.tsm_set_graphs(self._h, int(mode)))
 
     def hp_precision_name(self) -> str:

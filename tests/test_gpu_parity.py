@@ -1008,3 +1008,42 @@ def test_async_solves_match_synchronous_ones(medium, tsm_mod):
         c.t.solve_wait(0)
     assert e.value.code == tsm_mod.ESTATE
     c.t.loops_reset(False)
+
+
+@pytest.mark.parametrize("dims,recon", [((8, 8, 8, 16), 18), ((6, 10, 4, 6), 18), ((16, 16, 16, 32), 12), ((4, 4, 4, 8), 18)])
+def test_persistent_cg_kernel(tsm_mod, dims, recon):
+    """tsm_set_graphs(3): the whole CG loop in one cooperative launch of k_cg_persistent (grid barriers between the
+    phases, dot products summed from per-tile partials by every CTA, stopping test on the device).  Its phases are the
+    code of the kernel-by-kernel path, so with k_dslash as the stencil of that path (forced where k_dslash_small would
+    be chosen) the iterates are BIT-identical: fixed-iteration and residual mode, fp64 and fp32, 1, 3 and 4 sources,
+    a batch whose sources stop at different iterations, and the mixed-precision HP solver on top of it; fp64 also
+    against the oracle at 1e-12 and by true residual."""
+    c = Case(tsm_mod, dims, 0.5, 57, 0.157, 0.01, -1, max_nrhs=4, recon=recon)
+    c.t.set_stencil_kernel(1)
+    seed = 99
+    cases = [(F64, 0.0, 9, [1, 2, 3]), (F32, 0.0, 13, [4]), (F32, 1e-4, 500, [5, 6, 7, 8]), (F64, 1e-9, 2000, [2, 9]), (3, 1e-10, 2000, [1, 2, 3])]
+    ref = {}
+    for mode in (0, 3):
+        c.t.set_graphs(mode)
+        for k, (prec, tol, it, ids) in enumerate(cases):
+            n0 = c.t.launch_count()
+            rc, info = c.t.solve(seed, ids, prec, tol, it, slot=0, want_true_resid=(prec != F32))
+            got = ([i["iters"] for i in info], [i["status"] for i in info], [c.t.get_solution(0, j) for j in range(len(ids))])
+            if mode == 0:
+                ref[k] = got
+            else:
+                assert rc == 0 and got[0] == ref[k][0] and got[1] == ref[k][1], (dims, k, got[0], ref[k][0])
+                for j in range(len(ids)):
+                    assert np.array_equal(got[2][j], ref[k][2][j]), (dims, k, j)
+            if prec != F32 and tol > 0:
+                assert all(i["rel_resid_true"] < 20 * tol for i in info), (dims, k)
+    eta = oracle.noise(dims, seed, 2)
+    s_ref, _ = oracle.solve(dims, -1, c.kappa, c.mu, c.U, eta, 0.0, 9)
+    c.t.set_graphs(3)
+    rc, info = c.t.solve(seed, [1, 2, 3], F64, 0.0, 9, slot=0)
+    assert rel(c.t.get_solution(0, 1), s_ref) < 1e-12
+    # a single launch for the loop: noise, twist, 3 stencils, init, ONE persistent launch, reconstruction
+    n0 = c.t.launch_count()
+    c.t.solve(seed, [4], F32, 0.0, 13, slot=0)
+    assert c.t.launch_count() - n0 == 6 + 1 + 1
+    c.t.close()
