@@ -204,15 +204,17 @@ const char* tsm_stencil_kernel_name(const tsm_ctx* ctx, int prec, int nrhs);
  * fp32 / bf16 batches k_dslash_tile), 1 = k_dslash, 2 = k_dslash_tile (fp32 / bf16), 3 = k_dslash_box (fp32, lattice
  * permitting), 5 = k_dslash_small (fp64 / fp32).  A forced kernel that cannot serve a call falls back to the
  * automatic choice.  k_dslash and k_dslash_tile give a source bit-identical results; k_dslash_box and k_dslash_small
- * each differ from them in rounding, so a context should stay with one choice while results are being compared.  tsm_set_graphs: how the CG iterations are launched: 1 (default) = cached CUDA graphs
+ * each differ from them in rounding, so a context should stay with one choice while results are being compared.  tsm_set_graphs: how the CG iterations are launched: 4 (default) = automatic: mode 3
+ * on the lattices served by k_dslash_small (where it measures 34-42 % faster), mode 1 elsewhere; 1 = cached CUDA graphs
  * of 4 iterations, the host reads the all-done flag between them in residual mode; 2 = the whole iteration loop as
  * ONE graph launch, a WHILE node whose body is one captured iteration and whose condition (a source is still live
  * and the iteration budget is not used up) is set on the device by the last kernel of the body: no host round trip,
  * but measured 4.5 us per pass slower than mode 1 on this driver; 3 = the whole loop in ONE
  * cooperative launch of a persistent kernel (grid-wide barriers between the phases of an iteration, stopping test on
  * the device; fp64 / fp32, lattices of at most 131 072 sites per parity, other cases fall back to mode 1) whose
- * stencil arithmetic is k_dslash's; 0 = kernel by kernel.  Modes 0, 1, 2 give bit-identical iterates; so does mode 3
- * whenever the other modes run k_dslash / k_dslash_tile (i.e. not on the lattices served by k_dslash_small). */
+ * stencil arithmetic is that of the context's stencil kernel (k_dslash's with 128-site tiles, k_dslash_small's with
+ * 32-site blocks); 0 = kernel by kernel.  All modes give bit-identical iterates for fp64 / fp32 sources (for a batch of
+ * 2 or more fp32 sources with k_dslash_tile as the stencil, mode 3 agrees with it because k_dslash_tile and k_dslash do). */
 int tsm_set_stencil_kernel(tsm_ctx* ctx, int which);
 int tsm_set_graphs(tsm_ctx* ctx, int mode);
 

@@ -117,7 +117,7 @@ int tsm_create(tsm_ctx** out, const int dims[4], int t_boundary, int device)
     ctx->prof_on = false;
     ctx->loops_ready = false;
     ctx->stencil_choice = 0;
-    ctx->graphs_on = 1;
+    ctx->graphs_on = 4;
     ctx->loop_per_pass = 0;
     ctx->cg = nullptr; ctx->cg_host = nullptr; ctx->host_small = nullptr; ctx->ids_dev = nullptr;
     for (int s = 0; s < 2; s++) { ctx->slot_prec[s] = -1; ctx->slot_nrhs[s] = 0; }

@@ -178,7 +178,9 @@ int cg_run(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, void* r,
     const int poll = 4;
     const bool use_graph = graphs_enabled(ctx);
     // mode 3: the whole loop in ONE cooperative launch of k_cg_persistent (dslash.cu), where the lattice allows it
-    if (ctx->graphs_on == 3 && !ctx->prof_on && cg_persistent_supported(ctx, prec, nrhs))
+    // mode 4 (default): that launch where it measures faster (the lattices of k_dslash_small), graphs of 4 iterations elsewhere
+    if (!ctx->prof_on && ((ctx->graphs_on == 3 && cg_persistent_supported(ctx, prec, nrhs)) ||
+                          (ctx->graphs_on == 4 && cg_persistent_preferred(ctx, prec, nrhs))))
         return launch_cg_persistent(ctx, prec, nrhs, x, r, p, w, t, {tw.zero, tw.Rinv}, {tw.R, tw.mk2}, {tw.zero, tw.Rbinv}, {tw.Rb, tw.mk2},
                                     tol, max_iter);
     if (use_graph && (ctx->graphs_on == 2 || (no_poll && tol > 0))) {   // an enqueue-only solve in residual mode must not poll
@@ -487,8 +489,8 @@ int tsm_loops_reset(tsm_ctx* ctx, int ops)
 int tsm_set_graphs(tsm_ctx* ctx, int mode)
 {
     if (!ctx) return TSM_EINVAL;
-    if (mode < 0 || mode > 3)
-        return tsm_fail(ctx, TSM_EINVAL, "graphs: 0 off, 1 chunks of 4 iterations, 2 device-side loop, 3 persistent cooperative kernel");
+    if (mode < 0 || mode > 4)
+        return tsm_fail(ctx, TSM_EINVAL, "graphs: 0 off, 1 chunks of 4 iterations, 2 device-side loop, 3 persistent cooperative kernel, 4 automatic");
     ctx->graphs_on = mode;
     return TSM_OK;
 }

@@ -359,17 +359,6 @@ namespace {
 
 namespace cgp = cooperative_groups;
 
-struct PcgArgs {
-    Geom g;
-    int nrhs, ntiles, slab, max_iter;
-    double tol;
-    const void* pack[2];            // link packs of output parity 0 / 1
-    void *x, *r, *p, *w, *t;
-    DslashCoef c1, c2, c3, c4;      // the four stencil launches of cg_iteration (api_solve.cu)
-    double* partials;               // [2][nrhs][ntiles]: |w|^2 per tile, |r|^2 per tile
-    CgScalars* cg;
-};
-
 template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI>
 __device__ __forceinline__ void pcg_stencil(const PcgArgs& a, const int par, const void* in_, const void* x_, void* out_, const DslashCoef& cf,
                                             const double* s_alpha, double* partials, double* smem)
@@ -533,6 +522,13 @@ bool cg_persistent_supported(const tsm_ctx* ctx, int prec, int nrhs)
     return (prec == TSM_F64 || prec == TSM_F32) && ntiles <= FUSE_NTILES && (size_t)2 * nrhs * ntiles <= ctx->norm_partials_count;
 }
 
+// Where the persistent solver is the better choice (measured): the lattices whose stencil is
+// k_dslash_small (+34 % / +42 % LP solves/s at 4^3 x 8 / 8^3 x 16); with 128-site tiles it loses (-12 % at 16^3 x 32).
+bool cg_persistent_preferred(const tsm_ctx* ctx, int prec, int nrhs)
+{
+    return cg_persistent_supported(ctx, prec, nrhs) && stencil_kernel_for(ctx, prec, nrhs) == 5;
+}
+
 // max_iter iterations of O5 (or until every source is frozen) in ONE cooperative launch.  c1..c4: the coefficient pairs of
 // the four stencil launches of cg_iteration, in order.
 int launch_cg_persistent(tsm_ctx* ctx, int prec, int nrhs, void* x, void* r, void* p, void* w, void* t, const DslashCoef& c1,
@@ -542,7 +538,8 @@ int launch_cg_persistent(tsm_ctx* ctx, int prec, int nrhs, void* x, void* r, voi
     PcgArgs a;
     a.g = ctx->g;
     a.nrhs = nrhs;
-    a.ntiles = (ctx->g.Vh + TILE - 1) / TILE;
+    const bool small = stencil_kernel_for(ctx, prec, nrhs) == 5;   // where k_dslash_small is the stencil, its persistent form
+    a.ntiles = small ? (int)(padded_sites(ctx->g.Vh) / LB) : (ctx->g.Vh + TILE - 1) / TILE;
     a.slab = (ctx->g.S % TILE == 0) ? 1 : 0;
     a.max_iter = max_iter;
     a.tol = tol;
@@ -553,9 +550,11 @@ int launch_cg_persistent(tsm_ctx* ctx, int prec, int nrhs, void* x, void* r, voi
     ctx->norm_reduced = false;
     if (prec == TSM_F64) {
         a.pack[0] = ctx->gauge64[0]; a.pack[1] = ctx->gauge64[1];
-        return launch_pcg_t<TSM_F64, 18>(ctx, a);
+    } else {
+        a.pack[0] = ctx->gauge32[0]; a.pack[1] = ctx->gauge32[1];
     }
-    a.pack[0] = ctx->gauge32[0]; a.pack[1] = ctx->gauge32[1];
+    if (small) return launch_cg_persistent_small(ctx, prec, a);
+    if (prec == TSM_F64) return launch_pcg_t<TSM_F64, 18>(ctx, a);
     if (ctx->recon == 18) return launch_pcg_t<TSM_F32, 18>(ctx, a);
     return launch_pcg_t<TSM_F32, 12>(ctx, a);
 }

@@ -55,7 +55,7 @@ template <int PREC> __device__ __forceinline__ void store_spin(void* f, int i, i
 }
 
 // both hops of direction MU of site i into part[24] (zero on entry)
-template <int PREC, int RECON, bool DAGGER, int MU>
+template <int PREC, int RECON, bool DAGGER, int MU, bool NC>
 __device__ __forceinline__ void two_hops(const void* pack, const char* in, int i, int nf, int nbk, typename PT<PREC>::real ph_f,
                                          typename PT<PREC>::real ph_b, typename PT<PREC>::real* part)
 {
@@ -63,8 +63,8 @@ __device__ __forceinline__ void two_hops(const void* pack, const char* in, int i
     constexpr int SF = DAGGER ? +1 : -1;   // forward hop carries (1 - g_mu), dagger swaps
     T uf[18], ub[18], pf[24], pb[24], h[12], gq[12];
     load_link_pair<PREC, RECON>(pack, i, MU, uf, ub);
-    load_spinor<PREC>(in, nf, pf);
-    load_spinor<PREC>(in, nbk, pb);
+    load_spinor<PREC, NC>(in, nf, pf);
+    load_spinor<PREC, NC>(in, nbk, pb);
     project<T, MU, SF>(pf, h);
     if (MU == 3 && ph_f != 1) {   // time-boundary phase (A22)
 #pragma unroll
@@ -83,20 +83,21 @@ __device__ __forceinline__ void two_hops(const void* pack, const char* in, int i
     accumulate<T, MU, -SF>(gq, part);
 }
 
-template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI>
-__global__ void __launch_bounds__(128) k_dslash_small(const Geom g, const int par, const void* __restrict__ pack, const void* __restrict__ in_,
-                                                      const void* __restrict__ x_, void* out_, const DslashCoef cf,
-                                                      double* __restrict__ partials, CgScalars* __restrict__ cg, const int check_done)
+// One 32-site layout block `blk` of one source: four warps = four directions, then four warps = four spin components.
+// in / xf / out point at that source's fields; sm, red: the CTA's exchange buffers (the caller puts a barrier between two
+// calls).  Returns, in thread 0, the block's contribution to the fused norm.  NC: gather through ld.global.nc (false inside
+// the persistent CG kernel, where the gathered field is rewritten between two phases of the same launch).  Shared by
+// k_dslash_small and k_cg_persistent_small, so that the two give a source bit-identical results.
+template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI, bool NC>
+__device__ __forceinline__ double small_block(const Geom& g, const int par, const int blk, const void* pack, const char* in, const char* xf,
+                                              char* out, const DslashCoef& cf, const typename PT<PREC>::real alpha,
+                                              typename PT<PREC>::real (*sm)[24][32], double* red)
 {
     using T = typename PT<PREC>::real;
-    __shared__ T sm[4][24][32];
-    __shared__ double red[4];
-    if (check_done && cg->all_done) return;
     const int Vh = g.Vh;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;   // w: direction in the first half, spin component in the second
-    const int rhs = blockIdx.y, i = blockIdx.x * LB + lane;
+    const int i = blk * LB + lane;
     const bool live = i < Vh;
-    const size_t fb = field_bytes(PREC, Vh, 1);
     {
         T part[24];
 #pragma unroll
@@ -106,12 +107,11 @@ __global__ void __launch_bounds__(128) k_dslash_small(const Geom g, const int pa
             int nb[8];
             neighbours(g, i, s, nb);
             const T ph_f = (s.t == g.L[3] - 1) ? (T)g.theta : (T)1, ph_b = (s.t == 0) ? (T)g.theta : (T)1;
-            const char* in = (const char*)in_ + fb * rhs;
             switch (w) {   // warp-uniform
-                case 0: two_hops<PREC, RECON, DAGGER, 0>(pack, in, i, nb[0], nb[1], ph_f, ph_b, part); break;
-                case 1: two_hops<PREC, RECON, DAGGER, 1>(pack, in, i, nb[2], nb[3], ph_f, ph_b, part); break;
-                case 2: two_hops<PREC, RECON, DAGGER, 2>(pack, in, i, nb[4], nb[5], ph_f, ph_b, part); break;
-                default: two_hops<PREC, RECON, DAGGER, 3>(pack, in, i, nb[6], nb[7], ph_f, ph_b, part); break;
+                case 0: two_hops<PREC, RECON, DAGGER, 0, NC>(pack, in, i, nb[0], nb[1], ph_f, ph_b, part); break;
+                case 1: two_hops<PREC, RECON, DAGGER, 1, NC>(pack, in, i, nb[2], nb[3], ph_f, ph_b, part); break;
+                case 2: two_hops<PREC, RECON, DAGGER, 2, NC>(pack, in, i, nb[4], nb[5], ph_f, ph_b, part); break;
+                default: two_hops<PREC, RECON, DAGGER, 3, NC>(pack, in, i, nb[6], nb[7], ph_f, ph_b, part); break;
             }
         }
 #pragma unroll
@@ -134,33 +134,55 @@ __global__ void __launch_bounds__(128) k_dslash_small(const Geom g, const int pa
         if (XPAY) {
             const T cxr = (T)(a < 2 ? cf.x.up_re : cf.x.lo_re), cxi = (T)(a < 2 ? cf.x.up_im : cf.x.lo_im);
             T xv[6];
-            load_spin<PREC, true>((const char*)x_ + fb * rhs, i, a, xv);
+            load_spin<PREC, NC>(xf, i, a, xv);
 #pragma unroll
             for (int c = 0; c < 3; c++) {
                 o[2 * c] += cxr * xv[2 * c] - cxi * xv[2 * c + 1];
                 o[2 * c + 1] += cxr * xv[2 * c + 1] + cxi * xv[2 * c];
             }
         }
-        if (EPI == EPI_RESID) {   // out_ is the CG residual r (same precision as the spinors here): r -= alpha q
-            const T alpha = (T)cg->alpha[rhs];
+        if (EPI == EPI_RESID) {   // out is the CG residual r (same precision as the spinors here): r -= alpha q
             T rv[6];
-            load_spin<PREC, false>((const char*)out_ + fb * rhs, i, a, rv);
+            load_spin<PREC, false>(out, i, a, rv);
 #pragma unroll
             for (int c = 0; c < 6; c++) { rv[c] -= alpha * o[c]; nrm += (double)rv[c] * (double)rv[c]; }
-            store_spin<PREC>((char*)out_ + fb * rhs, i, a, rv);
+            store_spin<PREC>(out, i, a, rv);
         } else {
-            store_spin<PREC>((char*)out_ + fb * rhs, i, a, o);
+            store_spin<PREC>(out, i, a, o);
             if (EPI == EPI_NORM) {
 #pragma unroll
                 for (int c = 0; c < 6; c++) nrm += (double)o[c] * (double)o[c];
             }
         }
     }
+    double tot = 0.0;
     if (EPI != EPI_NONE) {
-        const double tot = warp_sum(nrm);
-        if (lane == 0) red[w] = tot;
+        const double ws = warp_sum(nrm);
+        if (lane == 0) red[w] = ws;
         __syncthreads();
-        if (threadIdx.x == 0) partials[(size_t)rhs * gridDim.x + blockIdx.x] = (red[0] + red[1]) + (red[2] + red[3]);
+        if (threadIdx.x == 0) tot = (red[0] + red[1]) + (red[2] + red[3]);
+    }
+    return tot;
+}
+
+template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI>
+__global__ void __launch_bounds__(128) k_dslash_small(const Geom g, const int par, const void* __restrict__ pack, const void* __restrict__ in_,
+                                                      const void* __restrict__ x_, void* out_, const DslashCoef cf,
+                                                      double* __restrict__ partials, CgScalars* __restrict__ cg, const int check_done)
+{
+    using T = typename PT<PREC>::real;
+    __shared__ T sm[4][24][32];
+    __shared__ double red[4];
+    if (check_done && cg->all_done) return;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int rhs = blockIdx.y;
+    const size_t fb = field_bytes(PREC, g.Vh, 1);
+    T alpha = 0;
+    if (EPI == EPI_RESID) alpha = (T)cg->alpha[rhs];
+    const double tot = small_block<PREC, RECON, DAGGER, XPAY, EPI, true>(g, par, blockIdx.x, pack, (const char*)in_ + fb * rhs, (const char*)x_ + fb * rhs,
+                                                                         (char*)out_ + fb * rhs, cf, alpha, sm, red);
+    if (EPI != EPI_NONE) {
+        if (threadIdx.x == 0) partials[(size_t)rhs * gridDim.x + blockIdx.x] = tot;
         // The last block of the grid to finish sums every source's partials (one warp per source, an order that
         // depends on the number of blocks only) and does what k_cg_reduce would: on these lattices a separate
         // reduction launch costs as much as the stencil itself.
@@ -219,4 +241,168 @@ int launch_dslash_small(tsm_ctx* ctx, int prec, int out_parity, bool dagger, int
         return launch_small_p<TSM_F32, 12>(ctx, out_parity, dagger, nrhs, ctx->gauge32[out_parity], in, x, out, c, nm, chk);
     }
     return tsm_fail(ctx, TSM_EINVAL, "small-lattice stencil: unsupported precision");
+}
+
+// ------------------------------------------------------------------ the persistent CG kernel in this file's formulation
+// k_cg_persistent (dslash.cu) with small_block() as the stencil: one cooperative launch for the whole iteration loop of O5
+// on the lattices where k_dslash_small is the stencil (a phase is then two dependent gathers per thread instead of eight).
+// Same partials per 32-site block, same order over blocks (sum_partials_warp), same update formula as k_cg_update_xp: a
+// source's iterate is bit-identical to the kernel-by-kernel path with k_dslash_small.
+#include <cooperative_groups.h>
+
+namespace {
+
+namespace cgp = cooperative_groups;
+
+template <int PREC, int RECON, bool DAGGER, bool XPAY, int EPI>
+__device__ __forceinline__ void pcgs_stencil(const PcgArgs& a, const int par, const void* in_, const void* x_, void* out_, const DslashCoef& cf,
+                                             const double* s_alpha, double* partials, typename PT<PREC>::real (*sm)[24][32], double* red)
+{
+    using T = typename PT<PREC>::real;
+    const size_t fb = field_bytes(PREC, a.g.Vh, 1);
+    for (int blk = blockIdx.x; blk < a.ntiles; blk += gridDim.x)
+        for (int rhs = 0; rhs < a.nrhs; rhs++) {
+            T alpha = 0;
+            if (EPI == EPI_RESID) alpha = (T)s_alpha[rhs];
+            const double tot = small_block<PREC, RECON, DAGGER, XPAY, EPI, false>(a.g, par, blk, a.pack[par], (const char*)in_ + fb * rhs,
+                                                                                  (const char*)x_ + fb * rhs, (char*)out_ + fb * rhs, cf, alpha, sm, red);
+            if (EPI != EPI_NONE && threadIdx.x == 0) partials[(size_t)rhs * a.ntiles + blk] = tot;
+            __syncthreads();   // sm and red are reused by the next (block, source)
+        }
+}
+
+template <int PREC, int RECON>
+__global__ void __launch_bounds__(128) k_cg_persistent_small(const PcgArgs a)
+{
+    using T = typename PT<PREC>::real;
+    cgp::grid_group grid = cgp::this_grid();
+    __shared__ T sm[4][24][32];
+    __shared__ double red[4];
+    __shared__ double s_alpha[TSM_MAX_NRHS], s_rr[TSM_MAX_NRHS], s_rrnew[TSM_MAX_NRHS], s_beta[TSM_MAX_NRHS], s_pq[TSM_MAX_NRHS];
+    __shared__ int s_done[TSM_MAX_NRHS], s_iters[TSM_MAX_NRHS], s_status[TSM_MAX_NRHS];
+    __shared__ int s_all, s_broke;
+    CgScalars* cg = a.cg;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int Vh = a.g.Vh, nrhs = a.nrhs;
+    if (tid < nrhs) {
+        s_rr[tid] = cg->rr[tid]; s_done[tid] = cg->done[tid]; s_iters[tid] = cg->iters[tid]; s_status[tid] = cg->status[tid];
+        s_beta[tid] = cg->beta[tid]; s_pq[tid] = cg->pq[tid]; s_alpha[tid] = 0.0; s_rrnew[tid] = cg->rr_new[tid];
+    }
+    if (tid == 0) { s_all = cg->all_done; s_broke = 0; }
+    __syncthreads();
+    double* part_w = a.partials;
+    double* part_r = a.partials + (size_t)nrhs * a.ntiles;
+
+    for (int it = 0; it < a.max_iter && !s_all; it++) {
+        pcgs_stencil<PREC, RECON, false, false, EPI_NONE>(a, 1, a.p, nullptr, a.t, a.c1, s_alpha, nullptr, sm, red);   // t = R^-1 D_oe p
+        grid.sync();
+        pcgs_stencil<PREC, RECON, false, true, EPI_NORM>(a, 0, a.t, a.p, a.w, a.c2, s_alpha, part_w, sm, red);         // w = Mhat p; |w|^2
+        grid.sync();
+        for (int j = wid; j < nrhs; j += 4) {   // alpha = rr / |w|^2 (cg_after_reduction, which == 0)
+            const double v = sum_partials_warp(part_w, j, a.ntiles);
+            if (lane == 0) {
+                s_pq[j] = v;
+                double alpha = 0.0;
+                if (!s_done[j]) {
+                    const double rr = s_rr[j];
+                    if (!(v > 0) || !isfinite(v) || !(rr > 0) || !isfinite(rr)) { s_done[j] = 1; s_status[j] = TSM_EBREAKDOWN; s_broke = 1; }
+                    else alpha = rr / v;
+                }
+                s_alpha[j] = alpha;
+            }
+        }
+        __syncthreads();
+        pcgs_stencil<PREC, RECON, true, false, EPI_NONE>(a, 1, a.w, nullptr, a.t, a.c3, s_alpha, nullptr, sm, red);    // t = Rb^-1 D_oe^dag w
+        grid.sync();
+        pcgs_stencil<PREC, RECON, true, true, EPI_RESID>(a, 0, a.t, a.w, a.r, a.c4, s_alpha, part_r, sm, red);         // r -= alpha Mhat^dag w; |r|^2
+        grid.sync();
+        for (int j = wid; j < nrhs; j += 4) {   // rr' (which == 1)
+            const double v = sum_partials_warp(part_r, j, a.ntiles);
+            if (lane == 0) s_rrnew[j] = v;
+        }
+        __syncthreads();
+        // x += alpha p; p = r + beta p on this CTA's own blocks: 96 threads = 32 sites x 3 groups of 8 reals
+        const size_t fb = field_bytes(PREC, Vh, 1);
+        if (tid < 96) {
+            const int k8 = tid >> 5;
+            for (int rhs = 0; rhs < nrhs; rhs++) {
+                if (s_done[rhs]) continue;
+                const T alpha = (T)s_alpha[rhs];
+                const T beta = (T)(s_rrnew[rhs] / s_rr[rhs]);
+                char* x = (char*)a.x + fb * rhs;
+                char* p = (char*)a.p + fb * rhs;
+                const char* r = (const char*)a.r + fb * rhs;
+                for (int blk = blockIdx.x; blk < a.ntiles; blk += gridDim.x) {
+                    const int i = blk * LB + lane;
+                    if (i >= Vh) continue;
+                    T xv[8], pv[8], rv[8];
+                    load8<PREC, false>(x, i, k8, xv);
+                    load8<PREC, false>(p, i, k8, pv);
+                    load8<PREC, false>(r, i, k8, rv);
+#pragma unroll
+                    for (int k = 0; k < 8; k++) {
+                        xv[k] += alpha * pv[k];
+                        pv[k] = rv[k] + beta * pv[k];
+                    }
+                    store8<PREC>(x, i, k8, xv);
+                    store8<PREC>(p, i, k8, pv);
+                }
+            }
+        }
+        __syncthreads();
+        if (tid == 0) {   // the bookkeeping of k_cg_update_xp's last block
+            int all = 1;
+            for (int j = 0; j < nrhs; j++) {
+                if (!s_done[j]) {
+                    const double v = s_rrnew[j];
+                    s_iters[j] += 1;
+                    s_beta[j] = v / s_rr[j];
+                    s_rr[j] = v;
+                    if (a.tol > 0 && sqrt(v / cg->bb[j]) <= a.tol) s_done[j] = 1;
+                }
+                all &= s_done[j];
+            }
+            s_all = all;
+        }
+        grid.sync();
+    }
+    if (blockIdx.x == 0) {
+        __syncthreads();
+        if (tid < nrhs) {
+            cg->rr[tid] = s_rr[tid]; cg->done[tid] = s_done[tid]; cg->iters[tid] = s_iters[tid]; cg->status[tid] = s_status[tid];
+            cg->beta[tid] = s_beta[tid]; cg->pq[tid] = s_pq[tid]; cg->alpha[tid] = s_alpha[tid]; cg->rr_new[tid] = s_rrnew[tid];
+        }
+        if (tid == 0) {
+            cg->all_done = s_all;
+            if (s_broke) cg->sticky_breakdown = 1;
+        }
+    }
+}
+
+template <int PREC, int RECON> int launch_pcgs_t(tsm_ctx* ctx, PcgArgs& a)
+{
+    auto kern = k_cg_persistent_small<PREC, RECON>;
+    static int resident[64] = {0};
+    if (ctx->device >= 64) return tsm_fail(ctx, TSM_EINVAL, "persistent CG: device index beyond 63");
+    if (!resident[ctx->device]) {
+        int nb = 0;
+        TSM_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 128, 0));
+        if (nb < 1) return tsm_fail(ctx, TSM_ECUDA, "persistent CG kernel does not fit an SM");
+        resident[ctx->device] = nb;
+    }
+    int grid = ctx->nsm * resident[ctx->device];
+    if (grid > a.ntiles) grid = a.ntiles;
+    void* params[] = {(void*)&a};
+    TSM_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)kern, dim3(grid), dim3(128), params, 0, ctx->stream));
+    ctx->launches++;
+    return TSM_OK;
+}
+
+}  // namespace
+
+int launch_cg_persistent_small(tsm_ctx* ctx, int prec, PcgArgs& a)
+{
+    if (prec == TSM_F64) return launch_pcgs_t<TSM_F64, 18>(ctx, a);
+    if (ctx->recon == 18) return launch_pcgs_t<TSM_F32, 18>(ctx, a);
+    return launch_pcgs_t<TSM_F32, 12>(ctx, a);
 }

@@ -419,7 +419,7 @@ struct tsm_ctx {
     std::vector<CgGraph> graphs;     // cleared whenever kappa/mu, the gauge storage or the workspace change
     std::vector<BoxMapCache> box_maps;
     int stencil_choice;              // tsm_set_stencil_kernel: 0 automatic, 1 k_dslash, 2 k_dslash_tile, 3 k_dslash_box, 5 k_dslash_small
-    int graphs_on;                   // tsm_set_graphs: 0 off, 1 chunks of 4 iterations, 2 device-side loop
+    int graphs_on;                   // tsm_set_graphs: 0 off, 1 chunks of 4 iterations, 2 device-side loop, 3 persistent kernel, 4 automatic
     long long loop_per_pass;         // launch accounting of the last device-side loop: kernels per pass (0: none pending),
     int loop_eager, loop_nrhs;       // iterations run before the loop, sources of that solve (settled when the scalars are read)
     // per solution slot: what tsm_solve_wait needs to report on a solve that was only enqueued (tsm_solve_async)
@@ -529,7 +529,21 @@ int launch_mixed_axpy(tsm_ctx* ctx, int nrhs, void* x64, const void* e32);
 int launch_cg_update_xp(tsm_ctx* ctx, int prec, int nrhs, void* x, void* p, const void* r, double tol, unsigned long long loop = 0,
                         int in_loop = 0);
 int launch_cg_loop_begin(tsm_ctx* ctx, int n);
+// arguments of the persistent CG kernels (dslash.cu: 128-site tiles, k_dslash's arithmetic; dslash_small.cu: 32-site
+// blocks, k_dslash_small's arithmetic)
+struct PcgArgs {
+    Geom g;
+    int nrhs, ntiles, slab, max_iter;   // ntiles: 128-site tiles, or 32-site blocks for the small form
+    double tol;
+    const void* pack[2];            // link packs of output parity 0 / 1
+    void *x, *r, *p, *w, *t;
+    DslashCoef c1, c2, c3, c4;      // the four stencil launches of cg_iteration (api_solve.cu)
+    double* partials;               // [2][nrhs][ntiles]: |w|^2 per tile, |r|^2 per tile
+    CgScalars* cg;
+};
+int launch_cg_persistent_small(tsm_ctx* ctx, int prec, PcgArgs& a);
 bool cg_persistent_supported(const tsm_ctx* ctx, int prec, int nrhs);
+bool cg_persistent_preferred(const tsm_ctx* ctx, int prec, int nrhs);
 int launch_cg_persistent(tsm_ctx* ctx, int prec, int nrhs, void* x, void* r, void* p, void* w, void* t, const DslashCoef& c1,
                          const DslashCoef& c2, const DslashCoef& c3, const DslashCoef& c4, double tol, int max_iter);
 int launch_convert(tsm_ctx* ctx, int prec_in, int prec_out, int nrhs_fields, const void* in, void* out);

@@ -218,7 +218,7 @@ class Tsm:
         return us.value, err.value
 
     def set_graphs(self, mode):
-        """1 / True (default): cached graphs of 4 CG iterations; 2: the CG loop as one graph launch with a device-side
+        """4 (default): automatic (3 on the smallest lattices, else 1); 1 / True: cached graphs of 4 CG iterations; 2: the CG loop as one graph launch with a device-side
         WHILE node; 3: one cooperative launch of the persistent CG kernel (small lattices); 0 / False: kernel by kernel."""
         self._check(self.lib.tsm_set_graphs(self._h, int(mode)))
 

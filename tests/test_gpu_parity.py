@@ -505,7 +505,7 @@ def test_cuda_graph_chunks_equal_kernel_by_kernel_launches(medium):
     # and the same launch count: noise, twist, 3 stencils, init; per iteration 4 stencils + update (k_dslash_small
     # finishes its own reductions on this lattice); the loop's begin kernel; reconstruction
     ref = None
-    for mode in (0, 1, 1, 2, 2):
+    for mode in (0, 1, 1, 2, 2, 3, 4):
         c.t.set_graphs(mode)
         for tol, k in ((0.0, 12), (1e-4, 500)):
             n0 = c.t.launch_count()
@@ -513,7 +513,8 @@ def test_cuda_graph_chunks_equal_kernel_by_kernel_launches(medium):
             n_l = c.t.launch_count() - n0
             got = (info[0]["iters"], info[1]["iters"], c.t.get_solution(0, 0), c.t.get_solution(0, 1))
             if tol == 0.0:
-                assert n_l == 6 + 5 * 12 + 1 + (1 if mode == 2 else 0), (mode, n_l)
+                want_l = {0: 6 + 5 * 12 + 1, 1: 6 + 5 * 12 + 1, 2: 6 + 5 * 12 + 2, 3: 8, 4: 8}[mode]   # 3, 4: ONE launch for the loop
+                assert n_l == want_l, (mode, n_l)
                 if ref is None:
                     ref = got
                 assert got[0] == 12 and np.array_equal(got[2], ref[2]) and np.array_equal(got[3], ref[3]), mode
@@ -521,7 +522,7 @@ def test_cuda_graph_chunks_equal_kernel_by_kernel_launches(medium):
                 if mode == 0:
                     ref_t = got
                 assert got[:2] == ref_t[:2] and np.array_equal(got[2], ref_t[2]) and np.array_equal(got[3], ref_t[3]), mode
-    c.t.set_graphs(1)
+    c.t.set_graphs(4)
 
 
 # ---------------------------------------------------------------- N1: one-end trick loops (Eq. 2.5)
@@ -1010,16 +1011,19 @@ def test_async_solves_match_synchronous_ones(medium, tsm_mod):
     c.t.loops_reset(False)
 
 
+@pytest.mark.parametrize("stencil", [1, 0])
 @pytest.mark.parametrize("dims,recon", [((8, 8, 8, 16), 18), ((6, 10, 4, 6), 18), ((16, 16, 16, 32), 12), ((4, 4, 4, 8), 18)])
-def test_persistent_cg_kernel(tsm_mod, dims, recon):
+def test_persistent_cg_kernel(tsm_mod, dims, recon, stencil):
     """tsm_set_graphs(3): the whole CG loop in one cooperative launch of k_cg_persistent (grid barriers between the
     phases, dot products summed from per-tile partials by every CTA, stopping test on the device).  Its phases are the
     code of the kernel-by-kernel path, so with k_dslash as the stencil of that path (forced where k_dslash_small would
     be chosen) the iterates are BIT-identical: fixed-iteration and residual mode, fp64 and fp32, 1, 3 and 4 sources,
     a batch whose sources stop at different iterations, and the mixed-precision HP solver on top of it; fp64 also
-    against the oracle at 1e-12 and by true residual."""
+    against the oracle at 1e-12 and by true residual.  stencil = 0: the automatic choice -- on lattices of at most
+    16 384 sites per parity that is k_dslash_small, and the persistent kernel is then k_cg_persistent_small (the same
+    loop with small_block() as the stencil), again bit-identical to its kernel-by-kernel path."""
     c = Case(tsm_mod, dims, 0.5, 57, 0.157, 0.01, -1, max_nrhs=4, recon=recon)
-    c.t.set_stencil_kernel(1)
+    c.t.set_stencil_kernel(stencil)
     seed = 99
     cases = [(F64, 0.0, 9, [1, 2, 3]), (F32, 0.0, 13, [4]), (F32, 1e-4, 500, [5, 6, 7, 8]), (F64, 1e-9, 2000, [2, 9]), (3, 1e-10, 2000, [1, 2, 3])]
     ref = {}
