@@ -219,6 +219,12 @@ def oracle_baseline(wl, U, with_one_thread: bool):
         oracle.hop(wl.dims, wl.t_boundary, U, psi, -1)
         ts.append(time.perf_counter() - t0)
     detail["t_full_lattice_dslash_s_median_of_5"] = float(np.median(ts))
+    if wl.V <= 131072:   # configs 1-3: one HP solve of the oracle in full as well
+        eta_hp = oracle.noise(wl.dims, wl.noise_seed, 0)
+        t0 = time.perf_counter()
+        _, info_hp = oracle.solve(wl.dims, wl.t_boundary, wl.kappa, wl.mu, U, eta_hp, wl.hp_tol, 5000)
+        detail["t_hp_solve_s"] = time.perf_counter() - t0
+        detail["hp_iterations"] = info_hp["iters"]
     if with_one_thread and wl.V <= 131072:   # configs 1-3: the same on ONE host thread as well
         try:
             import ctypes
