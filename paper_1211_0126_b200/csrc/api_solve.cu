@@ -180,9 +180,12 @@ int cg_run(tsm_ctx* ctx, int prec, int nrhs, const Twists& tw, void* x, void* r,
     // mode 3: the whole loop in ONE cooperative launch of k_cg_persistent (dslash.cu), where the lattice allows it
     // mode 4 (default): that launch where it measures faster (the lattices of k_dslash_small), graphs of 4 iterations elsewhere
     if (!ctx->prof_on && ((ctx->graphs_on == 3 && cg_persistent_supported(ctx, prec, nrhs)) ||
-                          (ctx->graphs_on == 4 && cg_persistent_preferred(ctx, prec, nrhs))))
-        return launch_cg_persistent(ctx, prec, nrhs, x, r, p, w, t, {tw.zero, tw.Rinv}, {tw.R, tw.mk2}, {tw.zero, tw.Rbinv}, {tw.Rb, tw.mk2},
-                                    tol, max_iter);
+                          (ctx->graphs_on == 4 && cg_persistent_preferred(ctx, prec, nrhs)))) {
+        const int rcp = launch_cg_persistent(ctx, prec, nrhs, x, r, p, w, t, {tw.zero, tw.Rinv}, {tw.R, tw.mk2}, {tw.zero, tw.Rbinv},
+                                             {tw.Rb, tw.mk2}, tol, max_iter);
+        if (rcp == TSM_OK || ctx->graphs_on == 3) return rcp;
+        cudaGetLastError();   // automatic mode: a refused cooperative launch (nothing has run) falls back to the graph path
+    }
     if (use_graph && (ctx->graphs_on == 2 || (no_poll && tol > 0))) {   // an enqueue-only solve in residual mode must not poll
         // device-side loop: the first iteration of an argument set runs kernel by kernel (kernel attributes
         // cannot be set inside a capture), everything after it is one graph launch
