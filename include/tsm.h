@@ -205,7 +205,9 @@ const char* tsm_stencil_kernel_name(const tsm_ctx* ctx, int prec, int nrhs);
  * permitting), 5 = k_dslash_small (fp64 / fp32).  A forced kernel that cannot serve a call falls back to the
  * automatic choice.  k_dslash and k_dslash_tile give a source bit-identical results; k_dslash_box and k_dslash_small
  * each differ from them in rounding, so a context should stay with one choice while results are being compared.  tsm_set_graphs: how the CG iterations are launched: 4 (default) = automatic: mode 3
- * on the lattices served by k_dslash_small (where it measures 34-42 % faster), mode 1 elsewhere; 1 = cached CUDA graphs
+ * on the lattices served by k_dslash_small (where it measures 34-42 % faster; there the same launch also does the
+ * even-odd preparation, the CG start and the reconstruction of an fp64 / fp32 solve, so a solve is the noise kernel
+ * plus ONE launch), mode 1 elsewhere; 1 = cached CUDA graphs
  * of 4 iterations, the host reads the all-done flag between them in residual mode; 2 = the whole iteration loop as
  * ONE graph launch, a WHILE node whose body is one captured iteration and whose condition (a source is still live
  * and the iteration budget is not used up) is set on the device by the last kernel of the body: no host round trip,

@@ -340,14 +340,27 @@ int solve_enqueue(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int n
         Phase ph("tsm: noise");
         if ((rc = launch_noise(ctx, sp, nrhs, seed, ids_dev, kind, s_e))) return rc;
     }
-    {   // H4: bhat = eta_e + kappa D_eo R^-1 eta_o (into w);  b' = Mhat^dag bhat (into r)
+    // Automatic launch mode on the smallest lattices: everything after the noise in ONE cooperative launch (dslash_small.cu:
+    // k_cg_persistent_small in its whole-solve form; the same arithmetic in the same order as the steps below)
+    bool one_launch = false;
+    if (prec != TSM_MIXED && prec != TSM_BF16 && ctx->graphs_on == 4 && !ctx->prof_on && cg_persistent_preferred(ctx, prec, nrhs)) {
+        Phase ph("tsm: prepare + CG + reconstruct (one launch)");
+        PcgArgs wa{};
+        wa.s_o = s_o; wa.aux = aux; wa.tw_rinv = tw.Rinv;
+        wa.cp1 = {tw.one, tw.k}; wa.cp2 = {tw.zero, tw.Rbinv}; wa.cp3 = {tw.Rb, tw.mk2}; wa.crec = {tw.Rinv, tw.kRinv};
+        const int rcw = launch_cg_persistent(ctx, prec, nrhs, x, r, p, w, t, {tw.zero, tw.Rinv}, {tw.R, tw.mk2}, {tw.zero, tw.Rbinv},
+                                             {tw.Rb, tw.mk2}, tol, max_iter, &wa);
+        if (rcw == TSM_OK) one_launch = true;
+        else cudaGetLastError();   // refused (nothing has run): the step-by-step path below
+    }
+    if (!one_launch) {   // H4: bhat = eta_e + kappa D_eo R^-1 eta_o (into w);  b' = Mhat^dag bhat (into r)
         Phase ph("tsm: prepare");
         if ((rc = launch_twist(ctx, sp, nrhs, s_o, aux, tw.Rinv))) return rc;
         if ((rc = launch_dslash(ctx, sp, 0, false, nrhs, aux, s_e, w, {tw.one, tw.k}, 0))) return rc;
         if ((rc = launch_dslash(ctx, sp, 1, true, nrhs, w, nullptr, t, {tw.zero, tw.Rbinv}, 0))) return rc;
         if ((rc = launch_dslash(ctx, sp, 0, true, nrhs, t, w, r, {tw.Rb, tw.mk2}, 0))) return rc;
     }
-    {   // O5: x0 = 0 (x lives in the slot's even half), r0 = p0 = b'
+    if (!one_launch) {   // O5: x0 = 0 (x lives in the slot's even half), r0 = p0 = b'
         Phase ph(prec == TSM_MIXED ? "tsm: CG (mixed precision)" : "tsm: CG");
         if (prec == TSM_MIXED) {
             if ((rc = solve_mixed(ctx, nrhs, tw, s_e, tol, max_iter))) return rc;
@@ -356,7 +369,7 @@ int solve_enqueue(tsm_ctx* ctx, uint64_t seed, const uint32_t* source_ids, int n
             if ((rc = cg_run(ctx, prec, nrhs, tw, x, r, p, w, t, tol, max_iter, no_poll))) return rc;
         }
     }
-    {   // H7: s_e = x, s_o = R^-1 (eta_o + kappa D_oe x)
+    if (!one_launch) {   // H7: s_e = x, s_o = R^-1 (eta_o + kappa D_oe x)
         Phase ph("tsm: reconstruct");
         if ((rc = launch_dslash(ctx, sp, 1, false, nrhs, x, s_o, aux, {tw.Rinv, tw.kRinv}, 0))) return rc;
         TSM_CUDA(ctx, cudaMemcpyAsync(s_o, aux, field_bytes(sp, Vh, nrhs), cudaMemcpyDeviceToDevice, ctx->stream));

@@ -34,7 +34,7 @@ __global__ void __launch_bounds__(BLAS_BS) k_cg_init(const int Vh, const int nrh
         TP pv[8];
         load8<PV>(r, i, k8, rv);
 #pragma unroll
-        for (int k = 0; k < 8; k++) { sum += (double)rv[k] * (double)rv[k]; pv[k] = (TP)rv[k]; z[k] = 0; }
+        for (int k = 0; k < 8; k++) { sum = fma((double)rv[k], (double)rv[k], sum); pv[k] = (TP)rv[k]; z[k] = 0; }   // explicit: k_cg_persistent_small repeats this chain
         store8<PP>(p, i, k8, pv);
         store8<PV>(x, i, k8, z);
     }
@@ -159,6 +159,8 @@ inline dim3 blas_grid(const tsm_ctx* ctx, int nrhs)
 }
 
 }  // namespace
+
+int blas_grid_x(const tsm_ctx* ctx) { return (int)blas_grid(ctx, 1).x; }
 
 // prec is the solve precision: F64 / F32 keep every vector in that precision; BF16 keeps
 // x, r, q in fp32 and p in bf16.

@@ -532,7 +532,7 @@ bool cg_persistent_preferred(const tsm_ctx* ctx, int prec, int nrhs)
 // max_iter iterations of O5 (or until every source is frozen) in ONE cooperative launch.  c1..c4: the coefficient pairs of
 // the four stencil launches of cg_iteration, in order.
 int launch_cg_persistent(tsm_ctx* ctx, int prec, int nrhs, void* x, void* r, void* p, void* w, void* t, const DslashCoef& c1,
-                         const DslashCoef& c2, const DslashCoef& c3, const DslashCoef& c4, double tol, int max_iter)
+                         const DslashCoef& c2, const DslashCoef& c3, const DslashCoef& c4, double tol, int max_iter, const PcgArgs* whole)
 {
     if (!cg_persistent_supported(ctx, prec, nrhs)) return tsm_fail(ctx, TSM_EINVAL, "persistent CG: lattice or precision not supported");
     PcgArgs a;
@@ -547,6 +547,20 @@ int launch_cg_persistent(tsm_ctx* ctx, int prec, int nrhs, void* x, void* r, voi
     a.c1 = c1; a.c2 = c2; a.c3 = c3; a.c4 = c4;
     a.partials = ctx->norm_partials;
     a.cg = ctx->cg;
+    a.whole = 0;
+    a.s_o = a.aux = nullptr;
+    a.init_groups = nullptr;
+    a.init_gx = 0;
+    if (whole) {   // source preparation, CG initialisation and reconstruction in the same launch (small form only)
+        a.whole = 1;
+        a.s_o = whole->s_o; a.aux = whole->aux; a.tw_rinv = whole->tw_rinv;
+        a.cp1 = whole->cp1; a.cp2 = whole->cp2; a.cp3 = whole->cp3; a.crec = whole->crec;
+        a.init_groups = ctx->partials;
+        a.init_gx = blas_grid_x(ctx);
+        // k_cg_init's summation order can be reproduced only where each of its threads holds at most one item
+        if (!small || (size_t)nrhs * 3 * a.ntiles > ctx->partials_count || (long long)a.init_gx * 256 < 3LL * padded_sites(ctx->g.Vh))
+            return tsm_fail(ctx, TSM_EINVAL, "persistent CG: the whole-solve form does not apply to this lattice");
+    }
     ctx->norm_reduced = false;
     if (prec == TSM_F64) {
         a.pack[0] = ctx->gauge64[0]; a.pack[1] = ctx->gauge64[1];

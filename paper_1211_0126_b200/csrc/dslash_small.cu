@@ -279,19 +279,89 @@ __global__ void __launch_bounds__(128) k_cg_persistent_small(const PcgArgs a)
     __shared__ T sm[4][24][32];
     __shared__ double red[4];
     __shared__ double s_alpha[TSM_MAX_NRHS], s_rr[TSM_MAX_NRHS], s_rrnew[TSM_MAX_NRHS], s_beta[TSM_MAX_NRHS], s_pq[TSM_MAX_NRHS];
+    __shared__ double s_bb[TSM_MAX_NRHS];
     __shared__ int s_done[TSM_MAX_NRHS], s_iters[TSM_MAX_NRHS], s_status[TSM_MAX_NRHS];
     __shared__ int s_all, s_broke;
     CgScalars* cg = a.cg;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int Vh = a.g.Vh, nrhs = a.nrhs;
+    const size_t fb = field_bytes(PREC, Vh, 1);
     if (tid < nrhs) {
         s_rr[tid] = cg->rr[tid]; s_done[tid] = cg->done[tid]; s_iters[tid] = cg->iters[tid]; s_status[tid] = cg->status[tid];
         s_beta[tid] = cg->beta[tid]; s_pq[tid] = cg->pq[tid]; s_alpha[tid] = 0.0; s_rrnew[tid] = cg->rr_new[tid];
+        s_bb[tid] = cg->bb[tid];
     }
     if (tid == 0) { s_all = cg->all_done; s_broke = 0; }
     __syncthreads();
     double* part_w = a.partials;
     double* part_r = a.partials + (size_t)nrhs * a.ntiles;
+
+    if (a.whole) {
+        // ---- H4 (tsm_solve): aux = R^-1 eta_o; bhat = eta_e + kappa D_eo aux (into w); t = Rb^-1 D_oe^dag bhat; b' = Mhat^dag bhat (into r)
+        if (tid < 96) {   // 32 sites x 3 groups of 8 reals, k_twist's arithmetic
+            const int k8 = tid >> 5;
+            for (int rhs = 0; rhs < nrhs; rhs++)
+                for (int blk = blockIdx.x; blk < a.ntiles; blk += gridDim.x) {
+                    const int i = blk * LB + lane;
+                    if (i >= Vh) continue;
+                    T v[8], o[8];
+                    load8<PREC, false>((const char*)a.s_o + fb * rhs, i, k8, v);
+                    twist8<T>(a.tw_rinv, k8, v, o);
+                    store8<PREC>((char*)a.aux + fb * rhs, i, k8, o);
+                }
+        }
+        grid.sync();
+        pcgs_stencil<PREC, RECON, false, true, EPI_NONE>(a, 0, a.aux, a.x, a.w, a.cp1, s_alpha, nullptr, sm, red);
+        grid.sync();
+        pcgs_stencil<PREC, RECON, true, false, EPI_NONE>(a, 1, a.w, nullptr, a.t, a.cp2, s_alpha, nullptr, sm, red);
+        grid.sync();
+        pcgs_stencil<PREC, RECON, true, true, EPI_NONE>(a, 0, a.t, a.w, a.r, a.cp3, s_alpha, nullptr, sm, red);
+        // ---- O5 start (k_cg_init): x0 = 0, p0 = r0 = b', |b'|^2.  Own blocks only (this CTA's warps have just written them and
+        // pcgs_stencil ends on a block barrier).  |r|^2 is left per (block, group of 8 reals) = per warp of k_cg_init ...
+        if (tid < 96) {
+            const int k8 = tid >> 5;
+            for (int rhs = 0; rhs < nrhs; rhs++)
+                for (int blk = blockIdx.x; blk < a.ntiles; blk += gridDim.x) {
+                    const int i = blk * LB + lane;
+                    double sum = 0;
+                    if (i < Vh) {
+                        T rv[8], z[8];
+                        load8<PREC, false>((const char*)a.r + fb * rhs, i, k8, rv);
+#pragma unroll
+                        for (int k = 0; k < 8; k++) { sum = fma((double)rv[k], (double)rv[k], sum); z[k] = 0; }   // k_cg_init's chain, not left to contraction
+                        store8<PREC>((char*)a.p + fb * rhs, i, k8, rv);
+                        store8<PREC>((char*)a.x + fb * rhs, i, k8, z);
+                    }
+                    const double gsum = warp_sum(sum);
+                    if (lane == 0) a.init_groups[(size_t)rhs * 3 * a.ntiles + 3 * blk + k8] = gsum;
+                }
+        }
+        grid.sync();
+        // ... and summed in k_cg_init's order: its block b adds its 8 warps (groups 8b .. 8b+7) serially, then one warp adds
+        // the blocks lane-strided and by the shuffle tree (sum_partials_warp)
+        for (int j = wid; j < nrhs; j += 4) {
+            const double* gr = a.init_groups + (size_t)j * 3 * a.ntiles;
+            const int ng = 3 * a.ntiles;
+            double v = 0;
+            for (int b = lane; b < a.init_gx; b += 32) {
+                double pb = 0;
+                for (int k = 0; k < 8; k++) pb += (8 * b + k < ng) ? __ldcg(gr + 8 * b + k) : 0.0;
+                v += pb;
+            }
+            v = warp_sum(v);
+            if (lane == 0) {
+                s_rr[j] = v; s_bb[j] = v; s_pq[j] = 0; s_beta[j] = 0; s_iters[j] = 0; s_status[j] = TSM_OK; s_done[j] = !(v > 0);
+                s_alpha[j] = 0.0;
+            }
+        }
+        __syncthreads();
+        if (tid == 0) {
+            int all = 1;
+            for (int j = 0; j < nrhs; j++) all &= s_done[j];
+            s_all = all;
+        }
+        __syncthreads();
+    }
 
     for (int it = 0; it < a.max_iter && !s_all; it++) {
         pcgs_stencil<PREC, RECON, false, false, EPI_NONE>(a, 1, a.p, nullptr, a.t, a.c1, s_alpha, nullptr, sm, red);   // t = R^-1 D_oe p
@@ -322,7 +392,6 @@ __global__ void __launch_bounds__(128) k_cg_persistent_small(const PcgArgs a)
         }
         __syncthreads();
         // x += alpha p; p = r + beta p on this CTA's own blocks: 96 threads = 32 sites x 3 groups of 8 reals
-        const size_t fb = field_bytes(PREC, Vh, 1);
         if (tid < 96) {
             const int k8 = tid >> 5;
             for (int rhs = 0; rhs < nrhs; rhs++) {
@@ -358,7 +427,7 @@ __global__ void __launch_bounds__(128) k_cg_persistent_small(const PcgArgs a)
                     s_iters[j] += 1;
                     s_beta[j] = v / s_rr[j];
                     s_rr[j] = v;
-                    if (a.tol > 0 && sqrt(v / cg->bb[j]) <= a.tol) s_done[j] = 1;
+                    if (a.tol > 0 && sqrt(v / s_bb[j]) <= a.tol) s_done[j] = 1;
                 }
                 all &= s_done[j];
             }
@@ -366,9 +435,12 @@ __global__ void __launch_bounds__(128) k_cg_persistent_small(const PcgArgs a)
         }
         grid.sync();
     }
+    // ---- H7: s_o = R^-1 (eta_o + kappa D_oe x), in place (a thread reads and rewrites only its own components)
+    if (a.whole) pcgs_stencil<PREC, RECON, false, true, EPI_NONE>(a, 1, a.x, a.s_o, a.s_o, a.crec, s_alpha, nullptr, sm, red);
     if (blockIdx.x == 0) {
         __syncthreads();
         if (tid < nrhs) {
+            cg->bb[tid] = s_bb[tid];
             cg->rr[tid] = s_rr[tid]; cg->done[tid] = s_done[tid]; cg->iters[tid] = s_iters[tid]; cg->status[tid] = s_status[tid];
             cg->beta[tid] = s_beta[tid]; cg->pq[tid] = s_pq[tid]; cg->alpha[tid] = s_alpha[tid]; cg->rr_new[tid] = s_rrnew[tid];
         }

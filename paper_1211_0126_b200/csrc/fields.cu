@@ -171,13 +171,7 @@ __global__ void k_twist(const int Vh, const int nrhs, const void* __restrict__ i
         const size_t off = field_bytes(PREC, Vh, 1) * rhs;
         T v[8], o[8];
         load8<PREC>((const char*)in + off, i, k8, v);
-#pragma unroll
-        for (int j = 0; j < 4; j++) {
-            const int q = 4 * k8 + j;
-            const T cr = (T)(q < 6 ? c.up_re : c.lo_re), ci = (T)(q < 6 ? c.up_im : c.lo_im);
-            o[2 * j] = cr * v[2 * j] - ci * v[2 * j + 1];
-            o[2 * j + 1] = cr * v[2 * j + 1] + ci * v[2 * j];
-        }
+        twist8<T>(c, k8, v, o);
         store8<PREC>((char*)out + off, i, k8, o);
     }
 }

@@ -383,6 +383,20 @@ enum { EPI_NONE = 0, EPI_NORM = 1, EPI_RESID = 2 };
 struct TwistCoef { double up_re, up_im, lo_re, lo_im; };
 struct DslashCoef { TwistCoef x, d; };
 
+// o = c (x) v on reals 8 k8 .. 8 k8 + 7 of a site (c.up on spins 0, 1, c.lo on spins 2, 3): the arithmetic of k_twist,
+// shared with the whole-solve persistent kernel (dslash_small.cu) so that both give the same bits
+template <typename T> __device__ __forceinline__ void twist8(const TwistCoef& c, const int k8, const T* v, T* o)
+{
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        const int q = 4 * k8 + j;
+        const T cr = (T)(q < 6 ? c.up_re : c.lo_re), ci = (T)(q < 6 ? c.up_im : c.lo_im);
+        // explicit FMAs: left to the compiler, "a b - c d" is contracted differently in different kernels
+        o[2 * j] = fma_(-ci, v[2 * j + 1], cr * v[2 * j]);
+        o[2 * j + 1] = fma_(ci, v[2 * j], cr * v[2 * j + 1]);
+    }
+}
+
 // ------------------------------------------------------------------ context
 struct GammaTable {          // Gamma_{alpha, col[alpha]} = i^ph[alpha], all other entries 0
     int col[16][4];
@@ -540,12 +554,21 @@ struct PcgArgs {
     DslashCoef c1, c2, c3, c4;      // the four stencil launches of cg_iteration (api_solve.cu)
     double* partials;               // [2][nrhs][ntiles]: |w|^2 per tile, |r|^2 per tile
     CgScalars* cg;
+    // whole-solve form (small kernel only): source preparation, CG initialisation and reconstruction in the same launch
+    int whole;                      // 0: the iteration loop only
+    void *s_o, *aux;                // the slot's odd half (eta_o on entry, s_o on exit); scratch vector
+    TwistCoef tw_rinv;              // aux = R^-1 eta_o
+    DslashCoef cp1, cp2, cp3, crec; // bhat, t, b' (tsm_solve's three preparation stencils) and the reconstruction
+    double* init_groups;            // [nrhs][3 ntiles]: |r|^2 of every (32-site block, group of 8 reals)
+    int init_gx;                    // blocks of k_cg_init's grid on this lattice (its summation order is reproduced)
 };
 int launch_cg_persistent_small(tsm_ctx* ctx, int prec, PcgArgs& a);
 bool cg_persistent_supported(const tsm_ctx* ctx, int prec, int nrhs);
 bool cg_persistent_preferred(const tsm_ctx* ctx, int prec, int nrhs);
 int launch_cg_persistent(tsm_ctx* ctx, int prec, int nrhs, void* x, void* r, void* p, void* w, void* t, const DslashCoef& c1,
-                         const DslashCoef& c2, const DslashCoef& c3, const DslashCoef& c4, double tol, int max_iter);
+                         const DslashCoef& c2, const DslashCoef& c3, const DslashCoef& c4, double tol, int max_iter,
+                         const PcgArgs* whole = nullptr);
+int blas_grid_x(const tsm_ctx* ctx);
 int launch_convert(tsm_ctx* ctx, int prec_in, int prec_out, int nrhs_fields, const void* in, void* out);
 int launch_contract(tsm_ctx* ctx, int slot);
 int launch_accumulate(tsm_ctx* ctx, double* acc, const double* a, const double* b, int nrhs);
