@@ -128,8 +128,10 @@ __device__ __forceinline__ double small_block(const Geom& g, const int par, cons
         const T cdr = (T)(a < 2 ? cf.d.up_re : cf.d.lo_re), cdi = (T)(a < 2 ? cf.d.up_im : cf.d.lo_im);
 #pragma unroll
         for (int c = 0; c < 3; c++) {
-            o[2 * c] = cdr * v[2 * c] - cdi * v[2 * c + 1];
-            o[2 * c + 1] = cdr * v[2 * c + 1] + cdi * v[2 * c];
+            // explicit chains: k_dslash_small and k_cg_persistent_small must round alike, so which of two products is
+            // fused is not left to the compiler
+            o[2 * c] = fma_(cdr, v[2 * c], -(cdi * v[2 * c + 1]));
+            o[2 * c + 1] = fma_(cdr, v[2 * c + 1], cdi * v[2 * c]);
         }
         if (XPAY) {
             const T cxr = (T)(a < 2 ? cf.x.up_re : cf.x.lo_re), cxi = (T)(a < 2 ? cf.x.up_im : cf.x.lo_im);
@@ -137,21 +139,21 @@ __device__ __forceinline__ double small_block(const Geom& g, const int par, cons
             load_spin<PREC, NC>(xf, i, a, xv);
 #pragma unroll
             for (int c = 0; c < 3; c++) {
-                o[2 * c] += cxr * xv[2 * c] - cxi * xv[2 * c + 1];
-                o[2 * c + 1] += cxr * xv[2 * c + 1] + cxi * xv[2 * c];
+                o[2 * c] = fma_(cxr, xv[2 * c], fma_(-cxi, xv[2 * c + 1], o[2 * c]));
+                o[2 * c + 1] = fma_(cxr, xv[2 * c + 1], fma_(cxi, xv[2 * c], o[2 * c + 1]));
             }
         }
         if (EPI == EPI_RESID) {   // out is the CG residual r (same precision as the spinors here): r -= alpha q
             T rv[6];
             load_spin<PREC, false>(out, i, a, rv);
 #pragma unroll
-            for (int c = 0; c < 6; c++) { rv[c] -= alpha * o[c]; nrm += (double)rv[c] * (double)rv[c]; }
+            for (int c = 0; c < 6; c++) { rv[c] = fma_(-alpha, o[c], rv[c]); nrm = fma((double)rv[c], (double)rv[c], nrm); }
             store_spin<PREC>(out, i, a, rv);
         } else {
             store_spin<PREC>(out, i, a, o);
             if (EPI == EPI_NORM) {
 #pragma unroll
-                for (int c = 0; c < 6; c++) nrm += (double)o[c] * (double)o[c];
+                for (int c = 0; c < 6; c++) nrm = fma((double)o[c], (double)o[c], nrm);
             }
         }
     }
