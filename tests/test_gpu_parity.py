@@ -1051,4 +1051,21 @@ def test_persistent_cg_kernel(tsm_mod, dims, recon, stencil):
     n0 = c.t.launch_count()
     c.t.solve(seed, [4], F32, 0.0, 13, slot=0)
     assert c.t.launch_count() - n0 == 6 + 1 + 1
+    # automatic mode, solves only enqueued (tsm_solve_async): the same iterates as the kernel-by-kernel path, against
+    # the oracle too; where the one-launch solve applies a batch is the noise kernel plus ONE launch
+    c.t.set_graphs(4)
+    for k in (0, 2, 3):
+        prec, tol, it, ids = cases[k]
+        n0 = c.t.launch_count()
+        c.t.solve_async(seed, ids, prec, tol, it, slot=1)
+        n_l = c.t.launch_count() - n0
+        rc, info = c.t.solve_wait(1)
+        assert rc == 0 and [i["iters"] for i in info] == ref[k][0], (dims, k)
+        for j in range(len(ids)):
+            assert np.array_equal(c.t.get_solution(1, j), ref[k][2][j]), (dims, k, j)
+        if stencil == 0 and dims[0] * dims[1] * dims[2] * dims[3] // 2 <= 16384:
+            assert n_l == 2, (dims, k, n_l)
+    if dims[3] <= 16:   # (the oracle's converged solve of the largest lattice here would take a minute)
+        s_conv, _ = oracle.solve(dims, -1, c.kappa, c.mu, c.U, oracle.noise(dims, seed, 2), 1e-9, 2000)
+        assert rel(c.t.get_solution(1, 0), s_conv) < 1e-6
     c.t.close()
