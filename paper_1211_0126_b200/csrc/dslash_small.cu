@@ -98,6 +98,11 @@ __device__ __forceinline__ double small_block(const Geom& g, const int par, cons
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;   // w: direction in the first half, spin component in the second
     const int i = blk * LB + lane;
     const bool live = i < Vh;
+    // the own-site x and r vectors of the second half (spin component w) are requested BEFORE the hops: their latency then
+    // overlaps the gathers instead of following the barrier (the same values: nothing writes them in between)
+    T xv[6] = {}, rv[6] = {};
+    if (XPAY && live) load_spin<PREC, NC>(xf, i, w, xv);
+    if (EPI == EPI_RESID && live) load_spin<PREC, false>(out, i, w, rv);
     {
         T part[24];
 #pragma unroll
@@ -135,8 +140,6 @@ __device__ __forceinline__ double small_block(const Geom& g, const int par, cons
         }
         if (XPAY) {
             const T cxr = (T)(a < 2 ? cf.x.up_re : cf.x.lo_re), cxi = (T)(a < 2 ? cf.x.up_im : cf.x.lo_im);
-            T xv[6];
-            load_spin<PREC, NC>(xf, i, a, xv);
 #pragma unroll
             for (int c = 0; c < 3; c++) {
                 o[2 * c] = fma_(cxr, xv[2 * c], fma_(-cxi, xv[2 * c + 1], o[2 * c]));
@@ -144,8 +147,6 @@ __device__ __forceinline__ double small_block(const Geom& g, const int par, cons
             }
         }
         if (EPI == EPI_RESID) {   // out is the CG residual r (same precision as the spinors here): r -= alpha q
-            T rv[6];
-            load_spin<PREC, false>(out, i, a, rv);
 #pragma unroll
             for (int c = 0; c < 6; c++) { rv[c] = fma_(-alpha, o[c], rv[c]); nrm = fma((double)rv[c], (double)rv[c], nrm); }
             store_spin<PREC>(out, i, a, rv);
